@@ -1,0 +1,146 @@
+/*
+ * epsgrad.h -- C ABI of the B200-native parametrization chain  C -> eps_hat  on the
+ * Yee grid and of its reverse pass (arxiv 2505.03352, "Accelerated inverse design of
+ * passive Si photonics").  "P:L<n>" = line n of the paper text; "S<n>" =
+ * the readings of silent / ambiguous points listed in DESIGN.md section 3.
+ *
+ * What the library computes
+ *   forward (Fig. 2/3):
+ *     Eq. (2)  Phi  = sum_ab C_ab b(x-x_a, y-y_b)   on a mask with `subpixel` pixels per
+ *              Yee cell (normalised density-filter form by default, S2)
+ *     Eq. (3)/(6)  rho = 1/2 (1 + tanh(beta (Phi - eta)))
+ *     mixing   eps = rho eps_core + (1-rho) eps_clad
+ *     Eq. (8)  cell averages <eps>, <1/eps> on the half-cell-shifted E_x/E_y/E_z
+ *              footprints (finite sums on the mask)
+ *     normals  Sobel operators at FDTD resolution, normalised
+ *     Eq. (7)  eps_ii^-1 = n_i^2 <eps^-1> + (1-n_i^2) <eps>^-1
+ *     z-extrusion to the slab [z_lo, z_hi] with fractional faces              P:L45 (S7, S8)
+ *   reverse (Eq. (1); "VJP ... with arbitrary field"):
+ *     dF/dC = -2 Re( (d eps_hat/dC)^T (E_F (.) E_A) ),  summed over field pairs;
+ *     the product is the plain element-wise complex product.
+ *
+ * Conventions
+ *   - All arrays are dense, row-major, last index fastest (component first).
+ *       C     [B, Mx, My]             float32
+ *       eps   [B, 3, Nx, Ny, Nz]      float32   (eps_xx, eps_yy, eps_zz), Nx = upsample*Mx
+ *       E_F/A [B, 3, Nx, Ny, Nz]      complex64, interleaved (re, im) float32
+ *       dFdC  [B, Mx, My]             float32, OVERWRITTEN with the sum over the pairs
+ *   - Device entry points take DEVICE pointers (16-byte aligned) and enqueue all work on
+ *     `stream` (a cudaStream_t passed as void*; NULL = the legacy default stream).  They
+ *     never synchronise the host, never allocate, and never write an input.
+ *   - *_host entry points take HOST pointers (pinned memory recommended), stage through
+ *     the plan's staging buffer (epsgrad_plan_set_staging), enqueue H2D copies, the same
+ *     kernels, and D2H copies on `stream`, and return without synchronising.
+ *   - The caller owns every data buffer, the workspace and the staging buffer.  The
+ *     library owns the plan: a host struct plus a few KB of device tables (filter
+ *     weights, border normalisers, z weights) allocated in epsgrad_plan_create.
+ *   - Every function returns an int status: 0 = EPSGRAD_OK, negative = error (below).
+ *     No exceptions, no abort.  Asynchronous faults surface at the caller's next sync.
+ *   - There is no CPU path.  Without a CUDA device plan creation fails with EPSGRAD_ECUDA.
+ */
+#ifndef EPSGRAD_H_
+#define EPSGRAD_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define EPSGRAD_OK             0
+#define EPSGRAD_EINVAL        -1   /* null / misaligned pointer, bad size, beta <= 0, eps <= 0, ... */
+#define EPSGRAD_EUNSUPPORTED  -2   /* upsample*subpixel not in {2,4,6,8}, Nz % 4 != 0, tables too large */
+#define EPSGRAD_ENOWORKSPACE  -3   /* workspace / staging buffer missing or too small */
+#define EPSGRAD_ECUDA         -4   /* CUDA runtime error (no device, launch failure) */
+#define EPSGRAD_ENOMEM        -5   /* host allocation failed */
+
+#define EPSGRAD_FILTER_CONIC     0 /* b = max(0, 1 - r/R)                              (S1)  */
+#define EPSGRAD_FILTER_GAUSSIAN  1 /* b = exp(-r^2/2 sigma^2), |dx|,|dy| <= R per axis (S11) */
+
+#define EPSGRAD_MAX_PAIRS 8        /* field pairs fused into one z-reduction launch; more are chained */
+
+typedef struct epsgrad_plan epsgrad_plan_t;   /* opaque, library-owned */
+
+/* Geometry, filter and materials of a batch of B identical design regions (cell units). */
+typedef struct {
+    int32_t batch;            /* B >= 1 independent designs                                  */
+    int32_t mx, my;           /* control grid (Eq. (2) nodes, pixel-centred; S3)             */
+    int32_t upsample;         /* u: Yee cells per control pixel, Nx = u*Mx, Ny = u*My        */
+    int32_t subpixel;         /* s: mask pixels per Yee cell per axis, even (S4; default 2)  */
+    int32_t nz;               /* Yee cells in z (multiple of 4)                              */
+    int32_t filter_kind;      /* EPSGRAD_FILTER_*                                            */
+    int32_t filter_normalize; /* 1: density filter, renormalised at borders (S2); 0: raw Eq. (2) */
+    double  z_lo, z_hi;       /* slab extent in cell units, may be fractional (S8)           */
+    double  filter_radius;    /* R in Yee cells                                              */
+    double  filter_sigma;     /* Gaussian sigma in Yee cells                                 */
+    double  eta;              /* projection threshold: 0.5 -> Eq. (6), 0 -> Eq. (3) (S9)     */
+    double  eps_core, eps_clad;
+    double  normal_delta;     /* guard in n_c^2 = g_c^2/(|g|^2 + delta) (S6; default 1e-12)  */
+} epsgrad_config_t;
+
+/* ---- plan -------------------------------------------------------------------------- */
+/* Validates cfg, builds the tables on `device`.  *out is set only on success.           */
+int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsgrad_plan_t **out);
+int epsgrad_plan_destroy(epsgrad_plan_t *plan);
+
+/* Scratch the device entry points need (filter output Phi, reduced cotangent, mask
+ * cotangent, separable-filter temporaries).  The caller allocates it (e.g. a torch
+ * uint8 tensor) and keeps it alive and unshared while calls of this plan are in flight. */
+size_t epsgrad_workspace_bytes(const epsgrad_plan_t *plan);
+int    epsgrad_plan_set_workspace(epsgrad_plan_t *plan, void *dev_ptr, size_t bytes);
+
+/* Device staging for the *_host entry points: C, dFdC, eps and n_pairs field pairs.     */
+size_t epsgrad_staging_bytes(const epsgrad_plan_t *plan, int n_pairs);
+int    epsgrad_plan_set_staging(epsgrad_plan_t *plan, void *dev_ptr, size_t bytes);
+
+/* Reverse-pass field reads (P:L27 restricts Eq. (1) to Omega_D; in z only the slab cells
+ * have d eps/dC != 0).  0 (default): read only the 16-byte chunks of each z column that
+ * hold slab cells.  1: read every z cell (weights are zero outside the slab).  Results
+ * are identical; this is a measurement switch.                                           */
+int epsgrad_plan_set_dense_reads(epsgrad_plan_t *plan, int dense);
+
+/* Number of kernel launches the last eps_* call of this plan enqueued (for accounting). */
+int epsgrad_plan_last_launches(const epsgrad_plan_t *plan);
+
+/* ---- the hot path (device pointers) -------------------------------------------------- */
+/* eps_hat(C, beta): the whole forward chain.  beta > 0 (it changes every
+ * iteration, Eq. (14), hence a call argument).                                    */
+int eps_forward(epsgrad_plan_t *plan, const float *C, float beta, float *eps, void *stream);
+
+/* Eq. (1): dFdC = -2 Re((d eps/dC)^T (E_F (.) E_A)) summed over n_pairs >= 1
+ * pairs.  EF, EA: HOST arrays of n_pairs DEVICE pointers to complex64 [B,3,Nx,Ny,Nz].
+ * A real cotangent w can be fed as E_F = -w/2 + 0i, E_A = 1 + 0i.               */
+int eps_vjp(epsgrad_plan_t *plan, const float *C, float beta, int n_pairs,
+            const void *const *EF, const void *const *EA, float *dFdC, void *stream);
+
+/* Both in one call; the filter output (Phi) is computed once and shared.                */
+int eps_forward_vjp(epsgrad_plan_t *plan, const float *C, float beta, int n_pairs,
+                    const void *const *EF, const void *const *EA,
+                    float *eps, float *dFdC, void *stream);
+
+/* ---- the same calls on HOST buffers (end-to-end path; copies included) --------------- */
+/* eps_host / dFdC_host may be NULL to skip that output (and its work).                  */
+int eps_forward_vjp_host(epsgrad_plan_t *plan, const float *C_host, float beta, int n_pairs,
+                         const void *const *EF_host, const void *const *EA_host,
+                         float *eps_host, float *dFdC_host, void *stream);
+/* bytes the last *_host call copied host->device and device->host                       */
+int epsgrad_plan_last_copy_bytes(const epsgrad_plan_t *plan, uint64_t *h2d, uint64_t *d2h);
+
+/* ---- stage taps (device pointers; for stage-by-stage parity tests) ------------------- */
+/* Phi - eta0 on the mask [B, s*Nx, s*Ny] (eta0 = eta if filter_normalize else 0).       */
+int epsgrad_stage_filter(epsgrad_plan_t *plan, const float *C, float *phi_centred, void *stream);
+/* eps2d [B,3,Nx,Ny]: the 2-D stage before z-extrusion (steps 1-6).                      */
+int epsgrad_stage_eps2d(epsgrad_plan_t *plan, const float *C, float beta, float *eps2d, void *stream);
+/* z-reduced cotangent [B,5,Nx,Ny]: planes x, y, z(full cells), z(lower face), z(upper face). */
+int epsgrad_stage_zreduce(epsgrad_plan_t *plan, int n_pairs, const void *const *EF,
+                          const void *const *EA, float *gbar, void *stream);
+
+const char *epsgrad_status_string(int status);
+/* library version: major*10000 + minor*100 + patch */
+int epsgrad_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* EPSGRAD_H_ */

@@ -1,0 +1,265 @@
+"""Thin ctypes binding of ``include/epsgrad.h`` -- argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of ``libepsgrad.so``; torch is used for
+device memory (tensors, workspace) and the current CUDA stream.  There is no CPU path: a
+missing library or a missing CUDA device is a hard error.  Names follow the C ABI.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Sequence
+
+from . import build as _build
+
+OK, EINVAL, EUNSUPPORTED, ENOWORKSPACE, ECUDA, ENOMEM = 0, -1, -2, -3, -4, -5
+FILTER_CONIC, FILTER_GAUSSIAN = 0, 1
+
+EXPORTS = (
+    "epsgrad_plan_create", "epsgrad_plan_destroy", "epsgrad_workspace_bytes",
+    "epsgrad_plan_set_workspace", "epsgrad_staging_bytes", "epsgrad_plan_set_staging",
+    "epsgrad_plan_set_dense_reads", "epsgrad_plan_last_launches", "epsgrad_plan_last_copy_bytes",
+    "eps_forward", "eps_vjp", "eps_forward_vjp", "eps_forward_vjp_host",
+    "epsgrad_stage_filter", "epsgrad_stage_eps2d", "epsgrad_stage_zreduce",
+    "epsgrad_status_string", "epsgrad_version",
+)
+
+
+class EpsgradError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: {status_string(status)} ({status})")
+
+
+class Config(ctypes.Structure):
+    """epsgrad_config_t (include/epsgrad.h)."""
+    _fields_ = [
+        ("batch", ctypes.c_int32), ("mx", ctypes.c_int32), ("my", ctypes.c_int32),
+        ("upsample", ctypes.c_int32), ("subpixel", ctypes.c_int32), ("nz", ctypes.c_int32),
+        ("filter_kind", ctypes.c_int32), ("filter_normalize", ctypes.c_int32),
+        ("z_lo", ctypes.c_double), ("z_hi", ctypes.c_double),
+        ("filter_radius", ctypes.c_double), ("filter_sigma", ctypes.c_double),
+        ("eta", ctypes.c_double), ("eps_core", ctypes.c_double), ("eps_clad", ctypes.c_double),
+        ("normal_delta", ctypes.c_double),
+    ]
+
+    @property
+    def nx(self) -> int:
+        return self.upsample * self.mx
+
+    @property
+    def ny(self) -> int:
+        return self.upsample * self.my
+
+
+def make_config(*, batch=1, mx, my, nz, z_lo, z_hi, upsample=2, subpixel=2, filter_kind=FILTER_CONIC,
+                filter_radius=4.0, filter_sigma=1.0, filter_normalize=1, eta=0.5, eps_core=12.11,
+                eps_clad=2.085, normal_delta=1e-12) -> Config:
+    return Config(batch, mx, my, upsample, subpixel, nz, filter_kind, filter_normalize, z_lo, z_hi,
+                  filter_radius, filter_sigma, eta, eps_core, eps_clad, normal_delta)
+
+
+def config_of(w) -> Config:
+    """Config of a ``workloads.Workload``."""
+    return make_config(batch=w.batch, mx=w.mx, my=w.my, nz=w.nz, z_lo=w.z_lo, z_hi=w.z_hi, upsample=w.upsample,
+                       subpixel=w.subpixel, filter_kind=w.filter_kind, filter_radius=w.radius,
+                       filter_sigma=w.sigma if w.sigma > 0 else 1.0, eta=w.eta, eps_core=w.eps_core,
+                       eps_clad=w.eps_clad, normal_delta=w.normal_delta)
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load (building if stale and nvcc is present) libepsgrad.so; raises if it cannot be had."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if _build.stale():
+        try:
+            path = _build.build()
+        except Exception as e:  # no nvcc on this box: use the shipped library if there is one
+            if not os.path.exists(path):
+                raise RuntimeError(f"libepsgrad.so is missing and could not be built: {e}") from e
+    L = ctypes.CDLL(path)
+    vp, i32, f32, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_float, ctypes.c_size_t
+    L.epsgrad_plan_create.argtypes = [ctypes.POINTER(Config), i32, ctypes.POINTER(vp)]
+    L.epsgrad_plan_destroy.argtypes = [vp]
+    L.epsgrad_workspace_bytes.argtypes = [vp]
+    L.epsgrad_workspace_bytes.restype = sz
+    L.epsgrad_plan_set_workspace.argtypes = [vp, vp, sz]
+    L.epsgrad_staging_bytes.argtypes = [vp, i32]
+    L.epsgrad_staging_bytes.restype = sz
+    L.epsgrad_plan_set_staging.argtypes = [vp, vp, sz]
+    L.epsgrad_plan_set_dense_reads.argtypes = [vp, i32]
+    L.epsgrad_plan_last_launches.argtypes = [vp]
+    L.epsgrad_plan_last_copy_bytes.argtypes = [vp, ctypes.POINTER(ctypes.c_uint64), ctypes.POINTER(ctypes.c_uint64)]
+    L.eps_forward.argtypes = [vp, vp, f32, vp, vp]
+    L.eps_vjp.argtypes = [vp, vp, f32, i32, vp, vp, vp, vp]
+    L.eps_forward_vjp.argtypes = [vp, vp, f32, i32, vp, vp, vp, vp, vp]
+    L.eps_forward_vjp_host.argtypes = [vp, vp, f32, i32, vp, vp, vp, vp, vp]
+    L.epsgrad_stage_filter.argtypes = [vp, vp, vp, vp]
+    L.epsgrad_stage_eps2d.argtypes = [vp, vp, f32, vp, vp]
+    L.epsgrad_stage_zreduce.argtypes = [vp, i32, vp, vp, vp, vp]
+    L.epsgrad_status_string.argtypes = [i32]
+    L.epsgrad_status_string.restype = ctypes.c_char_p
+    L.epsgrad_version.restype = i32
+    _lib = L
+    return L
+
+
+def status_string(status: int) -> str:
+    return lib().epsgrad_status_string(int(status)).decode()
+
+
+def _check(status: int, where: str) -> None:
+    if status != OK:
+        raise EpsgradError(status, where)
+
+
+def _ptr_array(tensors: Sequence) -> ctypes.Array:
+    return (ctypes.c_void_p * len(tensors))(*[t.data_ptr() for t in tensors])
+
+
+class Plan:
+    """epsgrad_plan_t plus its torch-allocated workspace.  Methods mirror the C entry points."""
+
+    def __init__(self, cfg: Config, device: int = 0):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("epsgrad needs a CUDA device (sm_100a); there is no CPU path")
+        self._torch = torch
+        self.cfg = cfg
+        self.device = torch.device("cuda", device)
+        self._h = ctypes.c_void_p()
+        _check(lib().epsgrad_plan_create(ctypes.byref(cfg), device, ctypes.byref(self._h)), "epsgrad_plan_create")
+        nbytes = lib().epsgrad_workspace_bytes(self._h)
+        self._ws = torch.empty(max(nbytes, 256), dtype=torch.uint8, device=self.device)
+        _check(lib().epsgrad_plan_set_workspace(self._h, self._ws.data_ptr(), self._ws.numel()),
+               "epsgrad_plan_set_workspace")
+        self._stg = None
+        self._stg_pairs = -1
+
+    def close(self) -> None:
+        if getattr(self, "_h", None):
+            lib().epsgrad_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- shapes
+    @property
+    def eps_shape(self):
+        c = self.cfg
+        return (c.batch, 3, c.nx, c.ny, c.nz)
+
+    @property
+    def ctrl_shape(self):
+        return (self.cfg.batch, self.cfg.mx, self.cfg.my)
+
+    @property
+    def mask_shape(self):
+        c = self.cfg
+        return (c.batch, c.subpixel * c.nx, c.subpixel * c.ny)
+
+    def _stream(self) -> int:
+        return self._torch.cuda.current_stream(self.device).cuda_stream
+
+    def _c(self, C):
+        t = self._torch
+        assert C.is_cuda and C.dtype == t.float32 and C.is_contiguous() and tuple(C.shape) == self.ctrl_shape, \
+            (C.shape, self.ctrl_shape)
+        return C
+
+    def _fields(self, EF, EA):
+        t = self._torch
+        assert len(EF) == len(EA) and len(EF) >= 1
+        for f in list(EF) + list(EA):
+            assert f.is_cuda and f.dtype == t.complex64 and f.is_contiguous() and tuple(f.shape) == self.eps_shape, \
+                (f.shape, f.dtype, self.eps_shape)
+        return _ptr_array(EF), _ptr_array(EA)
+
+    def _out(self, out, shape):
+        t = self._torch
+        if out is None:
+            return t.empty(shape, dtype=t.float32, device=self.device)
+        assert out.is_cuda and out.dtype == t.float32 and out.is_contiguous() and tuple(out.shape) == tuple(shape)
+        return out
+
+    # ---- options
+    def set_dense_reads(self, dense: bool) -> None:
+        _check(lib().epsgrad_plan_set_dense_reads(self._h, int(bool(dense))), "epsgrad_plan_set_dense_reads")
+
+    def last_launches(self) -> int:
+        return int(lib().epsgrad_plan_last_launches(self._h))
+
+    def last_copy_bytes(self):
+        a, b = ctypes.c_uint64(), ctypes.c_uint64()
+        _check(lib().epsgrad_plan_last_copy_bytes(self._h, ctypes.byref(a), ctypes.byref(b)), "last_copy_bytes")
+        return int(a.value), int(b.value)
+
+    # ---- hot path (device tensors)
+    def eps_forward(self, C, beta: float, out=None):
+        eps = self._out(out, self.eps_shape)
+        _check(lib().eps_forward(self._h, self._c(C).data_ptr(), beta, eps.data_ptr(), self._stream()), "eps_forward")
+        return eps
+
+    def eps_vjp(self, C, beta: float, EF: Sequence, EA: Sequence, out=None):
+        pf, pa = self._fields(EF, EA)
+        g = self._out(out, self.ctrl_shape)
+        _check(lib().eps_vjp(self._h, self._c(C).data_ptr(), beta, len(EF), pf, pa, g.data_ptr(), self._stream()),
+               "eps_vjp")
+        return g
+
+    def eps_forward_vjp(self, C, beta: float, EF: Sequence, EA: Sequence, eps_out=None, grad_out=None):
+        pf, pa = self._fields(EF, EA)
+        eps = self._out(eps_out, self.eps_shape)
+        g = self._out(grad_out, self.ctrl_shape)
+        _check(lib().eps_forward_vjp(self._h, self._c(C).data_ptr(), beta, len(EF), pf, pa, eps.data_ptr(),
+                                     g.data_ptr(), self._stream()), "eps_forward_vjp")
+        return eps, g
+
+    # ---- the same on host (CPU, ideally pinned) tensors; outputs are written asynchronously:
+    # synchronise the stream before reading them
+    def eps_forward_vjp_host(self, C, beta: float, EF: Sequence, EA: Sequence, eps_out, grad_out):
+        t = self._torch
+        n = len(EF) if grad_out is not None else 0
+        if self._stg is None or self._stg_pairs < n:
+            nbytes = lib().epsgrad_staging_bytes(self._h, n)
+            self._stg = t.empty(nbytes, dtype=t.uint8, device=self.device)
+            self._stg_pairs = n
+            _check(lib().epsgrad_plan_set_staging(self._h, self._stg.data_ptr(), nbytes), "epsgrad_plan_set_staging")
+        for x in [C, *EF, *EA] + [o for o in (eps_out, grad_out) if o is not None]:
+            assert not x.is_cuda and x.is_contiguous()
+        pf, pa = _ptr_array(EF), _ptr_array(EA)
+        _check(lib().eps_forward_vjp_host(
+            self._h, C.data_ptr(), beta, len(EF), pf, pa,
+            eps_out.data_ptr() if eps_out is not None else None,
+            grad_out.data_ptr() if grad_out is not None else None, self._stream()), "eps_forward_vjp_host")
+
+    # ---- stage taps
+    def stage_filter(self, C):
+        out = self._out(None, self.mask_shape)
+        _check(lib().epsgrad_stage_filter(self._h, self._c(C).data_ptr(), out.data_ptr(), self._stream()),
+               "epsgrad_stage_filter")
+        return out
+
+    def stage_eps2d(self, C, beta: float):
+        c = self.cfg
+        out = self._out(None, (c.batch, 3, c.nx, c.ny))
+        _check(lib().epsgrad_stage_eps2d(self._h, self._c(C).data_ptr(), beta, out.data_ptr(), self._stream()),
+               "epsgrad_stage_eps2d")
+        return out
+
+    def stage_zreduce(self, EF: Sequence, EA: Sequence):
+        c = self.cfg
+        pf, pa = self._fields(EF, EA)
+        out = self._out(None, (c.batch, 5, c.nx, c.ny))
+        _check(lib().epsgrad_stage_zreduce(self._h, len(EF), pf, pa, out.data_ptr(), self._stream()),
+               "epsgrad_stage_zreduce")
+        return out

@@ -1,0 +1,705 @@
+// epsgrad.cu -- C ABI (include/epsgrad.h), plan / table construction and kernel launches.
+// Product code for sm_100a; shares nothing with oracle/.
+#include "../../include/epsgrad.h"
+
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "common.cuh"
+#include "filter.cuh"
+#include "filter_sep.cuh"
+#include "forward.cuh"
+#include "reverse2d.cuh"
+#include "zreduce.cuh"
+
+using namespace epsgrad;
+
+#define EPSGRAD_VERSION 100   /* 0.1.0 */
+
+struct epsgrad_plan {
+    epsgrad_config_t cfg;
+    int device;
+    int nx, ny, px, py, m;
+    int T, NT, KX, KY;
+    int separable;
+    int conic_tile;            // TA = TB of the transposed conic filter (16 or 8)
+    // device tables (one allocation)
+    void *d_tables;
+    float *d_w;                // conic [NT][NT][m][m] | separable [NT][m]
+    int *d_tyrange;            // conic [NT][2]
+    float *d_invden;           // conic [KX*m][KY*m] | separable [KX*m] + [KY*m]
+    float *d_zw;               // [5][nz]
+    // z windows (chunks of 2 cells) for {x,y} and {z}; face weights
+    int ch0[2], nch[2];
+    float w_lo, w_hi;
+    int dense;
+    // scalars
+    float eta0, eta_r, eps_clad, deps, delta;
+    // caller-owned buffers
+    void *ws; size_t ws_bytes;
+    void *stg; size_t stg_bytes;
+    // workspace carve-up (byte offsets)
+    size_t off_phi, off_v, off_gbar, off_tmp, ws_need;
+    int last_launches;
+    uint64_t last_h2d, last_d2h;
+};
+
+static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+static double basis(const epsgrad_config_t &c, double dx, double dy)
+{
+    if (c.filter_kind == EPSGRAD_FILTER_CONIC) {                   // S1: max(0, 1 - r/R)
+        const double w = 1.0 - std::sqrt(dx * dx + dy * dy) / c.filter_radius;
+        return w > 0.0 ? w : 0.0;
+    }
+    if (std::fabs(dx) > c.filter_radius || std::fabs(dy) > c.filter_radius) return 0.0;   // S11
+    return std::exp(-(dx * dx + dy * dy) / (2.0 * c.filter_sigma * c.filter_sigma));
+}
+
+static double basis1(const epsgrad_config_t &c, double d)       // separable factor (Gaussian only)
+{
+    if (std::fabs(d) > c.filter_radius) return 0.0;
+    return std::exp(-d * d / (2.0 * c.filter_sigma * c.filter_sigma));
+}
+
+// representative control index of border class k (inverse of border_class)
+static int class_rep(int k, int M, int T, int K)
+{
+    if (K == M) return k;
+    return k <= T ? k : M - 1 - (2 * T - k);
+}
+
+static double overlap(double a0, double a1, double b0, double b1)
+{
+    const double lo = a0 > b0 ? a0 : b0, hi = a1 < b1 ? a1 : b1;
+    return hi > lo ? hi - lo : 0.0;
+}
+
+static int validate(const epsgrad_config_t *c)
+{
+    if (!c) return EPSGRAD_EINVAL;
+    if (c->batch < 1 || c->mx < 1 || c->my < 1 || c->upsample < 1 || c->nz < 1) return EPSGRAD_EINVAL;
+    if (c->subpixel < 2 || (c->subpixel & 1)) return EPSGRAD_EINVAL;
+    if (!(c->z_hi > c->z_lo)) return EPSGRAD_EINVAL;
+    if (!(c->filter_radius > 0.0)) return EPSGRAD_EINVAL;
+    if (c->filter_kind != EPSGRAD_FILTER_CONIC && c->filter_kind != EPSGRAD_FILTER_GAUSSIAN) return EPSGRAD_EINVAL;
+    if (c->filter_kind == EPSGRAD_FILTER_GAUSSIAN && !(c->filter_sigma > 0.0)) return EPSGRAD_EINVAL;
+    if (!(c->eps_core > 0.0) || !(c->eps_clad > 0.0) || c->eps_core == c->eps_clad) return EPSGRAD_EINVAL;
+    if (!(c->normal_delta >= 0.0)) return EPSGRAD_EINVAL;
+    const int m = c->upsample * c->subpixel;
+    if (m != 2 && m != 4 && m != 6 && m != 8) return EPSGRAD_EUNSUPPORTED;
+    if (c->nz % 4) return EPSGRAD_EUNSUPPORTED;
+    const double cells = (double)c->batch * 3.0 * c->upsample * c->mx * c->upsample * c->my;
+    if (cells * c->subpixel * c->subpixel > 2.0e9) return EPSGRAD_EUNSUPPORTED;   // 32-bit plane indices
+    return EPSGRAD_OK;
+}
+
+// ------------------------------------------------------------------------------------ plan
+extern "C" int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsgrad_plan_t **out)
+{
+    if (!out) return EPSGRAD_EINVAL;
+    int rc = validate(cfg);
+    if (rc) return rc;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
+        cudaGetLastError();
+        return EPSGRAD_ECUDA;
+    }
+    epsgrad_plan *P = new (std::nothrow) epsgrad_plan();
+    if (!P) return EPSGRAD_ENOMEM;
+    std::memset(P, 0, sizeof(*P));
+    P->cfg = *cfg;
+    P->device = device;
+    const int u = cfg->upsample, s = cfg->subpixel, m = u * s;
+    P->m = m;
+    P->nx = u * cfg->mx; P->ny = u * cfg->my;
+    P->px = s * P->nx;   P->py = s * P->ny;
+    P->separable = cfg->filter_kind == EPSGRAD_FILTER_GAUSSIAN;
+    // taps: X_p - x_a = delta_f - u t, |delta_f| < u/2  =>  |t| <= floor((R + u/2)/u)
+    const int T = (int)std::floor((cfg->filter_radius + 0.5 * u) / u);
+    const int NT = 2 * T + 1;
+    P->T = T; P->NT = NT;
+    P->KX = cfg->mx >= NT ? NT : cfg->mx;
+    P->KY = cfg->my >= NT ? NT : cfg->my;
+    P->eta0 = cfg->filter_normalize ? (float)cfg->eta : 0.0f;
+    P->eta_r = (float)(cfg->eta - (double)P->eta0);
+    P->eps_clad = (float)cfg->eps_clad;
+    P->deps = (float)(cfg->eps_core - cfg->eps_clad);
+    P->delta = (float)cfg->normal_delta;
+
+    // ---- filter tables (float64 on the host, rounded once to fp32)
+    std::vector<double> d1(m);                       // delta_f = (f + 1/2)/s - u/2
+    for (int f = 0; f < m; ++f) d1[f] = (f + 0.5) / s - 0.5 * u;
+    std::vector<float> w;
+    std::vector<int> tyr(2 * NT, 0);
+    std::vector<float> invden;
+    if (!P->separable) {
+        w.assign((size_t)NT * NT * m * m, 0.0f);
+        for (int tx = 0; tx < NT; ++tx) {
+            int lo = NT, hi = -1;
+            for (int ty = 0; ty < NT; ++ty) {
+                bool any = false;
+                for (int fx = 0; fx < m; ++fx)
+                    for (int fy = 0; fy < m; ++fy) {
+                        const double v = basis(*cfg, d1[fx] - (double)u * (tx - T), d1[fy] - (double)u * (ty - T));
+                        w[(((size_t)tx * NT + ty) * m + fx) * m + fy] = (float)v;
+                        any |= v != 0.0;
+                    }
+                if (any) { if (ty < lo) lo = ty; hi = ty; }
+            }
+            tyr[2 * tx] = lo; tyr[2 * tx + 1] = hi;   // empty row: lo > hi
+        }
+        const int RX = P->KX * m, RY = P->KY * m;
+        invden.assign((size_t)RX * RY, 1.0f);
+        if (cfg->filter_normalize)
+            for (int kx = 0; kx < P->KX; ++kx)
+                for (int ky = 0; ky < P->KY; ++ky) {
+                    const int a0 = class_rep(kx, cfg->mx, T, P->KX), b0 = class_rep(ky, cfg->my, T, P->KY);
+                    for (int fx = 0; fx < m; ++fx)
+                        for (int fy = 0; fy < m; ++fy) {
+                            double den = 0.0;
+                            for (int tx = 0; tx < NT; ++tx) {
+                                const int a = a0 + tx - T;
+                                if (a < 0 || a >= cfg->mx) continue;
+                                for (int ty = 0; ty < NT; ++ty) {
+                                    const int b = b0 + ty - T;
+                                    if (b < 0 || b >= cfg->my) continue;
+                                    den += (double)w[(((size_t)tx * NT + ty) * m + fx) * m + fy];
+                                }
+                            }
+                            invden[(size_t)(kx * m + fx) * RY + ky * m + fy] = (float)(1.0 / den);
+                        }
+                }
+    } else {
+        w.assign((size_t)NT * m, 0.0f);
+        for (int t = 0; t < NT; ++t)
+            for (int f = 0; f < m; ++f) w[(size_t)t * m + f] = (float)basis1(*cfg, d1[f] - (double)u * (t - T));
+        const int RX = P->KX * m, RY = P->KY * m;
+        invden.assign((size_t)RX + RY, 1.0f);
+        if (cfg->filter_normalize)
+            for (int ax = 0; ax < 2; ++ax) {
+                const int K = ax ? P->KY : P->KX, M = ax ? cfg->my : cfg->mx;
+                for (int k = 0; k < K; ++k) {
+                    const int a0 = class_rep(k, M, T, K);
+                    for (int f = 0; f < m; ++f) {
+                        double den = 0.0;
+                        for (int t = 0; t < NT; ++t) {
+                            const int a = a0 + t - T;
+                            if (a >= 0 && a < M) den += (double)w[(size_t)t * m + f];
+                        }
+                        invden[(ax ? RX : 0) + k * m + f] = (float)(1.0 / den);
+                    }
+                }
+            }
+    }
+
+    // ---- z tables (S7, S8): wxy_k = |[k,k+1] ^ slab|, wz_k = |[k+1/2,k+3/2] ^ slab|
+    const int nz = cfg->nz;
+    std::vector<float> zw((size_t)5 * nz, 0.0f);
+    int kmin[2] = {nz, nz}, kmax[2] = {-1, -1};
+    int n_face = 0;
+    for (int k = 0; k < nz; ++k) {
+        const double wxy = overlap(k, k + 1.0, cfg->z_lo, cfg->z_hi);
+        const double wz = overlap(k + 0.5, k + 1.5, cfg->z_lo, cfg->z_hi);
+        zw[k] = (float)wxy;
+        zw[nz + k] = (float)wz;
+        if (wxy > 0.0) { if (k < kmin[0]) kmin[0] = k; kmax[0] = k; }
+        if (wz > 0.0) {
+            if (k < kmin[1]) kmin[1] = k;
+            kmax[1] = k;
+            if ((float)wz == 1.0f) zw[2 * nz + k] = 1.0f;
+            else if (n_face == 0) { zw[3 * nz + k] = 1.0f; P->w_lo = (float)wz; ++n_face; }
+            else if (n_face == 1) { zw[4 * nz + k] = 1.0f; P->w_hi = (float)wz; ++n_face; }
+            else { delete P; return EPSGRAD_EINVAL; }   // cannot happen for an interval slab
+        }
+    }
+    for (int g = 0; g < 2; ++g) {
+        if (kmax[g] < 0) { P->ch0[g] = 0; P->nch[g] = 0; }
+        else { P->ch0[g] = kmin[g] / 2; P->nch[g] = kmax[g] / 2 - P->ch0[g] + 1; }
+    }
+
+    // ---- tile choice of the transposed conic filter by shared memory
+    P->conic_tile = 16;
+    if (!P->separable) {
+        auto need = [&](int t) { return ((size_t)NT * NT * m * m + (size_t)m * (t + 2 * T) * m * (t + 2 * T) + 2 * NT) * 4; };
+        if (need(16) > 200 * 1024) P->conic_tile = 8;
+        if (need(P->conic_tile) > 200 * 1024) { delete P; return EPSGRAD_EUNSUPPORTED; }
+    }
+    if (fwd_smem_floats(s, nz) * 4 > 200 * 1024 || rev_smem_floats(s) * 4 > 200 * 1024) { delete P; return EPSGRAD_EUNSUPPORTED; }
+
+    // ---- upload
+    int prev = 0;
+    cudaGetDevice(&prev);
+    cudaSetDevice(device);
+    const size_t b_w = align_up(w.size() * 4, 256), b_ty = align_up(tyr.size() * 4, 256);
+    const size_t b_id = align_up(invden.size() * 4, 256), b_zw = align_up(zw.size() * 4, 256);
+    cudaError_t ce = cudaMalloc(&P->d_tables, b_w + b_ty + b_id + b_zw);
+    if (ce == cudaSuccess) {
+        char *base = (char *)P->d_tables;
+        P->d_w = (float *)base;
+        P->d_tyrange = (int *)(base + b_w);
+        P->d_invden = (float *)(base + b_w + b_ty);
+        P->d_zw = (float *)(base + b_w + b_ty + b_id);
+        ce = cudaMemcpy(P->d_w, w.data(), w.size() * 4, cudaMemcpyHostToDevice);
+        if (ce == cudaSuccess) ce = cudaMemcpy(P->d_tyrange, tyr.data(), tyr.size() * 4, cudaMemcpyHostToDevice);
+        if (ce == cudaSuccess) ce = cudaMemcpy(P->d_invden, invden.data(), invden.size() * 4, cudaMemcpyHostToDevice);
+        if (ce == cudaSuccess) ce = cudaMemcpy(P->d_zw, zw.data(), zw.size() * 4, cudaMemcpyHostToDevice);
+    }
+    cudaSetDevice(prev);
+    if (ce != cudaSuccess) {
+        cudaGetLastError();
+        if (P->d_tables) cudaFree(P->d_tables);
+        delete P;
+        return EPSGRAD_ECUDA;
+    }
+
+    // ---- workspace carve-up
+    const size_t n_mask = (size_t)cfg->batch * P->px * P->py, n_cell = (size_t)cfg->batch * P->nx * P->ny;
+    size_t off = 0;
+    P->off_phi = off;  off += align_up(n_mask * 4, 256);
+    P->off_v = off;    off += align_up(n_mask * 4, 256);
+    P->off_gbar = off; off += align_up(n_cell * 5 * 4, 256);
+    P->off_tmp = off;  off += P->separable ? align_up((size_t)cfg->batch * cfg->mx * P->py * 4, 256) : 0;
+    P->ws_need = off;
+    *out = P;
+    return EPSGRAD_OK;
+}
+
+extern "C" int epsgrad_plan_destroy(epsgrad_plan_t *P)
+{
+    if (!P) return EPSGRAD_EINVAL;
+    if (P->d_tables) cudaFree(P->d_tables);
+    delete P;
+    return EPSGRAD_OK;
+}
+
+extern "C" size_t epsgrad_workspace_bytes(const epsgrad_plan_t *P) { return P ? P->ws_need : 0; }
+
+extern "C" int epsgrad_plan_set_workspace(epsgrad_plan_t *P, void *p, size_t bytes)
+{
+    if (!P || !p || ((uintptr_t)p & 255)) return EPSGRAD_EINVAL;
+    if (bytes < P->ws_need) return EPSGRAD_ENOWORKSPACE;
+    P->ws = p; P->ws_bytes = bytes;
+    return EPSGRAD_OK;
+}
+
+static size_t n_eps(const epsgrad_plan_t *P) { return (size_t)P->cfg.batch * 3 * P->nx * P->ny * P->cfg.nz; }
+static size_t n_ctrl(const epsgrad_plan_t *P) { return (size_t)P->cfg.batch * P->cfg.mx * P->cfg.my; }
+
+extern "C" size_t epsgrad_staging_bytes(const epsgrad_plan_t *P, int n_pairs)
+{
+    if (!P || n_pairs < 0) return 0;
+    return 2 * align_up(n_ctrl(P) * 4, 256) + align_up(n_eps(P) * 4, 256) + (size_t)2 * n_pairs * align_up(n_eps(P) * 8, 256);
+}
+
+extern "C" int epsgrad_plan_set_staging(epsgrad_plan_t *P, void *p, size_t bytes)
+{
+    if (!P || !p || ((uintptr_t)p & 255)) return EPSGRAD_EINVAL;
+    P->stg = p; P->stg_bytes = bytes;
+    return EPSGRAD_OK;
+}
+
+extern "C" int epsgrad_plan_set_dense_reads(epsgrad_plan_t *P, int dense)
+{
+    if (!P) return EPSGRAD_EINVAL;
+    P->dense = dense != 0;
+    return EPSGRAD_OK;
+}
+
+extern "C" int epsgrad_plan_last_launches(const epsgrad_plan_t *P) { return P ? P->last_launches : 0; }
+
+extern "C" int epsgrad_plan_last_copy_bytes(const epsgrad_plan_t *P, uint64_t *h2d, uint64_t *d2h)
+{
+    if (!P) return EPSGRAD_EINVAL;
+    if (h2d) *h2d = P->last_h2d;
+    if (d2h) *d2h = P->last_d2h;
+    return EPSGRAD_OK;
+}
+
+extern "C" const char *epsgrad_status_string(int st)
+{
+    switch (st) {
+    case EPSGRAD_OK: return "ok";
+    case EPSGRAD_EINVAL: return "invalid argument";
+    case EPSGRAD_EUNSUPPORTED: return "unsupported configuration";
+    case EPSGRAD_ENOWORKSPACE: return "workspace or staging buffer missing or too small";
+    case EPSGRAD_ECUDA: return "CUDA runtime error";
+    case EPSGRAD_ENOMEM: return "host allocation failed";
+    default: return "unknown status";
+    }
+}
+
+extern "C" int epsgrad_version(void) { return EPSGRAD_VERSION; }
+
+// ------------------------------------------------------------------------------------ launches
+namespace {
+
+inline int cdiv(int a, int b) { return (a + b - 1) / b; }
+
+template <typename K>
+int set_smem(K kernel, size_t bytes)
+{
+    if (bytes > 48 * 1024 &&
+        cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess) {
+        cudaGetLastError();
+        return EPSGRAD_ECUDA;
+    }
+    return EPSGRAD_OK;
+}
+
+int check_launch(epsgrad_plan *P)
+{
+    ++P->last_launches;
+    return cudaGetLastError() == cudaSuccess ? EPSGRAD_OK : EPSGRAD_ECUDA;
+}
+
+Normaliser make_nrm(const epsgrad_plan *P)
+{
+    Normaliser n;
+    n.tab = P->d_invden; n.mx = P->cfg.mx; n.my = P->cfg.my; n.m = P->m; n.T = P->T;
+    n.KX = P->KX; n.KY = P->KY; n.separable = P->separable;
+    return n;
+}
+
+float *ws_phi(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_phi); }
+float *ws_v(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_v); }
+float *ws_gbar(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_gbar); }
+float *ws_tmp(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_tmp); }
+
+// ---- F1: C -> centred Phi on the mask
+template <int M>
+int launch_filter_m(epsgrad_plan *P, const float *C, float *phi, cudaStream_t st)
+{
+    const int B = P->cfg.batch, mx = P->cfg.mx, my = P->cfg.my, T = P->T, NT = P->NT;
+    if (!P->separable) {
+        constexpr int TA = 16, TB = 16;
+        FilterParams fp;
+        fp.C = C; fp.phi = phi; fp.w = P->d_w; fp.tyrange = P->d_tyrange; fp.nrm = make_nrm(P);
+        fp.mx = mx; fp.my = my; fp.px = P->px; fp.py = P->py; fp.T = T; fp.NT = NT; fp.eta0 = P->eta0;
+        const size_t smem = ((size_t)NT * NT * M * M + (size_t)(TA + 2 * T) * (TB + 2 * T + 1) + 2 * NT) * 4;
+        if (smem > 200 * 1024) return EPSGRAD_EUNSUPPORTED;
+        int rc = set_smem(k_filter_conic<M, TA, TB>, smem);
+        if (rc) return rc;
+        k_filter_conic<M, TA, TB><<<dim3(cdiv(my, TB), cdiv(mx, TA), B), TA * TB, smem, st>>>(fp);
+        return check_launch(P);
+    }
+    SepParams sp;
+    sp.w1 = P->d_w; sp.nrm = make_nrm(P);
+    sp.mx = mx; sp.my = my; sp.px = P->px; sp.py = P->py; sp.T = T; sp.NT = NT; sp.eta0 = P->eta0;
+    {
+        sp.in = C; sp.out = ws_tmp(P);
+        const size_t smem = ((size_t)NT * M + (size_t)8 * (32 + 2 * T)) * 4;
+        int rc = set_smem(k_sep_up_y<M>, smem);
+        if (rc) return rc;
+        k_sep_up_y<M><<<dim3(cdiv(my, 32), cdiv(mx, 8), B), SEP_THREADS, smem, st>>>(sp);
+        if ((rc = check_launch(P))) return rc;
+    }
+    {
+        sp.in = ws_tmp(P); sp.out = phi;
+        const size_t smem = ((size_t)NT * M + (size_t)(8 + 2 * T) * 128) * 4;
+        if (smem > 200 * 1024) return EPSGRAD_EUNSUPPORTED;
+        int rc = set_smem(k_sep_up_x<M>, smem);
+        if (rc) return rc;
+        k_sep_up_x<M><<<dim3(cdiv(P->py, 128), cdiv(mx, 8), B), SEP_THREADS, smem, st>>>(sp);
+        return check_launch(P);
+    }
+}
+
+// ---- R6: mask cotangent v -> dF/dC
+template <int M, int TT>
+int launch_filterT_conic(epsgrad_plan *P, const float *v, float *dC, cudaStream_t st)
+{
+    const int T = P->T, NT = P->NT;
+    FilterTParams fp;
+    fp.v = v; fp.dC = dC; fp.w = P->d_w; fp.tyrange = P->d_tyrange;
+    fp.mx = P->cfg.mx; fp.my = P->cfg.my; fp.px = P->px; fp.py = P->py; fp.T = T; fp.NT = NT;
+    const size_t smem = ((size_t)NT * NT * M * M + (size_t)M * (TT + 2 * T) * M * (TT + 2 * T) + 2 * NT) * 4;
+    int rc = set_smem(k_filterT_conic<M, TT, TT>, smem);
+    if (rc) return rc;
+    k_filterT_conic<M, TT, TT><<<dim3(cdiv(fp.my, TT), cdiv(fp.mx, TT), P->cfg.batch), TT * TT, smem, st>>>(fp);
+    return check_launch(P);
+}
+
+template <int M>
+int launch_filterT_m(epsgrad_plan *P, const float *v, float *dC, cudaStream_t st)
+{
+    if (!P->separable)
+        return P->conic_tile == 16 ? launch_filterT_conic<M, 16>(P, v, dC, st) : launch_filterT_conic<M, 8>(P, v, dC, st);
+    const int B = P->cfg.batch, mx = P->cfg.mx, my = P->cfg.my, T = P->T, NT = P->NT;
+    SepParams sp;
+    sp.w1 = P->d_w; sp.nrm = make_nrm(P);
+    sp.mx = mx; sp.my = my; sp.px = P->px; sp.py = P->py; sp.T = T; sp.NT = NT; sp.eta0 = 0.0f;
+    {
+        sp.in = v; sp.out = ws_tmp(P);
+        const size_t smem = ((size_t)NT * M + (size_t)M * (8 + 2 * T) * 64) * 4;
+        if (smem > 200 * 1024) return EPSGRAD_EUNSUPPORTED;
+        int rc = set_smem(k_sep_down_x<M>, smem);
+        if (rc) return rc;
+        k_sep_down_x<M><<<dim3(cdiv(P->py, 64), cdiv(mx, 8), B), SEP_THREADS, smem, st>>>(sp);
+        if ((rc = check_launch(P))) return rc;
+    }
+    {
+        sp.in = ws_tmp(P); sp.out = dC;
+        const size_t smem = ((size_t)NT * M + (size_t)8 * M * (32 + 2 * T)) * 4;
+        if (smem > 200 * 1024) return EPSGRAD_EUNSUPPORTED;
+        int rc = set_smem(k_sep_down_y<M>, smem);
+        if (rc) return rc;
+        k_sep_down_y<M><<<dim3(cdiv(my, 32), cdiv(mx, 8), B), SEP_THREADS, smem, st>>>(sp);
+        return check_launch(P);
+    }
+}
+
+int launch_filter(epsgrad_plan *P, const float *C, float *phi, cudaStream_t st)
+{
+    switch (P->m) {
+    case 2: return launch_filter_m<2>(P, C, phi, st);
+    case 4: return launch_filter_m<4>(P, C, phi, st);
+    case 6: return launch_filter_m<6>(P, C, phi, st);
+    case 8: return launch_filter_m<8>(P, C, phi, st);
+    }
+    return EPSGRAD_EUNSUPPORTED;
+}
+
+int launch_filterT(epsgrad_plan *P, const float *v, float *dC, cudaStream_t st)
+{
+    switch (P->m) {
+    case 2: return launch_filterT_m<2>(P, v, dC, st);
+    case 4: return launch_filterT_m<4>(P, v, dC, st);
+    case 6: return launch_filterT_m<6>(P, v, dC, st);
+    case 8: return launch_filterT_m<8>(P, v, dC, st);
+    }
+    return EPSGRAD_EUNSUPPORTED;
+}
+
+// ---- F2..F6
+int launch_forward(epsgrad_plan *P, const float *phi, float beta, float *eps, float *eps2d, cudaStream_t st)
+{
+    FwdParams fp;
+    fp.phi = phi; fp.eps = eps; fp.eps2d = eps2d; fp.zw = P->d_zw;
+    fp.nx = P->nx; fp.ny = P->ny; fp.nz = P->cfg.nz; fp.px = P->px; fp.py = P->py; fp.s = P->cfg.subpixel;
+    fp.beta = beta; fp.eta_r = P->eta_r; fp.eps_clad = P->eps_clad; fp.deps = P->deps; fp.delta = P->delta;
+    const size_t smem = fwd_smem_floats(fp.s, fp.nz) * 4;
+    int rc = set_smem(k_forward, smem);
+    if (rc) return rc;
+    k_forward<<<dim3(cdiv(P->ny, FWD_TJ), cdiv(P->nx, FWD_TI), P->cfg.batch), FWD_THREADS, smem, st>>>(fp);
+    return check_launch(P);
+}
+
+// ---- R1
+int next_pow2(int x) { int p = 1; while (p < x) p <<= 1; return p; }
+
+int launch_zreduce(epsgrad_plan *P, int n_pairs, const void *const *EF, const void *const *EA, float *gbar, cudaStream_t st)
+{
+    ZredParams zp;
+    zp.gbar = gbar; zp.zw = P->d_zw; zp.ncol = P->nx * P->ny; zp.nz = P->cfg.nz;
+    int maxblocks = 1;
+    for (int g = 0; g < 2; ++g) {
+        zp.ch0[g] = P->dense ? 0 : P->ch0[g];
+        zp.nch[g] = P->dense ? P->cfg.nz / 2 : P->nch[g];
+        int L = next_pow2(zp.nch[g] < 1 ? 1 : zp.nch[g]);
+        if (L > 32) L = 32;
+        zp.L[g] = L;
+        const int cols_per_block = (ZR_THREADS / L) * ZR_UNROLL;
+        const int nb = cdiv(zp.ncol, cols_per_block);
+        if (nb > maxblocks) maxblocks = nb;
+    }
+    for (int p0 = 0; p0 < n_pairs; p0 += ZR_MAX_PAIRS) {
+        const int np = n_pairs - p0 < ZR_MAX_PAIRS ? n_pairs - p0 : ZR_MAX_PAIRS;
+        for (int p = 0; p < ZR_MAX_PAIRS; ++p) {
+            zp.ef[p] = (const float4 *)(p < np ? EF[p0 + p] : nullptr);
+            zp.ea[p] = (const float4 *)(p < np ? EA[p0 + p] : nullptr);
+        }
+        zp.n_pairs = np; zp.accumulate = p0 > 0;
+        k_zreduce<<<dim3(maxblocks, 3 * P->cfg.batch), ZR_THREADS, 0, st>>>(zp);
+        int rc = check_launch(P);
+        if (rc) return rc;
+    }
+    return EPSGRAD_OK;
+}
+
+// ---- R2..R5
+int launch_reverse2d(epsgrad_plan *P, const float *phi, float beta, const float *gbar, float *v, cudaStream_t st)
+{
+    Rev2dParams rp;
+    rp.phi = phi; rp.gbar = gbar; rp.v = v; rp.nrm = make_nrm(P);
+    rp.nx = P->nx; rp.ny = P->ny; rp.px = P->px; rp.py = P->py; rp.s = P->cfg.subpixel;
+    rp.beta = beta; rp.eta_r = P->eta_r; rp.eps_clad = P->eps_clad; rp.deps = P->deps; rp.delta = P->delta;
+    rp.w_lo = P->w_lo; rp.w_hi = P->w_hi;
+    const size_t smem = rev_smem_floats(rp.s) * 4;
+    int rc = set_smem(k_reverse2d, smem);
+    if (rc) return rc;
+    k_reverse2d<<<dim3(cdiv(P->ny, REV_TJ), cdiv(P->nx, REV_TI), P->cfg.batch), REV_THREADS, smem, st>>>(rp);
+    return check_launch(P);
+}
+
+bool aligned16(const void *p) { return p && !((uintptr_t)p & 15); }
+
+int check_common(epsgrad_plan *P, const float *C, float beta)
+{
+    if (!P || !aligned16(C) || !(beta > 0.0f) || !std::isfinite(beta)) return EPSGRAD_EINVAL;
+    if (!P->ws) return EPSGRAD_ENOWORKSPACE;
+    return EPSGRAD_OK;
+}
+
+int check_pairs(int n_pairs, const void *const *EF, const void *const *EA)
+{
+    if (n_pairs < 1 || !EF || !EA) return EPSGRAD_EINVAL;
+    for (int p = 0; p < n_pairs; ++p)
+        if (!aligned16(EF[p]) || !aligned16(EA[p])) return EPSGRAD_EINVAL;
+    return EPSGRAD_OK;
+}
+
+struct DeviceGuard {
+    int prev;
+    explicit DeviceGuard(int dev) { cudaGetDevice(&prev); if (prev != dev) cudaSetDevice(dev); else prev = -1; }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+int run_vjp(epsgrad_plan *P, float beta, int n_pairs, const void *const *EF, const void *const *EA,
+            float *dFdC, cudaStream_t st)
+{
+    int rc = launch_zreduce(P, n_pairs, EF, EA, ws_gbar(P), st);
+    if (!rc) rc = launch_reverse2d(P, ws_phi(P), beta, ws_gbar(P), ws_v(P), st);
+    if (!rc) rc = launch_filterT(P, ws_v(P), dFdC, st);
+    return rc;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------ hot path
+extern "C" int eps_forward(epsgrad_plan_t *P, const float *C, float beta, float *eps, void *stream)
+{
+    int rc = check_common(P, C, beta);
+    if (rc) return rc;
+    if (!aligned16(eps)) return EPSGRAD_EINVAL;
+    DeviceGuard g(P->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    P->last_launches = 0;
+    rc = launch_filter(P, C, ws_phi(P), st);
+    if (!rc) rc = launch_forward(P, ws_phi(P), beta, eps, nullptr, st);
+    return rc;
+}
+
+extern "C" int eps_vjp(epsgrad_plan_t *P, const float *C, float beta, int n_pairs,
+                       const void *const *EF, const void *const *EA, float *dFdC, void *stream)
+{
+    int rc = check_common(P, C, beta);
+    if (!rc) rc = check_pairs(n_pairs, EF, EA);
+    if (rc) return rc;
+    if (!aligned16(dFdC)) return EPSGRAD_EINVAL;
+    DeviceGuard g(P->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    P->last_launches = 0;
+    rc = launch_filter(P, C, ws_phi(P), st);
+    if (!rc) rc = run_vjp(P, beta, n_pairs, EF, EA, dFdC, st);
+    return rc;
+}
+
+extern "C" int eps_forward_vjp(epsgrad_plan_t *P, const float *C, float beta, int n_pairs,
+                               const void *const *EF, const void *const *EA,
+                               float *eps, float *dFdC, void *stream)
+{
+    int rc = check_common(P, C, beta);
+    if (!rc) rc = check_pairs(n_pairs, EF, EA);
+    if (rc) return rc;
+    if (!aligned16(eps) || !aligned16(dFdC)) return EPSGRAD_EINVAL;
+    DeviceGuard g(P->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    P->last_launches = 0;
+    rc = launch_filter(P, C, ws_phi(P), st);
+    if (!rc) rc = launch_forward(P, ws_phi(P), beta, eps, nullptr, st);
+    if (!rc) rc = run_vjp(P, beta, n_pairs, EF, EA, dFdC, st);
+    return rc;
+}
+
+// ------------------------------------------------------------------------------------ host buffers
+extern "C" int eps_forward_vjp_host(epsgrad_plan_t *P, const float *C_host, float beta, int n_pairs,
+                                    const void *const *EF_host, const void *const *EA_host,
+                                    float *eps_host, float *dFdC_host, void *stream)
+{
+    if (!P || !C_host || !(beta > 0.0f) || !std::isfinite(beta)) return EPSGRAD_EINVAL;
+    if (!eps_host && !dFdC_host) return EPSGRAD_EINVAL;
+    if (dFdC_host) {
+        if (n_pairs < 1 || !EF_host || !EA_host) return EPSGRAD_EINVAL;
+        for (int p = 0; p < n_pairs; ++p)
+            if (!EF_host[p] || !EA_host[p]) return EPSGRAD_EINVAL;
+    } else {
+        n_pairs = 0;
+    }
+    if (!P->ws) return EPSGRAD_ENOWORKSPACE;
+    if (!P->stg || P->stg_bytes < epsgrad_staging_bytes(P, n_pairs)) return EPSGRAD_ENOWORKSPACE;
+    DeviceGuard g(P->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    P->last_launches = 0;
+    P->last_h2d = P->last_d2h = 0;
+
+    const size_t b_c = n_ctrl(P) * 4, b_e = n_eps(P) * 4, b_f = n_eps(P) * 8;
+    char *base = (char *)P->stg;
+    float *dC = (float *)base;              base += align_up(b_c, 256);
+    float *dG = (float *)base;              base += align_up(b_c, 256);
+    float *dE = (float *)base;              base += align_up(b_e, 256);
+    std::vector<const void *> ef(n_pairs), ea(n_pairs);
+    bool ok = cudaMemcpyAsync(dC, C_host, b_c, cudaMemcpyHostToDevice, st) == cudaSuccess;
+    P->last_h2d += b_c;
+    for (int p = 0; p < n_pairs && ok; ++p) {
+        ef[p] = base; base += align_up(b_f, 256);
+        ea[p] = base; base += align_up(b_f, 256);
+        ok = cudaMemcpyAsync((void *)ef[p], EF_host[p], b_f, cudaMemcpyHostToDevice, st) == cudaSuccess &&
+             cudaMemcpyAsync((void *)ea[p], EA_host[p], b_f, cudaMemcpyHostToDevice, st) == cudaSuccess;
+        P->last_h2d += 2 * b_f;
+    }
+    if (!ok) { cudaGetLastError(); return EPSGRAD_ECUDA; }
+    int rc = launch_filter(P, dC, ws_phi(P), st);
+    if (!rc && eps_host) rc = launch_forward(P, ws_phi(P), beta, dE, nullptr, st);
+    if (!rc && dFdC_host) rc = run_vjp(P, beta, n_pairs, ef.data(), ea.data(), dG, st);
+    if (rc) return rc;
+    if (eps_host) {
+        ok = ok && cudaMemcpyAsync(eps_host, dE, b_e, cudaMemcpyDeviceToHost, st) == cudaSuccess;
+        P->last_d2h += b_e;
+    }
+    if (dFdC_host) {
+        ok = ok && cudaMemcpyAsync(dFdC_host, dG, b_c, cudaMemcpyDeviceToHost, st) == cudaSuccess;
+        P->last_d2h += b_c;
+    }
+    if (!ok) { cudaGetLastError(); return EPSGRAD_ECUDA; }
+    return EPSGRAD_OK;
+}
+
+// ------------------------------------------------------------------------------------ stage taps
+extern "C" int epsgrad_stage_filter(epsgrad_plan_t *P, const float *C, float *phi_centred, void *stream)
+{
+    int rc = check_common(P, C, 1.0f);
+    if (rc) return rc;
+    if (!aligned16(phi_centred)) return EPSGRAD_EINVAL;
+    DeviceGuard g(P->device);
+    P->last_launches = 0;
+    return launch_filter(P, C, phi_centred, (cudaStream_t)stream);
+}
+
+extern "C" int epsgrad_stage_eps2d(epsgrad_plan_t *P, const float *C, float beta, float *eps2d, void *stream)
+{
+    int rc = check_common(P, C, beta);
+    if (rc) return rc;
+    if (!aligned16(eps2d)) return EPSGRAD_EINVAL;
+    DeviceGuard g(P->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    P->last_launches = 0;
+    rc = launch_filter(P, C, ws_phi(P), st);
+    if (!rc) rc = launch_forward(P, ws_phi(P), beta, nullptr, eps2d, st);
+    return rc;
+}
+
+extern "C" int epsgrad_stage_zreduce(epsgrad_plan_t *P, int n_pairs, const void *const *EF,
+                                     const void *const *EA, float *gbar, void *stream)
+{
+    if (!P) return EPSGRAD_EINVAL;
+    int rc = check_pairs(n_pairs, EF, EA);
+    if (rc) return rc;
+    if (!aligned16(gbar)) return EPSGRAD_EINVAL;
+    DeviceGuard g(P->device);
+    P->last_launches = 0;
+    return launch_zreduce(P, n_pairs, EF, EA, gbar, (cudaStream_t)stream);
+}

@@ -1,0 +1,70 @@
+"""Shared pieces of the GPU parity tests: run the CUDA path (through the C ABI binding) and
+the float64 oracle on the same seeded inputs and compare.  Tolerances are BASELINE.json's:
+relative 1e-5 on eps (element-wise; eps >= eps_clad > 0) and 1e-4 on dF/dC (S14: max-norm
+and 2-norm relative error; element-wise is meaningless at sign changes)."""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+import oracle as O
+from helpers import rel_inf, rel_l2
+from paper_2505_03352_b200 import binding as B
+
+TOL_EPS = 1e-5
+TOL_GRAD = 1e-4
+
+
+def oracle_cfg(cfg: B.Config) -> O.OracleConfig:
+    return O.OracleConfig(mx=cfg.mx, my=cfg.my, nx=cfg.nx, ny=cfg.ny, nz=cfg.nz, z_lo=cfg.z_lo, z_hi=cfg.z_hi,
+                          s=cfg.subpixel, filter_kind=cfg.filter_kind, radius=cfg.filter_radius,
+                          sigma=cfg.filter_sigma, normalize=cfg.filter_normalize, eta=cfg.eta,
+                          eps_core=cfg.eps_core, eps_clad=cfg.eps_clad, delta=cfg.normal_delta)
+
+
+def rand_C(cfg: B.Config, seed: int) -> np.ndarray:
+    return np.random.default_rng(seed).random((cfg.batch, cfg.mx, cfg.my), dtype=np.float32)
+
+
+def rand_fields(cfg: B.Config, n_pairs: int, seed: int):
+    """n_pairs x (E_F, E_A), complex64 [B,3,nx,ny,nz], i.i.d. N(0,1) re and im."""
+    rng = np.random.default_rng([seed, 7])
+    shape = (cfg.batch, 3, cfg.nx, cfg.ny, cfg.nz)
+
+    def one():
+        a = np.empty(shape, np.complex64)
+        rng.standard_normal(out=a.view(np.float32).reshape(-1), dtype=np.float32)
+        return a
+    return [one() for _ in range(n_pairs)], [one() for _ in range(n_pairs)]
+
+
+def dev(a: np.ndarray) -> torch.Tensor:
+    return torch.from_numpy(a).cuda()
+
+
+def max_rel(a: np.ndarray, ref: np.ndarray) -> float:
+    return float(np.max(np.abs(a - ref) / np.abs(ref)))
+
+
+def check_forward(cfg: B.Config, C: np.ndarray, beta: float, plan: B.Plan | None = None, tol=TOL_EPS):
+    plan = plan or B.Plan(cfg)
+    eps = plan.eps_forward(dev(C), beta).cpu().numpy().astype(np.float64)
+    oc = oracle_cfg(cfg)
+    worst = 0.0
+    for b in range(cfg.batch):
+        ref = O.forward(oc, C[b], beta)
+        worst = max(worst, max_rel(eps[b], ref))
+    assert worst < tol, f"eps max relative error {worst:.3e} >= {tol}"
+    return worst
+
+
+def check_vjp(cfg: B.Config, C: np.ndarray, beta: float, EF, EA, plan: B.Plan | None = None, tol=TOL_GRAD):
+    plan = plan or B.Plan(cfg)
+    g = plan.eps_vjp(dev(C), beta, [dev(f) for f in EF], [dev(f) for f in EA]).cpu().numpy().astype(np.float64)
+    oc = oracle_cfg(cfg)
+    worst = 0.0
+    for b in range(cfg.batch):
+        ref = O.vjp(oc, C[b], beta, [f[b] for f in EF], [f[b] for f in EA])
+        worst = max(worst, rel_inf(g[b], ref), rel_l2(g[b], ref))
+    assert worst < tol, f"dF/dC relative error {worst:.3e} >= {tol}"
+    return worst

@@ -1,0 +1,171 @@
+"""GPU parity: the CUDA path (through the C ABI) against the float64 oracle, element by
+element on the same seeded inputs.  Small cases span several tiles (16x16 Yee cells per
+CTA) with ragged tails; the BASELINE.json configs follow in test_gpu_configs.py."""
+import numpy as np
+import pytest
+import torch
+
+import oracle as O
+from gpu_common import (TOL_EPS, TOL_GRAD, check_forward, check_vjp, dev, max_rel, oracle_cfg, rand_C,
+                        rand_fields)
+from helpers import rel_inf, rel_l2
+from paper_2505_03352_b200 import binding as B
+
+pytestmark = pytest.mark.gpu
+
+# name -> (config kwargs, beta)
+CASES = {
+    "conic_ragged": (dict(mx=37, my=29, nz=16, z_lo=6.25, z_hi=9.75, filter_radius=4.0), 8.0),
+    "conic_r8_beta64": (dict(mx=41, my=50, nz=64, z_lo=28.25, z_hi=35.75, filter_radius=8.0), 64.0),
+    "conic_fractional_radius": (dict(mx=24, my=33, nz=8, z_lo=2.25, z_hi=5.75, filter_radius=3.3), 12.0),
+    "subpixel4": (dict(mx=19, my=23, nz=8, z_lo=2.25, z_hi=5.75, filter_radius=3.0, subpixel=4), 10.0),
+    "upsample1": (dict(mx=40, my=35, nz=8, z_lo=1.5, z_hi=6.0, filter_radius=2.5, upsample=1), 9.0),
+    "upsample3": (dict(mx=13, my=17, nz=12, z_lo=3.25, z_hi=8.5, filter_radius=5.0, upsample=3), 7.0),
+    "upsample4": (dict(mx=11, my=9, nz=8, z_lo=2.0, z_hi=6.0, filter_radius=6.0, upsample=4), 6.0),
+    "gaussian": (dict(mx=45, my=38, nz=32, z_lo=14.25, z_hi=17.75, filter_kind=1, filter_radius=8.0,
+                      filter_sigma=2.5), 8.0),
+    "gaussian_wide": (dict(mx=70, my=40, nz=8, z_lo=2.25, z_hi=5.75, filter_kind=1, filter_radius=32.0,
+                           filter_sigma=10.0), 8.0),
+    "raw_eq2_eq3": (dict(mx=20, my=22, nz=8, z_lo=2.25, z_hi=5.75, filter_radius=3.0, filter_normalize=0,
+                         eta=0.0), 0.5),
+    "grid_smaller_than_filter": (dict(mx=5, my=7, nz=8, z_lo=2.25, z_hi=5.75, filter_radius=8.0), 8.0),
+    "single_control_row": (dict(mx=1, my=40, nz=8, z_lo=2.25, z_hi=5.75, filter_radius=3.0), 8.0),
+    "thin_slab_in_one_cell": (dict(mx=18, my=18, nz=8, z_lo=3.6, z_hi=3.9, filter_radius=3.0), 8.0),
+    "slab_fills_z": (dict(mx=18, my=18, nz=8, z_lo=0.0, z_hi=8.0, filter_radius=3.0), 8.0),
+    "slab_half_cell_faces": (dict(mx=18, my=18, nz=8, z_lo=2.5, z_hi=5.5, filter_radius=3.0), 8.0),
+    "batch3": (dict(batch=3, mx=21, my=19, nz=8, z_lo=2.25, z_hi=5.75, filter_radius=3.0), 8.0),
+}
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_forward_matches_oracle(name):
+    kw, beta = CASES[name]
+    cfg = B.make_config(**kw)
+    check_forward(cfg, rand_C(cfg, 11), beta)
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_vjp_matches_oracle(name):
+    kw, beta = CASES[name]
+    cfg = B.make_config(**kw)
+    EF, EA = rand_fields(cfg, 1, 5)
+    check_vjp(cfg, rand_C(cfg, 11), beta, EF, EA)
+
+
+@pytest.mark.parametrize("name", ["conic_ragged", "subpixel4", "gaussian", "raw_eq2_eq3", "upsample3"])
+def test_stage_filter_and_eps2d(name):
+    kw, beta = CASES[name]
+    cfg = B.make_config(**kw)
+    C = rand_C(cfg, 3)
+    plan = B.Plan(cfg)
+    oc = oracle_cfg(cfg)
+    phi = plan.stage_filter(dev(C)).cpu().numpy().astype(np.float64)
+    e2 = plan.stage_eps2d(dev(C), beta).cpu().numpy().astype(np.float64)
+    eta0 = cfg.eta if cfg.filter_normalize else 0.0
+    for b in range(cfg.batch):
+        st = O.forward_stages(oc, C[b], beta)
+        # the kernel stores Phi - eta0; fp32 rounding of a sum of <= ~1e3 O(1) terms
+        assert np.max(np.abs(phi[b] - (st["Phi"] - eta0))) < 2e-6 * max(1.0, np.max(np.abs(st["Phi"])))
+        assert max_rel(e2[b], st["eps2d"]) < TOL_EPS
+
+
+@pytest.mark.parametrize("n_pairs", [2, 3, 9])
+def test_pairs_accumulate(n_pairs):
+    # Eq. (1) summed over field pairs (multi-wavelength, BASELINE configs[2]); 9 > EPSGRAD_MAX_PAIRS chains launches
+    cfg = B.make_config(mx=17, my=21, nz=16, z_lo=6.25, z_hi=9.75, filter_radius=4.0)
+    EF, EA = rand_fields(cfg, n_pairs, 21)
+    check_vjp(cfg, rand_C(cfg, 2), 8.0, EF, EA)
+
+
+def test_zreduce_planes_match_definition():
+    cfg = B.make_config(batch=2, mx=9, my=11, nz=16, z_lo=6.25, z_hi=9.75, filter_radius=3.0)
+    EF, EA = rand_fields(cfg, 2, 8)
+    plan = B.Plan(cfg)
+    g = plan.stage_zreduce([dev(f) for f in EF], [dev(f) for f in EA]).cpu().numpy().astype(np.float64)
+    G3 = sum(-2.0 * (f.astype(np.complex128) * a.astype(np.complex128)).real for f, a in zip(EF, EA))
+    wxy, wz = O.zweights(oracle_cfg(cfg))
+    ref = np.stack([G3[:, 0] @ wxy, G3[:, 1] @ wxy, G3[:, 2] @ (wz == 1.0), G3[:, 2, :, :, 5], G3[:, 2, :, :, 9]], axis=1)
+    assert rel_inf(g, ref) < 1e-5
+
+
+def test_dense_reads_give_the_same_gradient():
+    cfg = B.make_config(mx=23, my=18, nz=64, z_lo=28.25, z_hi=35.75, filter_radius=4.0)
+    C = rand_C(cfg, 4)
+    EF, EA = rand_fields(cfg, 1, 9)
+    plan = B.Plan(cfg)
+    check_vjp(cfg, C, 16.0, EF, EA, plan=plan)
+    plan.set_dense_reads(True)
+    check_vjp(cfg, C, 16.0, EF, EA, plan=plan)
+
+
+def test_forward_vjp_equals_separate_calls_and_keeps_inputs():
+    cfg = B.make_config(mx=30, my=26, nz=16, z_lo=6.25, z_hi=9.75, filter_radius=4.0)
+    C = dev(rand_C(cfg, 6))
+    EFn, EAn = rand_fields(cfg, 2, 10)
+    EF, EA = [dev(f) for f in EFn], [dev(f) for f in EAn]
+    C0, F0 = C.clone(), EF[0].clone()
+    plan = B.Plan(cfg)
+    eps1 = plan.eps_forward(C, 8.0)
+    g1 = plan.eps_vjp(C, 8.0, EF, EA)
+    eps2, g2 = plan.eps_forward_vjp(C, 8.0, EF, EA)
+    torch.cuda.synchronize()
+    assert torch.equal(eps1, eps2) and torch.equal(g1, g2)
+    assert torch.equal(C, C0) and torch.equal(EF[0], F0)
+    assert plan.last_launches() >= 5
+
+
+def test_real_cotangent_special_case():
+    # VJP with an arbitrary (real) field w: E_F = -w/2, E_A = 1
+    cfg = B.make_config(mx=12, my=14, nz=8, z_lo=2.25, z_hi=5.75, filter_radius=3.0)
+    C = rand_C(cfg, 1)
+    w = np.random.default_rng(5).standard_normal((1, 3, cfg.nx, cfg.ny, cfg.nz))
+    EF = [(-0.5 * w).astype(np.complex64)]
+    EA = [np.ones_like(EF[0])]
+    g = B.Plan(cfg).eps_vjp(dev(C), 8.0, [dev(EF[0])], [dev(EA[0])]).cpu().numpy().astype(np.float64)
+    ref = O.vjp_real(oracle_cfg(cfg), C[0], 8.0, (-2.0 * (EF[0].astype(np.complex128) * EA[0]).real)[0])
+    assert rel_inf(g[0], ref) < TOL_GRAD and rel_l2(g[0], ref) < TOL_GRAD
+
+
+def test_uniform_control_gives_uniform_mixing_value():
+    # north_star invariant, on the GPU path itself
+    cfg = B.make_config(mx=33, my=20, nz=16, z_lo=6.25, z_hi=9.75, filter_radius=4.0)
+    plan = B.Plan(cfg)
+    for c0 in (0.0, 0.43, 1.0):
+        e2 = plan.stage_eps2d(torch.full(plan.ctrl_shape, c0, device="cuda"), 8.0).cpu().numpy().astype(np.float64)
+        rho = 0.5 * (1 + np.tanh(8.0 * (np.float64(np.float32(c0)) - 0.5)))
+        ref = rho * cfg.eps_core + (1 - rho) * cfg.eps_clad
+        assert np.max(np.abs(e2 - ref)) < 2e-6 * ref
+    eps = plan.eps_forward(torch.rand(plan.ctrl_shape, device="cuda"), 300.0).cpu().numpy()
+    assert eps.min() >= np.float32(cfg.eps_clad) * (1 - 1e-6) and eps.max() <= np.float32(cfg.eps_core) * (1 + 1e-6)
+
+
+def test_host_entry_point_matches_device_entry_point():
+    cfg = B.make_config(mx=20, my=24, nz=16, z_lo=6.25, z_hi=9.75, filter_radius=4.0)
+    Cn = rand_C(cfg, 12)
+    EFn, EAn = rand_fields(cfg, 2, 13)
+    plan = B.Plan(cfg)
+    eps_d, g_d = plan.eps_forward_vjp(dev(Cn), 8.0, [dev(f) for f in EFn], [dev(f) for f in EAn])
+    pin = lambda a: torch.from_numpy(a).pin_memory()
+    eps_h = torch.empty(plan.eps_shape, dtype=torch.float32).pin_memory()
+    g_h = torch.empty(plan.ctrl_shape, dtype=torch.float32).pin_memory()
+    plan.eps_forward_vjp_host(pin(Cn), 8.0, [pin(f) for f in EFn], [pin(f) for f in EAn], eps_h, g_h)
+    torch.cuda.synchronize()
+    assert torch.equal(eps_h, eps_d.cpu()) and torch.equal(g_h, g_d.cpu())
+    h2d, d2h = plan.last_copy_bytes()
+    assert h2d == Cn.nbytes + sum(f.nbytes for f in EFn + EAn) and d2h == eps_h.numel() * 4 + g_h.numel() * 4
+
+
+def test_error_codes():
+    with pytest.raises(B.EpsgradError) as e:
+        B.Plan(B.make_config(mx=8, my=8, nz=8, z_lo=2.0, z_hi=1.0))
+    assert e.value.status == B.EINVAL
+    with pytest.raises(B.EpsgradError) as e:
+        B.Plan(B.make_config(mx=8, my=8, nz=8, z_lo=2.0, z_hi=5.0, subpixel=3))
+    assert e.value.status == B.EINVAL
+    with pytest.raises(B.EpsgradError) as e:
+        B.Plan(B.make_config(mx=8, my=8, nz=6, z_lo=2.0, z_hi=5.0))
+    assert e.value.status == B.EUNSUPPORTED
+    plan = B.Plan(B.make_config(mx=8, my=8, nz=8, z_lo=2.0, z_hi=5.0))
+    with pytest.raises(B.EpsgradError) as e:
+        plan.eps_forward(torch.rand(plan.ctrl_shape, device="cuda"), -1.0)
+    assert e.value.status == B.EINVAL
