@@ -1,0 +1,346 @@
+#!/usr/bin/env python
+"""bench.py -- eps forward+VJP throughput (Yee-cells/s) and HBM roofline fraction on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config paper] [--impl ours|reference]
+
+A step is one pass of the whole hot path -- eps_forward_vjp: filter, fused 2-D chain +
+z-extrusion, Eq. (1) z-reduction, 2-D reverse chain, transposed filter -- over one batch of
+synthetic input (BASELINE.json configs[1] "paper": 250x250 controls -> 500x500x64 Yee cells,
+one field pair) that is already resident in HBM.  Field buffers rotate over 3 sets and eps
+(192 MB > L2) is rewritten every step, so no step finds its inputs in L2.
+One JSON line on stdout (rank 0); see DESIGN.md section 7 for every key.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "eps forward+VJP Yee-cells/s and achieved HBM GB/s vs B200 peak (1 GPU)"
+UNIT = "Yee-cells/s"
+N_SETS = 3
+
+
+def measured_peak_gbs():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler(threading.Thread):
+    """SM clock and throttle reasons via NVML while the timed region runs."""
+
+    def __init__(self, index: int, period_s: float = 0.002):
+        super().__init__(daemon=True)
+        self.index, self.period, self.samples, self.reasons, self.max_mhz = index, period_s, [], set(), None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception:
+            pass
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+        }
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    mask = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    mask = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for bit, name in names.items():
+                    if mask & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2)
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2] if s else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(s)}
+
+
+def visible_device_index(local_rank: int) -> int:
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[local_rank])
+        except Exception:
+            pass
+    return local_rank
+
+
+def zreduce_sector_bytes(w, n_pairs: int) -> int:
+    """Algorithmic bytes of the Eq. (1) field read: the 32-byte sectors of every z column that hold
+    cells with d eps/dC != 0 (x,y: wxy_k > 0; z: wz_k > 0), E_F and E_A, all pairs."""
+    import math
+
+    kxy0, kxy1 = int(math.floor(w.z_lo)), int(math.ceil(w.z_hi)) - 1
+    kz0, kz1 = int(math.floor(w.z_lo - 0.5)), int(math.ceil(w.z_hi - 0.5)) - 1
+    kxy0, kz0 = max(kxy0, 0), max(kz0, 0)
+    kxy1, kz1 = min(kxy1, w.nz - 1), min(kz1, w.nz - 1)
+    sec = lambda a, b: (b // 4 - a // 4 + 1) * 32          # 4 complex64 cells per 32-byte sector
+    per_column = 2 * sec(kxy0, kxy1) + sec(kz0, kz1)
+    return w.batch * w.nx * w.ny * per_column * 2 * n_pairs
+
+
+def oracle_cfg(w, mx=None, my=None):
+    import oracle as O
+    mx, my = mx or w.mx, my or w.my
+    return O.OracleConfig(mx=mx, my=my, nx=w.upsample * mx, ny=w.upsample * my, nz=w.nz, z_lo=w.z_lo, z_hi=w.z_hi,
+                          s=w.subpixel, filter_kind=w.filter_kind, radius=w.radius, sigma=w.sigma or 1.0, eta=w.eta,
+                          eps_core=w.eps_core, eps_clad=w.eps_clad, delta=w.normal_delta)
+
+
+def oracle_step_inputs(w, mx, my):
+    from dataclasses import replace
+    from paper_2505_03352_b200 import workloads as W
+    ws = replace(w, mx=mx, my=my, batch=1)
+    C = W.make_C(ws)[0]
+    EF = [W.make_field(ws, p, 0) for p in range(w.n_pairs)]
+    EA = [W.make_field(ws, p, 1) for p in range(w.n_pairs)]
+    return ws, C, EF, EA
+
+
+def oracle_step(cfg, C, betas, EF, EA):
+    import oracle as O
+    for beta in betas:
+        O.forward(cfg, C, beta)
+        O.vjp(cfg, C, beta, EF, EA)
+
+
+def time_oracle(w, budget_s: float, steps: int, warmup: int):
+    """Time the float64 oracle (as it stands) on a crop of workload w sized so that
+    (steps + warmup) steps take about budget_s.  Returns (cells/s, seconds/step, sample text, threads)."""
+    import oracle as O
+    # calibrate on a 32x32-control crop
+    ws, C, EF, EA = oracle_step_inputs(w, min(32, w.mx), min(32, w.my))
+    cfg = oracle_cfg(w, ws.mx, ws.my)
+    oracle_step(cfg, C, w.betas, EF, EA)
+    t0 = time.perf_counter()
+    oracle_step(cfg, C, w.betas, EF, EA)
+    rate = ws.nx * ws.ny * ws.nz / (time.perf_counter() - t0)          # cells/s, rough
+    target_cells = rate * budget_s / max(1, steps + warmup)
+    full = w.nx * w.ny * w.nz
+    if target_cells >= full:
+        mx, my = w.mx, w.my
+    else:
+        f = (target_cells / full) ** 0.5
+        mx, my = max(16, int(w.mx * f)), max(16, int(w.my * f))
+    ws, C, EF, EA = oracle_step_inputs(w, mx, my)
+    cfg = oracle_cfg(w, mx, my)
+    for _ in range(warmup):
+        oracle_step(cfg, C, w.betas, EF, EA)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        oracle_step(cfg, C, w.betas, EF, EA)
+    dt = (time.perf_counter() - t0) / steps
+    cells = ws.nx * ws.ny * ws.nz                                        # one design of the batch
+    sample = (f"{steps} step(s) of forward+VJP on a {mx}x{my}-control crop ({ws.nx}x{ws.ny}x{ws.nz} Yee cells, "
+              f"{w.n_pairs} pair(s), {len(w.betas)} beta) of '{w.name}'"
+              + (" = the full workload" if (mx, my, w.batch) == (w.mx, w.my, 1) else ""))
+    return cells / dt, dt, sample, O.num_threads()
+
+
+def base_line(w, args, n_gpus):
+    return {
+        "metric": METRIC, "unit": UNIT, "n_gpus": n_gpus, "steps": args.steps, "warmup": args.warmup,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "data": "synthetic",
+        "config": {"workload": f"{w.name}: C {w.batch}x{w.mx}x{w.my} -> Yee {w.nx}x{w.ny}x{w.nz}, "
+                               f"{'conic' if w.filter_kind == 0 else 'gaussian'} R={w.radius:g}, beta={list(w.betas)}, "
+                               f"{w.n_pairs} field pair(s), slab [{w.z_lo},{w.z_hi}]",
+                   "per_gpu": "one such design batch per GPU (independent designs, no collective)",
+                   "cache": f"field buffers rotate over {N_SETS} sets; eps ({w.cells * 12 / 1e6:.0f} MB) rewritten every step"},
+    }
+
+
+def run_reference(args, w):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    val, dt, sample, threads = time_oracle(w, 150.0, args.steps, args.warmup)
+    line = base_line(w, args, args.gpus)
+    line.update({"impl": "reference", "value": val, "ms_per_step": dt * 1e3, "dtype": "f64", "scaling": "weak",
+                 "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+                 "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                 "gpu_launches": 0})
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args, w):
+    import torch
+    from paper_2505_03352_b200 import binding as B
+    from paper_2505_03352_b200 import workloads as W
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the epsgrad path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+
+    plan = B.Plan(B.config_of(w), local)
+    from dataclasses import replace
+    C = torch.from_numpy(W.make_C(replace(w, index=w.index + 1000 * rank))).to(dev)
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(1234 + rank)
+    shape = plan.eps_shape
+
+    def field():
+        return torch.view_as_complex(torch.randn(*shape, 2, device=dev, dtype=torch.float32, generator=gen))
+    EF = [[field() for _ in range(w.n_pairs)] for _ in range(N_SETS)]
+    EA = [[field() for _ in range(w.n_pairs)] for _ in range(N_SETS)]
+    eps = torch.empty(shape, dtype=torch.float32, device=dev)
+    grad = torch.empty(plan.ctrl_shape, dtype=torch.float32, device=dev)
+
+    def step(i):
+        s = i % N_SETS
+        for beta in w.betas:
+            plan.eps_forward_vjp(C, beta, EF[s], EA[s], eps, grad)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for i in range(max(args.warmup, 3)):
+        step(i)
+    launches_per_step = plan.last_launches() * len(w.betas)
+    sampler = ClockSampler(visible_device_index(local))
+    barrier()
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for i in range(args.steps):
+        step(i)
+    e1.record()
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    if dist is not None:
+        t = torch.tensor([ms_total], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    cells_step = w.cells * len(w.betas)
+    value = world * cells_step * args.steps / (ms_total * 1e-3)
+
+    # ---- per-kernel durations, live, with CUDA events on the launching stream
+    plan.set_profiling(True)
+    acc, n_prof = {}, min(args.steps, 100)
+    for i in range(n_prof):
+        s = i % N_SETS
+        for beta in w.betas:
+            plan.eps_forward_vjp(C, beta, EF[s], EA[s], eps, grad)
+            for name, ms in plan.last_kernel_times():
+                acc[name] = acc.get(name, 0.0) + ms
+    plan.set_profiling(False)
+    calls = n_prof * len(w.betas)
+    kernels = {k: v / calls for k, v in acc.items()}                    # ms per launch
+    peak, peak_src = measured_peak_gbs()
+    alg = {"forward": w.cells * 12, "zreduce": zreduce_sector_bytes(w, w.n_pairs)}
+    dom = max((k for k in kernels if k in alg), key=lambda k: kernels[k])
+    traffic = None
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            traffic = json.load(f).get(w.name, {}).get(dom)
+    except Exception:
+        pass
+    achieved = alg[dom] / (kernels[dom] * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                "algorithmic_bytes": alg[dom], "kernel_ms": kernels[dom],
+                "kernels_ms": kernels,
+                "others": {k: {"algorithmic_bytes": alg[k], "GB/s": alg[k] / (kernels[k] * 1e-3) / 1e9,
+                               "frac": alg[k] / (kernels[k] * 1e-3) / 1e9 / peak} for k in alg if k != dom}}
+
+    # ---- end to end through the host-buffer entry point: H2D of C and the fields, D2H of eps and dF/dC
+    pin = lambda t: t.cpu().pin_memory()
+    Ch, EFh, EAh = pin(C), [pin(f) for f in EF[0]], [pin(f) for f in EA[0]]
+    eps_h = torch.empty(shape, dtype=torch.float32).pin_memory()
+    grad_h = torch.empty(plan.ctrl_shape, dtype=torch.float32).pin_memory()
+    n_e2e = max(1, min(args.steps, 10))
+
+    def e2e_step():
+        for beta in w.betas:
+            plan.eps_forward_vjp_host(Ch, beta, EFh, EAh, eps_h, grad_h)
+    for _ in range(2):
+        e2e_step()
+    h2d, d2h = plan.last_copy_bytes()
+    barrier()
+    e0.record()
+    for _ in range(n_e2e):
+        e2e_step()
+    e1.record()
+    barrier()
+    ms_e2e = e0.elapsed_time(e1)
+    if dist is not None:
+        t = torch.tensor([ms_e2e], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_e2e = float(t.item())
+    e2e = {"value": world * cells_step * n_e2e / (ms_e2e * 1e-3), "unit": UNIT,
+           "h2d_bytes_per_step": h2d * len(w.betas), "d2h_bytes_per_step": d2h * len(w.betas),
+           "steps": n_e2e, "ms_per_step": ms_e2e / n_e2e}
+
+    if rank == 0:
+        line = base_line(w, args, world)
+        line.update({"value": value, "ms_per_step": ms_total / args.steps, "dtype": "f32",
+                     "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
+                     "roofline": roofline})
+        if world == 1:
+            val, dt, sample, threads = time_oracle(w, 15.0, 3, 1)
+            line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample}
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=300)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--config", default="paper")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    args = ap.parse_args()
+    from paper_2505_03352_b200 import workloads as W
+    w = W.BY_NAME[args.config]
+    if args.impl == "reference":
+        run_reference(args, w)
+    else:
+        run_ours(args, w)
+
+
+if __name__ == "__main__":
+    main()

@@ -103,6 +103,16 @@ int epsgrad_plan_set_dense_reads(epsgrad_plan_t *plan, int dense);
 /* Number of kernel launches the last eps_* call of this plan enqueued (for accounting). */
 int epsgrad_plan_last_launches(const epsgrad_plan_t *plan);
 
+/* Per-kernel timing for roofline accounting.  When enabled, every eps_* / stage call also
+ * records a CUDA event on `stream` before its first and after each of its kernels (at most
+ * 16).  epsgrad_plan_last_kernel_times waits (host-blocking: the one exception to "never
+ * synchronises") for the last call's events and returns the number n of kernels it
+ * launched, writing ms[i] = device time between the events around kernel i (it includes
+ * the launch gap before it) and names[i] = a static string naming the kernel; ms[i] = -1
+ * when profiling was off.  Negative return = error.                                     */
+int epsgrad_plan_set_profiling(epsgrad_plan_t *plan, int enable);
+int epsgrad_plan_last_kernel_times(epsgrad_plan_t *plan, int max_n, float *ms, const char **names);
+
 /* ---- the hot path (device pointers) -------------------------------------------------- */
 /* eps_hat(C, beta): the whole forward chain.  beta > 0 (it changes every
  * iteration, Eq. (14), hence a call argument).                                    */

@@ -19,6 +19,7 @@ EXPORTS = (
     "epsgrad_plan_create", "epsgrad_plan_destroy", "epsgrad_workspace_bytes",
     "epsgrad_plan_set_workspace", "epsgrad_staging_bytes", "epsgrad_plan_set_staging",
     "epsgrad_plan_set_dense_reads", "epsgrad_plan_last_launches", "epsgrad_plan_last_copy_bytes",
+    "epsgrad_plan_set_profiling", "epsgrad_plan_last_kernel_times",
     "eps_forward", "eps_vjp", "eps_forward_vjp", "eps_forward_vjp_host",
     "epsgrad_stage_filter", "epsgrad_stage_eps2d", "epsgrad_stage_zreduce",
     "epsgrad_status_string", "epsgrad_version",
@@ -95,6 +96,8 @@ def lib() -> ctypes.CDLL:
     L.epsgrad_plan_set_dense_reads.argtypes = [vp, i32]
     L.epsgrad_plan_last_launches.argtypes = [vp]
     L.epsgrad_plan_last_copy_bytes.argtypes = [vp, ctypes.POINTER(ctypes.c_uint64), ctypes.POINTER(ctypes.c_uint64)]
+    L.epsgrad_plan_set_profiling.argtypes = [vp, i32]
+    L.epsgrad_plan_last_kernel_times.argtypes = [vp, i32, ctypes.POINTER(f32), ctypes.POINTER(ctypes.c_char_p)]
     L.eps_forward.argtypes = [vp, vp, f32, vp, vp]
     L.eps_vjp.argtypes = [vp, vp, f32, i32, vp, vp, vp, vp]
     L.eps_forward_vjp.argtypes = [vp, vp, f32, i32, vp, vp, vp, vp, vp]
@@ -202,6 +205,18 @@ class Plan:
         a, b = ctypes.c_uint64(), ctypes.c_uint64()
         _check(lib().epsgrad_plan_last_copy_bytes(self._h, ctypes.byref(a), ctypes.byref(b)), "last_copy_bytes")
         return int(a.value), int(b.value)
+
+    def set_profiling(self, enable: bool) -> None:
+        _check(lib().epsgrad_plan_set_profiling(self._h, int(bool(enable))), "epsgrad_plan_set_profiling")
+
+    def last_kernel_times(self):
+        """[(kernel name, ms)] of the last call (blocks until its events have completed)."""
+        ms = (ctypes.c_float * 16)()
+        names = (ctypes.c_char_p * 16)()
+        n = lib().epsgrad_plan_last_kernel_times(self._h, 16, ms, names)
+        if n < 0:
+            raise EpsgradError(n, "epsgrad_plan_last_kernel_times")
+        return [(names[i].decode(), float(ms[i])) for i in range(n)]
 
     # ---- hot path (device tensors)
     def eps_forward(self, C, beta: float, out=None):

@@ -18,6 +18,7 @@
 using namespace epsgrad;
 
 #define EPSGRAD_VERSION 100   /* 0.1.0 */
+#define EPSGRAD_MAX_KERNELS 16
 
 struct epsgrad_plan {
     epsgrad_config_t cfg;
@@ -45,6 +46,10 @@ struct epsgrad_plan {
     size_t off_phi, off_v, off_gbar, off_tmp, ws_need;
     int last_launches;
     uint64_t last_h2d, last_d2h;
+    // optional per-kernel timing (epsgrad_plan_set_profiling)
+    int prof;
+    cudaEvent_t ev[EPSGRAD_MAX_KERNELS + 1];
+    const char *kname[EPSGRAD_MAX_KERNELS];
 };
 
 static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
@@ -272,8 +277,45 @@ extern "C" int epsgrad_plan_destroy(epsgrad_plan_t *P)
 {
     if (!P) return EPSGRAD_EINVAL;
     if (P->d_tables) cudaFree(P->d_tables);
+    if (P->ev[0])
+        for (int i = 0; i <= EPSGRAD_MAX_KERNELS; ++i) cudaEventDestroy(P->ev[i]);
     delete P;
     return EPSGRAD_OK;
+}
+
+extern "C" int epsgrad_plan_set_profiling(epsgrad_plan_t *P, int enable)
+{
+    if (!P) return EPSGRAD_EINVAL;
+    if (enable && !P->ev[0]) {
+        int prev = 0;
+        cudaGetDevice(&prev);
+        cudaSetDevice(P->device);
+        bool ok = true;
+        for (int i = 0; i <= EPSGRAD_MAX_KERNELS && ok; ++i) ok = cudaEventCreate(&P->ev[i]) == cudaSuccess;
+        cudaSetDevice(prev);
+        if (!ok) { cudaGetLastError(); return EPSGRAD_ECUDA; }
+    }
+    P->prof = enable != 0;
+    return EPSGRAD_OK;
+}
+
+extern "C" int epsgrad_plan_last_kernel_times(epsgrad_plan_t *P, int max_n, float *ms, const char **names)
+{
+    if (!P || max_n < 0 || (max_n > 0 && (!ms || !names))) return EPSGRAD_EINVAL;
+    int n = P->last_launches < EPSGRAD_MAX_KERNELS ? P->last_launches : EPSGRAD_MAX_KERNELS;
+    if (n > max_n) n = max_n;
+    for (int i = 0; i < n; ++i) {
+        names[i] = P->kname[i];
+        ms[i] = -1.0f;
+        if (P->prof) {
+            if (cudaEventSynchronize(P->ev[i + 1]) != cudaSuccess ||
+                cudaEventElapsedTime(&ms[i], P->ev[i], P->ev[i + 1]) != cudaSuccess) {
+                cudaGetLastError();
+                return EPSGRAD_ECUDA;
+            }
+        }
+    }
+    return n;
 }
 
 extern "C" size_t epsgrad_workspace_bytes(const epsgrad_plan_t *P) { return P ? P->ws_need : 0; }
@@ -350,9 +392,19 @@ int set_smem(K kernel, size_t bytes)
     return EPSGRAD_OK;
 }
 
-int check_launch(epsgrad_plan *P)
+void begin_call(epsgrad_plan *P, cudaStream_t st)
 {
-    ++P->last_launches;
+    P->last_launches = 0;
+    if (P->prof) cudaEventRecord(P->ev[0], st);
+}
+
+int check_launch(epsgrad_plan *P, const char *name, cudaStream_t st)
+{
+    const int idx = P->last_launches++;
+    if (idx < EPSGRAD_MAX_KERNELS) {
+        P->kname[idx] = name;
+        if (P->prof) cudaEventRecord(P->ev[idx + 1], st);
+    }
     return cudaGetLastError() == cudaSuccess ? EPSGRAD_OK : EPSGRAD_ECUDA;
 }
 
@@ -384,7 +436,7 @@ int launch_filter_m(epsgrad_plan *P, const float *C, float *phi, cudaStream_t st
         int rc = set_smem(k_filter_conic<M, TA, TB>, smem);
         if (rc) return rc;
         k_filter_conic<M, TA, TB><<<dim3(cdiv(my, TB), cdiv(mx, TA), B), TA * TB, smem, st>>>(fp);
-        return check_launch(P);
+        return check_launch(P, "filter", st);
     }
     SepParams sp;
     sp.w1 = P->d_w; sp.nrm = make_nrm(P);
@@ -395,7 +447,7 @@ int launch_filter_m(epsgrad_plan *P, const float *C, float *phi, cudaStream_t st
         int rc = set_smem(k_sep_up_y<M>, smem);
         if (rc) return rc;
         k_sep_up_y<M><<<dim3(cdiv(my, 32), cdiv(mx, 8), B), SEP_THREADS, smem, st>>>(sp);
-        if ((rc = check_launch(P))) return rc;
+        if ((rc = check_launch(P, "filter_up_y", st))) return rc;
     }
     {
         sp.in = ws_tmp(P); sp.out = phi;
@@ -404,7 +456,7 @@ int launch_filter_m(epsgrad_plan *P, const float *C, float *phi, cudaStream_t st
         int rc = set_smem(k_sep_up_x<M>, smem);
         if (rc) return rc;
         k_sep_up_x<M><<<dim3(cdiv(P->py, 128), cdiv(mx, 8), B), SEP_THREADS, smem, st>>>(sp);
-        return check_launch(P);
+        return check_launch(P, "filter_up_x", st);
     }
 }
 
@@ -420,7 +472,7 @@ int launch_filterT_conic(epsgrad_plan *P, const float *v, float *dC, cudaStream_
     int rc = set_smem(k_filterT_conic<M, TT, TT>, smem);
     if (rc) return rc;
     k_filterT_conic<M, TT, TT><<<dim3(cdiv(fp.my, TT), cdiv(fp.mx, TT), P->cfg.batch), TT * TT, smem, st>>>(fp);
-    return check_launch(P);
+    return check_launch(P, "filterT", st);
 }
 
 template <int M>
@@ -439,7 +491,7 @@ int launch_filterT_m(epsgrad_plan *P, const float *v, float *dC, cudaStream_t st
         int rc = set_smem(k_sep_down_x<M>, smem);
         if (rc) return rc;
         k_sep_down_x<M><<<dim3(cdiv(P->py, 64), cdiv(mx, 8), B), SEP_THREADS, smem, st>>>(sp);
-        if ((rc = check_launch(P))) return rc;
+        if ((rc = check_launch(P, "filterT_down_x", st))) return rc;
     }
     {
         sp.in = ws_tmp(P); sp.out = dC;
@@ -448,7 +500,7 @@ int launch_filterT_m(epsgrad_plan *P, const float *v, float *dC, cudaStream_t st
         int rc = set_smem(k_sep_down_y<M>, smem);
         if (rc) return rc;
         k_sep_down_y<M><<<dim3(cdiv(my, 32), cdiv(mx, 8), B), SEP_THREADS, smem, st>>>(sp);
-        return check_launch(P);
+        return check_launch(P, "filterT_down_y", st);
     }
 }
 
@@ -485,7 +537,7 @@ int launch_forward(epsgrad_plan *P, const float *phi, float beta, float *eps, fl
     int rc = set_smem(k_forward, smem);
     if (rc) return rc;
     k_forward<<<dim3(cdiv(P->ny, FWD_TJ), cdiv(P->nx, FWD_TI), P->cfg.batch), FWD_THREADS, smem, st>>>(fp);
-    return check_launch(P);
+    return check_launch(P, "forward", st);
 }
 
 // ---- R1
@@ -514,7 +566,7 @@ int launch_zreduce(epsgrad_plan *P, int n_pairs, const void *const *EF, const vo
         }
         zp.n_pairs = np; zp.accumulate = p0 > 0;
         k_zreduce<<<dim3(maxblocks, 3 * P->cfg.batch), ZR_THREADS, 0, st>>>(zp);
-        int rc = check_launch(P);
+        int rc = check_launch(P, "zreduce", st);
         if (rc) return rc;
     }
     return EPSGRAD_OK;
@@ -532,7 +584,7 @@ int launch_reverse2d(epsgrad_plan *P, const float *phi, float beta, const float 
     int rc = set_smem(k_reverse2d, smem);
     if (rc) return rc;
     k_reverse2d<<<dim3(cdiv(P->ny, REV_TJ), cdiv(P->nx, REV_TI), P->cfg.batch), REV_THREADS, smem, st>>>(rp);
-    return check_launch(P);
+    return check_launch(P, "reverse2d", st);
 }
 
 bool aligned16(const void *p) { return p && !((uintptr_t)p & 15); }
@@ -577,7 +629,7 @@ extern "C" int eps_forward(epsgrad_plan_t *P, const float *C, float beta, float 
     if (!aligned16(eps)) return EPSGRAD_EINVAL;
     DeviceGuard g(P->device);
     cudaStream_t st = (cudaStream_t)stream;
-    P->last_launches = 0;
+    begin_call(P, st);
     rc = launch_filter(P, C, ws_phi(P), st);
     if (!rc) rc = launch_forward(P, ws_phi(P), beta, eps, nullptr, st);
     return rc;
@@ -592,7 +644,7 @@ extern "C" int eps_vjp(epsgrad_plan_t *P, const float *C, float beta, int n_pair
     if (!aligned16(dFdC)) return EPSGRAD_EINVAL;
     DeviceGuard g(P->device);
     cudaStream_t st = (cudaStream_t)stream;
-    P->last_launches = 0;
+    begin_call(P, st);
     rc = launch_filter(P, C, ws_phi(P), st);
     if (!rc) rc = run_vjp(P, beta, n_pairs, EF, EA, dFdC, st);
     return rc;
@@ -608,7 +660,7 @@ extern "C" int eps_forward_vjp(epsgrad_plan_t *P, const float *C, float beta, in
     if (!aligned16(eps) || !aligned16(dFdC)) return EPSGRAD_EINVAL;
     DeviceGuard g(P->device);
     cudaStream_t st = (cudaStream_t)stream;
-    P->last_launches = 0;
+    begin_call(P, st);
     rc = launch_filter(P, C, ws_phi(P), st);
     if (!rc) rc = launch_forward(P, ws_phi(P), beta, eps, nullptr, st);
     if (!rc) rc = run_vjp(P, beta, n_pairs, EF, EA, dFdC, st);
@@ -633,7 +685,7 @@ extern "C" int eps_forward_vjp_host(epsgrad_plan_t *P, const float *C_host, floa
     if (!P->stg || P->stg_bytes < epsgrad_staging_bytes(P, n_pairs)) return EPSGRAD_ENOWORKSPACE;
     DeviceGuard g(P->device);
     cudaStream_t st = (cudaStream_t)stream;
-    P->last_launches = 0;
+    begin_call(P, st);
     P->last_h2d = P->last_d2h = 0;
 
     const size_t b_c = n_ctrl(P) * 4, b_e = n_eps(P) * 4, b_f = n_eps(P) * 8;
@@ -675,7 +727,7 @@ extern "C" int epsgrad_stage_filter(epsgrad_plan_t *P, const float *C, float *ph
     if (rc) return rc;
     if (!aligned16(phi_centred)) return EPSGRAD_EINVAL;
     DeviceGuard g(P->device);
-    P->last_launches = 0;
+    begin_call(P, (cudaStream_t)stream);
     return launch_filter(P, C, phi_centred, (cudaStream_t)stream);
 }
 
@@ -686,7 +738,7 @@ extern "C" int epsgrad_stage_eps2d(epsgrad_plan_t *P, const float *C, float beta
     if (!aligned16(eps2d)) return EPSGRAD_EINVAL;
     DeviceGuard g(P->device);
     cudaStream_t st = (cudaStream_t)stream;
-    P->last_launches = 0;
+    begin_call(P, st);
     rc = launch_filter(P, C, ws_phi(P), st);
     if (!rc) rc = launch_forward(P, ws_phi(P), beta, nullptr, eps2d, st);
     return rc;
@@ -700,6 +752,6 @@ extern "C" int epsgrad_stage_zreduce(epsgrad_plan_t *P, int n_pairs, const void 
     if (rc) return rc;
     if (!aligned16(gbar)) return EPSGRAD_EINVAL;
     DeviceGuard g(P->device);
-    P->last_launches = 0;
+    begin_call(P, (cudaStream_t)stream);
     return launch_zreduce(P, n_pairs, EF, EA, gbar, (cudaStream_t)stream);
 }
