@@ -22,22 +22,33 @@ __device__ __forceinline__ int border_class(int a0, int M, int T, int K)
     return d < T ? 2 * T - d : T;
 }
 
-// streaming 16-byte load that does not allocate in L1 (fields are read exactly once)
+// streaming 16-byte load that does not allocate in L1 (fields are read exactly once).
+// SPARSE: the access touches only a 64..96-byte window of each 512-byte z column.  By default a
+// miss fills the whole 128-byte line from DRAM (measured: 256 B fetched per column for a window
+// that straddles a line boundary); the L2::64B prefetch-size qualifier halves that -- 64 B is the
+// smallest fill granularity this part honours (profiles/r1b_zreduce_granularity.md).
+template <bool SPARSE>
 __device__ __forceinline__ float4 ld_stream(const float4 *p)
 {
     float4 r;
-    asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
-                 : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
+    if (SPARSE)
+        asm volatile("ld.global.nc.L1::no_allocate.L2::64B.v4.f32 {%0,%1,%2,%3}, [%4];"
+                     : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
+    else
+        asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
+                     : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
     return r;
 }
 
 // Projection + mixing rule of one mask pixel (Eq. (3)/(6) P:L54,L74):
-//   t = beta (Phi - eta), rho = (1 + tanh t)/2, e = eps_clad + (eps_core - eps_clad) rho.
-// phi_c is the centred filter output Phi - eta0; eta_r = eta - eta0.
+//   t = beta (Phi - eta), rho = (1 + tanh t)/2 = 1/(1 + exp(-2t)), e = eps_clad + (eps_core - eps_clad) rho.
+// phi_c is the centred filter output Phi - eta0; eta_r = eta - eta0.  exp(-2t) -> +inf gives rho = 0,
+// -> 0 gives rho = 1: no NaN.  |d rho| <= rho (1-rho) * relerr(exp) < 1e-7 with the ex2.approx path
+// (DESIGN.md 6.2); the reciprocal is correctly rounded.
 __device__ __forceinline__ float project_mix(float phi_c, float beta, float eta_r, float eps_clad, float deps)
 {
     const float t = beta * (phi_c - eta_r);
-    const float rho = 0.5f * (1.0f + tanhf(t));
+    const float rho = __frcp_rn(1.0f + __expf(-2.0f * t));
     return fmaf(deps, rho, eps_clad);
 }
 
@@ -46,21 +57,43 @@ __device__ __forceinline__ float project_mix(float phi_c, float beta, float eta_
 __device__ __forceinline__ float project_slope(float phi_c, float beta, float eta_r)
 {
     const float t = beta * (phi_c - eta_r);
-    const float a = expf(-2.0f * fabsf(t));
-    const float d = 1.0f + a;
-    return 2.0f * beta * a / (d * d);
+    const float a = __expf(-2.0f * fabsf(t));
+    const float d = __frcp_rn(1.0f + a);
+    return 2.0f * beta * a * d * d;
+}
+
+// load N consecutive floats from shared memory (N even; 16-byte vectors when N % 4 == 0 and p is 16-byte aligned)
+template <int N>
+__device__ __forceinline__ void lds_vec(const float *p, float *out)
+{
+    if (N % 4 == 0) {
+#pragma unroll
+        for (int q = 0; q < N / 4; ++q) {
+            const float4 t = reinterpret_cast<const float4 *>(p)[q];
+            out[4 * q] = t.x; out[4 * q + 1] = t.y; out[4 * q + 2] = t.z; out[4 * q + 3] = t.w;
+        }
+    } else {
+#pragma unroll
+        for (int q = 0; q < N / 2; ++q) {
+            const float2 t = reinterpret_cast<const float2 *>(p)[q];
+            out[2 * q] = t.x; out[2 * q + 1] = t.y;
+        }
+    }
 }
 
 struct Normaliser {          // 1/sum_w lookup (S2), DESIGN.md 5.1
     const float *tab;        // conic: [KX*m][KY*m]; separable: x table [KX*m] then y table [KY*m]
     int mx, my, m, T, KX, KY, separable;
-    __device__ __forceinline__ float at(int p, int q) const
+    // table row / column of mask pixel p = m*a0 + f along x / y
+    __device__ __forceinline__ int ix(int a0, int f) const { return border_class(a0, mx, T, KX) * m + f; }
+    __device__ __forceinline__ int iy(int b0, int f) const { return border_class(b0, my, T, KY) * m + f; }
+    __device__ __forceinline__ int ix_of(int p) const { const int a0 = p / m; return ix(a0, p - a0 * m); }
+    __device__ __forceinline__ int iy_of(int q) const { const int b0 = q / m; return iy(b0, q - b0 * m); }
+    __device__ __forceinline__ float at_index(int i, int j) const
     {
-        const int a0 = p / m, fx = p - a0 * m, b0 = q / m, fy = q - b0 * m;
-        const int ix = border_class(a0, mx, T, KX) * m + fx;
-        const int iy = border_class(b0, my, T, KY) * m + fy;
-        return separable ? tab[ix] * tab[KX * m + iy] : tab[ix * (KY * m) + iy];
+        return separable ? tab[i] * tab[KX * m + j] : tab[i * (KY * m) + j];
     }
+    __device__ __forceinline__ float at(int p, int q) const { return at_index(ix_of(p), iy_of(q)); }
 };
 
 }  // namespace epsgrad

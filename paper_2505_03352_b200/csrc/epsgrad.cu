@@ -26,13 +26,12 @@ struct epsgrad_plan {
     int nx, ny, px, py, m;
     int T, NT, KX, KY;
     int separable;
-    int conic_tile;            // TA = TB of the transposed conic filter (16 or 8)
     // device tables (one allocation)
     void *d_tables;
     float *d_w;                // conic [NT][NT][m][m] | separable [NT][m]
     int *d_tyrange;            // conic [NT][2]
     float *d_invden;           // conic [KX*m][KY*m] | separable [KX*m] + [KY*m]
-    float *d_zw;               // [5][nz]
+    float *d_zw;               // [7][nz]: wxy, wz, z-full / lower-face / upper-face indicators, eps_clad(1-wxy), eps_clad[wz=0]
     // z windows (chunks of 2 cells) for {x,y} and {z}; face weights
     int ch0[2], nch[2];
     float w_lo, w_hi;
@@ -203,7 +202,7 @@ extern "C" int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsg
 
     // ---- z tables (S7, S8): wxy_k = |[k,k+1] ^ slab|, wz_k = |[k+1/2,k+3/2] ^ slab|
     const int nz = cfg->nz;
-    std::vector<float> zw((size_t)5 * nz, 0.0f);
+    std::vector<float> zw((size_t)7 * nz, 0.0f);
     int kmin[2] = {nz, nz}, kmax[2] = {-1, -1};
     int n_face = 0;
     for (int k = 0; k < nz; ++k) {
@@ -211,6 +210,8 @@ extern "C" int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsg
         const double wz = overlap(k + 0.5, k + 1.5, cfg->z_lo, cfg->z_hi);
         zw[k] = (float)wxy;
         zw[nz + k] = (float)wz;
+        zw[5 * nz + k] = (float)(cfg->eps_clad * (1.0 - wxy));
+        zw[6 * nz + k] = wz > 0.0 ? 0.0f : (float)cfg->eps_clad;
         if (wxy > 0.0) { if (k < kmin[0]) kmin[0] = k; kmax[0] = k; }
         if (wz > 0.0) {
             if (k < kmin[1]) kmin[1] = k;
@@ -226,12 +227,11 @@ extern "C" int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsg
         else { P->ch0[g] = kmin[g] / 2; P->nch[g] = kmax[g] / 2 - P->ch0[g] + 1; }
     }
 
-    // ---- tile choice of the transposed conic filter by shared memory
-    P->conic_tile = 16;
+    // ---- shared-memory budget of the transposed conic filter (v tile + weight table)
     if (!P->separable) {
-        auto need = [&](int t) { return ((size_t)NT * NT * m * m + (size_t)m * (t + 2 * T) * m * (t + 2 * T) + 2 * NT) * 4; };
-        if (need(16) > 200 * 1024) P->conic_tile = 8;
-        if (need(P->conic_tile) > 200 * 1024) { delete P; return EPSGRAD_EUNSUPPORTED; }
+        const int sp = m % 4 == 0 ? 4 : 2, tb = 32 / sp, ta = 8;
+        const size_t need = ((size_t)NT * NT * m * m + (size_t)m * (ta + 2 * T) * m * (tb + 2 * T) + 2 * NT) * 4;
+        if (need > 200 * 1024) { delete P; return EPSGRAD_EUNSUPPORTED; }
     }
     if (fwd_smem_floats(s, nz) * 4 > 200 * 1024 || rev_smem_floats(s) * 4 > 200 * 1024) { delete P; return EPSGRAD_EUNSUPPORTED; }
 
@@ -427,7 +427,7 @@ int launch_filter_m(epsgrad_plan *P, const float *C, float *phi, cudaStream_t st
 {
     const int B = P->cfg.batch, mx = P->cfg.mx, my = P->cfg.my, T = P->T, NT = P->NT;
     if (!P->separable) {
-        constexpr int TA = 16, TB = 16;
+        constexpr int TA = 8, TB = 16;
         FilterParams fp;
         fp.C = C; fp.phi = phi; fp.w = P->d_w; fp.tyrange = P->d_tyrange; fp.nrm = make_nrm(P);
         fp.mx = mx; fp.my = my; fp.px = P->px; fp.py = P->py; fp.T = T; fp.NT = NT; fp.eta0 = P->eta0;
@@ -461,17 +461,19 @@ int launch_filter_m(epsgrad_plan *P, const float *C, float *phi, cudaStream_t st
 }
 
 // ---- R6: mask cotangent v -> dF/dC
-template <int M, int TT>
+template <int M>
 int launch_filterT_conic(epsgrad_plan *P, const float *v, float *dC, cudaStream_t st)
 {
+    using S = FilterTShape<M>;
     const int T = P->T, NT = P->NT;
     FilterTParams fp;
     fp.v = v; fp.dC = dC; fp.w = P->d_w; fp.tyrange = P->d_tyrange;
     fp.mx = P->cfg.mx; fp.my = P->cfg.my; fp.px = P->px; fp.py = P->py; fp.T = T; fp.NT = NT;
-    const size_t smem = ((size_t)NT * NT * M * M + (size_t)M * (TT + 2 * T) * M * (TT + 2 * T) + 2 * NT) * 4;
-    int rc = set_smem(k_filterT_conic<M, TT, TT>, smem);
+    const size_t smem = ((size_t)NT * NT * M * M + (size_t)M * (S::TA + 2 * T) * M * (S::TB + 2 * T) + 2 * NT) * 4;
+    if (smem > 200 * 1024) return EPSGRAD_EUNSUPPORTED;
+    int rc = set_smem(k_filterT_conic<M>, smem);
     if (rc) return rc;
-    k_filterT_conic<M, TT, TT><<<dim3(cdiv(fp.my, TT), cdiv(fp.mx, TT), P->cfg.batch), TT * TT, smem, st>>>(fp);
+    k_filterT_conic<M><<<dim3(cdiv(fp.my, S::TB), cdiv(fp.mx, S::TA), P->cfg.batch), S::NTHR, smem, st>>>(fp);
     return check_launch(P, "filterT", st);
 }
 
@@ -479,7 +481,7 @@ template <int M>
 int launch_filterT_m(epsgrad_plan *P, const float *v, float *dC, cudaStream_t st)
 {
     if (!P->separable)
-        return P->conic_tile == 16 ? launch_filterT_conic<M, 16>(P, v, dC, st) : launch_filterT_conic<M, 8>(P, v, dC, st);
+        return launch_filterT_conic<M>(P, v, dC, st);
     const int B = P->cfg.batch, mx = P->cfg.mx, my = P->cfg.my, T = P->T, NT = P->NT;
     SepParams sp;
     sp.w1 = P->d_w; sp.nrm = make_nrm(P);
@@ -533,10 +535,12 @@ int launch_forward(epsgrad_plan *P, const float *phi, float beta, float *eps, fl
     fp.phi = phi; fp.eps = eps; fp.eps2d = eps2d; fp.zw = P->d_zw;
     fp.nx = P->nx; fp.ny = P->ny; fp.nz = P->cfg.nz; fp.px = P->px; fp.py = P->py; fp.s = P->cfg.subpixel;
     fp.beta = beta; fp.eta_r = P->eta_r; fp.eps_clad = P->eps_clad; fp.deps = P->deps; fp.delta = P->delta;
+    fp.w_lo = P->w_lo; fp.w_hi = P->w_hi;
     const size_t smem = fwd_smem_floats(fp.s, fp.nz) * 4;
-    int rc = set_smem(k_forward, smem);
+    auto kern = fp.s == 2 ? k_forward<2> : (fp.s == 4 ? k_forward<4> : k_forward<0>);
+    int rc = set_smem(kern, smem);
     if (rc) return rc;
-    k_forward<<<dim3(cdiv(P->ny, FWD_TJ), cdiv(P->nx, FWD_TI), P->cfg.batch), FWD_THREADS, smem, st>>>(fp);
+    kern<<<dim3(cdiv(P->ny, FWD_TJ), cdiv(P->nx, FWD_TI), P->cfg.batch), FWD_THREADS, smem, st>>>(fp);
     return check_launch(P, "forward", st);
 }
 
@@ -547,15 +551,21 @@ int launch_zreduce(epsgrad_plan *P, int n_pairs, const void *const *EF, const vo
 {
     ZredParams zp;
     zp.gbar = gbar; zp.zw = P->d_zw; zp.ncol = P->nx * P->ny; zp.nz = P->cfg.nz;
-    int maxblocks = 1;
+    int maxnch = 1;
     for (int g = 0; g < 2; ++g) {
         zp.ch0[g] = P->dense ? 0 : P->ch0[g];
         zp.nch[g] = P->dense ? P->cfg.nz / 2 : P->nch[g];
         int L = next_pow2(zp.nch[g] < 1 ? 1 : zp.nch[g]);
         if (L > 32) L = 32;
         zp.L[g] = L;
-        const int cols_per_block = (ZR_THREADS / L) * ZR_UNROLL;
-        const int nb = cdiv(zp.ncol, cols_per_block);
+        if (zp.nch[g] > maxnch) maxnch = zp.nch[g];
+    }
+    // windows of at most 128 bytes per column: ask for 64-byte fills and keep fewer columns in flight
+    const bool sparse = maxnch * 16 <= 128 && zp.nz * 8 > 128;
+    const int unroll = sparse ? ZR_UNROLL_SPARSE : ZR_UNROLL_DENSE;
+    int maxblocks = 1;
+    for (int g = 0; g < 2; ++g) {
+        const int nb = cdiv(zp.ncol, (ZR_THREADS / zp.L[g]) * unroll);
         if (nb > maxblocks) maxblocks = nb;
     }
     for (int p0 = 0; p0 < n_pairs; p0 += ZR_MAX_PAIRS) {
@@ -565,7 +575,9 @@ int launch_zreduce(epsgrad_plan *P, int n_pairs, const void *const *EF, const vo
             zp.ea[p] = (const float4 *)(p < np ? EA[p0 + p] : nullptr);
         }
         zp.n_pairs = np; zp.accumulate = p0 > 0;
-        k_zreduce<<<dim3(maxblocks, 3 * P->cfg.batch), ZR_THREADS, 0, st>>>(zp);
+        const dim3 grid(maxblocks, 3 * P->cfg.batch);
+        if (sparse) k_zreduce<ZR_UNROLL_SPARSE, true><<<grid, ZR_THREADS, 0, st>>>(zp);
+        else k_zreduce<ZR_UNROLL_DENSE, false><<<grid, ZR_THREADS, 0, st>>>(zp);
         int rc = check_launch(P, "zreduce", st);
         if (rc) return rc;
     }
@@ -581,9 +593,10 @@ int launch_reverse2d(epsgrad_plan *P, const float *phi, float beta, const float 
     rp.beta = beta; rp.eta_r = P->eta_r; rp.eps_clad = P->eps_clad; rp.deps = P->deps; rp.delta = P->delta;
     rp.w_lo = P->w_lo; rp.w_hi = P->w_hi;
     const size_t smem = rev_smem_floats(rp.s) * 4;
-    int rc = set_smem(k_reverse2d, smem);
+    auto kern = rp.s == 2 ? k_reverse2d<2> : (rp.s == 4 ? k_reverse2d<4> : k_reverse2d<0>);
+    int rc = set_smem(kern, smem);
     if (rc) return rc;
-    k_reverse2d<<<dim3(cdiv(P->ny, REV_TJ), cdiv(P->nx, REV_TI), P->cfg.batch), REV_THREADS, smem, st>>>(rp);
+    kern<<<dim3(cdiv(P->ny, REV_TJ), cdiv(P->nx, REV_TI), P->cfg.batch), REV_THREADS, smem, st>>>(rp);
     return check_launch(P, "reverse2d", st);
 }
 

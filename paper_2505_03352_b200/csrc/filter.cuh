@@ -64,7 +64,8 @@ __global__ void __launch_bounds__(TA *TB) k_filter_conic(const FilterParams P)
         const float *crow = c_s + (la + tx) * CW + lb;
         for (int ty = ty0; ty <= ty1; ++ty) {
             const float cv = crow[ty];
-            const float *wt = w_s + (tx * NT + ty) * (M * M);
+            float wt[M * M];
+            lds_vec<M * M>(w_s + (tx * NT + ty) * (M * M), wt);      // warp-uniform address: broadcast
 #pragma unroll
             for (int i = 0; i < M; ++i)
 #pragma unroll
@@ -73,6 +74,7 @@ __global__ void __launch_bounds__(TA *TB) k_filter_conic(const FilterParams P)
     }
     if (a0 >= P.mx || b0 >= P.my) return;
     float *out = P.phi + (size_t)b * P.px * P.py;
+    const int nix = P.nrm.ix(a0, 0), niy = P.nrm.iy(b0, 0);   // all m x m pixels of a control pixel share its border class
 #pragma unroll
     for (int i = 0; i < M; ++i) {
         const int p = M * a0 + i;
@@ -80,8 +82,8 @@ __global__ void __launch_bounds__(TA *TB) k_filter_conic(const FilterParams P)
 #pragma unroll
         for (int j = 0; j < M; j += 2) {
             float2 o;
-            o.x = acc[i][j] * P.nrm.at(p, M * b0 + j);
-            o.y = acc[i][j + 1] * P.nrm.at(p, M * b0 + j + 1);
+            o.x = acc[i][j] * P.nrm.at_index(nix + i, niy + j);
+            o.y = acc[i][j + 1] * P.nrm.at_index(nix + i, niy + j + 1);
             *reinterpret_cast<float2 *>(row + j) = o;
         }
     }
@@ -96,17 +98,28 @@ struct FilterTParams {
     int mx, my, px, py, T, NT;
 };
 
-// grid (ceil(my/TB), ceil(mx/TA), B), block TA*TB; thread <-> control pixel (a,b).
-template <int M, int TA, int TB>
-__global__ void __launch_bounds__(TA *TB) k_filterT_conic(const FilterTParams P)
+// One warp per row of TB control pixels; SP lanes share a control pixel, each taking M/SP of its m phase
+// rows, and reduce with xor-shuffles (4x the parallelism of one thread per pixel: the grid is only
+// (mx/8) x (my/TB) CTAs).  Lane = sp*TB + lb keeps a quarter-warp on 8 neighbouring pixels, so the
+// M-float reads of v are contiguous across lanes (no bank conflicts).
+template <int M> struct FilterTShape {
+    static constexpr int SP = (M % 4 == 0) ? 4 : 2;     // lanes per control pixel
+    static constexpr int TB = 32 / SP, TA = 8, NTHR = 32 * TA, ROWS = M / SP;
+};
+
+// grid (ceil(my/TB), ceil(mx/TA), B)
+template <int M>
+__global__ void __launch_bounds__(FilterTShape<M>::NTHR) k_filterT_conic(const FilterTParams P)
 {
+    using S = FilterTShape<M>;
+    constexpr int TA = S::TA, TB = S::TB, SP = S::SP, ROWS = S::ROWS, nthr = S::NTHR;
     extern __shared__ __align__(16) float sm[];
     const int T = P.T, NT = P.NT;
     const int VH = M * (TA + 2 * T), VW = M * (TB + 2 * T);   // v tile
     float *w_s = sm;                               // NT*NT*M*M
     float *v_s = w_s + NT * NT * M * M;            // VH*VW
     int *ty_s = reinterpret_cast<int *>(v_s + VH * VW);
-    const int tid = threadIdx.x, nthr = TA * TB;
+    const int tid = threadIdx.x;
     const int a_base = blockIdx.y * TA, b_base = blockIdx.x * TB, b = blockIdx.z;
 
     for (int i = tid; i < NT * NT * M * M; i += nthr) w_s[i] = P.w[i];
@@ -122,24 +135,34 @@ __global__ void __launch_bounds__(TA *TB) k_filterT_conic(const FilterTParams P)
     }
     __syncthreads();
 
-    const int la = tid / TB, lb = tid - la * TB;
+    const int la = tid >> 5, lane = tid & 31, sp = lane / TB, lb = lane - sp * TB;
     const int a = a_base + la, bb = b_base + lb;
-    if (a >= P.mx || bb >= P.my) return;
-    float acc = 0.0f;
+    float part[M];                                 // independent partial sums: no serial FMA chain
+#pragma unroll
+    for (int j = 0; j < M; ++j) part[j] = 0.0f;
     for (int tx = 0; tx < NT; ++tx) {
         const int ty0 = ty_s[2 * tx], ty1 = ty_s[2 * tx + 1];
         // forward used node a = a0 + (tx-T)  ->  source block a0 = a - (tx-T); local block la + 2T - tx
-        const float *vrow = v_s + (M * (la + 2 * T - tx)) * VW;
+        const float *vrow = v_s + (M * (la + 2 * T - tx) + sp * ROWS) * VW;
         for (int ty = ty0; ty <= ty1; ++ty) {
             const float *vt = vrow + M * (lb + 2 * T - ty);
-            const float *wt = w_s + (tx * NT + ty) * (M * M);
+            float wt[ROWS * M];
+            lds_vec<ROWS * M>(w_s + (tx * NT + ty) * (M * M) + sp * ROWS * M, wt);
 #pragma unroll
-            for (int i = 0; i < M; ++i)
+            for (int i = 0; i < ROWS; ++i) {
+                float vv[M];
+                lds_vec<M>(vt + i * VW, vv);
 #pragma unroll
-                for (int j = 0; j < M; ++j) acc = fmaf(wt[i * M + j], vt[i * VW + j], acc);
+                for (int j = 0; j < M; ++j) part[j] = fmaf(wt[i * M + j], vv[j], part[j]);
+            }
         }
     }
-    P.dC[((size_t)b * P.mx + a) * P.my + bb] = acc;
+    float acc = 0.0f;
+#pragma unroll
+    for (int j = 0; j < M; ++j) acc += part[j];
+#pragma unroll
+    for (int off = TB; off < 32; off <<= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
+    if (sp == 0 && a < P.mx && bb < P.my) P.dC[((size_t)b * P.mx + a) * P.my + bb] = acc;
 }
 
 }  // namespace epsgrad

@@ -16,9 +16,11 @@ struct FwdParams {
     const float *phi;      // [B,px,py]
     float *eps;            // [B,3,nx,ny,nz] or nullptr
     float *eps2d;          // [B,3,nx,ny] or nullptr (stage tap)
-    const float *zw;       // [2][nz]: wxy_k, wz_k (overlaps of the z footprints with the slab)
+    const float *zw;       // [7][nz] z tables (epsgrad.cu): wxy, wz, z-full, z-lower-face, z-upper-face indicators,
+                           //          eps_clad (1 - wxy), eps_clad [wz == 0]
     int nx, ny, nz, px, py, s;
     float beta, eta_r, eps_clad, deps, delta;
+    float w_lo, w_hi;      // fractional z-face weights of eps_zz (0 if that face cell is absent)
 };
 
 constexpr int FWD_TI = 16, FWD_TJ = 16, FWD_THREADS = 256;
@@ -27,16 +29,17 @@ __host__ __device__ inline size_t fwd_smem_floats(int s, int nz)
 {
     const int CI = FWD_TI + 2, CJ = FWD_TJ + 2;
     const int MP = s * CI + s / 2, MQ = s * CJ + s / 2;
-    return (size_t)2 * MP * MQ + 4 * CI * CJ + 3 * FWD_TI * FWD_TJ + 2 * (size_t)nz;
+    return (size_t)2 * MP * MQ + 4 * CI * CJ + 5 * FWD_TI * FWD_TJ + 7 * (size_t)nz;
 }
 
-// grid (ceil(ny/TJ), ceil(nx/TI), B)
+// grid (ceil(ny/TJ), ceil(nx/TI), B).  S > 0: compile-time subpixel count (index divisions fold to shifts); S = 0: runtime P.s.
+template <int S>
 __global__ void __launch_bounds__(FWD_THREADS) k_forward(const FwdParams P)
 {
     extern __shared__ __align__(16) float sm[];
     constexpr int TI = FWD_TI, TJ = FWD_TJ, NTH = FWD_THREADS;
     constexpr int CI = TI + 2, CJ = TJ + 2;
-    const int s = P.s, hs = s >> 1;
+    const int s = S > 0 ? S : P.s, hs = s >> 1;
     const int MP = s * CI + hs, MQ = s * CJ + hs;
     float *e_s = sm;
     float *r_s = e_s + MP * MQ;
@@ -44,15 +47,15 @@ __global__ void __launch_bounds__(FWD_THREADS) k_forward(const FwdParams P)
     float *Hx = Ax + CI * CJ;
     float *Ay = Hx + CI * CJ;
     float *Hy = Ay + CI * CJ;
-    float *e2 = Hy + CI * CJ;          // [3][TI*TJ]
-    float *zw = e2 + 3 * TI * TJ;      // [2][nz]
+    float *e2 = Hy + CI * CJ;          // [5][TI*TJ]: eps2d_x, eps2d_y, eps2d_z, eps_zz on the lower / upper face cell
+    float *zw = e2 + 5 * TI * TJ;      // [7][nz]
 
     const int tid = threadIdx.x;
     const int i0 = blockIdx.y * TI, j0 = blockIdx.x * TJ, b = blockIdx.z;
     const int nx = P.nx, ny = P.ny, nz = P.nz;
     const float inv_s2 = 1.0f / (float)(s * s);
 
-    for (int k = tid; k < 2 * nz; k += NTH) zw[k] = P.zw[k];
+    for (int k = tid; k < 7 * nz; k += NTH) zw[k] = P.zw[k];
 
     // ---- stage 1: mask tile (replicate outside the region, S5): e and r = 1/e
     {
@@ -63,7 +66,7 @@ __global__ void __launch_bounds__(FWD_THREADS) k_forward(const FwdParams P)
             const int p = clampi(p_base + lp, 0, P.px - 1), q = clampi(q_base + lq, 0, P.py - 1);
             const float e = project_mix(phib[(size_t)p * P.py + q], P.beta, P.eta_r, P.eps_clad, P.deps);
             e_s[i] = e;
-            r_s[i] = 1.0f / e;
+            r_s[i] = __frcp_rn(e);
         }
     }
     __syncthreads();
@@ -108,9 +111,9 @@ __global__ void __launch_bounds__(FWD_THREADS) k_forward(const FwdParams P)
                 }
             gx *= inv_deps; gy *= inv_deps;
             const float gc = c == 0 ? gx : gy;
-            const float n2 = gc * gc / (gx * gx + gy * gy + P.delta);
+            const float n2 = gc * gc * __frcp_rn(gx * gx + gy * gy + P.delta);
             const int ic = (ii + 1) * CJ + jj + 1;
-            out[c] = 1.0f / (n2 * H[ic] + (1.0f - n2) / A[ic]);
+            out[c] = __frcp_rn(n2 * H[ic] + (1.0f - n2) * __frcp_rn(A[ic]));
         }
         {
             float az = 0.f;
@@ -124,34 +127,68 @@ __global__ void __launch_bounds__(FWD_THREADS) k_forward(const FwdParams P)
             e2[c * TI * TJ + it] = out[c];
             if (P.eps2d) P.eps2d[(((size_t)b * 3 + c) * nx + i) * ny + j] = out[c];
         }
+        // Eq. (7) with n = z_hat on the (at most two) fractional face cells of E_z (S7): once per column
+        const float inv_ec = 1.0f / P.eps_clad;
+        const float rz = __frcp_rn(out[2]);
+        e2[3 * TI * TJ + it] = P.w_lo > 0.f ? __frcp_rn(P.w_lo * rz + (1.0f - P.w_lo) * inv_ec) : 0.f;
+        e2[4 * TI * TJ + it] = P.w_hi > 0.f ? __frcp_rn(P.w_hi * rz + (1.0f - P.w_hi) * inv_ec) : 0.f;
     }
     if (!P.eps) return;
     __syncthreads();
 
-    // ---- stage 4: z-extrusion, 16-byte streaming stores; a (c,i) row of the tile is contiguous
+    // ---- stage 4: z-extrusion, 16-byte streaming stores.  Every output is affine in the staged per-column values:
+    //   eps_cc[k] = eps_clad (1 - wxy_k) + wxy_k eps2d_c          (c = x, y)
+    //   eps_zz[k] = eps_clad [wz_k = 0] + [wz_k = 1] eps2d_z + [k = lower face] v_lo + [k = upper face] v_hi
     const int TIv = min(TI, nx - i0), TJv = min(TJ, ny - j0);
-    const int nz4 = nz >> 2, n4 = TJv * nz4;
-    const float ec = P.eps_clad, inv_ec = 1.0f / P.eps_clad;
-    for (int r = 0; r < 3 * TIv; ++r) {
-        const int c = r / TIv, ii = r - c * TIv;
-        float4 *dst = reinterpret_cast<float4 *>(P.eps + ((((size_t)b * 3 + c) * nx + i0 + ii) * ny + j0) * nz);
-        const float *vrow = e2 + c * TI * TJ + ii * TJ;
-        for (int f = tid; f < n4; f += NTH) {
-            const int jj = f / nz4, k = (f - jj * nz4) << 2;
-            const float v = vrow[jj];
-            float o[4];
-            if (c < 2) {
-                const float dv = v - ec;
+    const int nz4 = nz >> 2;
+    const float *w_xy = zw, *b_xy = zw + 5 * nz, *b_z = zw + 6 * nz, *i_f = zw + 2 * nz, *i_l = zw + 3 * nz, *i_h = zw + 4 * nz;
+    if (NTH % nz4 == 0) {
+        // a thread keeps its 4 z cells for the whole tile: weights live in registers
+        const int kc = tid % nz4, k = kc << 2, cstep = NTH / nz4;
+        float wx[4], bx[4], bz[4], zf[4], zl[4], zh[4];
 #pragma unroll
-                for (int x = 0; x < 4; ++x) o[x] = fmaf(zw[k + x], dv, ec);
-            } else {
-#pragma unroll
-                for (int x = 0; x < 4; ++x) {
-                    const float w = zw[nz + k + x];
-                    o[x] = w == 0.0f ? ec : (w == 1.0f ? v : 1.0f / (w / v + (1.0f - w) * inv_ec));
+        for (int x = 0; x < 4; ++x) {
+            wx[x] = w_xy[k + x]; bx[x] = b_xy[k + x]; bz[x] = b_z[k + x];
+            zf[x] = i_f[k + x]; zl[x] = i_l[k + x]; zh[x] = i_h[k + x];
+        }
+        for (int c = 0; c < 3; ++c) {
+            float *base = P.eps + ((((size_t)b * 3 + c) * nx + i0) * ny + j0) * nz + k;   // tile-relative offsets fit 32 bits
+            const float *vc = e2 + c * TI * TJ;
+            const int row_stride = ny * nz;
+            for (int cell = tid / nz4; cell < TIv * TJ; cell += cstep) {
+                const int ii = cell / TJ, jj = cell - ii * TJ;
+                if (jj >= TJv) continue;
+                const float v = vc[cell];
+                float4 o;
+                if (c < 2) {
+                    o.x = fmaf(wx[0], v, bx[0]); o.y = fmaf(wx[1], v, bx[1]);
+                    o.z = fmaf(wx[2], v, bx[2]); o.w = fmaf(wx[3], v, bx[3]);
+                } else {
+                    const float vl = e2[3 * TI * TJ + cell], vh = e2[4 * TI * TJ + cell];
+                    o.x = fmaf(zf[0], v, fmaf(zl[0], vl, fmaf(zh[0], vh, bz[0])));
+                    o.y = fmaf(zf[1], v, fmaf(zl[1], vl, fmaf(zh[1], vh, bz[1])));
+                    o.z = fmaf(zf[2], v, fmaf(zl[2], vl, fmaf(zh[2], vh, bz[2])));
+                    o.w = fmaf(zf[3], v, fmaf(zl[3], vl, fmaf(zh[3], vh, bz[3])));
                 }
+                __stcs(reinterpret_cast<float4 *>(base + (ii * row_stride + jj * nz)), o);
             }
-            __stcs(dst + f, make_float4(o[0], o[1], o[2], o[3]));
+        }
+    } else {
+        for (int c = 0; c < 3; ++c) {
+            float *base = P.eps + ((((size_t)b * 3 + c) * nx + i0) * ny + j0) * nz;
+            const float *vc = e2 + c * TI * TJ;
+            for (int f = tid; f < TIv * TJ * nz4; f += NTH) {
+                const int cell = f / nz4, k = (f - cell * nz4) << 2;
+                const int ii = cell / TJ, jj = cell - ii * TJ;
+                if (jj >= TJv) continue;
+                const float v = vc[cell], vl = e2[3 * TI * TJ + cell], vh = e2[4 * TI * TJ + cell];
+                float o[4];
+#pragma unroll
+                for (int x = 0; x < 4; ++x)
+                    o[x] = c < 2 ? fmaf(w_xy[k + x], v, b_xy[k + x])
+                                 : fmaf(i_f[k + x], v, fmaf(i_l[k + x], vl, fmaf(i_h[k + x], vh, b_z[k + x])));
+                __stcs(reinterpret_cast<float4 *>(base + ((size_t)ii * ny + jj) * nz + k), make_float4(o[0], o[1], o[2], o[3]));
+            }
         }
     }
 }

@@ -34,22 +34,23 @@ constexpr int REV_CI = REV_TI + 5, REV_CJ = REV_TJ + 5;
 __host__ __device__ inline size_t rev_smem_floats(int s)
 {
     const int MP = s * REV_CI + s / 2, MQ = s * REV_CJ + s / 2;
-    return (size_t)2 * MP * MQ + 14 * REV_CI * REV_CJ + REV_TI * REV_TJ;
+    return (size_t)2 * MP * MQ + 14 * REV_CI * REV_CJ + REV_TI * REV_TJ + (size_t)s * (REV_TI + REV_TJ);
 }
 
 // d eps_zz / d eps2d_z on a face cell of weight w:  w (eps_zz/v)^2, eps_zz/v = 1/(w + (1-w) v/eps_clad)
 __device__ __forceinline__ float face_factor(float w, float v, float inv_ec)
 {
-    const float f = 1.0f / (w + (1.0f - w) * v * inv_ec);
+    const float f = __frcp_rn(w + (1.0f - w) * v * inv_ec);
     return w * f * f;
 }
 
-// grid (ceil(ny/TJ), ceil(nx/TI), B)
+// grid (ceil(ny/TJ), ceil(nx/TI), B).  S > 0: compile-time subpixel count; S = 0: runtime P.s.
+template <int S>
 __global__ void __launch_bounds__(REV_THREADS) k_reverse2d(const Rev2dParams P)
 {
     extern __shared__ __align__(16) float sm[];
     constexpr int TI = REV_TI, TJ = REV_TJ, NTH = REV_THREADS, CI = REV_CI, CJ = REV_CJ, NC = CI * CJ;
-    const int s = P.s, hs = s >> 1;
+    const int s = S > 0 ? S : P.s, hs = s >> 1;
     const int MP = s * CI + hs, MQ = s * CJ + hs;
     float *e_s = sm;
     float *r_s = e_s + MP * MQ;
@@ -61,6 +62,7 @@ __global__ void __launch_bounds__(REV_THREADS) k_reverse2d(const Rev2dParams P)
         ptr += 7 * NC;
     }
     float *AbZ = ptr;                  // [TI*TJ]
+    int *nidx = reinterpret_cast<int *>(AbZ + TI * TJ);   // normaliser table row of each tile mask row, then column of each mask column
 
     const int tid = threadIdx.x;
     const int i0 = blockIdx.y * TI, j0 = blockIdx.x * TJ, b = blockIdx.z;
@@ -70,6 +72,11 @@ __global__ void __launch_bounds__(REV_THREADS) k_reverse2d(const Rev2dParams P)
     const float *phib = P.phi + (size_t)b * P.px * P.py;
     const float *gb = P.gbar + (size_t)b * 5 * ncol;
 
+    for (int k = tid; k < s * (TI + TJ); k += NTH) {
+        const int along_x = k < s * TI;
+        const int pix = along_x ? s * i0 + k : s * j0 + (k - s * TI);
+        nidx[k] = along_x ? P.nrm.ix_of(min(pix, P.px - 1)) : P.nrm.iy_of(min(pix, P.py - 1));
+    }
     // ---- A: mask tile e, r (replicate)
     {
         const int p_base = s * oi, q_base = s * oj;
@@ -78,7 +85,7 @@ __global__ void __launch_bounds__(REV_THREADS) k_reverse2d(const Rev2dParams P)
             const int p = clampi(p_base + lp, 0, P.px - 1), q = clampi(q_base + lq, 0, P.py - 1);
             const float e = project_mix(phib[(size_t)p * P.py + q], P.beta, P.eta_r, P.eps_clad, P.deps);
             e_s[i] = e;
-            r_s[i] = 1.0f / e;
+            r_s[i] = __frcp_rn(e);
         }
     }
     __syncthreads();
@@ -101,71 +108,91 @@ __global__ void __launch_bounds__(REV_THREADS) k_reverse2d(const Rev2dParams P)
     __syncthreads();
 
     // ---- C: R2 + first half of R3 on the 2-cell ring: Hbar, Abar, gxbar, gybar per component
-    for (int it = tid; it < 2 * NC; it += NTH) {
-        const int c = it / NC, i_ = it - c * NC;
-        const int ci = i_ / CJ, cj = i_ - ci * CJ;
-        const int i = oi + ci, j = oj + cj;
-        float hb = 0.f, ab = 0.f, gxb = 0.f, gyb = 0.f;
-        if (ci >= 1 && ci <= TI + 3 && cj >= 1 && cj <= TJ + 3 && i >= 0 && i < nx && j >= 0 && j < ny) {
-            const float *Ac = A[c];
-            float gx = 0.f, gy = 0.f;
+    {
+        constexpr int RI = TI + 3, RJ = TJ + 3;           // cells ci in [1, TI+3], cj in [1, TJ+3]
+        for (int it = tid; it < 2 * RI * RJ; it += NTH) {
+            const int c = it / (RI * RJ), rem = it - c * (RI * RJ);
+            const int ci = 1 + rem / RJ, cj = 1 + rem % RJ, i_ = ci * CJ + cj;
+            const int i = oi + ci, j = oj + cj;
+            float hb = 0.f, ab = 0.f, gxb = 0.f, gyb = 0.f;
+            if (i >= 0 && i < nx && j >= 0 && j < ny) {
+                const float *Ac = A[c];
+                float gx = 0.f, gy = 0.f;
 #pragma unroll
-            for (int di = -1; di <= 1; ++di)
+                for (int di = -1; di <= 1; ++di)
 #pragma unroll
-                for (int dj = -1; dj <= 1; ++dj) {
-                    const int ni = clampi(i + di, 0, nx - 1) - oi, nj = clampi(j + dj, 0, ny - 1) - oj;
-                    const float d = Ac[ni * CJ + nj];
-                    gx = fmaf((float)(di * (2 - (dj < 0 ? -dj : dj))) * 0.125f, d, gx);
-                    gy = fmaf((float)(dj * (2 - (di < 0 ? -di : di))) * 0.125f, d, gy);
-                }
-            gx *= inv_deps; gy *= inv_deps;
-            const float gc = c == 0 ? gx : gy, go = c == 0 ? gy : gx;
-            const float S = gc * gc + go * go + P.delta;
-            const float n2 = gc * gc / S;
-            const float a = Ac[i_], h = H[c][i_];
-            const float q = n2 * h + (1.0f - n2) / a;
-            const float G = gb[(size_t)c * ncol + (size_t)i * ny + j];
-            const float qbar = -G / (q * q);
-            hb = n2 * qbar;
-            ab = -(1.0f - n2) * qbar / (a * a);
-            const float n2bar = (h - 1.0f / a) * qbar;
-            const float k2 = 2.0f * n2bar * gc / (S * S);
-            const float gcb = k2 * (go * go + P.delta), gob = -k2 * gc * go;
-            gxb = c == 0 ? gcb : gob;
-            gyb = c == 0 ? gob : gcb;
+                    for (int dj = -1; dj <= 1; ++dj) {
+                        const int ni = clampi(i + di, 0, nx - 1) - oi, nj = clampi(j + dj, 0, ny - 1) - oj;
+                        const float d = Ac[ni * CJ + nj];
+                        gx = fmaf((float)(di * (2 - (dj < 0 ? -dj : dj))) * 0.125f, d, gx);
+                        gy = fmaf((float)(dj * (2 - (di < 0 ? -di : di))) * 0.125f, d, gy);
+                    }
+                gx *= inv_deps; gy *= inv_deps;
+                const float gc = c == 0 ? gx : gy, go = c == 0 ? gy : gx;
+                const float rS = __frcp_rn(gc * gc + go * go + P.delta);
+                const float n2 = gc * gc * rS;
+                const float ra = __frcp_rn(Ac[i_]), h = H[c][i_];
+                const float e2d = __frcp_rn(n2 * h + (1.0f - n2) * ra);       // eps2d_c = 1/q
+                const float G = gb[(size_t)c * ncol + (size_t)i * ny + j];
+                const float qbar = -G * e2d * e2d;
+                hb = n2 * qbar;
+                ab = -(1.0f - n2) * qbar * ra * ra;
+                const float n2bar = (h - ra) * qbar;
+                const float k2 = 2.0f * n2bar * gc * rS * rS;
+                const float gcb = k2 * (go * go + P.delta), gob = -k2 * gc * go;
+                gxb = c == 0 ? gcb : gob;
+                gyb = c == 0 ? gob : gcb;
+            }
+            Hb[c][i_] = hb; Ab[c][i_] = ab; Gx[c][i_] = gxb; Gy[c][i_] = gyb;
         }
-        Hb[c][i_] = hb; Ab[c][i_] = ab; Gx[c][i_] = gxb; Gy[c][i_] = gyb;
     }
     __syncthreads();
 
     // ---- D: Sobel^T with the replicate padding folded back (second half of R3); z component
-    for (int it = tid; it < 2 * NC; it += NTH) {
-        const int c = it / NC, i_ = it - c * NC;
-        const int ci = i_ / CJ, cj = i_ - ci * CJ;
-        const int ii = oi + ci, jj = oj + cj;
-        float out = 0.f;
-        if (ci >= 2 && ci <= TI + 2 && cj >= 2 && cj <= TJ + 2 && ii >= 0 && ii < nx && jj >= 0 && jj < ny) {
-            float dbar = 0.f;
-            // sources (i,di) with clamp(i+di) == ii: i = ii-di in range, plus the folded border terms
-            for (int cx = 0; cx < 5; ++cx) {
-                int di, i;
-                if (cx < 3) { di = cx - 1; i = ii - di; if (i < 0 || i >= nx) continue; }
-                else if (cx == 3) { if (ii != 0) continue; di = -1; i = 0; }
-                else { if (ii != nx - 1) continue; di = 1; i = nx - 1; }
-                for (int cy = 0; cy < 5; ++cy) {
-                    int dj, j;
-                    if (cy < 3) { dj = cy - 1; j = jj - dj; if (j < 0 || j >= ny) continue; }
-                    else if (cy == 3) { if (jj != 0) continue; dj = -1; j = 0; }
-                    else { if (jj != ny - 1) continue; dj = 1; j = ny - 1; }
-                    const int src = (i - oi) * CJ + (j - oj);
-                    const float kx = (float)(di * (2 - (dj < 0 ? -dj : dj))) * 0.125f;
-                    const float ky = (float)(dj * (2 - (di < 0 ? -di : di))) * 0.125f;
-                    dbar = fmaf(kx, Gx[c][src], fmaf(ky, Gy[c][src], dbar));
+    {
+        constexpr int RI = TI + 1, RJ = TJ + 1;           // cells ci in [2, TI+2], cj in [2, TJ+2]
+        for (int it = tid; it < 2 * RI * RJ; it += NTH) {
+            const int c = it / (RI * RJ), rem = it - c * (RI * RJ);
+            const int ci = 2 + rem / RJ, cj = 2 + rem % RJ, i_ = ci * CJ + cj;
+            const int ii = oi + ci, jj = oj + cj;
+            float out = 0.f;
+            if (ii >= 0 && ii < nx && jj >= 0 && jj < ny) {
+                float dbar = 0.f;
+                const float *gxs = Gx[c], *gys = Gy[c];
+                if (ii >= 1 && ii <= nx - 2 && jj >= 1 && jj <= ny - 2) {
+                    // interior: the cell (ii-di, jj-dj) reached (ii,jj) through its stencil entry (di,dj)
+#pragma unroll
+                    for (int di = -1; di <= 1; ++di)
+#pragma unroll
+                        for (int dj = -1; dj <= 1; ++dj) {
+                            const int src = i_ - di * CJ - dj;
+                            const float kx = (float)(di * (2 - (dj < 0 ? -dj : dj))) * 0.125f;
+                            const float ky = (float)(dj * (2 - (di < 0 ? -di : di))) * 0.125f;
+                            dbar = fmaf(kx, gxs[src], fmaf(ky, gys[src], dbar));
+                        }
+                } else {
+                    // border: sources (i,di) with clamp(i+di) == ii: i = ii-di in range, plus the folded terms
+                    for (int cx = 0; cx < 5; ++cx) {
+                        int di, i;
+                        if (cx < 3) { di = cx - 1; i = ii - di; if (i < 0 || i >= nx) continue; }
+                        else if (cx == 3) { if (ii != 0) continue; di = -1; i = 0; }
+                        else { if (ii != nx - 1) continue; di = 1; i = nx - 1; }
+                        for (int cy = 0; cy < 5; ++cy) {
+                            int dj, j;
+                            if (cy < 3) { dj = cy - 1; j = jj - dj; if (j < 0 || j >= ny) continue; }
+                            else if (cy == 3) { if (jj != 0) continue; dj = -1; j = 0; }
+                            else { if (jj != ny - 1) continue; dj = 1; j = ny - 1; }
+                            const int src = (i - oi) * CJ + (j - oj);
+                            const float kx = (float)(di * (2 - (dj < 0 ? -dj : dj))) * 0.125f;
+                            const float ky = (float)(dj * (2 - (di < 0 ? -di : di))) * 0.125f;
+                            dbar = fmaf(kx, gxs[src], fmaf(ky, gys[src], dbar));
+                        }
+                    }
                 }
+                out = Ab[c][i_] + dbar * inv_deps;
             }
-            out = Ab[c][i_] + dbar * inv_deps;
+            AbF[c][i_] = out;
         }
-        AbF[c][i_] = out;
     }
     for (int it = tid; it < TI * TJ; it += NTH) {
         const int ti = it / TJ, tj = it - ti * TJ;
@@ -209,10 +236,10 @@ __global__ void __launch_bounds__(REV_THREADS) k_reverse2d(const Rev2dParams P)
             ebar = fmaf(mlt, AbF[1][idx], ebar);
             rbar = fmaf(mlt, Hb[1][idx], rbar);
         }
-        const float e = e_s[(tp + 3 * s) * MQ + tq + 3 * s];
-        const float rhobar = P.deps * inv_s2 * (ebar - rbar / (e * e));
+        const float r = r_s[(tp + 3 * s) * MQ + tq + 3 * s];           // 1/e
+        const float rhobar = P.deps * inv_s2 * (ebar - rbar * r * r);
         const float slope = project_slope(phib[(size_t)p * P.py + q], P.beta, P.eta_r);
-        vb[(size_t)p * P.py + q] = rhobar * slope * P.nrm.at(p, q);
+        vb[(size_t)p * P.py + q] = rhobar * slope * P.nrm.at_index(nidx[tp], nidx[TP + tq]);
     }
 }
 

@@ -9,13 +9,16 @@
 // Only the 16-byte chunks (2 complex64 cells) of a z column that hold slab cells are read
 // ("|Omega_D"; d eps/dC = 0 elsewhere); `dense` plans read every chunk.  L lanes
 // (a power of two) share a column and reduce with xor-shuffles; each thread keeps
-// ZR_UNROLL columns in flight so that 2*ZR_UNROLL 16-byte loads are issued before use.
+// ZR_UNROLL columns in flight so that 2*ZR_UNROLL 16-byte loads are issued before use.  Consecutive
+// lane groups take consecutive columns, so one warp instruction covers 32/L neighbouring columns.
+// SPARSE windows (<= 128 B of a column) use 64-byte L2 fills (common.cuh ld_stream).
 #pragma once
 #include "common.cuh"
 
 namespace epsgrad {
 
-constexpr int ZR_THREADS = 256, ZR_UNROLL = 4, ZR_MAX_PAIRS = 8;
+constexpr int ZR_THREADS = 256, ZR_MAX_PAIRS = 8;
+constexpr int ZR_UNROLL_SPARSE = 2, ZR_UNROLL_DENSE = 4;   // columns in flight per thread (swept on B200: profiles/r1b_notes.md)
 
 struct ZredParams {
     const float4 *ef[ZR_MAX_PAIRS];
@@ -28,7 +31,8 @@ struct ZredParams {
 };
 
 // grid (blocks over columns, 3*B)
-__global__ void __launch_bounds__(ZR_THREADS) k_zreduce(const ZredParams P)
+template <int ZR_UNROLL, bool SPARSE>
+__global__ void __launch_bounds__(ZR_THREADS, 4) k_zreduce(const ZredParams P)
 {
     const int c = blockIdx.y % 3, b = blockIdx.y / 3;
     const int grp = c == 2;
@@ -38,10 +42,13 @@ __global__ void __launch_bounds__(ZR_THREADS) k_zreduce(const ZredParams P)
     const int nzc = P.nz >> 1;                       // chunks per column
     const size_t plane = ((size_t)b * 3 + c) * P.ncol;
 
-    int col[ZR_UNROLL];
+    // thread's columns: colbase + u*GPB (consecutive lane groups take consecutive columns)
+    const int colbase = blockIdx.x * (ZR_UNROLL * GPB) + g;
+    if (colbase - g >= P.ncol) return;               // whole block past the end (uniform)
+    bool live[ZR_UNROLL];
 #pragma unroll
-    for (int u = 0; u < ZR_UNROLL; ++u) col[u] = (blockIdx.x * ZR_UNROLL + u) * GPB + g;
-    if (col[0] - g >= P.ncol) return;                // whole block past the end (uniform)
+    for (int u = 0; u < ZR_UNROLL; ++u) live[u] = colbase + u * GPB < P.ncol;
+    const int ustride = GPB * nzc;                   // float4 stride between a thread's columns
 
     float acc[ZR_UNROLL][3];
 #pragma unroll
@@ -57,14 +64,15 @@ __global__ void __launch_bounds__(ZR_THREADS) k_zreduce(const ZredParams P)
 #pragma unroll
             for (int o = 0; o < 3; ++o) { w[o][0] = P.zw[(2 + o) * P.nz + k]; w[o][1] = P.zw[(2 + o) * P.nz + k + 1]; }
         }
+        const size_t off0 = (plane + colbase) * nzc + ch0 + ch;
         for (int p = 0; p < P.n_pairs; ++p) {
+            const float4 *pf = P.ef[p] + off0, *pa = P.ea[p] + off0;
             float4 f[ZR_UNROLL], a[ZR_UNROLL];
 #pragma unroll
             for (int u = 0; u < ZR_UNROLL; ++u) {
-                if (col[u] < P.ncol) {
-                    const size_t idx = (plane + col[u]) * nzc + ch0 + ch;
-                    f[u] = ld_stream(P.ef[p] + idx);
-                    a[u] = ld_stream(P.ea[p] + idx);
+                if (live[u]) {
+                    f[u] = ld_stream<SPARSE>(pf + u * ustride);
+                    a[u] = ld_stream<SPARSE>(pa + u * ustride);
                 } else {
                     f[u] = make_float4(0.f, 0.f, 0.f, 0.f);
                     a[u] = f[u];
@@ -93,9 +101,9 @@ __global__ void __launch_bounds__(ZR_THREADS) k_zreduce(const ZredParams P)
     if (l != 0) return;
 #pragma unroll
     for (int u = 0; u < ZR_UNROLL; ++u) {
-        if (col[u] >= P.ncol) continue;
+        if (!live[u]) continue;
         for (int o = 0; o < nout; ++o) {
-            float *dst = P.gbar + ((size_t)b * 5 + (grp ? 2 + o : c)) * P.ncol + col[u];
+            float *dst = P.gbar + ((size_t)b * 5 + (grp ? 2 + o : c)) * P.ncol + colbase + u * GPB;
             *dst = P.accumulate ? *dst + acc[u][o] : acc[u][o];
         }
     }
