@@ -100,6 +100,19 @@ int    epsgrad_plan_set_staging(epsgrad_plan_t *plan, void *dev_ptr, size_t byte
  * are identical; this is a measurement switch.                                           */
 int epsgrad_plan_set_dense_reads(epsgrad_plan_t *plan, int dense);
 
+/* Fused HBM streams (default on): eps_forward_vjp runs the forward tile kernel (eps writes) and
+ * the Eq. (1) z-reduction (field reads) as ONE launch whose CTAs interleave both roles, so reads
+ * and writes overlap.  0 = separate launches.  Per-kernel profiling always uses separate launches. */
+int epsgrad_plan_set_fused_streams(epsgrad_plan_t *plan, int enable);
+
+/* Two-stream schedule (default off; an alternative to the fused launch).  The Eq. (1) field stream does not depend on the filter, so
+ * calls that compute dF/dC fork the plan's auxiliary stream from `stream` (event), run
+ * zreduce -> reverse2d -> filterT there while filter -> forward run on `stream`, and join it back
+ * (event) before returning: to the caller everything is still ordered on `stream`, with no host
+ * synchronisation, and the calls remain CUDA-graph capturable.  0 = one stream, strictly serial
+ * (also used while per-kernel profiling is on).                                              */
+int epsgrad_plan_set_overlap(epsgrad_plan_t *plan, int enable);
+
 /* Number of kernel launches the last eps_* call of this plan enqueued (for accounting). */
 int epsgrad_plan_last_launches(const epsgrad_plan_t *plan);
 

@@ -40,15 +40,24 @@ __device__ __forceinline__ float4 ld_stream(const float4 *p)
     return r;
 }
 
+// 1/x on the special-function unit (MUFU.RCP, <= 1 ulp; 1/inf = 0).  The 2-D chain needs ~1e-7
+// relative accuracy (tolerances 1e-5 / 1e-4), not IEEE rounding.
+__device__ __forceinline__ float fast_rcp(float x)
+{
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
 // Projection + mixing rule of one mask pixel (Eq. (3)/(6) P:L54,L74):
 //   t = beta (Phi - eta), rho = (1 + tanh t)/2 = 1/(1 + exp(-2t)), e = eps_clad + (eps_core - eps_clad) rho.
 // phi_c is the centred filter output Phi - eta0; eta_r = eta - eta0.  exp(-2t) -> +inf gives rho = 0,
 // -> 0 gives rho = 1: no NaN.  |d rho| <= rho (1-rho) * relerr(exp) < 1e-7 with the ex2.approx path
-// (DESIGN.md 6.2); the reciprocal is correctly rounded.
+// (DESIGN.md 6.2).
 __device__ __forceinline__ float project_mix(float phi_c, float beta, float eta_r, float eps_clad, float deps)
 {
     const float t = beta * (phi_c - eta_r);
-    const float rho = __frcp_rn(1.0f + __expf(-2.0f * t));
+    const float rho = fast_rcp(1.0f + __expf(-2.0f * t));
     return fmaf(deps, rho, eps_clad);
 }
 
@@ -58,7 +67,7 @@ __device__ __forceinline__ float project_slope(float phi_c, float beta, float et
 {
     const float t = beta * (phi_c - eta_r);
     const float a = __expf(-2.0f * fabsf(t));
-    const float d = __frcp_rn(1.0f + a);
+    const float d = fast_rcp(1.0f + a);
     return 2.0f * beta * a * d * d;
 }
 

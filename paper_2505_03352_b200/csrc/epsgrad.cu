@@ -10,10 +10,12 @@
 
 #include "common.cuh"
 #include "filter.cuh"
+#include "filter4.cuh"
 #include "filter_sep.cuh"
 #include "forward.cuh"
 #include "reverse2d.cuh"
 #include "zreduce.cuh"
+#include "stream.cuh"
 
 using namespace epsgrad;
 
@@ -48,6 +50,10 @@ struct epsgrad_plan {
     // optional per-kernel timing (epsgrad_plan_set_profiling)
     int prof;
     cudaEvent_t ev[EPSGRAD_MAX_KERNELS + 1];
+    // two-stream overlap of the field stream (zreduce -> reverse2d -> filterT) with filter -> forward
+    int overlap, fuse_streams;
+    cudaStream_t aux;
+    cudaEvent_t ev_fork, ev_filter, ev_join;
     const char *kname[EPSGRAD_MAX_KERNELS];
 };
 
@@ -261,6 +267,21 @@ extern "C" int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsg
         return EPSGRAD_ECUDA;
     }
 
+    // ---- auxiliary stream and fork/join events (no timing) for the two-stream schedule
+    {
+        int prev2 = 0;
+        cudaGetDevice(&prev2);
+        cudaSetDevice(device);
+        bool ok = cudaStreamCreateWithFlags(&P->aux, cudaStreamNonBlocking) == cudaSuccess &&
+                  cudaEventCreateWithFlags(&P->ev_fork, cudaEventDisableTiming) == cudaSuccess &&
+                  cudaEventCreateWithFlags(&P->ev_filter, cudaEventDisableTiming) == cudaSuccess &&
+                  cudaEventCreateWithFlags(&P->ev_join, cudaEventDisableTiming) == cudaSuccess;
+        cudaSetDevice(prev2);
+        if (!ok) { cudaGetLastError(); epsgrad_plan_destroy(P); return EPSGRAD_ECUDA; }
+        P->overlap = 0;
+        P->fuse_streams = 1;
+    }
+
     // ---- workspace carve-up
     const size_t n_mask = (size_t)cfg->batch * P->px * P->py, n_cell = (size_t)cfg->batch * P->nx * P->ny;
     size_t off = 0;
@@ -277,6 +298,10 @@ extern "C" int epsgrad_plan_destroy(epsgrad_plan_t *P)
 {
     if (!P) return EPSGRAD_EINVAL;
     if (P->d_tables) cudaFree(P->d_tables);
+    if (P->aux) cudaStreamDestroy(P->aux);
+    if (P->ev_fork) cudaEventDestroy(P->ev_fork);
+    if (P->ev_filter) cudaEventDestroy(P->ev_filter);
+    if (P->ev_join) cudaEventDestroy(P->ev_join);
     if (P->ev[0])
         for (int i = 0; i <= EPSGRAD_MAX_KERNELS; ++i) cudaEventDestroy(P->ev[i]);
     delete P;
@@ -348,6 +373,20 @@ extern "C" int epsgrad_plan_set_dense_reads(epsgrad_plan_t *P, int dense)
 {
     if (!P) return EPSGRAD_EINVAL;
     P->dense = dense != 0;
+    return EPSGRAD_OK;
+}
+
+extern "C" int epsgrad_plan_set_overlap(epsgrad_plan_t *P, int enable)
+{
+    if (!P) return EPSGRAD_EINVAL;
+    P->overlap = enable != 0;
+    return EPSGRAD_OK;
+}
+
+extern "C" int epsgrad_plan_set_fused_streams(epsgrad_plan_t *P, int enable)
+{
+    if (!P) return EPSGRAD_EINVAL;
+    P->fuse_streams = enable != 0;
     return EPSGRAD_OK;
 }
 
@@ -431,6 +470,14 @@ int launch_filter_m(epsgrad_plan *P, const float *C, float *phi, cudaStream_t st
         FilterParams fp;
         fp.C = C; fp.phi = phi; fp.w = P->d_w; fp.tyrange = P->d_tyrange; fp.nrm = make_nrm(P);
         fp.mx = mx; fp.my = my; fp.px = P->px; fp.py = P->py; fp.T = T; fp.NT = NT; fp.eta0 = P->eta0;
+        if (M == 4 && (NT == 5 || NT == 9 || NT == 13)) {      // fast path (filter4.cuh)
+            auto kern = NT == 5 ? k_filter_conic4<5> : (NT == 9 ? k_filter_conic4<9> : k_filter_conic4<13>);
+            const size_t smem4 = filter4_smem_floats(NT) * 4;
+            int rc4 = set_smem(kern, smem4);
+            if (rc4) return rc4;
+            kern<<<dim3(cdiv(my, F4_TB), cdiv(mx, F4_TA), B), F4_THREADS, smem4, st>>>(fp);
+            return check_launch(P, "filter", st);
+        }
         const size_t smem = ((size_t)NT * NT * M * M + (size_t)(TA + 2 * T) * (TB + 2 * T + 1) + 2 * NT) * 4;
         if (smem > 200 * 1024) return EPSGRAD_EUNSUPPORTED;
         int rc = set_smem(k_filter_conic<M, TA, TB>, smem);
@@ -469,6 +516,14 @@ int launch_filterT_conic(epsgrad_plan *P, const float *v, float *dC, cudaStream_
     FilterTParams fp;
     fp.v = v; fp.dC = dC; fp.w = P->d_w; fp.tyrange = P->d_tyrange;
     fp.mx = P->cfg.mx; fp.my = P->cfg.my; fp.px = P->px; fp.py = P->py; fp.T = T; fp.NT = NT;
+    if (M == 4 && (NT == 5 || NT == 9 || NT == 13)) {          // fast path (filter4.cuh)
+        auto kern = NT == 5 ? k_filterT_conic4<5> : (NT == 9 ? k_filterT_conic4<9> : k_filterT_conic4<13>);
+        const size_t smem4 = filterT4_smem_floats(NT) * 4;
+        int rc4 = set_smem(kern, smem4);
+        if (rc4) return rc4;
+        kern<<<dim3(cdiv(fp.my, F4_TB), cdiv(fp.mx, F4_TA), P->cfg.batch), F4_THREADS, smem4, st>>>(fp);
+        return check_launch(P, "filterT", st);
+    }
     const size_t smem = ((size_t)NT * NT * M * M + (size_t)M * (S::TA + 2 * T) * M * (S::TB + 2 * T) + 2 * NT) * 4;
     if (smem > 200 * 1024) return EPSGRAD_EUNSUPPORTED;
     int rc = set_smem(k_filterT_conic<M>, smem);
@@ -529,13 +584,73 @@ int launch_filterT(epsgrad_plan *P, const float *v, float *dC, cudaStream_t st)
 }
 
 // ---- F2..F6
-int launch_forward(epsgrad_plan *P, const float *phi, float beta, float *eps, float *eps2d, cudaStream_t st)
+FwdParams make_fwd(const epsgrad_plan *P, const float *phi, float beta, float *eps, float *eps2d)
 {
     FwdParams fp;
     fp.phi = phi; fp.eps = eps; fp.eps2d = eps2d; fp.zw = P->d_zw;
     fp.nx = P->nx; fp.ny = P->ny; fp.nz = P->cfg.nz; fp.px = P->px; fp.py = P->py; fp.s = P->cfg.subpixel;
     fp.beta = beta; fp.eta_r = P->eta_r; fp.eps_clad = P->eps_clad; fp.deps = P->deps; fp.delta = P->delta;
     fp.w_lo = P->w_lo; fp.w_hi = P->w_hi;
+    return fp;
+}
+
+// z windows, lanes per column, load flavour and block counts of the z-reduction
+struct ZredShape { bool sparse; int unroll; int nb[2]; };
+ZredShape make_zred(const epsgrad_plan *P, ZredParams &zp, float *gbar)
+{
+    zp.gbar = gbar; zp.zw = P->d_zw; zp.ncol = P->nx * P->ny; zp.nz = P->cfg.nz;
+    int maxnch = 1;
+    for (int g = 0; g < 2; ++g) {
+        zp.ch0[g] = P->dense ? 0 : P->ch0[g];
+        zp.nch[g] = P->dense ? P->cfg.nz / 2 : P->nch[g];
+        int L = 1;
+        while (L < zp.nch[g]) L <<= 1;
+        if (L > 32) L = 32;
+        zp.L[g] = L;
+        if (zp.nch[g] > maxnch) maxnch = zp.nch[g];
+    }
+    ZredShape zs;
+    // windows of at most 128 bytes per column: ask for 64-byte fills and keep fewer columns in flight
+    zs.sparse = maxnch * 16 <= 128 && zp.nz * 8 > 128;
+    zs.unroll = zs.sparse ? ZR_UNROLL_SPARSE : ZR_UNROLL_DENSE;
+    for (int g = 0; g < 2; ++g) zs.nb[g] = cdiv(zp.ncol, (ZR_THREADS / zp.L[g]) * zs.unroll);
+    return zs;
+}
+
+void set_pairs(ZredParams &zp, int np, const void *const *EF, const void *const *EA, int accumulate)
+{
+    for (int p = 0; p < ZR_MAX_PAIRS; ++p) {
+        zp.ef[p] = (const float4 *)(p < np ? EF[p] : nullptr);
+        zp.ea[p] = (const float4 *)(p < np ? EA[p] : nullptr);
+    }
+    zp.n_pairs = np; zp.accumulate = accumulate;
+}
+
+// ---- F2..F6 and R1 in one launch (stream.cuh); n_pairs <= ZR_MAX_PAIRS
+int launch_stream(epsgrad_plan *P, const float *phi, float beta, float *eps, int n_pairs,
+                  const void *const *EF, const void *const *EA, float *gbar, cudaStream_t st)
+{
+    StreamParams sp;
+    sp.F = make_fwd(P, phi, beta, eps, nullptr);
+    const ZredShape zs = make_zred(P, sp.Z, gbar);
+    set_pairs(sp.Z, n_pairs, EF, EA, 0);
+    sp.fx = cdiv(P->ny, FWD_TJ); sp.fy = cdiv(P->nx, FWD_TI); sp.nf = sp.fx * sp.fy * P->cfg.batch;
+    sp.nbz[0] = zs.nb[0]; sp.nbz[1] = zs.nb[1];
+    sp.nz_blocks = P->cfg.batch * (2 * zs.nb[0] + zs.nb[1]);
+    const size_t smem = fwd_smem_floats(sp.F.s, sp.F.nz) * 4;
+    const int s = sp.F.s;
+    void (*kern)(const StreamParams);
+    if (zs.sparse) kern = s == 2 ? k_stream<2, ZR_UNROLL_SPARSE, true> : (s == 4 ? k_stream<4, ZR_UNROLL_SPARSE, true> : k_stream<0, ZR_UNROLL_SPARSE, true>);
+    else kern = s == 2 ? k_stream<2, ZR_UNROLL_DENSE, false> : (s == 4 ? k_stream<4, ZR_UNROLL_DENSE, false> : k_stream<0, ZR_UNROLL_DENSE, false>);
+    int rc = set_smem(kern, smem);
+    if (rc) return rc;
+    kern<<<sp.nf + sp.nz_blocks, FWD_THREADS, smem, st>>>(sp);
+    return check_launch(P, "stream", st);
+}
+
+int launch_forward(epsgrad_plan *P, const float *phi, float beta, float *eps, float *eps2d, cudaStream_t st)
+{
+    const FwdParams fp = make_fwd(P, phi, beta, eps, eps2d);
     const size_t smem = fwd_smem_floats(fp.s, fp.nz) * 4;
     auto kern = fp.s == 2 ? k_forward<2> : (fp.s == 4 ? k_forward<4> : k_forward<0>);
     int rc = set_smem(kern, smem);
@@ -545,38 +660,16 @@ int launch_forward(epsgrad_plan *P, const float *phi, float beta, float *eps, fl
 }
 
 // ---- R1
-int next_pow2(int x) { int p = 1; while (p < x) p <<= 1; return p; }
-
-int launch_zreduce(epsgrad_plan *P, int n_pairs, const void *const *EF, const void *const *EA, float *gbar, cudaStream_t st)
+int launch_zreduce(epsgrad_plan *P, int n_pairs, const void *const *EF, const void *const *EA, float *gbar,
+                   cudaStream_t st, int first_accumulates = 0)
 {
     ZredParams zp;
-    zp.gbar = gbar; zp.zw = P->d_zw; zp.ncol = P->nx * P->ny; zp.nz = P->cfg.nz;
-    int maxnch = 1;
-    for (int g = 0; g < 2; ++g) {
-        zp.ch0[g] = P->dense ? 0 : P->ch0[g];
-        zp.nch[g] = P->dense ? P->cfg.nz / 2 : P->nch[g];
-        int L = next_pow2(zp.nch[g] < 1 ? 1 : zp.nch[g]);
-        if (L > 32) L = 32;
-        zp.L[g] = L;
-        if (zp.nch[g] > maxnch) maxnch = zp.nch[g];
-    }
-    // windows of at most 128 bytes per column: ask for 64-byte fills and keep fewer columns in flight
-    const bool sparse = maxnch * 16 <= 128 && zp.nz * 8 > 128;
-    const int unroll = sparse ? ZR_UNROLL_SPARSE : ZR_UNROLL_DENSE;
-    int maxblocks = 1;
-    for (int g = 0; g < 2; ++g) {
-        const int nb = cdiv(zp.ncol, (ZR_THREADS / zp.L[g]) * unroll);
-        if (nb > maxblocks) maxblocks = nb;
-    }
+    const ZredShape zs = make_zred(P, zp, gbar);
+    const dim3 grid(zs.nb[0] > zs.nb[1] ? zs.nb[0] : zs.nb[1], 3 * P->cfg.batch);
     for (int p0 = 0; p0 < n_pairs; p0 += ZR_MAX_PAIRS) {
         const int np = n_pairs - p0 < ZR_MAX_PAIRS ? n_pairs - p0 : ZR_MAX_PAIRS;
-        for (int p = 0; p < ZR_MAX_PAIRS; ++p) {
-            zp.ef[p] = (const float4 *)(p < np ? EF[p0 + p] : nullptr);
-            zp.ea[p] = (const float4 *)(p < np ? EA[p0 + p] : nullptr);
-        }
-        zp.n_pairs = np; zp.accumulate = p0 > 0;
-        const dim3 grid(maxblocks, 3 * P->cfg.batch);
-        if (sparse) k_zreduce<ZR_UNROLL_SPARSE, true><<<grid, ZR_THREADS, 0, st>>>(zp);
+        set_pairs(zp, np, EF + p0, EA + p0, p0 > 0 || first_accumulates);
+        if (zs.sparse) k_zreduce<ZR_UNROLL_SPARSE, true><<<grid, ZR_THREADS, 0, st>>>(zp);
         else k_zreduce<ZR_UNROLL_DENSE, false><<<grid, ZR_THREADS, 0, st>>>(zp);
         int rc = check_launch(P, "zreduce", st);
         if (rc) return rc;
@@ -623,12 +716,50 @@ struct DeviceGuard {
     ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
 };
 
-int run_vjp(epsgrad_plan *P, float beta, int n_pairs, const void *const *EF, const void *const *EA,
-            float *dFdC, cudaStream_t st)
+// The whole path.  eps == nullptr skips F2-F6, dFdC == nullptr skips R1-R6.
+// Dependencies: forward <- filter;  reverse2d <- filter, zreduce;  filterT <- reverse2d.  zreduce
+// depends on nothing, so with overlap on (and a reverse pass requested) it starts at once on the
+// plan's auxiliary stream, the 2-D reverse chain follows it there, and filter -> forward run on the
+// caller's stream; the call joins the auxiliary stream back before returning (no host sync).
+int run_chain(epsgrad_plan *P, const float *C, float beta, int n_pairs, const void *const *EF,
+              const void *const *EA, float *eps, float *dFdC, cudaStream_t st)
 {
-    int rc = launch_zreduce(P, n_pairs, EF, EA, ws_gbar(P), st);
-    if (!rc) rc = launch_reverse2d(P, ws_phi(P), beta, ws_gbar(P), ws_v(P), st);
-    if (!rc) rc = launch_filterT(P, ws_v(P), dFdC, st);
+    int rc = EPSGRAD_OK;
+    if (eps && dFdC && P->fuse_streams && !P->prof) {
+        // filter -> [forward + zreduce in one launch] -> reverse2d -> filterT; pairs beyond the
+        // first ZR_MAX_PAIRS are accumulated by plain zreduce launches
+        const int np0 = n_pairs < ZR_MAX_PAIRS ? n_pairs : ZR_MAX_PAIRS;
+        rc = launch_filter(P, C, ws_phi(P), st);
+        if (!rc) rc = launch_stream(P, ws_phi(P), beta, eps, np0, EF, EA, ws_gbar(P), st);
+        if (!rc && n_pairs > np0) rc = launch_zreduce(P, n_pairs - np0, EF + np0, EA + np0, ws_gbar(P), st, 1);
+        if (!rc) rc = launch_reverse2d(P, ws_phi(P), beta, ws_gbar(P), ws_v(P), st);
+        if (!rc) rc = launch_filterT(P, ws_v(P), dFdC, st);
+        return rc;
+    }
+    if (!dFdC || !P->overlap || P->prof) {
+        rc = launch_filter(P, C, ws_phi(P), st);
+        if (!rc && eps) rc = launch_forward(P, ws_phi(P), beta, eps, nullptr, st);
+        if (!rc && dFdC) rc = launch_zreduce(P, n_pairs, EF, EA, ws_gbar(P), st);
+        if (!rc && dFdC) rc = launch_reverse2d(P, ws_phi(P), beta, ws_gbar(P), ws_v(P), st);
+        if (!rc && dFdC) rc = launch_filterT(P, ws_v(P), dFdC, st);
+        return rc;
+    }
+    cudaStream_t ax = P->aux;
+    if (cudaEventRecord(P->ev_fork, st) != cudaSuccess || cudaStreamWaitEvent(ax, P->ev_fork, 0) != cudaSuccess) {
+        cudaGetLastError();
+        return EPSGRAD_ECUDA;
+    }
+    rc = launch_zreduce(P, n_pairs, EF, EA, ws_gbar(P), ax);
+    if (!rc) rc = launch_filter(P, C, ws_phi(P), st);
+    if (!rc && (cudaEventRecord(P->ev_filter, st) != cudaSuccess || cudaStreamWaitEvent(ax, P->ev_filter, 0) != cudaSuccess)) rc = EPSGRAD_ECUDA;
+    if (!rc) rc = launch_reverse2d(P, ws_phi(P), beta, ws_gbar(P), ws_v(P), ax);
+    if (!rc) rc = launch_filterT(P, ws_v(P), dFdC, ax);
+    if (!rc && eps) rc = launch_forward(P, ws_phi(P), beta, eps, nullptr, st);
+    // always join, even on error, so that the auxiliary stream never outlives the call
+    if (cudaEventRecord(P->ev_join, ax) != cudaSuccess || cudaStreamWaitEvent(st, P->ev_join, 0) != cudaSuccess) {
+        cudaGetLastError();
+        if (!rc) rc = EPSGRAD_ECUDA;
+    }
     return rc;
 }
 
@@ -643,9 +774,7 @@ extern "C" int eps_forward(epsgrad_plan_t *P, const float *C, float beta, float 
     DeviceGuard g(P->device);
     cudaStream_t st = (cudaStream_t)stream;
     begin_call(P, st);
-    rc = launch_filter(P, C, ws_phi(P), st);
-    if (!rc) rc = launch_forward(P, ws_phi(P), beta, eps, nullptr, st);
-    return rc;
+    return run_chain(P, C, beta, 0, nullptr, nullptr, eps, nullptr, st);
 }
 
 extern "C" int eps_vjp(epsgrad_plan_t *P, const float *C, float beta, int n_pairs,
@@ -658,9 +787,7 @@ extern "C" int eps_vjp(epsgrad_plan_t *P, const float *C, float beta, int n_pair
     DeviceGuard g(P->device);
     cudaStream_t st = (cudaStream_t)stream;
     begin_call(P, st);
-    rc = launch_filter(P, C, ws_phi(P), st);
-    if (!rc) rc = run_vjp(P, beta, n_pairs, EF, EA, dFdC, st);
-    return rc;
+    return run_chain(P, C, beta, n_pairs, EF, EA, nullptr, dFdC, st);
 }
 
 extern "C" int eps_forward_vjp(epsgrad_plan_t *P, const float *C, float beta, int n_pairs,
@@ -674,10 +801,7 @@ extern "C" int eps_forward_vjp(epsgrad_plan_t *P, const float *C, float beta, in
     DeviceGuard g(P->device);
     cudaStream_t st = (cudaStream_t)stream;
     begin_call(P, st);
-    rc = launch_filter(P, C, ws_phi(P), st);
-    if (!rc) rc = launch_forward(P, ws_phi(P), beta, eps, nullptr, st);
-    if (!rc) rc = run_vjp(P, beta, n_pairs, EF, EA, dFdC, st);
-    return rc;
+    return run_chain(P, C, beta, n_pairs, EF, EA, eps, dFdC, st);
 }
 
 // ------------------------------------------------------------------------------------ host buffers
@@ -717,9 +841,7 @@ extern "C" int eps_forward_vjp_host(epsgrad_plan_t *P, const float *C_host, floa
         P->last_h2d += 2 * b_f;
     }
     if (!ok) { cudaGetLastError(); return EPSGRAD_ECUDA; }
-    int rc = launch_filter(P, dC, ws_phi(P), st);
-    if (!rc && eps_host) rc = launch_forward(P, ws_phi(P), beta, dE, nullptr, st);
-    if (!rc && dFdC_host) rc = run_vjp(P, beta, n_pairs, ef.data(), ea.data(), dG, st);
+    int rc = run_chain(P, dC, beta, n_pairs, ef.data(), ea.data(), eps_host ? dE : nullptr, dFdC_host ? dG : nullptr, st);
     if (rc) return rc;
     if (eps_host) {
         ok = ok && cudaMemcpyAsync(eps_host, dE, b_e, cudaMemcpyDeviceToHost, st) == cudaSuccess;

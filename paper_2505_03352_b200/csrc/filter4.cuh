@@ -1,0 +1,175 @@
+// filter4.cuh -- fast paths of the conic polyphase stencil (filter.cuh) for m = u*s = 4 and a
+// compile-time tap count NTC = 2T+1 in {5, 9, 13} (R = 4, 8, 12 cells at u = 2).
+//
+// Both directions use the same decomposition:
+//   - 4 lanes per group of NB = 4 neighbouring control pixels along y; lane `sp` owns phase row
+//     fx = sp of those pixels (4 phase columns fy), so 16 (forward) / 16 (reverse) independent
+//     accumulators per lane and 4x the warps of a thread-per-pixel mapping;
+//   - per tap row tx the lane first pulls the NTC weight vectors W[tx][*][sp][0..3] into registers
+//     (warp-wide that is one 64-byte broadcast each), then sweeps the NTC+3 source columns, each
+//     loaded value feeding up to NB outputs:  shared-memory wavefronts per FMA drop from 1.25
+//     (reverse) / 0.31 (forward) to 0.40 / 0.15 -- the earlier kernels were shared-memory bound
+//     (profiles/r1b_ncu_full_summary.md).
+// Forward reads c' (control resolution, scalar, conflict-free); reverse reads the v tile staged with
+// one padding block after every 4 (block c at float offset 4(c + c/4)): lanes of a quarter-warp then
+// hit 8 distinct 16-byte bank groups.
+#pragma once
+#include "filter.cuh"
+
+namespace epsgrad {
+
+constexpr int F4_NB = 4, F4_TA = 4, F4_TB = 8 * F4_NB, F4_THREADS = 32 * F4_TA;
+
+__host__ __device__ inline size_t filter4_smem_floats(int NT)
+{
+    const int T = (NT - 1) / 2;
+    return (size_t)NT * NT * 16 + (size_t)(F4_TA + 2 * T) * (F4_TB + 2 * T + 1);
+}
+
+// grid (ceil(my/32), ceil(mx/4), B), 128 threads: warp <-> control row la, lane = sp*8 + lb
+template <int NTC>
+__global__ void __launch_bounds__(F4_THREADS) k_filter_conic4(const FilterParams P)
+{
+    constexpr int T = (NTC - 1) / 2, TA = F4_TA, TB = F4_TB, NB = F4_NB, CW = TB + 2 * T + 1;
+    extern __shared__ __align__(16) float sm[];
+    float *w_s = sm;                               // [NTC][NTC][4][4]
+    float *c_s = w_s + NTC * NTC * 16;             // [(TA+2T)][CW]
+    const int tid = threadIdx.x;
+    const int a_base = blockIdx.y * TA, b_base = blockIdx.x * TB, b = blockIdx.z;
+
+    for (int i = tid; i < NTC * NTC * 4; i += F4_THREADS)
+        reinterpret_cast<float4 *>(w_s)[i] = reinterpret_cast<const float4 *>(P.w)[i];
+    const float *Cb = P.C + (size_t)b * P.mx * P.my;
+    for (int r = tid >> 5; r < TA + 2 * T; r += F4_THREADS / 32) {
+        const int a = a_base - T + r;
+        for (int c = tid & 31; c < TB + 2 * T; c += 32) {
+            const int bb = b_base - T + c;
+            float v = 0.0f;
+            if (a >= 0 && a < P.mx && bb >= 0 && bb < P.my) v = Cb[(size_t)a * P.my + bb] - P.eta0;
+            c_s[r * CW + c] = v;
+        }
+    }
+    __syncthreads();
+
+    const int la = tid >> 5, lane = tid & 31, sp = lane >> 3, lb = lane & 7;
+    float acc[NB][4];
+#pragma unroll
+    for (int jb = 0; jb < NB; ++jb)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[jb][j] = 0.0f;
+
+#pragma unroll 1
+    for (int tx = 0; tx < NTC; ++tx) {
+        float wr[NTC][4];
+#pragma unroll
+        for (int ty = 0; ty < NTC; ++ty) lds_vec<4>(w_s + ((tx * NTC + ty) * 4 + sp) * 4, wr[ty]);
+        const float *crow = c_s + (la + tx) * CW + NB * lb;
+#pragma unroll
+        for (int k = 0; k < NTC + NB - 1; ++k) {       // source column b0 + jb + ty - T, k = jb + ty
+            const float cv = crow[k];
+#pragma unroll
+            for (int jb = 0; jb < NB; ++jb) {
+                const int ty = k - jb;
+                if (ty >= 0 && ty < NTC) {
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) acc[jb][j] = fmaf(wr[ty][j], cv, acc[jb][j]);
+                }
+            }
+        }
+    }
+    const int a0 = a_base + la;
+    if (a0 >= P.mx) return;
+    const int p = 4 * a0 + sp, nix = P.nrm.ix(a0, sp);
+    float *row = P.phi + ((size_t)b * P.px + p) * P.py;
+#pragma unroll
+    for (int jb = 0; jb < NB; ++jb) {
+        const int b0 = b_base + NB * lb + jb;
+        if (b0 >= P.my) continue;
+        const int niy = P.nrm.iy(b0, 0);
+        float4 o;
+        o.x = acc[jb][0] * P.nrm.at_index(nix, niy);
+        o.y = acc[jb][1] * P.nrm.at_index(nix, niy + 1);
+        o.z = acc[jb][2] * P.nrm.at_index(nix, niy + 2);
+        o.w = acc[jb][3] * P.nrm.at_index(nix, niy + 3);
+        *reinterpret_cast<float4 *>(row + 4 * b0) = o;
+    }
+}
+
+// ---------------------------------------------------------------- transpose
+__host__ __device__ inline int filterT4_pitch(int T) { const int nb = F4_TB + 2 * T; return 4 * (nb + (nb + 3) / 4); }
+__host__ __device__ inline size_t filterT4_smem_floats(int NT)
+{
+    const int T = (NT - 1) / 2;
+    return (size_t)NT * NT * 16 + (size_t)4 * (F4_TA + 2 * T) * filterT4_pitch(T);
+}
+
+// grid (ceil(my/32), ceil(mx/4), B), 128 threads
+template <int NTC>
+__global__ void __launch_bounds__(F4_THREADS) k_filterT_conic4(const FilterTParams P)
+{
+    constexpr int T = (NTC - 1) / 2, TA = F4_TA, TB = F4_TB, NB = F4_NB;
+    constexpr int VH = 4 * (TA + 2 * T), VB = TB + 2 * T;       // v tile: rows, blocks of 4 floats per row
+    extern __shared__ __align__(16) float sm[];
+    const int pitch = filterT4_pitch(T);
+    float *w_s = sm;                               // [NTC][NTC][4][4]
+    float *v_s = w_s + NTC * NTC * 16;             // [VH][pitch], block c at 4(c + c/4)
+    const int tid = threadIdx.x;
+    const int a_base = blockIdx.y * TA, b_base = blockIdx.x * TB, b = blockIdx.z;
+
+    for (int i = tid; i < NTC * NTC * 4; i += F4_THREADS)
+        reinterpret_cast<float4 *>(w_s)[i] = reinterpret_cast<const float4 *>(P.w)[i];
+    const float *vb = P.v + (size_t)b * P.px * P.py;
+    const int p_base = 4 * (a_base - T), q_base = 4 * (b_base - T);
+    for (int r = tid >> 5; r < VH; r += F4_THREADS / 32) {
+        const int p = p_base + r;
+        const bool rin = p >= 0 && p < P.px;
+        for (int c = tid & 31; c < VB; c += 32) {
+            const int q = q_base + 4 * c;
+            float4 x = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (rin && q >= 0 && q < P.py) x = *reinterpret_cast<const float4 *>(vb + (size_t)p * P.py + q);
+            *reinterpret_cast<float4 *>(v_s + r * pitch + 4 * (c + (c >> 2))) = x;
+        }
+    }
+    __syncthreads();
+
+    const int la = tid >> 5, lane = tid & 31, sp = lane >> 3, lb = lane & 7;
+    float acc[NB][4];
+#pragma unroll
+    for (int jb = 0; jb < NB; ++jb)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[jb][j] = 0.0f;
+
+#pragma unroll 1
+    for (int tx = 0; tx < NTC; ++tx) {
+        float wr[NTC][4];
+#pragma unroll
+        for (int ty = 0; ty < NTC; ++ty) lds_vec<4>(w_s + ((tx * NTC + ty) * 4 + sp) * 4, wr[ty]);
+        // forward used node a = a0 + (tx-T): source block row a - (tx-T), local la + 2T - tx; phase row sp
+        const float *vrow = v_s + (4 * (la + 2 * T - tx) + sp) * pitch;
+#pragma unroll
+        for (int k = 0; k < NTC + NB - 1; ++k) {       // source block column NB*lb + k;  k = jb + 2T - ty
+            const int c = NB * lb + k;
+            float vv[4];
+            lds_vec<4>(vrow + 4 * (c + (c >> 2)), vv);
+#pragma unroll
+            for (int jb = 0; jb < NB; ++jb) {
+                const int ty = jb + 2 * T - k;
+                if (ty >= 0 && ty < NTC) {
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) acc[jb][j] = fmaf(wr[ty][j], vv[j], acc[jb][j]);
+                }
+            }
+        }
+    }
+    const int a = a_base + la;
+#pragma unroll
+    for (int jb = 0; jb < NB; ++jb) {
+        float s = (acc[jb][0] + acc[jb][1]) + (acc[jb][2] + acc[jb][3]);
+        s += __shfl_xor_sync(0xffffffffu, s, 8);
+        s += __shfl_xor_sync(0xffffffffu, s, 16);
+        const int bb = b_base + NB * lb + jb;
+        if (sp == 0 && a < P.mx && bb < P.my) P.dC[((size_t)b * P.mx + a) * P.my + bb] = s;
+    }
+}
+
+}  // namespace epsgrad

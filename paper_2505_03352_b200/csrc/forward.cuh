@@ -32,11 +32,11 @@ __host__ __device__ inline size_t fwd_smem_floats(int s, int nz)
     return (size_t)2 * MP * MQ + 4 * CI * CJ + 5 * FWD_TI * FWD_TJ + 7 * (size_t)nz;
 }
 
-// grid (ceil(ny/TJ), ceil(nx/TI), B).  S > 0: compile-time subpixel count (index divisions fold to shifts); S = 0: runtime P.s.
+// One tile (bx, by) of design bz.  S > 0: compile-time subpixel count (index divisions fold to shifts);
+// S = 0: runtime P.s.  sm: fwd_smem_floats(s, nz) floats of shared memory.
 template <int S>
-__global__ void __launch_bounds__(FWD_THREADS) k_forward(const FwdParams P)
+__device__ __forceinline__ void forward_tile(const FwdParams &P, float *sm, int bx, int by, int bz)
 {
-    extern __shared__ __align__(16) float sm[];
     constexpr int TI = FWD_TI, TJ = FWD_TJ, NTH = FWD_THREADS;
     constexpr int CI = TI + 2, CJ = TJ + 2;
     const int s = S > 0 ? S : P.s, hs = s >> 1;
@@ -51,7 +51,7 @@ __global__ void __launch_bounds__(FWD_THREADS) k_forward(const FwdParams P)
     float *zw = e2 + 5 * TI * TJ;      // [7][nz]
 
     const int tid = threadIdx.x;
-    const int i0 = blockIdx.y * TI, j0 = blockIdx.x * TJ, b = blockIdx.z;
+    const int i0 = by * TI, j0 = bx * TJ, b = bz;
     const int nx = P.nx, ny = P.ny, nz = P.nz;
     const float inv_s2 = 1.0f / (float)(s * s);
 
@@ -64,9 +64,9 @@ __global__ void __launch_bounds__(FWD_THREADS) k_forward(const FwdParams P)
         for (int i = tid; i < MP * MQ; i += NTH) {
             const int lp = i / MQ, lq = i - lp * MQ;
             const int p = clampi(p_base + lp, 0, P.px - 1), q = clampi(q_base + lq, 0, P.py - 1);
-            const float e = project_mix(phib[(size_t)p * P.py + q], P.beta, P.eta_r, P.eps_clad, P.deps);
+            const float e = project_mix(phib[p * P.py + q], P.beta, P.eta_r, P.eps_clad, P.deps);
             e_s[i] = e;
-            r_s[i] = __frcp_rn(e);
+            r_s[i] = fast_rcp(e);
         }
     }
     __syncthreads();
@@ -90,6 +90,7 @@ __global__ void __launch_bounds__(FWD_THREADS) k_forward(const FwdParams P)
 
     // ---- stage 3: Sobel normals of D_c = (A_c - eps_clad)/deps, Eq. (7); eps2d_z = <e>_z
     const float inv_deps = 1.0f / P.deps;
+    const bool inner = i0 >= 1 && j0 >= 1 && i0 + TI <= nx - 1 && j0 + TJ <= ny - 1;   // 1-cell ring inside the region
     for (int it = tid; it < TI * TJ; it += NTH) {
         const int ii = it / TJ, jj = it - ii * TJ;
         const int i = i0 + ii, j = j0 + jj;
@@ -98,22 +99,31 @@ __global__ void __launch_bounds__(FWD_THREADS) k_forward(const FwdParams P)
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
             const float *A = c == 0 ? Ax : Ay, *H = c == 0 ? Hx : Hy;
-            float gx = 0.f, gy = 0.f;
+            float gx, gy;
+            if (inner) {
+                const float *q1 = A + (ii + 1) * CJ + jj + 1, *q0 = q1 - CJ, *q2 = q1 + CJ;
+                const float a00 = q0[-1], a01 = q0[0], a02 = q0[1], a10 = q1[-1], a12 = q1[1];
+                const float a20 = q2[-1], a21 = q2[0], a22 = q2[1];
+                gx = ((a20 - a00) + 2.0f * (a21 - a01) + (a22 - a02)) * 0.125f;
+                gy = ((a02 - a00) + 2.0f * (a12 - a10) + (a22 - a20)) * 0.125f;
+            } else {
+                gx = 0.f; gy = 0.f;
 #pragma unroll
-            for (int di = -1; di <= 1; ++di)
+                for (int di = -1; di <= 1; ++di)
 #pragma unroll
-                for (int dj = -1; dj <= 1; ++dj) {
-                    const int ni = clampi(i + di, 0, nx - 1) - (i0 - 1);
-                    const int nj = clampi(j + dj, 0, ny - 1) - (j0 - 1);
-                    const float d = A[ni * CJ + nj];
-                    gx = fmaf((float)(di * (2 - (dj < 0 ? -dj : dj))) * 0.125f, d, gx);
-                    gy = fmaf((float)(dj * (2 - (di < 0 ? -di : di))) * 0.125f, d, gy);
-                }
+                    for (int dj = -1; dj <= 1; ++dj) {
+                        const int ni = clampi(i + di, 0, nx - 1) - (i0 - 1);
+                        const int nj = clampi(j + dj, 0, ny - 1) - (j0 - 1);
+                        const float d = A[ni * CJ + nj];
+                        gx = fmaf((float)(di * (2 - (dj < 0 ? -dj : dj))) * 0.125f, d, gx);
+                        gy = fmaf((float)(dj * (2 - (di < 0 ? -di : di))) * 0.125f, d, gy);
+                    }
+            }
             gx *= inv_deps; gy *= inv_deps;
             const float gc = c == 0 ? gx : gy;
-            const float n2 = gc * gc * __frcp_rn(gx * gx + gy * gy + P.delta);
+            const float n2 = gc * gc * fast_rcp(gx * gx + gy * gy + P.delta);
             const int ic = (ii + 1) * CJ + jj + 1;
-            out[c] = __frcp_rn(n2 * H[ic] + (1.0f - n2) * __frcp_rn(A[ic]));
+            out[c] = fast_rcp(n2 * H[ic] + (1.0f - n2) * fast_rcp(A[ic]));
         }
         {
             float az = 0.f;
@@ -129,9 +139,9 @@ __global__ void __launch_bounds__(FWD_THREADS) k_forward(const FwdParams P)
         }
         // Eq. (7) with n = z_hat on the (at most two) fractional face cells of E_z (S7): once per column
         const float inv_ec = 1.0f / P.eps_clad;
-        const float rz = __frcp_rn(out[2]);
-        e2[3 * TI * TJ + it] = P.w_lo > 0.f ? __frcp_rn(P.w_lo * rz + (1.0f - P.w_lo) * inv_ec) : 0.f;
-        e2[4 * TI * TJ + it] = P.w_hi > 0.f ? __frcp_rn(P.w_hi * rz + (1.0f - P.w_hi) * inv_ec) : 0.f;
+        const float rz = fast_rcp(out[2]);
+        e2[3 * TI * TJ + it] = P.w_lo > 0.f ? fast_rcp(P.w_lo * rz + (1.0f - P.w_lo) * inv_ec) : 0.f;
+        e2[4 * TI * TJ + it] = P.w_hi > 0.f ? fast_rcp(P.w_hi * rz + (1.0f - P.w_hi) * inv_ec) : 0.f;
     }
     if (!P.eps) return;
     __syncthreads();
@@ -191,6 +201,14 @@ __global__ void __launch_bounds__(FWD_THREADS) k_forward(const FwdParams P)
             }
         }
     }
+}
+
+// grid (ceil(ny/TJ), ceil(nx/TI), B)
+template <int S>
+__global__ void __launch_bounds__(FWD_THREADS) k_forward(const FwdParams P)
+{
+    extern __shared__ __align__(16) float sm[];
+    forward_tile<S>(P, sm, blockIdx.x, blockIdx.y, blockIdx.z);
 }
 
 }  // namespace epsgrad

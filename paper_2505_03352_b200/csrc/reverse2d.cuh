@@ -40,7 +40,7 @@ __host__ __device__ inline size_t rev_smem_floats(int s)
 // d eps_zz / d eps2d_z on a face cell of weight w:  w (eps_zz/v)^2, eps_zz/v = 1/(w + (1-w) v/eps_clad)
 __device__ __forceinline__ float face_factor(float w, float v, float inv_ec)
 {
-    const float f = __frcp_rn(w + (1.0f - w) * v * inv_ec);
+    const float f = fast_rcp(w + (1.0f - w) * v * inv_ec);
     return w * f * f;
 }
 
@@ -71,6 +71,8 @@ __global__ void __launch_bounds__(REV_THREADS) k_reverse2d(const Rev2dParams P)
     const float inv_s2 = 1.0f / (float)(s * s), inv_deps = 1.0f / P.deps, inv_ec = 1.0f / P.eps_clad;
     const float *phib = P.phi + (size_t)b * P.px * P.py;
     const float *gb = P.gbar + (size_t)b * 5 * ncol;
+    // tile whose 3-cell ring lies inside the region: no clamping, no folded border terms (block-uniform)
+    const bool inner = i0 >= 3 && j0 >= 3 && i0 + TI + 2 <= nx - 1 && j0 + TJ + 2 <= ny - 1;
 
     for (int k = tid; k < s * (TI + TJ); k += NTH) {
         const int along_x = k < s * TI;
@@ -83,9 +85,9 @@ __global__ void __launch_bounds__(REV_THREADS) k_reverse2d(const Rev2dParams P)
         for (int i = tid; i < MP * MQ; i += NTH) {
             const int lp = i / MQ, lq = i - lp * MQ;
             const int p = clampi(p_base + lp, 0, P.px - 1), q = clampi(q_base + lq, 0, P.py - 1);
-            const float e = project_mix(phib[(size_t)p * P.py + q], P.beta, P.eta_r, P.eps_clad, P.deps);
+            const float e = project_mix(phib[p * P.py + q], P.beta, P.eta_r, P.eps_clad, P.deps);
             e_s[i] = e;
-            r_s[i] = __frcp_rn(e);
+            r_s[i] = fast_rcp(e);
         }
     }
     __syncthreads();
@@ -115,25 +117,34 @@ __global__ void __launch_bounds__(REV_THREADS) k_reverse2d(const Rev2dParams P)
             const int ci = 1 + rem / RJ, cj = 1 + rem % RJ, i_ = ci * CJ + cj;
             const int i = oi + ci, j = oj + cj;
             float hb = 0.f, ab = 0.f, gxb = 0.f, gyb = 0.f;
-            if (i >= 0 && i < nx && j >= 0 && j < ny) {
+            if (inner || (i >= 0 && i < nx && j >= 0 && j < ny)) {
                 const float *Ac = A[c];
-                float gx = 0.f, gy = 0.f;
+                float gx, gy;
+                if (inner) {
+                    const float *q0 = Ac + i_ - CJ, *q1 = Ac + i_, *q2 = Ac + i_ + CJ;
+                    const float a00 = q0[-1], a01 = q0[0], a02 = q0[1], a10 = q1[-1], a12 = q1[1];
+                    const float a20 = q2[-1], a21 = q2[0], a22 = q2[1];
+                    gx = ((a20 - a00) + 2.0f * (a21 - a01) + (a22 - a02)) * 0.125f;
+                    gy = ((a02 - a00) + 2.0f * (a12 - a10) + (a22 - a20)) * 0.125f;
+                } else {
+                    gx = 0.f; gy = 0.f;
 #pragma unroll
-                for (int di = -1; di <= 1; ++di)
+                    for (int di = -1; di <= 1; ++di)
 #pragma unroll
-                    for (int dj = -1; dj <= 1; ++dj) {
-                        const int ni = clampi(i + di, 0, nx - 1) - oi, nj = clampi(j + dj, 0, ny - 1) - oj;
-                        const float d = Ac[ni * CJ + nj];
-                        gx = fmaf((float)(di * (2 - (dj < 0 ? -dj : dj))) * 0.125f, d, gx);
-                        gy = fmaf((float)(dj * (2 - (di < 0 ? -di : di))) * 0.125f, d, gy);
-                    }
+                        for (int dj = -1; dj <= 1; ++dj) {
+                            const int ni = clampi(i + di, 0, nx - 1) - oi, nj = clampi(j + dj, 0, ny - 1) - oj;
+                            const float d = Ac[ni * CJ + nj];
+                            gx = fmaf((float)(di * (2 - (dj < 0 ? -dj : dj))) * 0.125f, d, gx);
+                            gy = fmaf((float)(dj * (2 - (di < 0 ? -di : di))) * 0.125f, d, gy);
+                        }
+                }
                 gx *= inv_deps; gy *= inv_deps;
                 const float gc = c == 0 ? gx : gy, go = c == 0 ? gy : gx;
-                const float rS = __frcp_rn(gc * gc + go * go + P.delta);
+                const float rS = fast_rcp(gc * gc + go * go + P.delta);
                 const float n2 = gc * gc * rS;
-                const float ra = __frcp_rn(Ac[i_]), h = H[c][i_];
-                const float e2d = __frcp_rn(n2 * h + (1.0f - n2) * ra);       // eps2d_c = 1/q
-                const float G = gb[(size_t)c * ncol + (size_t)i * ny + j];
+                const float ra = fast_rcp(Ac[i_]), h = H[c][i_];
+                const float e2d = fast_rcp(n2 * h + (1.0f - n2) * ra);       // eps2d_c = 1/q
+                const float G = gb[c * ncol + i * ny + j];
                 const float qbar = -G * e2d * e2d;
                 hb = n2 * qbar;
                 ab = -(1.0f - n2) * qbar * ra * ra;
@@ -156,10 +167,10 @@ __global__ void __launch_bounds__(REV_THREADS) k_reverse2d(const Rev2dParams P)
             const int ci = 2 + rem / RJ, cj = 2 + rem % RJ, i_ = ci * CJ + cj;
             const int ii = oi + ci, jj = oj + cj;
             float out = 0.f;
-            if (ii >= 0 && ii < nx && jj >= 0 && jj < ny) {
+            if (inner || (ii >= 0 && ii < nx && jj >= 0 && jj < ny)) {
                 float dbar = 0.f;
                 const float *gxs = Gx[c], *gys = Gy[c];
-                if (ii >= 1 && ii <= nx - 2 && jj >= 1 && jj <= ny - 2) {
+                if (inner || (ii >= 1 && ii <= nx - 2 && jj >= 1 && jj <= ny - 2)) {
                     // interior: the cell (ii-di, jj-dj) reached (ii,jj) through its stencil entry (di,dj)
 #pragma unroll
                     for (int di = -1; di <= 1; ++di)
@@ -204,10 +215,10 @@ __global__ void __launch_bounds__(REV_THREADS) k_reverse2d(const Rev2dParams P)
             for (int a = 0; a < s; ++a)
                 for (int bb = 0; bb < s; ++bb) az += e_s[(lp0 + a) * MQ + lq0 + bb];
             az *= inv_s2;                                   // eps2d_z
-            const size_t cell = (size_t)i * ny + j;
-            out = gb[2 * (size_t)ncol + cell];
-            if (P.w_lo > 0.f) out = fmaf(face_factor(P.w_lo, az, inv_ec), gb[3 * (size_t)ncol + cell], out);
-            if (P.w_hi > 0.f) out = fmaf(face_factor(P.w_hi, az, inv_ec), gb[4 * (size_t)ncol + cell], out);
+            const int cell = i * ny + j;
+            out = gb[2 * ncol + cell];
+            if (P.w_lo > 0.f) out = fmaf(face_factor(P.w_lo, az, inv_ec), gb[3 * ncol + cell], out);
+            if (P.w_hi > 0.f) out = fmaf(face_factor(P.w_hi, az, inv_ec), gb[4 * ncol + cell], out);
         }
         AbZ[it] = out;
     }
@@ -238,8 +249,8 @@ __global__ void __launch_bounds__(REV_THREADS) k_reverse2d(const Rev2dParams P)
         }
         const float r = r_s[(tp + 3 * s) * MQ + tq + 3 * s];           // 1/e
         const float rhobar = P.deps * inv_s2 * (ebar - rbar * r * r);
-        const float slope = project_slope(phib[(size_t)p * P.py + q], P.beta, P.eta_r);
-        vb[(size_t)p * P.py + q] = rhobar * slope * P.nrm.at_index(nidx[tp], nidx[TP + tq]);
+        const float slope = project_slope(phib[p * P.py + q], P.beta, P.eta_r);
+        vb[p * P.py + q] = rhobar * slope * P.nrm.at_index(nidx[tp], nidx[TP + tq]);
     }
 }
 

@@ -30,11 +30,10 @@ struct ZredParams {
     int ch0[2], nch[2], L[2];   // chunk window (chunk = 2 cells) and lanes per column for {x,y} and {z}
 };
 
-// grid (blocks over columns, 3*B)
+// One block of columns (index bx) of component c of design b.
 template <int ZR_UNROLL, bool SPARSE>
-__global__ void __launch_bounds__(ZR_THREADS, 4) k_zreduce(const ZredParams P)
+__device__ __forceinline__ void zreduce_block(const ZredParams &P, int bx, int c, int b)
 {
-    const int c = blockIdx.y % 3, b = blockIdx.y / 3;
     const int grp = c == 2;
     const int L = P.L[grp], ch0 = P.ch0[grp], nch = P.nch[grp];
     const int tid = threadIdx.x;
@@ -43,7 +42,7 @@ __global__ void __launch_bounds__(ZR_THREADS, 4) k_zreduce(const ZredParams P)
     const size_t plane = ((size_t)b * 3 + c) * P.ncol;
 
     // thread's columns: colbase + u*GPB (consecutive lane groups take consecutive columns)
-    const int colbase = blockIdx.x * (ZR_UNROLL * GPB) + g;
+    const int colbase = bx * (ZR_UNROLL * GPB) + g;
     if (colbase - g >= P.ncol) return;               // whole block past the end (uniform)
     bool live[ZR_UNROLL];
 #pragma unroll
@@ -107,6 +106,13 @@ __global__ void __launch_bounds__(ZR_THREADS, 4) k_zreduce(const ZredParams P)
             *dst = P.accumulate ? *dst + acc[u][o] : acc[u][o];
         }
     }
+}
+
+// grid (blocks over columns, 3*B)
+template <int ZR_UNROLL, bool SPARSE>
+__global__ void __launch_bounds__(ZR_THREADS, 4) k_zreduce(const ZredParams P)
+{
+    zreduce_block<ZR_UNROLL, SPARSE>(P, blockIdx.x, blockIdx.y % 3, blockIdx.y / 3);
 }
 
 }  // namespace epsgrad

@@ -17,6 +17,8 @@ pytestmark = pytest.mark.gpu
 CASES = {
     "conic_ragged": (dict(mx=37, my=29, nz=16, z_lo=6.25, z_hi=9.75, filter_radius=4.0), 8.0),
     "conic_r8_beta64": (dict(mx=41, my=50, nz=64, z_lo=28.25, z_hi=35.75, filter_radius=8.0), 64.0),
+    "conic_r12_beta32": (dict(mx=45, my=39, nz=8, z_lo=2.25, z_hi=5.75, filter_radius=12.0), 32.0),
+    "conic_r6_generic_taps": (dict(mx=30, my=41, nz=8, z_lo=2.25, z_hi=5.75, filter_radius=6.0), 10.0),
     "conic_fractional_radius": (dict(mx=24, my=33, nz=8, z_lo=2.25, z_hi=5.75, filter_radius=3.3), 12.0),
     "subpixel4": (dict(mx=19, my=23, nz=8, z_lo=2.25, z_hi=5.75, filter_radius=3.0, subpixel=4), 10.0),
     "upsample1": (dict(mx=40, my=35, nz=8, z_lo=1.5, z_hi=6.0, filter_radius=2.5, upsample=1), 9.0),
@@ -111,7 +113,49 @@ def test_forward_vjp_equals_separate_calls_and_keeps_inputs():
     torch.cuda.synchronize()
     assert torch.equal(eps1, eps2) and torch.equal(g1, g2)
     assert torch.equal(C, C0) and torch.equal(EF[0], F0)
-    assert plan.last_launches() >= 5
+    assert plan.last_launches() >= 4
+
+
+@pytest.mark.parametrize("n_pairs", [1, 9])
+def test_schedules_agree_bitwise(n_pairs):
+    # fused forward+zreduce launch (default), separate launches, and the two-stream schedule
+    cfg = B.make_config(batch=2, mx=27, my=22, nz=16, z_lo=6.25, z_hi=9.75, filter_radius=4.0)
+    C = dev(rand_C(cfg, 16))
+    EFn, EAn = rand_fields(cfg, n_pairs, 17)
+    EF, EA = [dev(f) for f in EFn], [dev(f) for f in EAn]
+    plan = B.Plan(cfg)
+    eps0, g0 = plan.eps_forward_vjp(C, 8.0, EF, EA)
+    n_fused = plan.last_launches()
+    plan.set_fused_streams(False)
+    eps1, g1 = plan.eps_forward_vjp(C, 8.0, EF, EA)
+    assert plan.last_launches() == n_fused + 1
+    plan.set_overlap(True)
+    eps2, g2 = plan.eps_forward_vjp(C, 8.0, EF, EA)
+    g3 = plan.eps_vjp(C, 8.0, EF, EA)
+    torch.cuda.synchronize()
+    assert torch.equal(eps0, eps1) and torch.equal(g0, g1) and torch.equal(eps0, eps2) and torch.equal(g0, g2)
+    assert torch.equal(g0, g3)
+
+
+def test_calls_are_cuda_graph_capturable():
+    cfg = B.make_config(mx=25, my=31, nz=16, z_lo=6.25, z_hi=9.75, filter_radius=4.0)
+    C = dev(rand_C(cfg, 18))
+    EFn, EAn = rand_fields(cfg, 1, 19)
+    EF, EA = [dev(f) for f in EFn], [dev(f) for f in EAn]
+    plan = B.Plan(cfg)
+    eps_ref, g_ref = plan.eps_forward_vjp(C, 8.0, EF, EA)
+    eps, g = torch.zeros_like(eps_ref), torch.zeros_like(g_ref)
+    torch.cuda.synchronize()
+    for overlap in (False, True):
+        plan.set_overlap(overlap)
+        plan.set_fused_streams(not overlap)
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):
+            plan.eps_forward_vjp(C, 8.0, EF, EA, eps, g)
+        eps.zero_(); g.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(eps, eps_ref) and torch.equal(g, g_ref)
 
 
 def test_real_cotangent_special_case():
