@@ -198,6 +198,7 @@ def run_reference(args, w):
 def run_ours(args, w):
     import torch
     from paper_2505_03352_b200 import binding as B
+    from paper_2505_03352_b200 import sharding
     from paper_2505_03352_b200 import workloads as W
 
     rank = int(os.environ.get("RANK", "0"))
@@ -271,12 +272,9 @@ def run_ours(args, w):
     barrier()
     ms_total = e0.elapsed_time(e1)
     clocks = sampler.stop()
-    if dist is not None:
-        t = torch.tensor([ms_total], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = sharding.max_over_ranks(ms_total, device=dev)
     cells_step = w.cells * len(w.betas)
-    value = world * cells_step * args.steps / (ms_total * 1e-3)
+    value = sharding.job_throughput(cells_step, args.steps, ms_total, world)
 
     # ---- per-kernel durations, live, with CUDA events on the launching stream
     plan.set_profiling(True)
@@ -327,11 +325,8 @@ def run_ours(args, w):
     e1.record()
     barrier()
     ms_e2e = e0.elapsed_time(e1)
-    if dist is not None:
-        t = torch.tensor([ms_e2e], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_e2e = float(t.item())
-    e2e = {"value": world * cells_step * n_e2e / (ms_e2e * 1e-3), "unit": UNIT,
+    ms_e2e = sharding.max_over_ranks(ms_e2e, device=dev)
+    e2e = {"value": sharding.job_throughput(cells_step, n_e2e, ms_e2e, world), "unit": UNIT,
            "h2d_bytes_per_step": h2d * len(w.betas), "d2h_bytes_per_step": d2h * len(w.betas),
            "steps": n_e2e, "ms_per_step": ms_e2e / n_e2e}
 

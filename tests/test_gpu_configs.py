@@ -1,0 +1,128 @@
+"""GPU parity on the five BASELINE.json configs at FULL size, in the launch configuration bench.py
+times (eps_forward_vjp, fused streams).
+
+Tiny, Paper-scale and Multi-wavelength are compared with the float64 oracle element by element.
+Large (2000x2000x64) and Wide batch (8 x 2048x2048x32) are too big for the oracle to finish in
+seconds, so they are checked on sampled outputs the oracle can compute one by one: every output has
+a bounded dependency cone -- eps at a Yee cell depends on C within R+3 cells,
+dF/dC at a control node on C within 2R+5 cells and on the fields within R+4 cells -- so the oracle
+is run on windows cut out of the full problem and compared where the window's artificial edges
+cannot be felt (its real edges, at region corners, are compared up to the border).  The fields of
+those windows are drawn on the host (numpy) and pasted into the otherwise device-generated fields.
+"""
+import math
+from dataclasses import replace
+
+import numpy as np
+import pytest
+import torch
+
+import oracle as O
+from gpu_common import TOL_EPS, TOL_GRAD, dev, max_rel
+from helpers import cfg_of, rel_inf, rel_l2
+from paper_2505_03352_b200 import binding as B
+from paper_2505_03352_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+def _full_fields(w):
+    EF = [W.make_field(w, p, 0)[None] for p in range(w.n_pairs)]
+    EA = [W.make_field(w, p, 1)[None] for p in range(w.n_pairs)]
+    return EF, EA
+
+
+@pytest.mark.parametrize("name", ["tiny", "paper", "multiwavelength"])
+def test_full_size_elementwise(name):
+    w = W.BY_NAME[name]
+    assert w.batch == 1
+    C = W.make_C(w)
+    EF, EA = _full_fields(w)
+    plan = B.Plan(B.config_of(w))
+    dEF, dEA = [dev(f) for f in EF], [dev(f) for f in EA]
+    oc = cfg_of(w)
+    for beta in w.betas:                                        # S12: one run per beta, all pairs each
+        eps, g = plan.eps_forward_vjp(dev(C), beta, dEF, dEA)
+        eps, g = eps.cpu().numpy()[0], g.cpu().numpy().astype(np.float64)[0]
+        ref = O.forward(oc, C[0], beta)
+        err_e = float(np.max(np.abs(eps - ref) / ref))
+        del ref
+        gref = O.vjp(oc, C[0], beta, [f[0] for f in EF], [f[0] for f in EA])
+        err_g = max(rel_inf(g, gref), rel_l2(g, gref))
+        print(f"{name} beta={beta}: eps {err_e:.2e}  dF/dC {err_g:.2e}")
+        assert err_e < TOL_EPS, (name, beta, err_e)
+        assert err_g < TOL_GRAD, (name, beta, err_g)
+
+
+def _device_fields(plan, w, seed):
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(seed)
+    mk = lambda: torch.view_as_complex(torch.randn(*plan.eps_shape, 2, device="cuda", generator=gen))
+    return [mk() for _ in range(w.n_pairs)], [mk() for _ in range(w.n_pairs)]
+
+
+def _window_patch(w, K, seed):
+    rng = np.random.default_rng(seed)
+    a = np.empty((3, w.upsample * K, w.upsample * K, w.nz), np.complex64)
+    rng.standard_normal(out=a.view(np.float32).reshape(-1), dtype=np.float32)
+    return a
+
+
+def _check_windows(w, windows, K):
+    """windows: list of (design, a0, b0) control-pixel origins of K x K windows."""
+    u, R = w.upsample, w.radius
+    m_rev = int(math.ceil((2 * R + 5) / u)) + 1                 # control pixels an artificial edge can reach (reverse)
+    m_fwd = int(math.ceil(R + 3)) + u                           # Yee cells (forward)
+    assert K > 2 * m_rev + 8
+    C = W.make_C(w)
+    plan = B.Plan(B.config_of(w))
+    EF, EA = _device_fields(plan, w, 100 + w.index)
+    patches = []
+    for n, (b, a0, b0) in enumerate(windows):
+        pf = [_window_patch(w, K, [w.index, n, p, 0]) for p in range(w.n_pairs)]
+        pa = [_window_patch(w, K, [w.index, n, p, 1]) for p in range(w.n_pairs)]
+        for p in range(w.n_pairs):
+            EF[p][b, :, u * a0:u * (a0 + K), u * b0:u * (b0 + K), :] = dev(pf[p])
+            EA[p][b, :, u * a0:u * (a0 + K), u * b0:u * (b0 + K), :] = dev(pa[p])
+        patches.append((pf, pa))
+    beta = w.betas[0]
+    eps, g = plan.eps_forward_vjp(dev(C), beta, EF, EA)
+    torch.cuda.synchronize()
+    g = g.cpu().numpy().astype(np.float64)
+    oc = cfg_of(replace(w, mx=K, my=K, batch=1))
+    for (b, a0, b0), (pf, pa) in zip(windows, patches):
+        Cw = np.ascontiguousarray(C[b, a0:a0 + K, b0:b0 + K])
+        # sides of the window that are real region borders need no margin
+        lo_a = 0 if a0 == 0 else m_rev
+        hi_a = K if a0 + K == w.mx else K - m_rev
+        lo_b = 0 if b0 == 0 else m_rev
+        hi_b = K if b0 + K == w.my else K - m_rev
+        gref = O.vjp(oc, Cw, beta, pf, pa)[lo_a:hi_a, lo_b:hi_b]
+        ggpu = g[b, a0 + lo_a:a0 + hi_a, b0 + lo_b:b0 + hi_b]
+        err_g = max(rel_inf(ggpu, gref), rel_l2(ggpu, gref))
+        fa = (0 if a0 == 0 else m_fwd, u * K if a0 + K == w.mx else u * K - m_fwd)
+        fb = (0 if b0 == 0 else m_fwd, u * K if b0 + K == w.my else u * K - m_fwd)
+        eref = O.forward(oc, Cw, beta)[:, fa[0]:fa[1], fb[0]:fb[1], :]
+        egpu = eps[b, :, u * a0 + fa[0]:u * a0 + fa[1], u * b0 + fb[0]:u * b0 + fb[1], :].cpu().numpy()
+        err_e = max_rel(egpu.astype(np.float64), eref)
+        print(f"{w.name} design {b} window ({a0},{b0})+{K}: eps {err_e:.2e} on {eref.size} cells, "
+              f"dF/dC {err_g:.2e} on {gref.size} nodes")
+        assert err_e < TOL_EPS and err_g < TOL_GRAD, (w.name, b, a0, b0, err_e, err_g)
+    # properties that hold at any size: bounds, and cladding outside the slab
+    lo, hi = float(eps.min()), float(eps.max())
+    assert lo >= np.float32(w.eps_clad) * (1 - 1e-6) and hi <= np.float32(w.eps_core) * (1 + 1e-6)
+    k_out = int(math.floor(w.z_lo - 0.5)) - 1
+    assert torch.all(eps[..., :k_out] == np.float32(w.eps_clad))
+    assert torch.isfinite(torch.from_numpy(g)).all()
+
+
+def test_large_full_size_sampled_windows():
+    w = W.BY_NAME["large"]                                      # 1000x1000 -> 2000x2000x64, conic R = 12, beta = 32
+    K = 96
+    _check_windows(w, [(0, 0, 0), (0, w.mx - K, w.my - K), (0, 0, w.my - K), (0, 437, 301), (0, 700, 64)], K)
+
+
+def test_widebatch_full_size_sampled_windows():
+    w = W.BY_NAME["widebatch"]                                  # 8 x 1024x1024 -> 2048x2048x32, Gaussian R = 32
+    K = 112
+    _check_windows(w, [(0, 0, 0), (3, 400, 512), (7, w.mx - K, w.my - K), (5, w.mx - K, 0)], K)

@@ -1,0 +1,71 @@
+"""Host-side logic of the N > 1 path on CPU: world_size-2 gloo processes.  Field pairs are sharded
+across ranks, each rank forms its partial dF/dC (here with the float64 oracle, the GPU being absent)
+and the partials are summed with the same all-reduce helper the GPU path uses; timing is reduced
+with the max-over-ranks helper bench.py uses."""
+import os
+import socket
+
+import numpy as np
+import pytest
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+from paper_2505_03352_b200 import sharding
+
+
+def test_shard_range_partitions():
+    for n in (0, 1, 3, 8, 17):
+        for world in (1, 2, 3, 8):
+            parts = [sharding.shard_range(n, r, world) for r in range(world)]
+            assert [i for p in parts for i in p] == list(range(n))
+            sizes = [len(p) for p in parts]
+            assert max(sizes) - min(sizes) <= 1
+    with pytest.raises(ValueError):
+        sharding.shard_range(4, 2, 2)
+
+
+def test_job_throughput():
+    assert sharding.job_throughput(16_000_000, 10, 2.0, 4) == pytest.approx(4 * 16e6 * 10 / 2e-3)
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    p = s.getsockname()[1]
+    s.close()
+    return p
+
+
+def _worker(rank, world, port, out_dir):
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    sys.path[:0] = [root, os.path.join(root, "tests")]
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import oracle as O
+    from helpers import small_cfg
+    cfg = small_cfg(mx=10, my=9, nz=8, z_lo=2.25, z_hi=5.75, radius=3.0)
+    rng = np.random.default_rng(7)                      # same stream on every rank: identical inputs
+    C = rng.random((cfg.mx, cfg.my)).astype(np.float32)
+    n_pairs = 3
+    shape = (3, cfg.nx, cfg.ny, cfg.nz)
+    mk = lambda: (rng.standard_normal(shape) + 1j * rng.standard_normal(shape)).astype(np.complex64)
+    EF, EA = [mk() for _ in range(n_pairs)], [mk() for _ in range(n_pairs)]
+    mine = sharding.shard_range(n_pairs, rank, world)
+    part = O.vjp(cfg, C, 8.0, [EF[p] for p in mine], [EA[p] for p in mine]) if len(mine) else np.zeros((cfg.mx, cfg.my))
+    g = sharding.sum_gradients(torch.from_numpy(part.copy()))
+    t = sharding.max_over_ranks(10.0 + rank)
+    if rank == 0:
+        full = O.vjp(cfg, C, 8.0, EF, EA)
+        np.save(os.path.join(out_dir, "res.npy"), np.array([np.max(np.abs(g.numpy() - full)) / np.max(np.abs(full)), t]))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_pair_sharded_gradient_sums_to_the_full_gradient(tmp_path):
+    world = 2
+    mp.spawn(_worker, args=(world, _free_port(), str(tmp_path)), nprocs=world, join=True)
+    err, t = np.load(tmp_path / "res.npy")
+    assert err < 1e-12            # linearity of Eq. (1) in the pairs
+    assert t == 11.0              # max over ranks
