@@ -84,8 +84,8 @@ typedef struct {
 int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsgrad_plan_t **out);
 int epsgrad_plan_destroy(epsgrad_plan_t *plan);
 
-/* Scratch the device entry points need (filter output Phi, reduced cotangent, mask
- * cotangent, separable-filter temporaries).  The caller allocates it (e.g. a torch
+/* Scratch the device entry points need (filter output Phi, per-cell reverse residual planes,
+ * mask cotangent, separable-filter temporaries).  The caller allocates it (e.g. a torch
  * uint8 tensor) and keeps it alive and unshared while calls of this plan are in flight. */
 size_t epsgrad_workspace_bytes(const epsgrad_plan_t *plan);
 int    epsgrad_plan_set_workspace(epsgrad_plan_t *plan, void *dev_ptr, size_t bytes);
@@ -99,19 +99,6 @@ int    epsgrad_plan_set_staging(epsgrad_plan_t *plan, void *dev_ptr, size_t byte
  * hold slab cells.  1: read every z cell (weights are zero outside the slab).  Results
  * are identical; this is a measurement switch.                                           */
 int epsgrad_plan_set_dense_reads(epsgrad_plan_t *plan, int dense);
-
-/* Fused HBM streams (default on): eps_forward_vjp runs the forward tile kernel (eps writes) and
- * the Eq. (1) z-reduction (field reads) as ONE launch whose CTAs interleave both roles, so reads
- * and writes overlap.  0 = separate launches.  Per-kernel profiling always uses separate launches. */
-int epsgrad_plan_set_fused_streams(epsgrad_plan_t *plan, int enable);
-
-/* Two-stream schedule (default off; an alternative to the fused launch).  The Eq. (1) field stream does not depend on the filter, so
- * calls that compute dF/dC fork the plan's auxiliary stream from `stream` (event), run
- * zreduce -> reverse2d -> filterT there while filter -> forward run on `stream`, and join it back
- * (event) before returning: to the caller everything is still ordered on `stream`, with no host
- * synchronisation, and the calls remain CUDA-graph capturable.  0 = one stream, strictly serial
- * (also used while per-kernel profiling is on).                                              */
-int epsgrad_plan_set_overlap(epsgrad_plan_t *plan, int enable);
 
 /* Number of kernel launches the last eps_* call of this plan enqueued (for accounting). */
 int epsgrad_plan_last_launches(const epsgrad_plan_t *plan);
@@ -155,7 +142,8 @@ int epsgrad_plan_last_copy_bytes(const epsgrad_plan_t *plan, uint64_t *h2d, uint
 int epsgrad_stage_filter(epsgrad_plan_t *plan, const float *C, float *phi_centred, void *stream);
 /* eps2d [B,3,Nx,Ny]: the 2-D stage before z-extrusion (steps 1-6).                      */
 int epsgrad_stage_eps2d(epsgrad_plan_t *plan, const float *C, float beta, float *eps2d, void *stream);
-/* z-reduced cotangent [B,5,Nx,Ny]: planes x, y, z(full cells), z(lower face), z(upper face). */
+/* z-reduced cotangent [B,5,Nx,Ny]: planes x, y, z(full cells), z(lower face), z(upper face).
+ * Runs the tile kernel on a zeroed filter output, so it needs (and overwrites part of) the workspace. */
 int epsgrad_stage_zreduce(epsgrad_plan_t *plan, int n_pairs, const void *const *EF,
                           const void *const *EA, float *gbar, void *stream);
 

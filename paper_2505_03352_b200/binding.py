@@ -19,7 +19,7 @@ EXPORTS = (
     "epsgrad_plan_create", "epsgrad_plan_destroy", "epsgrad_workspace_bytes",
     "epsgrad_plan_set_workspace", "epsgrad_staging_bytes", "epsgrad_plan_set_staging",
     "epsgrad_plan_set_dense_reads", "epsgrad_plan_last_launches", "epsgrad_plan_last_copy_bytes",
-    "epsgrad_plan_set_profiling", "epsgrad_plan_last_kernel_times", "epsgrad_plan_set_overlap", "epsgrad_plan_set_fused_streams",
+    "epsgrad_plan_set_profiling", "epsgrad_plan_last_kernel_times", 
     "eps_forward", "eps_vjp", "eps_forward_vjp", "eps_forward_vjp_host",
     "epsgrad_stage_filter", "epsgrad_stage_eps2d", "epsgrad_stage_zreduce",
     "epsgrad_status_string", "epsgrad_version",
@@ -96,8 +96,6 @@ def lib() -> ctypes.CDLL:
     L.epsgrad_plan_set_dense_reads.argtypes = [vp, i32]
     L.epsgrad_plan_last_launches.argtypes = [vp]
     L.epsgrad_plan_last_copy_bytes.argtypes = [vp, ctypes.POINTER(ctypes.c_uint64), ctypes.POINTER(ctypes.c_uint64)]
-    L.epsgrad_plan_set_overlap.argtypes = [vp, i32]
-    L.epsgrad_plan_set_fused_streams.argtypes = [vp, i32]
     L.epsgrad_plan_set_profiling.argtypes = [vp, i32]
     L.epsgrad_plan_last_kernel_times.argtypes = [vp, i32, ctypes.POINTER(f32), ctypes.POINTER(ctypes.c_char_p)]
     L.eps_forward.argtypes = [vp, vp, f32, vp, vp]
@@ -207,12 +205,6 @@ class Plan:
         a, b = ctypes.c_uint64(), ctypes.c_uint64()
         _check(lib().epsgrad_plan_last_copy_bytes(self._h, ctypes.byref(a), ctypes.byref(b)), "last_copy_bytes")
         return int(a.value), int(b.value)
-
-    def set_fused_streams(self, enable: bool) -> None:
-        _check(lib().epsgrad_plan_set_fused_streams(self._h, int(bool(enable))), "epsgrad_plan_set_fused_streams")
-
-    def set_overlap(self, enable: bool) -> None:
-        _check(lib().epsgrad_plan_set_overlap(self._h, int(bool(enable))), "epsgrad_plan_set_overlap")
 
     def set_profiling(self, enable: bool) -> None:
         _check(lib().epsgrad_plan_set_profiling(self._h, int(bool(enable))), "epsgrad_plan_set_profiling")

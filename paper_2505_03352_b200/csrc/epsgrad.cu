@@ -12,10 +12,8 @@
 #include "filter.cuh"
 #include "filter4.cuh"
 #include "filter_sep.cuh"
-#include "forward.cuh"
-#include "reverse2d.cuh"
-#include "zreduce.cuh"
-#include "stream.cuh"
+#include "tile.cuh"
+#include "maskgrad.cuh"
 
 using namespace epsgrad;
 
@@ -44,16 +42,12 @@ struct epsgrad_plan {
     void *ws; size_t ws_bytes;
     void *stg; size_t stg_bytes;
     // workspace carve-up (byte offsets)
-    size_t off_phi, off_v, off_gbar, off_tmp, ws_need;
+    size_t off_phi, off_v, off_res, off_tmp, ws_need;
     int last_launches;
     uint64_t last_h2d, last_d2h;
     // optional per-kernel timing (epsgrad_plan_set_profiling)
     int prof;
     cudaEvent_t ev[EPSGRAD_MAX_KERNELS + 1];
-    // two-stream overlap of the field stream (zreduce -> reverse2d -> filterT) with filter -> forward
-    int overlap, fuse_streams;
-    cudaStream_t aux;
-    cudaEvent_t ev_fork, ev_filter, ev_join;
     const char *kname[EPSGRAD_MAX_KERNELS];
 };
 
@@ -239,7 +233,7 @@ extern "C" int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsg
         const size_t need = ((size_t)NT * NT * m * m + (size_t)m * (ta + 2 * T) * m * (tb + 2 * T) + 2 * NT) * 4;
         if (need > 200 * 1024) { delete P; return EPSGRAD_EUNSUPPORTED; }
     }
-    if (fwd_smem_floats(s, nz) * 4 > 200 * 1024 || rev_smem_floats(s) * 4 > 200 * 1024) { delete P; return EPSGRAD_EUNSUPPORTED; }
+    if (tile_smem_floats(s, nz) * 4 + (size_t)2 * TILE_STAGE_CELLS * 13 * 16 > 200 * 1024 || maskgrad_smem_floats(s) * 4 > 200 * 1024) { delete P; return EPSGRAD_EUNSUPPORTED; }
 
     // ---- upload
     int prev = 0;
@@ -267,27 +261,12 @@ extern "C" int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsg
         return EPSGRAD_ECUDA;
     }
 
-    // ---- auxiliary stream and fork/join events (no timing) for the two-stream schedule
-    {
-        int prev2 = 0;
-        cudaGetDevice(&prev2);
-        cudaSetDevice(device);
-        bool ok = cudaStreamCreateWithFlags(&P->aux, cudaStreamNonBlocking) == cudaSuccess &&
-                  cudaEventCreateWithFlags(&P->ev_fork, cudaEventDisableTiming) == cudaSuccess &&
-                  cudaEventCreateWithFlags(&P->ev_filter, cudaEventDisableTiming) == cudaSuccess &&
-                  cudaEventCreateWithFlags(&P->ev_join, cudaEventDisableTiming) == cudaSuccess;
-        cudaSetDevice(prev2);
-        if (!ok) { cudaGetLastError(); epsgrad_plan_destroy(P); return EPSGRAD_ECUDA; }
-        P->overlap = 0;
-        P->fuse_streams = 1;
-    }
-
     // ---- workspace carve-up
     const size_t n_mask = (size_t)cfg->batch * P->px * P->py, n_cell = (size_t)cfg->batch * P->nx * P->ny;
     size_t off = 0;
     P->off_phi = off;  off += align_up(n_mask * 4, 256);
     P->off_v = off;    off += align_up(n_mask * 4, 256);
-    P->off_gbar = off; off += align_up(n_cell * 5 * 4, 256);
+    P->off_res = off;  off += align_up(n_cell * TILE_NRES * 4, 256);
     P->off_tmp = off;  off += P->separable ? align_up((size_t)cfg->batch * cfg->mx * P->py * 4, 256) : 0;
     P->ws_need = off;
     *out = P;
@@ -298,10 +277,6 @@ extern "C" int epsgrad_plan_destroy(epsgrad_plan_t *P)
 {
     if (!P) return EPSGRAD_EINVAL;
     if (P->d_tables) cudaFree(P->d_tables);
-    if (P->aux) cudaStreamDestroy(P->aux);
-    if (P->ev_fork) cudaEventDestroy(P->ev_fork);
-    if (P->ev_filter) cudaEventDestroy(P->ev_filter);
-    if (P->ev_join) cudaEventDestroy(P->ev_join);
     if (P->ev[0])
         for (int i = 0; i <= EPSGRAD_MAX_KERNELS; ++i) cudaEventDestroy(P->ev[i]);
     delete P;
@@ -376,20 +351,6 @@ extern "C" int epsgrad_plan_set_dense_reads(epsgrad_plan_t *P, int dense)
     return EPSGRAD_OK;
 }
 
-extern "C" int epsgrad_plan_set_overlap(epsgrad_plan_t *P, int enable)
-{
-    if (!P) return EPSGRAD_EINVAL;
-    P->overlap = enable != 0;
-    return EPSGRAD_OK;
-}
-
-extern "C" int epsgrad_plan_set_fused_streams(epsgrad_plan_t *P, int enable)
-{
-    if (!P) return EPSGRAD_EINVAL;
-    P->fuse_streams = enable != 0;
-    return EPSGRAD_OK;
-}
-
 extern "C" int epsgrad_plan_last_launches(const epsgrad_plan_t *P) { return P ? P->last_launches : 0; }
 
 extern "C" int epsgrad_plan_last_copy_bytes(const epsgrad_plan_t *P, uint64_t *h2d, uint64_t *d2h)
@@ -457,7 +418,7 @@ Normaliser make_nrm(const epsgrad_plan *P)
 
 float *ws_phi(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_phi); }
 float *ws_v(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_v); }
-float *ws_gbar(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_gbar); }
+float *ws_res(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_res); }
 float *ws_tmp(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_tmp); }
 
 // ---- F1: C -> centred Phi on the mask
@@ -583,114 +544,68 @@ int launch_filterT(epsgrad_plan *P, const float *v, float *dC, cudaStream_t st)
     return EPSGRAD_EUNSUPPORTED;
 }
 
-// ---- F2..F6
-FwdParams make_fwd(const epsgrad_plan *P, const float *phi, float beta, float *eps, float *eps2d)
+// ---- F2..F6 + R1..R3a: the tile kernel (tile.cuh).  eps / eps2d / gtap / res may be null; n_pairs == 0 skips the reverse half.
+// More than TILE_MAX_PAIRS pairs are chained: R2/R3a are linear in the cotangent, so later launches accumulate into res.
+int launch_tile(epsgrad_plan *P, const float *phi, float beta, float *eps, float *eps2d, int n_pairs,
+                const void *const *EF, const void *const *EA, float *res, float *gtap, cudaStream_t st)
 {
-    FwdParams fp;
-    fp.phi = phi; fp.eps = eps; fp.eps2d = eps2d; fp.zw = P->d_zw;
-    fp.nx = P->nx; fp.ny = P->ny; fp.nz = P->cfg.nz; fp.px = P->px; fp.py = P->py; fp.s = P->cfg.subpixel;
-    fp.beta = beta; fp.eta_r = P->eta_r; fp.eps_clad = P->eps_clad; fp.deps = P->deps; fp.delta = P->delta;
-    fp.w_lo = P->w_lo; fp.w_hi = P->w_hi;
-    return fp;
-}
-
-// z windows, lanes per column, load flavour and block counts of the z-reduction
-struct ZredShape { bool sparse; int unroll; int nb[2]; };
-ZredShape make_zred(const epsgrad_plan *P, ZredParams &zp, float *gbar)
-{
-    zp.gbar = gbar; zp.zw = P->d_zw; zp.ncol = P->nx * P->ny; zp.nz = P->cfg.nz;
+    TileParams tp;
+    tp.phi = phi; tp.zw = P->d_zw;
+    tp.nx = P->nx; tp.ny = P->ny; tp.nz = P->cfg.nz; tp.px = P->px; tp.py = P->py; tp.s = P->cfg.subpixel;
+    tp.beta = beta; tp.eta_r = P->eta_r; tp.eps_clad = P->eps_clad; tp.deps = P->deps; tp.delta = P->delta;
+    tp.w_lo = P->w_lo; tp.w_hi = P->w_hi;
     int maxnch = 1;
     for (int g = 0; g < 2; ++g) {
-        zp.ch0[g] = P->dense ? 0 : P->ch0[g];
-        zp.nch[g] = P->dense ? P->cfg.nz / 2 : P->nch[g];
-        int L = 1;
-        while (L < zp.nch[g]) L <<= 1;
-        if (L > 32) L = 32;
-        zp.L[g] = L;
-        if (zp.nch[g] > maxnch) maxnch = zp.nch[g];
+        tp.ch0[g] = P->dense ? 0 : P->ch0[g];
+        tp.nch[g] = P->dense ? P->cfg.nz / 2 : P->nch[g];
+        if (tp.nch[g] > maxnch) maxnch = tp.nch[g];
+        tp.chs[g] = 0;
+        while ((1 << tp.chs[g]) < tp.nch[g]) ++tp.chs[g];
+        if (tp.chs[g] > 8) return EPSGRAD_EUNSUPPORTED;     // window wider than one CTA pass (nz > 1024)
     }
-    ZredShape zs;
-    // windows of at most 128 bytes per column: ask for 64-byte fills and keep fewer columns in flight
-    zs.sparse = maxnch * 16 <= 128 && zp.nz * 8 > 128;
-    zs.unroll = zs.sparse ? ZR_UNROLL_SPARSE : ZR_UNROLL_DENSE;
-    for (int g = 0; g < 2; ++g) zs.nb[g] = cdiv(zp.ncol, (ZR_THREADS / zp.L[g]) * zs.unroll);
-    return zs;
-}
-
-void set_pairs(ZredParams &zp, int np, const void *const *EF, const void *const *EA, int accumulate)
-{
-    for (int p = 0; p < ZR_MAX_PAIRS; ++p) {
-        zp.ef[p] = (const float4 *)(p < np ? EF[p] : nullptr);
-        zp.ea[p] = (const float4 *)(p < np ? EA[p] : nullptr);
-    }
-    zp.n_pairs = np; zp.accumulate = accumulate;
-}
-
-// ---- F2..F6 and R1 in one launch (stream.cuh); n_pairs <= ZR_MAX_PAIRS
-int launch_stream(epsgrad_plan *P, const float *phi, float beta, float *eps, int n_pairs,
-                  const void *const *EF, const void *const *EA, float *gbar, cudaStream_t st)
-{
-    StreamParams sp;
-    sp.F = make_fwd(P, phi, beta, eps, nullptr);
-    const ZredShape zs = make_zred(P, sp.Z, gbar);
-    set_pairs(sp.Z, n_pairs, EF, EA, 0);
-    sp.fx = cdiv(P->ny, FWD_TJ); sp.fy = cdiv(P->nx, FWD_TI); sp.nf = sp.fx * sp.fy * P->cfg.batch;
-    sp.nbz[0] = zs.nb[0]; sp.nbz[1] = zs.nb[1];
-    sp.nz_blocks = P->cfg.batch * (2 * zs.nb[0] + zs.nb[1]);
-    const size_t smem = fwd_smem_floats(sp.F.s, sp.F.nz) * 4;
-    const int s = sp.F.s;
-    void (*kern)(const StreamParams);
-    if (zs.sparse) kern = s == 2 ? k_stream<2, ZR_UNROLL_SPARSE, true> : (s == 4 ? k_stream<4, ZR_UNROLL_SPARSE, true> : k_stream<0, ZR_UNROLL_SPARSE, true>);
-    else kern = s == 2 ? k_stream<2, ZR_UNROLL_DENSE, false> : (s == 4 ? k_stream<4, ZR_UNROLL_DENSE, false> : k_stream<0, ZR_UNROLL_DENSE, false>);
+    const int rows = 2 * tp.nch[0] + tp.nch[1];
+    tp.ncp = tile_cells_per_pass(rows);
+    if (tp.ncp < 1) return EPSGRAD_EUNSUPPORTED;
+    // windows of at most 128 bytes per column: ask for 64-byte fills
+    tp.sparse = maxnch * 16 <= 128 && tp.nz * 8 > 128;
+    const size_t smem = tile_smem_floats(tp.s, tp.nz) * 4 + (n_pairs > 0 ? (size_t)2 * rows * tp.ncp * 16 : 0);
+    void (*kern)(const TileParams);
+    if (tp.sparse) kern = tp.s == 2 ? k_tile<2, true> : (tp.s == 4 ? k_tile<4, true> : k_tile<0, true>);
+    else kern = tp.s == 2 ? k_tile<2, false> : (tp.s == 4 ? k_tile<4, false> : k_tile<0, false>);
     int rc = set_smem(kern, smem);
     if (rc) return rc;
-    kern<<<sp.nf + sp.nz_blocks, FWD_THREADS, smem, st>>>(sp);
-    return check_launch(P, "stream", st);
-}
-
-int launch_forward(epsgrad_plan *P, const float *phi, float beta, float *eps, float *eps2d, cudaStream_t st)
-{
-    const FwdParams fp = make_fwd(P, phi, beta, eps, eps2d);
-    const size_t smem = fwd_smem_floats(fp.s, fp.nz) * 4;
-    auto kern = fp.s == 2 ? k_forward<2> : (fp.s == 4 ? k_forward<4> : k_forward<0>);
-    int rc = set_smem(kern, smem);
-    if (rc) return rc;
-    kern<<<dim3(cdiv(P->ny, FWD_TJ), cdiv(P->nx, FWD_TI), P->cfg.batch), FWD_THREADS, smem, st>>>(fp);
-    return check_launch(P, "forward", st);
-}
-
-// ---- R1
-int launch_zreduce(epsgrad_plan *P, int n_pairs, const void *const *EF, const void *const *EA, float *gbar,
-                   cudaStream_t st, int first_accumulates = 0)
-{
-    ZredParams zp;
-    const ZredShape zs = make_zred(P, zp, gbar);
-    const dim3 grid(zs.nb[0] > zs.nb[1] ? zs.nb[0] : zs.nb[1], 3 * P->cfg.batch);
-    for (int p0 = 0; p0 < n_pairs; p0 += ZR_MAX_PAIRS) {
-        const int np = n_pairs - p0 < ZR_MAX_PAIRS ? n_pairs - p0 : ZR_MAX_PAIRS;
-        set_pairs(zp, np, EF + p0, EA + p0, p0 > 0 || first_accumulates);
-        if (zs.sparse) k_zreduce<ZR_UNROLL_SPARSE, true><<<grid, ZR_THREADS, 0, st>>>(zp);
-        else k_zreduce<ZR_UNROLL_DENSE, false><<<grid, ZR_THREADS, 0, st>>>(zp);
-        int rc = check_launch(P, "zreduce", st);
+    const dim3 grid(cdiv(P->ny, TILE_TJ), cdiv(P->nx, TILE_TI), P->cfg.batch);
+    int p0 = 0;
+    do {
+        const int np = n_pairs - p0 < TILE_MAX_PAIRS ? n_pairs - p0 : TILE_MAX_PAIRS;
+        for (int p = 0; p < TILE_MAX_PAIRS; ++p) {
+            tp.ef[p] = (const float4 *)(p < np ? EF[p0 + p] : nullptr);
+            tp.ea[p] = (const float4 *)(p < np ? EA[p0 + p] : nullptr);
+        }
+        tp.n_pairs = np; tp.accumulate = p0 > 0;
+        tp.eps = p0 == 0 ? eps : nullptr; tp.eps2d = p0 == 0 ? eps2d : nullptr;
+        tp.res = res; tp.gtap = gtap;
+        kern<<<grid, TILE_THREADS, smem, st>>>(tp);
+        rc = check_launch(P, "tile", st);
         if (rc) return rc;
-    }
+        p0 += TILE_MAX_PAIRS;
+    } while (p0 < n_pairs);
     return EPSGRAD_OK;
 }
 
-// ---- R2..R5
-int launch_reverse2d(epsgrad_plan *P, const float *phi, float beta, const float *gbar, float *v, cudaStream_t st)
+// ---- R3b..R5
+int launch_maskgrad(epsgrad_plan *P, const float *phi, float beta, const float *res, float *v, cudaStream_t st)
 {
-    Rev2dParams rp;
-    rp.phi = phi; rp.gbar = gbar; rp.v = v; rp.nrm = make_nrm(P);
-    rp.nx = P->nx; rp.ny = P->ny; rp.px = P->px; rp.py = P->py; rp.s = P->cfg.subpixel;
-    rp.beta = beta; rp.eta_r = P->eta_r; rp.eps_clad = P->eps_clad; rp.deps = P->deps; rp.delta = P->delta;
-    rp.w_lo = P->w_lo; rp.w_hi = P->w_hi;
-    const size_t smem = rev_smem_floats(rp.s) * 4;
-    auto kern = rp.s == 2 ? k_reverse2d<2> : (rp.s == 4 ? k_reverse2d<4> : k_reverse2d<0>);
+    MaskGradParams mp;
+    mp.phi = phi; mp.res = res; mp.v = v; mp.nrm = make_nrm(P);
+    mp.nx = P->nx; mp.ny = P->ny; mp.px = P->px; mp.py = P->py; mp.s = P->cfg.subpixel;
+    mp.beta = beta; mp.eta_r = P->eta_r; mp.eps_clad = P->eps_clad; mp.deps = P->deps;
+    const size_t smem = maskgrad_smem_floats(mp.s) * 4;
+    auto kern = mp.s == 2 ? k_maskgrad<2> : (mp.s == 4 ? k_maskgrad<4> : k_maskgrad<0>);
     int rc = set_smem(kern, smem);
     if (rc) return rc;
-    kern<<<dim3(cdiv(P->ny, REV_TJ), cdiv(P->nx, REV_TI), P->cfg.batch), REV_THREADS, smem, st>>>(rp);
-    return check_launch(P, "reverse2d", st);
+    kern<<<dim3(cdiv(P->ny, MG_TJ), cdiv(P->nx, MG_TI), P->cfg.batch), MG_THREADS, smem, st>>>(mp);
+    return check_launch(P, "maskgrad", st);
 }
 
 bool aligned16(const void *p) { return p && !((uintptr_t)p & 15); }
@@ -716,50 +631,14 @@ struct DeviceGuard {
     ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
 };
 
-// The whole path.  eps == nullptr skips F2-F6, dFdC == nullptr skips R1-R6.
-// Dependencies: forward <- filter;  reverse2d <- filter, zreduce;  filterT <- reverse2d.  zreduce
-// depends on nothing, so with overlap on (and a reverse pass requested) it starts at once on the
-// plan's auxiliary stream, the 2-D reverse chain follows it there, and filter -> forward run on the
-// caller's stream; the call joins the auxiliary stream back before returning (no host sync).
+// The whole path: filter -> tile -> maskgrad -> filterT.  eps == nullptr skips F6, dFdC == nullptr skips R1-R6.
 int run_chain(epsgrad_plan *P, const float *C, float beta, int n_pairs, const void *const *EF,
               const void *const *EA, float *eps, float *dFdC, cudaStream_t st)
 {
-    int rc = EPSGRAD_OK;
-    if (eps && dFdC && P->fuse_streams && !P->prof) {
-        // filter -> [forward + zreduce in one launch] -> reverse2d -> filterT; pairs beyond the
-        // first ZR_MAX_PAIRS are accumulated by plain zreduce launches
-        const int np0 = n_pairs < ZR_MAX_PAIRS ? n_pairs : ZR_MAX_PAIRS;
-        rc = launch_filter(P, C, ws_phi(P), st);
-        if (!rc) rc = launch_stream(P, ws_phi(P), beta, eps, np0, EF, EA, ws_gbar(P), st);
-        if (!rc && n_pairs > np0) rc = launch_zreduce(P, n_pairs - np0, EF + np0, EA + np0, ws_gbar(P), st, 1);
-        if (!rc) rc = launch_reverse2d(P, ws_phi(P), beta, ws_gbar(P), ws_v(P), st);
-        if (!rc) rc = launch_filterT(P, ws_v(P), dFdC, st);
-        return rc;
-    }
-    if (!dFdC || !P->overlap || P->prof) {
-        rc = launch_filter(P, C, ws_phi(P), st);
-        if (!rc && eps) rc = launch_forward(P, ws_phi(P), beta, eps, nullptr, st);
-        if (!rc && dFdC) rc = launch_zreduce(P, n_pairs, EF, EA, ws_gbar(P), st);
-        if (!rc && dFdC) rc = launch_reverse2d(P, ws_phi(P), beta, ws_gbar(P), ws_v(P), st);
-        if (!rc && dFdC) rc = launch_filterT(P, ws_v(P), dFdC, st);
-        return rc;
-    }
-    cudaStream_t ax = P->aux;
-    if (cudaEventRecord(P->ev_fork, st) != cudaSuccess || cudaStreamWaitEvent(ax, P->ev_fork, 0) != cudaSuccess) {
-        cudaGetLastError();
-        return EPSGRAD_ECUDA;
-    }
-    rc = launch_zreduce(P, n_pairs, EF, EA, ws_gbar(P), ax);
-    if (!rc) rc = launch_filter(P, C, ws_phi(P), st);
-    if (!rc && (cudaEventRecord(P->ev_filter, st) != cudaSuccess || cudaStreamWaitEvent(ax, P->ev_filter, 0) != cudaSuccess)) rc = EPSGRAD_ECUDA;
-    if (!rc) rc = launch_reverse2d(P, ws_phi(P), beta, ws_gbar(P), ws_v(P), ax);
-    if (!rc) rc = launch_filterT(P, ws_v(P), dFdC, ax);
-    if (!rc && eps) rc = launch_forward(P, ws_phi(P), beta, eps, nullptr, st);
-    // always join, even on error, so that the auxiliary stream never outlives the call
-    if (cudaEventRecord(P->ev_join, ax) != cudaSuccess || cudaStreamWaitEvent(st, P->ev_join, 0) != cudaSuccess) {
-        cudaGetLastError();
-        if (!rc) rc = EPSGRAD_ECUDA;
-    }
+    int rc = launch_filter(P, C, ws_phi(P), st);
+    if (!rc) rc = launch_tile(P, ws_phi(P), beta, eps, nullptr, dFdC ? n_pairs : 0, EF, EA, dFdC ? ws_res(P) : nullptr, nullptr, st);
+    if (!rc && dFdC) rc = launch_maskgrad(P, ws_phi(P), beta, ws_res(P), ws_v(P), st);
+    if (!rc && dFdC) rc = launch_filterT(P, ws_v(P), dFdC, st);
     return rc;
 }
 
@@ -875,7 +754,7 @@ extern "C" int epsgrad_stage_eps2d(epsgrad_plan_t *P, const float *C, float beta
     cudaStream_t st = (cudaStream_t)stream;
     begin_call(P, st);
     rc = launch_filter(P, C, ws_phi(P), st);
-    if (!rc) rc = launch_forward(P, ws_phi(P), beta, nullptr, eps2d, st);
+    if (!rc) rc = launch_tile(P, ws_phi(P), beta, nullptr, eps2d, 0, nullptr, nullptr, nullptr, nullptr, st);
     return rc;
 }
 
@@ -887,6 +766,10 @@ extern "C" int epsgrad_stage_zreduce(epsgrad_plan_t *P, int n_pairs, const void 
     if (rc) return rc;
     if (!aligned16(gbar)) return EPSGRAD_EINVAL;
     DeviceGuard g(P->device);
+    if (!P->ws) return EPSGRAD_ENOWORKSPACE;
     begin_call(P, (cudaStream_t)stream);
-    return launch_zreduce(P, n_pairs, EF, EA, gbar, (cudaStream_t)stream);
+    // the tile kernel needs a filter output to run its forward half on; its value does not enter the reduced planes
+    rc = cudaMemsetAsync(ws_phi(P), 0, (size_t)P->cfg.batch * P->px * P->py * 4, (cudaStream_t)stream) == cudaSuccess ? EPSGRAD_OK : EPSGRAD_ECUDA;
+    if (rc) return rc;
+    return launch_tile(P, ws_phi(P), 1.0f, nullptr, nullptr, n_pairs, EF, EA, nullptr, gbar, (cudaStream_t)stream);
 }

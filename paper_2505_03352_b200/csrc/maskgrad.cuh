@@ -1,0 +1,155 @@
+// maskgrad.cuh -- second half of R3, R4 and R5 in gather form: from the nine per-cell residual planes
+// the tile kernel left (tile.cuh) to the mask cotangent  v[p,q] = Phibar[p,q] / den[p,q]  that the transposed
+// filter (R6) gathers.
+//   R3b Dbar_c = Sobel^T(gxbar_c, gybar_c) with the replicate padding folded back at the borders (S5);
+//       AbarF_c = Abar_c + Dbar_c / deps
+//   R4  averages^T: each mask pixel gathers from the E_x, E_y, E_z cells whose footprint holds it
+//       (the clamped last pixel is counted s/2+1 times)
+//   R5  mixing^T, projection^T: rhobar = deps (ebar - rbar/e^2), Phibar = rhobar (beta/2) sech^2 t,
+//       sech^2 in the overflow-free form (the paper's custom tanh derivative rule)
+// One CTA per TI x TJ cells (s TI x s TJ mask pixels); owners of a tile's pixels lie on [i0-1, i0+TI-1], their
+// Sobel^T sources on [i0-2, i0+TI].
+#pragma once
+#include "common.cuh"
+
+namespace epsgrad {
+
+struct MaskGradParams {
+    const float *phi;      // [B,px,py]
+    const float *res;      // [B,9,nx,ny]
+    float *v;              // [B,px,py]
+    Normaliser nrm;
+    int nx, ny, px, py, s;
+    float beta, eta_r, eps_clad, deps;
+};
+
+constexpr int MG_TI = 16, MG_TJ = 16, MG_THREADS = 256;
+constexpr int MG_CI = MG_TI + 3, MG_CJ = MG_TJ + 3;        // staged cells: [i0-2, i0+TI] x [j0-2, j0+TJ]
+
+__host__ __device__ inline size_t maskgrad_smem_floats(int s)
+{
+    return (size_t)10 * MG_CI * MG_CJ + MG_TI * MG_TJ + (size_t)s * (MG_TI + MG_TJ);
+}
+
+// grid (ceil(ny/TJ), ceil(nx/TI), B).  S > 0: compile-time subpixel count; S = 0: runtime P.s.
+template <int S>
+__global__ void __launch_bounds__(MG_THREADS) k_maskgrad(const __grid_constant__ MaskGradParams P)
+{
+    extern __shared__ __align__(16) float sm[];
+    constexpr int TI = MG_TI, TJ = MG_TJ, NTH = MG_THREADS, CI = MG_CI, CJ = MG_CJ, NC = CI * CJ;
+    const int s = S > 0 ? S : P.s, hs = s >> 1;
+    float *R = sm;                     // [8][NC] staged residual planes: Hb, Ab, Gx, Gy for c = x then c = y
+    float *AbF = sm + 8 * NC;          // [2][NC]
+    float *AbZ = sm + 10 * NC;         // [TI*TJ]
+    int *nidx = reinterpret_cast<int *>(AbZ + TI * TJ);   // normaliser table row of each tile mask row, then column of each mask column
+
+    const int tid = threadIdx.x;
+    const int i0 = blockIdx.y * TI, j0 = blockIdx.x * TJ, b = blockIdx.z;
+    const int oi = i0 - 2, oj = j0 - 2;            // cell origin of the staged arrays
+    const int nx = P.nx, ny = P.ny, ncol = nx * ny;
+    const float inv_s2 = 1.0f / (float)(s * s), inv_deps = 1.0f / P.deps;
+    const float *rb = P.res + (size_t)b * 9 * ncol;
+    // tile whose 2-cell ring lies strictly inside the region: no folded border terms (block-uniform)
+    const bool inner = i0 >= 3 && j0 >= 3 && i0 + TI + 1 <= nx - 1 && j0 + TJ + 1 <= ny - 1;
+
+    for (int k = tid; k < s * (TI + TJ); k += NTH) {
+        const int along_x = k < s * TI;
+        const int pix = along_x ? s * i0 + k : s * j0 + (k - s * TI);
+        nidx[k] = along_x ? P.nrm.ix_of(min(pix, P.px - 1)) : P.nrm.iy_of(min(pix, P.py - 1));
+    }
+    for (int it = tid; it < 8 * NC; it += NTH) {
+        const int o = it / NC, rem = it - o * NC, ci = rem / CJ, cj = rem - ci * CJ;
+        const int i = oi + ci, j = oj + cj;
+        R[it] = (i >= 0 && i < nx && j >= 0 && j < ny) ? rb[(size_t)o * ncol + i * ny + j] : 0.0f;
+    }
+    for (int it = tid; it < TI * TJ; it += NTH) {
+        const int ti = it / TJ, tj = it - ti * TJ, i = i0 + ti, j = j0 + tj;
+        AbZ[it] = (i < nx && j < ny) ? rb[(size_t)8 * ncol + i * ny + j] : 0.0f;
+    }
+    __syncthreads();
+
+    // ---- Sobel^T with the replicate padding folded back, on the owner cells [i0-1, i0+TI-1] x [j0-1, j0+TJ-1]
+    {
+        constexpr int RI = TI + 1, RJ = TJ + 1;           // ci in [1, TI+1], cj in [1, TJ+1]
+        for (int it = tid; it < 2 * RI * RJ; it += NTH) {
+            const int c = it / (RI * RJ), rem = it - c * (RI * RJ);
+            const int ci = 1 + rem / RJ, cj = 1 + rem % RJ, i_ = ci * CJ + cj;
+            const int ii = oi + ci, jj = oj + cj;
+            float out = 0.f;
+            if (inner || (ii >= 0 && ii < nx && jj >= 0 && jj < ny)) {
+                float dbar = 0.f;
+                const float *gxs = R + (4 * c + 2) * NC, *gys = R + (4 * c + 3) * NC;
+                if (inner || (ii >= 1 && ii <= nx - 2 && jj >= 1 && jj <= ny - 2)) {
+                    // interior: the cell (ii-di, jj-dj) reached (ii,jj) through its stencil entry (di,dj)
+#pragma unroll
+                    for (int di = -1; di <= 1; ++di)
+#pragma unroll
+                        for (int dj = -1; dj <= 1; ++dj) {
+                            const int src = i_ - di * CJ - dj;
+                            const float kx = (float)(di * (2 - (dj < 0 ? -dj : dj))) * 0.125f;
+                            const float ky = (float)(dj * (2 - (di < 0 ? -di : di))) * 0.125f;
+                            dbar = fmaf(kx, gxs[src], fmaf(ky, gys[src], dbar));
+                        }
+                } else {
+                    // border: sources (i,di) with clamp(i+di) == ii: i = ii-di in range, plus the folded terms
+                    for (int cx = 0; cx < 5; ++cx) {
+                        int di, i;
+                        if (cx < 3) { di = cx - 1; i = ii - di; if (i < 0 || i >= nx) continue; }
+                        else if (cx == 3) { if (ii != 0) continue; di = -1; i = 0; }
+                        else { if (ii != nx - 1) continue; di = 1; i = nx - 1; }
+                        for (int cy = 0; cy < 5; ++cy) {
+                            int dj, j;
+                            if (cy < 3) { dj = cy - 1; j = jj - dj; if (j < 0 || j >= ny) continue; }
+                            else if (cy == 3) { if (jj != 0) continue; dj = -1; j = 0; }
+                            else { if (jj != ny - 1) continue; dj = 1; j = ny - 1; }
+                            const int src = (i - oi) * CJ + (j - oj);
+                            const float kx = (float)(di * (2 - (dj < 0 ? -dj : dj))) * 0.125f;
+                            const float ky = (float)(dj * (2 - (di < 0 ? -di : di))) * 0.125f;
+                            dbar = fmaf(kx, gxs[src], fmaf(ky, gys[src], dbar));
+                        }
+                    }
+                }
+                out = R[(4 * c + 1) * NC + i_] + dbar * inv_deps;
+            }
+            AbF[c * NC + i_] = out;
+        }
+    }
+    __syncthreads();
+
+    // ---- R4 + R5 per mask pixel of the tile
+    const int TP = s * TI, TQ = s * TJ;
+    const float *phib = P.phi + (size_t)b * P.px * P.py;
+    float *vb = P.v + (size_t)b * P.px * P.py;
+    for (int it = tid; it < TP * TQ; it += NTH) {
+        const int tp = it / TQ, tq = it - tp * TQ;
+        const int p = s * i0 + tp, q = s * j0 + tq;
+        if (p >= P.px || q >= P.py) continue;
+        const int iz = p / s, jz = q / s;
+        float ebar = AbZ[(iz - i0) * TJ + (jz - j0)], rbar = 0.f;
+        if (p >= hs) {                                       // E_x owner
+            const int ix = (p - hs) / s;
+            const float mlt = p == P.px - 1 ? (float)(1 + hs) : 1.0f;
+            const int idx = (ix - oi) * CJ + (jz - oj);
+            ebar = fmaf(mlt, AbF[idx], ebar);
+            rbar = fmaf(mlt, R[idx], rbar);
+        }
+        if (q >= hs) {                                       // E_y owner
+            const int jy = (q - hs) / s;
+            const float mlt = q == P.py - 1 ? (float)(1 + hs) : 1.0f;
+            const int idx = (iz - oi) * CJ + (jy - oj);
+            ebar = fmaf(mlt, AbF[NC + idx], ebar);
+            rbar = fmaf(mlt, R[4 * NC + idx], rbar);
+        }
+        // one exponential serves rho and its slope: a = exp(-2|t|), rho = 1/(1+a) or a/(1+a), slope = 2 beta a/(1+a)^2
+        const float t = P.beta * (phib[p * P.py + q] - P.eta_r);
+        const float a = __expf(-2.0f * fabsf(t));
+        const float d = fast_rcp(1.0f + a);
+        const float rho = t >= 0.f ? d : a * d;
+        const float r = fast_rcp(fmaf(P.deps, rho, P.eps_clad));   // 1/e
+        const float slope = 2.0f * P.beta * a * d * d;
+        const float rhobar = P.deps * inv_s2 * (ebar - rbar * r * r);
+        vb[p * P.py + q] = rhobar * slope * P.nrm.at_index(nidx[tp], nidx[TP + tq]);
+    }
+}
+
+}  // namespace epsgrad

@@ -116,25 +116,25 @@ def test_forward_vjp_equals_separate_calls_and_keeps_inputs():
     assert plan.last_launches() >= 4
 
 
-@pytest.mark.parametrize("n_pairs", [1, 9])
-def test_schedules_agree_bitwise(n_pairs):
-    # fused forward+zreduce launch (default), separate launches, and the two-stream schedule
+@pytest.mark.parametrize("n_pairs", [1, 9, 17])
+def test_entry_points_agree_bitwise(n_pairs):
+    # eps_forward_vjp, eps_forward and eps_vjp run the same tile kernel with halves switched off; more than
+    # EPSGRAD_MAX_PAIRS pairs are chained through accumulating launches
     cfg = B.make_config(batch=2, mx=27, my=22, nz=16, z_lo=6.25, z_hi=9.75, filter_radius=4.0)
     C = dev(rand_C(cfg, 16))
     EFn, EAn = rand_fields(cfg, n_pairs, 17)
     EF, EA = [dev(f) for f in EFn], [dev(f) for f in EAn]
     plan = B.Plan(cfg)
     eps0, g0 = plan.eps_forward_vjp(C, 8.0, EF, EA)
-    n_fused = plan.last_launches()
-    plan.set_fused_streams(False)
-    eps1, g1 = plan.eps_forward_vjp(C, 8.0, EF, EA)
-    assert plan.last_launches() == n_fused + 1
-    plan.set_overlap(True)
-    eps2, g2 = plan.eps_forward_vjp(C, 8.0, EF, EA)
-    g3 = plan.eps_vjp(C, 8.0, EF, EA)
+    assert plan.last_launches() == 3 + (n_pairs + 7) // 8
+    eps1 = plan.eps_forward(C, 8.0)
+    g1 = plan.eps_vjp(C, 8.0, EF, EA)
     torch.cuda.synchronize()
-    assert torch.equal(eps0, eps1) and torch.equal(g0, g1) and torch.equal(eps0, eps2) and torch.equal(g0, g2)
-    assert torch.equal(g0, g3)
+    assert torch.equal(eps0, eps1) and torch.equal(g0, g1)
+    if n_pairs > 1:
+        # linearity in the pairs: the sum of single-pair gradients
+        gs = sum(plan.eps_vjp(C, 8.0, [f], [a]).double() for f, a in zip(EF, EA))
+        assert float((gs - g0.double()).abs().max()) < 1e-5 * float(g0.abs().max())
 
 
 def test_calls_are_cuda_graph_capturable():
@@ -146,16 +146,13 @@ def test_calls_are_cuda_graph_capturable():
     eps_ref, g_ref = plan.eps_forward_vjp(C, 8.0, EF, EA)
     eps, g = torch.zeros_like(eps_ref), torch.zeros_like(g_ref)
     torch.cuda.synchronize()
-    for overlap in (False, True):
-        plan.set_overlap(overlap)
-        plan.set_fused_streams(not overlap)
-        graph = torch.cuda.CUDAGraph()
-        with torch.cuda.graph(graph):
-            plan.eps_forward_vjp(C, 8.0, EF, EA, eps, g)
-        eps.zero_(); g.zero_()
-        graph.replay()
-        torch.cuda.synchronize()
-        assert torch.equal(eps, eps_ref) and torch.equal(g, g_ref)
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        plan.eps_forward_vjp(C, 8.0, EF, EA, eps, g)
+    eps.zero_(); g.zero_()
+    graph.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(eps, eps_ref) and torch.equal(g, g_ref)
 
 
 def test_real_cotangent_special_case():
