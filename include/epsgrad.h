@@ -84,8 +84,8 @@ typedef struct {
 int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsgrad_plan_t **out);
 int epsgrad_plan_destroy(epsgrad_plan_t *plan);
 
-/* Scratch the device entry points need (filter output Phi, per-cell reverse residual planes,
- * mask cotangent, separable-filter temporaries).  The caller allocates it (e.g. a torch
+/* Scratch the device entry points need (filter output Phi, 2-D stage and reverse coefficient planes,
+ * reduced cotangent, mask cotangent, separable-filter temporaries).  The caller allocates it (e.g. a torch
  * uint8 tensor) and keeps it alive and unshared while calls of this plan are in flight. */
 size_t epsgrad_workspace_bytes(const epsgrad_plan_t *plan);
 int    epsgrad_plan_set_workspace(epsgrad_plan_t *plan, void *dev_ptr, size_t bytes);
@@ -100,6 +100,14 @@ int    epsgrad_plan_set_staging(epsgrad_plan_t *plan, void *dev_ptr, size_t byte
  * are identical; this is a measurement switch.                                           */
 int epsgrad_plan_set_dense_reads(epsgrad_plan_t *plan, int dense);
 
+/* Two-stream schedule (default on).  The path has two HBM-bound kernels -- the Eq. (1) field reads, which depend
+ * on nothing, and the eps stores -- and four small L2-resident ones.  Calls that compute dF/dC fork the plan's auxiliary
+ * stream from `stream` (event), run the field reads there beside filter -> 2-D chain, then the 2-D reverse chain and the
+ * transposed filter there beside the eps stores, and join it back (event) before returning: to the caller everything is
+ * still ordered on `stream`, with no host synchronisation, and the calls remain CUDA-graph capturable.  0 = one stream,
+ * strictly serial (also used while per-kernel profiling is on).  Results are bitwise identical.                        */
+int epsgrad_plan_set_overlap(epsgrad_plan_t *plan, int enable);
+
 /* Number of kernel launches the last eps_* call of this plan enqueued (for accounting). */
 int epsgrad_plan_last_launches(const epsgrad_plan_t *plan);
 
@@ -112,6 +120,14 @@ int epsgrad_plan_last_launches(const epsgrad_plan_t *plan);
  * when profiling was off.  Negative return = error.                                     */
 int epsgrad_plan_set_profiling(epsgrad_plan_t *plan, int enable);
 int epsgrad_plan_last_kernel_times(epsgrad_plan_t *plan, int max_n, float *ms, const char **names);
+
+/* Timeline of one call (diagnostic; default off).  When enabled, a one-thread kernel that stores the device clock
+ * (%globaltimer, ns) is enqueued at the start of a two-stream call and after each kernel on that kernel's stream (up to
+ * 32 stamps), so the stamps show when each kernel of either stream ended.  epsgrad_plan_read_timeline synchronises the
+ * device (host-blocking) and returns the number n of stamps of the last call with their names ("begin" or the kernel
+ * whose end they mark).  The extra kernels perturb the schedule slightly; not for timed runs.                          */
+int epsgrad_plan_set_timeline(epsgrad_plan_t *plan, int enable);
+int epsgrad_plan_read_timeline(epsgrad_plan_t *plan, int max_n, uint64_t *ns, const char **names);
 
 /* ---- the hot path (device pointers) -------------------------------------------------- */
 /* eps_hat(C, beta): the whole forward chain.  beta > 0 (it changes every
@@ -142,8 +158,7 @@ int epsgrad_plan_last_copy_bytes(const epsgrad_plan_t *plan, uint64_t *h2d, uint
 int epsgrad_stage_filter(epsgrad_plan_t *plan, const float *C, float *phi_centred, void *stream);
 /* eps2d [B,3,Nx,Ny]: the 2-D stage before z-extrusion (steps 1-6).                      */
 int epsgrad_stage_eps2d(epsgrad_plan_t *plan, const float *C, float beta, float *eps2d, void *stream);
-/* z-reduced cotangent [B,5,Nx,Ny]: planes x, y, z(full cells), z(lower face), z(upper face).
- * Runs the tile kernel on a zeroed filter output, so it needs (and overwrites part of) the workspace. */
+/* z-reduced cotangent [B,5,Nx,Ny]: planes x, y, z(full cells), z(lower face), z(upper face). */
 int epsgrad_stage_zreduce(epsgrad_plan_t *plan, int n_pairs, const void *const *EF,
                           const void *const *EA, float *gbar, void *stream);
 

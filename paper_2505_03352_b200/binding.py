@@ -19,7 +19,7 @@ EXPORTS = (
     "epsgrad_plan_create", "epsgrad_plan_destroy", "epsgrad_workspace_bytes",
     "epsgrad_plan_set_workspace", "epsgrad_staging_bytes", "epsgrad_plan_set_staging",
     "epsgrad_plan_set_dense_reads", "epsgrad_plan_last_launches", "epsgrad_plan_last_copy_bytes",
-    "epsgrad_plan_set_profiling", "epsgrad_plan_last_kernel_times", 
+    "epsgrad_plan_set_profiling", "epsgrad_plan_last_kernel_times", "epsgrad_plan_set_overlap", "epsgrad_plan_set_timeline", "epsgrad_plan_read_timeline", 
     "eps_forward", "eps_vjp", "eps_forward_vjp", "eps_forward_vjp_host",
     "epsgrad_stage_filter", "epsgrad_stage_eps2d", "epsgrad_stage_zreduce",
     "epsgrad_status_string", "epsgrad_version",
@@ -104,6 +104,9 @@ def lib() -> ctypes.CDLL:
     L.eps_forward_vjp_host.argtypes = [vp, vp, f32, i32, vp, vp, vp, vp, vp]
     L.epsgrad_stage_filter.argtypes = [vp, vp, vp, vp]
     L.epsgrad_stage_eps2d.argtypes = [vp, vp, f32, vp, vp]
+    L.epsgrad_plan_set_overlap.argtypes = [vp, i32]
+    L.epsgrad_plan_set_timeline.argtypes = [vp, i32]
+    L.epsgrad_plan_read_timeline.argtypes = [vp, i32, vp, vp]
     L.epsgrad_stage_zreduce.argtypes = [vp, i32, vp, vp, vp, vp]
     L.epsgrad_status_string.argtypes = [i32]
     L.epsgrad_status_string.restype = ctypes.c_char_p
@@ -205,6 +208,20 @@ class Plan:
         a, b = ctypes.c_uint64(), ctypes.c_uint64()
         _check(lib().epsgrad_plan_last_copy_bytes(self._h, ctypes.byref(a), ctypes.byref(b)), "last_copy_bytes")
         return int(a.value), int(b.value)
+
+    def set_overlap(self, enable: bool) -> None:
+        _check(lib().epsgrad_plan_set_overlap(self._h, int(bool(enable))), "epsgrad_plan_set_overlap")
+
+    def set_timeline(self, enable: bool) -> None:
+        _check(lib().epsgrad_plan_set_timeline(self._h, int(bool(enable))), "epsgrad_plan_set_timeline")
+
+    def read_timeline(self):
+        """[(name, ns since the first stamp)] of the last call (synchronises the device)"""
+        ns = (ctypes.c_uint64 * 32)()
+        names = (ctypes.c_char_p * 32)()
+        n = lib().epsgrad_plan_read_timeline(self._h, 32, ns, names)
+        _check(min(n, 0), "epsgrad_plan_read_timeline")
+        return [(names[i].decode(), int(ns[i]) - int(ns[0])) for i in range(n)]
 
     def set_profiling(self, enable: bool) -> None:
         _check(lib().epsgrad_plan_set_profiling(self._h, int(bool(enable))), "epsgrad_plan_set_profiling")

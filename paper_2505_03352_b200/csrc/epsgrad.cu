@@ -12,7 +12,9 @@
 #include "filter.cuh"
 #include "filter4.cuh"
 #include "filter_sep.cuh"
-#include "tile.cuh"
+#include "fwd2d.cuh"
+#include "extrude.cuh"
+#include "zreduce.cuh"
 #include "maskgrad.cuh"
 
 using namespace epsgrad;
@@ -42,13 +44,27 @@ struct epsgrad_plan {
     void *ws; size_t ws_bytes;
     void *stg; size_t stg_bytes;
     // workspace carve-up (byte offsets)
-    size_t off_phi, off_v, off_res, off_tmp, ws_need;
+    size_t off_phi, off_v, off_gbar, off_e2d, off_coef, off_tmp, ws_need;
     int last_launches;
     uint64_t last_h2d, last_d2h;
     // optional per-kernel timing (epsgrad_plan_set_profiling)
     int prof;
     cudaEvent_t ev[EPSGRAD_MAX_KERNELS + 1];
+    // two-stream schedule: the field stream (zreduce) runs beside filter -> fwd2d, the 2-D reverse chain beside the eps stores
+    int overlap;
+    cudaStream_t aux;
+    cudaEvent_t ev_fork, ev_r, ev_2d, ev_join;
     const char *kname[EPSGRAD_MAX_KERNELS];
+    // optional device-clock stamps between the kernels of both streams (epsgrad_plan_set_timeline)
+    unsigned long long *d_tl;
+    int n_tl;
+    const char *tlname[2 * EPSGRAD_MAX_KERNELS];
+};
+
+struct DeviceGuardC {
+    int prev;
+    explicit DeviceGuardC(int dev) { cudaGetDevice(&prev); if (prev != dev) cudaSetDevice(dev); else prev = -1; }
+    ~DeviceGuardC() { if (prev >= 0) cudaSetDevice(prev); }
 };
 
 static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
@@ -233,7 +249,7 @@ extern "C" int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsg
         const size_t need = ((size_t)NT * NT * m * m + (size_t)m * (ta + 2 * T) * m * (tb + 2 * T) + 2 * NT) * 4;
         if (need > 200 * 1024) { delete P; return EPSGRAD_EUNSUPPORTED; }
     }
-    if (tile_smem_floats(s, nz) * 4 + (size_t)2 * TILE_STAGE_CELLS * 13 * 16 > 200 * 1024 || maskgrad_smem_floats(s) * 4 > 200 * 1024) { delete P; return EPSGRAD_EUNSUPPORTED; }
+    if (fwd2d_smem_floats(s) * 4 > 200 * 1024 || maskgrad_smem_floats(s) * 4 > 200 * 1024) { delete P; return EPSGRAD_EUNSUPPORTED; }
 
     // ---- upload
     int prev = 0;
@@ -261,12 +277,32 @@ extern "C" int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsg
         return EPSGRAD_ECUDA;
     }
 
+    // ---- auxiliary stream and fork/join events (no timing) for the two-stream schedule
+    {
+        int prev2 = 0;
+        cudaGetDevice(&prev2);
+        cudaSetDevice(device);
+        // highest priority: the small kernels it carries must get SM slots ahead of the pending CTAs of the HBM-bound kernels
+        int prio_least = 0, prio_greatest = 0;
+        cudaDeviceGetStreamPriorityRange(&prio_least, &prio_greatest);
+        bool ok = cudaStreamCreateWithPriority(&P->aux, cudaStreamNonBlocking, prio_greatest) == cudaSuccess &&
+                  cudaEventCreateWithFlags(&P->ev_fork, cudaEventDisableTiming) == cudaSuccess &&
+                  cudaEventCreateWithFlags(&P->ev_r, cudaEventDisableTiming) == cudaSuccess &&
+                  cudaEventCreateWithFlags(&P->ev_2d, cudaEventDisableTiming) == cudaSuccess &&
+                  cudaEventCreateWithFlags(&P->ev_join, cudaEventDisableTiming) == cudaSuccess;
+        cudaSetDevice(prev2);
+        if (!ok) { cudaGetLastError(); epsgrad_plan_destroy(P); return EPSGRAD_ECUDA; }
+        P->overlap = 1;
+    }
+
     // ---- workspace carve-up
     const size_t n_mask = (size_t)cfg->batch * P->px * P->py, n_cell = (size_t)cfg->batch * P->nx * P->ny;
     size_t off = 0;
     P->off_phi = off;  off += align_up(n_mask * 4, 256);
     P->off_v = off;    off += align_up(n_mask * 4, 256);
-    P->off_res = off;  off += align_up(n_cell * TILE_NRES * 4, 256);
+    P->off_gbar = off; off += align_up(n_cell * 5 * 4, 256);
+    P->off_e2d = off;  off += align_up(n_cell * F2_NE2D * 4, 256);
+    P->off_coef = off; off += align_up(n_cell * F2_NCOEF * 4, 256);
     P->off_tmp = off;  off += P->separable ? align_up((size_t)cfg->batch * cfg->mx * P->py * 4, 256) : 0;
     P->ws_need = off;
     *out = P;
@@ -277,6 +313,12 @@ extern "C" int epsgrad_plan_destroy(epsgrad_plan_t *P)
 {
     if (!P) return EPSGRAD_EINVAL;
     if (P->d_tables) cudaFree(P->d_tables);
+    if (P->d_tl) cudaFree(P->d_tl);
+    if (P->aux) cudaStreamDestroy(P->aux);
+    if (P->ev_fork) cudaEventDestroy(P->ev_fork);
+    if (P->ev_r) cudaEventDestroy(P->ev_r);
+    if (P->ev_2d) cudaEventDestroy(P->ev_2d);
+    if (P->ev_join) cudaEventDestroy(P->ev_join);
     if (P->ev[0])
         for (int i = 0; i <= EPSGRAD_MAX_KERNELS; ++i) cudaEventDestroy(P->ev[i]);
     delete P;
@@ -351,6 +393,39 @@ extern "C" int epsgrad_plan_set_dense_reads(epsgrad_plan_t *P, int dense)
     return EPSGRAD_OK;
 }
 
+extern "C" int epsgrad_plan_set_overlap(epsgrad_plan_t *P, int enable)
+{
+    if (!P) return EPSGRAD_EINVAL;
+    P->overlap = enable != 0;
+    return EPSGRAD_OK;
+}
+
+extern "C" int epsgrad_plan_set_timeline(epsgrad_plan_t *P, int enable)
+{
+    if (!P) return EPSGRAD_EINVAL;
+    if (enable && !P->d_tl) {
+        DeviceGuardC g(P->device);
+        if (cudaMalloc(&P->d_tl, 2 * EPSGRAD_MAX_KERNELS * sizeof(unsigned long long)) != cudaSuccess) { cudaGetLastError(); P->d_tl = nullptr; return EPSGRAD_ECUDA; }
+    } else if (!enable && P->d_tl) {
+        cudaFree(P->d_tl);
+        P->d_tl = nullptr;
+    }
+    P->n_tl = 0;
+    return EPSGRAD_OK;
+}
+
+extern "C" int epsgrad_plan_read_timeline(epsgrad_plan_t *P, int max_n, uint64_t *ns, const char **names)
+{
+    if (!P || max_n < 0 || (max_n > 0 && (!ns || !names))) return EPSGRAD_EINVAL;
+    if (!P->d_tl) return 0;
+    const int n = P->n_tl < max_n ? P->n_tl : max_n;
+    DeviceGuardC g(P->device);
+    if (cudaDeviceSynchronize() != cudaSuccess ||
+        cudaMemcpy(ns, P->d_tl, n * sizeof(unsigned long long), cudaMemcpyDeviceToHost) != cudaSuccess) { cudaGetLastError(); return EPSGRAD_ECUDA; }
+    for (int i = 0; i < n; ++i) names[i] = P->tlname[i];
+    return n;
+}
+
 extern "C" int epsgrad_plan_last_launches(const epsgrad_plan_t *P) { return P ? P->last_launches : 0; }
 
 extern "C" int epsgrad_plan_last_copy_bytes(const epsgrad_plan_t *P, uint64_t *h2d, uint64_t *d2h)
@@ -392,9 +467,25 @@ int set_smem(K kernel, size_t bytes)
     return EPSGRAD_OK;
 }
 
+__global__ void k_stamp(unsigned long long *slot)
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+    *slot = t;
+}
+
+// timeline on: a one-thread kernel that stores the device clock runs at this point of stream `st`
+void stamp(epsgrad_plan *P, const char *what, cudaStream_t st)
+{
+    if (!P->d_tl || P->n_tl >= 2 * EPSGRAD_MAX_KERNELS) return;
+    P->tlname[P->n_tl] = what;
+    k_stamp<<<1, 1, 0, st>>>(P->d_tl + P->n_tl++);
+}
+
 void begin_call(epsgrad_plan *P, cudaStream_t st)
 {
     P->last_launches = 0;
+    P->n_tl = 0;
     if (P->prof) cudaEventRecord(P->ev[0], st);
 }
 
@@ -405,6 +496,7 @@ int check_launch(epsgrad_plan *P, const char *name, cudaStream_t st)
         P->kname[idx] = name;
         if (P->prof) cudaEventRecord(P->ev[idx + 1], st);
     }
+    stamp(P, name, st);
     return cudaGetLastError() == cudaSuccess ? EPSGRAD_OK : EPSGRAD_ECUDA;
 }
 
@@ -418,7 +510,9 @@ Normaliser make_nrm(const epsgrad_plan *P)
 
 float *ws_phi(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_phi); }
 float *ws_v(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_v); }
-float *ws_res(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_res); }
+float *ws_gbar(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_gbar); }
+float *ws_e2d(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_e2d); }
+float *ws_coef(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_coef); }
 float *ws_tmp(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_tmp); }
 
 // ---- F1: C -> centred Phi on the mask
@@ -544,60 +638,74 @@ int launch_filterT(epsgrad_plan *P, const float *v, float *dC, cudaStream_t st)
     return EPSGRAD_EUNSUPPORTED;
 }
 
-// ---- F2..F6 + R1..R3a: the tile kernel (tile.cuh).  eps / eps2d / gtap / res may be null; n_pairs == 0 skips the reverse half.
-// More than TILE_MAX_PAIRS pairs are chained: R2/R3a are linear in the cotangent, so later launches accumulate into res.
-int launch_tile(epsgrad_plan *P, const float *phi, float beta, float *eps, float *eps2d, int n_pairs,
-                const void *const *EF, const void *const *EA, float *res, float *gtap, cudaStream_t st)
+// ---- F2..F5: the 2-D chain; e2d / coef / eps2d may be null
+int launch_fwd2d(epsgrad_plan *P, const float *phi, float beta, float *e2d, float *coef, float *eps2d, cudaStream_t st)
 {
-    TileParams tp;
-    tp.phi = phi; tp.zw = P->d_zw;
-    tp.nx = P->nx; tp.ny = P->ny; tp.nz = P->cfg.nz; tp.px = P->px; tp.py = P->py; tp.s = P->cfg.subpixel;
-    tp.beta = beta; tp.eta_r = P->eta_r; tp.eps_clad = P->eps_clad; tp.deps = P->deps; tp.delta = P->delta;
-    tp.w_lo = P->w_lo; tp.w_hi = P->w_hi;
-    int maxnch = 1;
-    for (int g = 0; g < 2; ++g) {
-        tp.ch0[g] = P->dense ? 0 : P->ch0[g];
-        tp.nch[g] = P->dense ? P->cfg.nz / 2 : P->nch[g];
-        if (tp.nch[g] > maxnch) maxnch = tp.nch[g];
-        tp.chs[g] = 0;
-        while ((1 << tp.chs[g]) < tp.nch[g]) ++tp.chs[g];
-        if (tp.chs[g] > 8) return EPSGRAD_EUNSUPPORTED;     // window wider than one CTA pass (nz > 1024)
-    }
-    const int rows = 2 * tp.nch[0] + tp.nch[1];
-    tp.ncp = tile_cells_per_pass(rows);
-    if (tp.ncp < 1) return EPSGRAD_EUNSUPPORTED;
-    // windows of at most 128 bytes per column: ask for 64-byte fills
-    tp.sparse = maxnch * 16 <= 128 && tp.nz * 8 > 128;
-    const size_t smem = tile_smem_floats(tp.s, tp.nz) * 4 + (n_pairs > 0 ? (size_t)2 * rows * tp.ncp * 16 : 0);
-    void (*kern)(const TileParams);
-    if (tp.sparse) kern = tp.s == 2 ? k_tile<2, true> : (tp.s == 4 ? k_tile<4, true> : k_tile<0, true>);
-    else kern = tp.s == 2 ? k_tile<2, false> : (tp.s == 4 ? k_tile<4, false> : k_tile<0, false>);
+    Fwd2dParams fp;
+    fp.phi = phi; fp.e2d = e2d; fp.coef = coef; fp.eps2d = eps2d;
+    fp.nx = P->nx; fp.ny = P->ny; fp.px = P->px; fp.py = P->py; fp.s = P->cfg.subpixel;
+    fp.beta = beta; fp.eta_r = P->eta_r; fp.eps_clad = P->eps_clad; fp.deps = P->deps; fp.delta = P->delta;
+    fp.w_lo = P->w_lo; fp.w_hi = P->w_hi;
+    const size_t smem = fwd2d_smem_floats(fp.s) * 4;
+    auto kern = fp.s == 2 ? k_fwd2d<2> : (fp.s == 4 ? k_fwd2d<4> : k_fwd2d<0>);
     int rc = set_smem(kern, smem);
     if (rc) return rc;
-    const dim3 grid(cdiv(P->ny, TILE_TJ), cdiv(P->nx, TILE_TI), P->cfg.batch);
-    int p0 = 0;
-    do {
-        const int np = n_pairs - p0 < TILE_MAX_PAIRS ? n_pairs - p0 : TILE_MAX_PAIRS;
-        for (int p = 0; p < TILE_MAX_PAIRS; ++p) {
-            tp.ef[p] = (const float4 *)(p < np ? EF[p0 + p] : nullptr);
-            tp.ea[p] = (const float4 *)(p < np ? EA[p0 + p] : nullptr);
+    kern<<<dim3(cdiv(P->ny, F2_TJ), cdiv(P->nx, F2_TI), P->cfg.batch), F2_THREADS, smem, st>>>(fp);
+    return check_launch(P, "fwd2d", st);
+}
+
+// ---- F6: the eps store stream
+int launch_extrude(epsgrad_plan *P, const float *e2d, float *eps, cudaStream_t st)
+{
+    ExtrudeParams ep;
+    ep.e2d = e2d; ep.eps = eps; ep.zw = P->d_zw; ep.ncol = P->nx * P->ny; ep.nz = P->cfg.nz;
+    k_extrude<<<dim3(cdiv(ep.ncol, extrude_cols_per_cta(ep.nz)), P->cfg.batch), EX_THREADS, 0, st>>>(ep);
+    return check_launch(P, "extrude", st);
+}
+
+// ---- R1: the field read stream; more than ZR_MAX_PAIRS pairs are chained through accumulating launches
+int launch_zreduce(epsgrad_plan *P, int n_pairs, const void *const *EF, const void *const *EA, float *gbar, cudaStream_t st)
+{
+    ZredParams zp;
+    zp.gbar = gbar; zp.zw = P->d_zw; zp.ncol = P->nx * P->ny; zp.nz = P->cfg.nz;
+    int maxnch = 1;
+    for (int g = 0; g < 2; ++g) {
+        zp.ch0[g] = P->dense ? 0 : P->ch0[g];
+        zp.nch[g] = P->dense ? P->cfg.nz / 2 : P->nch[g];
+        if (zp.nch[g] > maxnch) maxnch = zp.nch[g];
+        zp.chs[g] = 0;
+        while ((1 << zp.chs[g]) < zp.nch[g]) ++zp.chs[g];
+        if (zp.chs[g] > 8) return EPSGRAD_EUNSUPPORTED;     // window wider than one CTA pass (nz > 512)
+    }
+    const int rows = 2 * zp.nch[0] + zp.nch[1];
+    zp.ncp = zred_cols_per_pass(rows);
+    if (zp.ncp < 1) return EPSGRAD_EUNSUPPORTED;
+    // windows of at most 128 bytes per column: ask for 64-byte fills
+    const bool sparse = maxnch * 16 <= 128 && zp.nz * 8 > 128;
+    const size_t smem = (size_t)2 * rows * zp.ncp * 16 + (size_t)5 * zp.nz * 4;
+    auto kern = sparse ? k_zreduce<true> : k_zreduce<false>;
+    int rc = set_smem(kern, smem);
+    if (rc) return rc;
+    const dim3 grid(cdiv(zp.ncol, ZR_COLS), P->cfg.batch);
+    for (int p0 = 0; p0 < n_pairs; p0 += ZR_MAX_PAIRS) {
+        const int np = n_pairs - p0 < ZR_MAX_PAIRS ? n_pairs - p0 : ZR_MAX_PAIRS;
+        for (int p = 0; p < ZR_MAX_PAIRS; ++p) {
+            zp.ef[p] = (const float4 *)(p < np ? EF[p0 + p] : nullptr);
+            zp.ea[p] = (const float4 *)(p < np ? EA[p0 + p] : nullptr);
         }
-        tp.n_pairs = np; tp.accumulate = p0 > 0;
-        tp.eps = p0 == 0 ? eps : nullptr; tp.eps2d = p0 == 0 ? eps2d : nullptr;
-        tp.res = res; tp.gtap = gtap;
-        kern<<<grid, TILE_THREADS, smem, st>>>(tp);
-        rc = check_launch(P, "tile", st);
+        zp.n_pairs = np; zp.accumulate = p0 > 0;
+        kern<<<grid, ZR_THREADS, smem, st>>>(zp);
+        rc = check_launch(P, "zreduce", st);
         if (rc) return rc;
-        p0 += TILE_MAX_PAIRS;
-    } while (p0 < n_pairs);
+    }
     return EPSGRAD_OK;
 }
 
-// ---- R3b..R5
-int launch_maskgrad(epsgrad_plan *P, const float *phi, float beta, const float *res, float *v, cudaStream_t st)
+// ---- R2..R5
+int launch_maskgrad(epsgrad_plan *P, const float *phi, float beta, const float *gbar, const float *coef, float *v, cudaStream_t st)
 {
     MaskGradParams mp;
-    mp.phi = phi; mp.res = res; mp.v = v; mp.nrm = make_nrm(P);
+    mp.phi = phi; mp.gbar = gbar; mp.coef = coef; mp.v = v; mp.nrm = make_nrm(P);
     mp.nx = P->nx; mp.ny = P->ny; mp.px = P->px; mp.py = P->py; mp.s = P->cfg.subpixel;
     mp.beta = beta; mp.eta_r = P->eta_r; mp.eps_clad = P->eps_clad; mp.deps = P->deps;
     const size_t smem = maskgrad_smem_floats(mp.s) * 4;
@@ -631,14 +739,51 @@ struct DeviceGuard {
     ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
 };
 
-// The whole path: filter -> tile -> maskgrad -> filterT.  eps == nullptr skips F6, dFdC == nullptr skips R1-R6.
+// The whole path.  eps == nullptr skips F6, dFdC == nullptr skips R1-R6.
+// Dependencies: fwd2d <- filter;  extrude <- fwd2d;  maskgrad <- zreduce, fwd2d;  filterT <- maskgrad;  zreduce <- nothing.
+// Two HBM-bound kernels (zreduce: field reads; extrude: eps stores) and four small L2-resident ones.  Running the two
+// HBM streams at once gains nothing (measured: DRAM is the shared limit); hiding the small kernels under
+// them does.  With overlap on, the small kernels go to the plan's auxiliary stream, which has the highest priority so
+// that their CTAs are placed ahead of the pending CTAs of the big kernels: filter -> fwd2d run there beside zreduce,
+// then maskgrad -> filterT beside extrude (which follows zreduce on the caller's stream).  The call joins the auxiliary
+// stream back before returning: to the caller everything is ordered on `stream`, there is no host synchronisation, and
+// the call stays CUDA-graph capturable.
 int run_chain(epsgrad_plan *P, const float *C, float beta, int n_pairs, const void *const *EF,
               const void *const *EA, float *eps, float *dFdC, cudaStream_t st)
 {
-    int rc = launch_filter(P, C, ws_phi(P), st);
-    if (!rc) rc = launch_tile(P, ws_phi(P), beta, eps, nullptr, dFdC ? n_pairs : 0, EF, EA, dFdC ? ws_res(P) : nullptr, nullptr, st);
-    if (!rc && dFdC) rc = launch_maskgrad(P, ws_phi(P), beta, ws_res(P), ws_v(P), st);
-    if (!rc && dFdC) rc = launch_filterT(P, ws_v(P), dFdC, st);
+    int rc = EPSGRAD_OK;
+    if (!dFdC || !P->overlap || P->prof) {
+        rc = launch_filter(P, C, ws_phi(P), st);
+        if (!rc) rc = launch_fwd2d(P, ws_phi(P), beta, eps ? ws_e2d(P) : nullptr, dFdC ? ws_coef(P) : nullptr, nullptr, st);
+        if (!rc && dFdC) rc = launch_zreduce(P, n_pairs, EF, EA, ws_gbar(P), st);
+        if (!rc && eps) rc = launch_extrude(P, ws_e2d(P), eps, st);
+        if (!rc && dFdC) rc = launch_maskgrad(P, ws_phi(P), beta, ws_gbar(P), ws_coef(P), ws_v(P), st);
+        if (!rc && dFdC) rc = launch_filterT(P, ws_v(P), dFdC, st);
+        return rc;
+    }
+    cudaStream_t ax = P->aux;
+    stamp(P, "begin", st);
+    if (cudaEventRecord(P->ev_fork, st) != cudaSuccess || cudaStreamWaitEvent(ax, P->ev_fork, 0) != cudaSuccess) {
+        cudaGetLastError();
+        return EPSGRAD_ECUDA;
+    }
+    rc = launch_filter(P, C, ws_phi(P), ax);
+    if (!rc) rc = launch_zreduce(P, n_pairs, EF, EA, ws_gbar(P), st);
+    if (!rc && cudaEventRecord(P->ev_r, st) != cudaSuccess) rc = EPSGRAD_ECUDA;
+    if (!rc) rc = launch_fwd2d(P, ws_phi(P), beta, eps ? ws_e2d(P) : nullptr, ws_coef(P), nullptr, ax);
+    if (!rc && cudaEventRecord(P->ev_2d, ax) != cudaSuccess) rc = EPSGRAD_ECUDA;
+    if (!rc && cudaStreamWaitEvent(ax, P->ev_r, 0) != cudaSuccess) rc = EPSGRAD_ECUDA;
+    if (!rc) rc = launch_maskgrad(P, ws_phi(P), beta, ws_gbar(P), ws_coef(P), ws_v(P), ax);
+    if (!rc && eps) {
+        if (cudaStreamWaitEvent(st, P->ev_2d, 0) != cudaSuccess) rc = EPSGRAD_ECUDA;
+        if (!rc) rc = launch_extrude(P, ws_e2d(P), eps, st);
+    }
+    if (!rc) rc = launch_filterT(P, ws_v(P), dFdC, ax);
+    // always join, even on error, so that the auxiliary stream never outlives the call
+    if (cudaEventRecord(P->ev_join, ax) != cudaSuccess || cudaStreamWaitEvent(st, P->ev_join, 0) != cudaSuccess) {
+        cudaGetLastError();
+        if (!rc) rc = EPSGRAD_ECUDA;
+    }
     return rc;
 }
 
@@ -754,7 +899,7 @@ extern "C" int epsgrad_stage_eps2d(epsgrad_plan_t *P, const float *C, float beta
     cudaStream_t st = (cudaStream_t)stream;
     begin_call(P, st);
     rc = launch_filter(P, C, ws_phi(P), st);
-    if (!rc) rc = launch_tile(P, ws_phi(P), beta, nullptr, eps2d, 0, nullptr, nullptr, nullptr, nullptr, st);
+    if (!rc) rc = launch_fwd2d(P, ws_phi(P), beta, nullptr, nullptr, eps2d, st);
     return rc;
 }
 
@@ -766,10 +911,6 @@ extern "C" int epsgrad_stage_zreduce(epsgrad_plan_t *P, int n_pairs, const void 
     if (rc) return rc;
     if (!aligned16(gbar)) return EPSGRAD_EINVAL;
     DeviceGuard g(P->device);
-    if (!P->ws) return EPSGRAD_ENOWORKSPACE;
     begin_call(P, (cudaStream_t)stream);
-    // the tile kernel needs a filter output to run its forward half on; its value does not enter the reduced planes
-    rc = cudaMemsetAsync(ws_phi(P), 0, (size_t)P->cfg.batch * P->px * P->py * 4, (cudaStream_t)stream) == cudaSuccess ? EPSGRAD_OK : EPSGRAD_ECUDA;
-    if (rc) return rc;
-    return launch_tile(P, ws_phi(P), 1.0f, nullptr, nullptr, n_pairs, EF, EA, nullptr, gbar, (cudaStream_t)stream);
+    return launch_zreduce(P, n_pairs, EF, EA, gbar, (cudaStream_t)stream);
 }

@@ -1,6 +1,8 @@
-// maskgrad.cuh -- second half of R3, R4 and R5 in gather form: from the nine per-cell residual planes
-// the tile kernel left (tile.cuh) to the mask cotangent  v[p,q] = Phibar[p,q] / den[p,q]  that the transposed
-// filter (R6) gathers.
+// maskgrad.cuh -- R2..R5 in gather form: from the z-reduced cotangent G (zreduce.cuh) and the per-cell
+// coefficients the forward 2-D kernel left (fwd2d.cuh) to the mask cotangent  v[p,q] = Phibar[p,q] / den[p,q]  that the
+// transposed filter (R6) gathers.
+//   R2/R3a Eq. (7)^T and normals^T are linear in G and local to the cell: Hbar_c = hbk_c G_c, Abar_c = abk_c G_c,
+//       gxbar_c = gxk_c G_c, gybar_c = gyk_c G_c (c = x,y); Abar_z = G_zfull + flo G_zlo + fhi G_zhi -- formed while staging
 //   R3b Dbar_c = Sobel^T(gxbar_c, gybar_c) with the replicate padding folded back at the borders (S5);
 //       AbarF_c = Abar_c + Dbar_c / deps
 //   R4  averages^T: each mask pixel gathers from the E_x, E_y, E_z cells whose footprint holds it
@@ -16,7 +18,8 @@ namespace epsgrad {
 
 struct MaskGradParams {
     const float *phi;      // [B,px,py]
-    const float *res;      // [B,9,nx,ny]
+    const float *gbar;     // [B,5,nx,ny]  z-reduced cotangent: x, y, z-full, z-lower-face, z-upper-face
+    const float *coef;     // [B,10,nx,ny] [hbk, abk, gxk, gyk] for c = x, for c = y, flo, fhi
     float *v;              // [B,px,py]
     Normaliser nrm;
     int nx, ny, px, py, s;
@@ -48,7 +51,7 @@ __global__ void __launch_bounds__(MG_THREADS) k_maskgrad(const __grid_constant__
     const int oi = i0 - 2, oj = j0 - 2;            // cell origin of the staged arrays
     const int nx = P.nx, ny = P.ny, ncol = nx * ny;
     const float inv_s2 = 1.0f / (float)(s * s), inv_deps = 1.0f / P.deps;
-    const float *rb = P.res + (size_t)b * 9 * ncol;
+    const float *gb = P.gbar + (size_t)b * 5 * ncol, *cb = P.coef + (size_t)b * 10 * ncol;
     // tile whose 2-cell ring lies strictly inside the region: no folded border terms (block-uniform)
     const bool inner = i0 >= 3 && j0 >= 3 && i0 + TI + 1 <= nx - 1 && j0 + TJ + 1 <= ny - 1;
 
@@ -57,14 +60,34 @@ __global__ void __launch_bounds__(MG_THREADS) k_maskgrad(const __grid_constant__
         const int pix = along_x ? s * i0 + k : s * j0 + (k - s * TI);
         nidx[k] = along_x ? P.nrm.ix_of(min(pix, P.px - 1)) : P.nrm.iy_of(min(pix, P.py - 1));
     }
-    for (int it = tid; it < 8 * NC; it += NTH) {
-        const int o = it / NC, rem = it - o * NC, ci = rem / CJ, cj = rem - ci * CJ;
-        const int i = oi + ci, j = oj + cj;
-        R[it] = (i >= 0 && i < nx && j >= 0 && j < ny) ? rb[(size_t)o * ncol + i * ny + j] : 0.0f;
+    // staging: a warp per row of the (TI+3) x (TJ+3) cell block, a lane per cell; R2/R3a products formed on the way
+    static_assert(CJ <= 32, "one lane per staged column");
+    for (int ci = tid >> 5; ci < CI; ci += NTH / 32) {
+        const int cj = tid & 31, i = oi + ci, j = oj + cj;
+        if (cj < CJ) {
+            float r8[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+            if (i >= 0 && i < nx && j >= 0 && j < ny) {
+                const int cell = i * ny + j;
+                const float gx = gb[cell], gy = gb[ncol + cell];
+#pragma unroll
+                for (int o = 0; o < 4; ++o) {
+                    r8[o] = cb[(size_t)o * ncol + cell] * gx;
+                    r8[4 + o] = cb[(size_t)(4 + o) * ncol + cell] * gy;
+                }
+            }
+#pragma unroll
+            for (int o = 0; o < 8; ++o) R[o * NC + ci * CJ + cj] = r8[o];
+        }
     }
     for (int it = tid; it < TI * TJ; it += NTH) {
         const int ti = it / TJ, tj = it - ti * TJ, i = i0 + ti, j = j0 + tj;
-        AbZ[it] = (i < nx && j < ny) ? rb[(size_t)8 * ncol + i * ny + j] : 0.0f;
+        float az = 0.f;
+        if (i < nx && j < ny) {
+            const int cell = i * ny + j;
+            az = fmaf(cb[(size_t)8 * ncol + cell], gb[(size_t)3 * ncol + cell],
+                      fmaf(cb[(size_t)9 * ncol + cell], gb[(size_t)4 * ncol + cell], gb[(size_t)2 * ncol + cell]));
+        }
+        AbZ[it] = az;
     }
     __syncthreads();
 

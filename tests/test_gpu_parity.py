@@ -118,19 +118,23 @@ def test_forward_vjp_equals_separate_calls_and_keeps_inputs():
 
 @pytest.mark.parametrize("n_pairs", [1, 9, 17])
 def test_entry_points_agree_bitwise(n_pairs):
-    # eps_forward_vjp, eps_forward and eps_vjp run the same tile kernel with halves switched off; more than
-    # EPSGRAD_MAX_PAIRS pairs are chained through accumulating launches
+    # eps_forward_vjp, eps_forward and eps_vjp share their kernels; the two-stream schedule and the serial one give the
+    # same bits; more than EPSGRAD_MAX_PAIRS pairs are chained through accumulating launches
     cfg = B.make_config(batch=2, mx=27, my=22, nz=16, z_lo=6.25, z_hi=9.75, filter_radius=4.0)
     C = dev(rand_C(cfg, 16))
     EFn, EAn = rand_fields(cfg, n_pairs, 17)
     EF, EA = [dev(f) for f in EFn], [dev(f) for f in EAn]
     plan = B.Plan(cfg)
     eps0, g0 = plan.eps_forward_vjp(C, 8.0, EF, EA)
-    assert plan.last_launches() == 3 + (n_pairs + 7) // 8
+    assert plan.last_launches() == 5 + (n_pairs + 7) // 8
     eps1 = plan.eps_forward(C, 8.0)
     g1 = plan.eps_vjp(C, 8.0, EF, EA)
+    plan.set_overlap(False)
+    eps2, g2 = plan.eps_forward_vjp(C, 8.0, EF, EA)
+    g3 = plan.eps_vjp(C, 8.0, EF, EA)
+    plan.set_overlap(True)
     torch.cuda.synchronize()
-    assert torch.equal(eps0, eps1) and torch.equal(g0, g1)
+    assert torch.equal(eps0, eps1) and torch.equal(g0, g1) and torch.equal(eps0, eps2) and torch.equal(g0, g2) and torch.equal(g0, g3)
     if n_pairs > 1:
         # linearity in the pairs: the sum of single-pair gradients
         gs = sum(plan.eps_vjp(C, 8.0, [f], [a]).double() for f, a in zip(EF, EA))
@@ -146,13 +150,15 @@ def test_calls_are_cuda_graph_capturable():
     eps_ref, g_ref = plan.eps_forward_vjp(C, 8.0, EF, EA)
     eps, g = torch.zeros_like(eps_ref), torch.zeros_like(g_ref)
     torch.cuda.synchronize()
-    graph = torch.cuda.CUDAGraph()
-    with torch.cuda.graph(graph):
-        plan.eps_forward_vjp(C, 8.0, EF, EA, eps, g)
-    eps.zero_(); g.zero_()
-    graph.replay()
-    torch.cuda.synchronize()
-    assert torch.equal(eps, eps_ref) and torch.equal(g, g_ref)
+    for overlap in (True, False):
+        plan.set_overlap(overlap)
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):
+            plan.eps_forward_vjp(C, 8.0, EF, EA, eps, g)
+        eps.zero_(); g.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(eps, eps_ref) and torch.equal(g, g_ref)
 
 
 def test_real_cotangent_special_case():
