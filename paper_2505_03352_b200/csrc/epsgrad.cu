@@ -24,7 +24,7 @@ using namespace epsgrad;
 
 struct epsgrad_plan {
     epsgrad_config_t cfg;
-    int device;
+    int device, n_sm;
     int nx, ny, px, py, m;
     int T, NT, KX, KY;
     int separable;
@@ -133,6 +133,7 @@ extern "C" int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsg
     std::memset(P, 0, sizeof(*P));
     P->cfg = *cfg;
     P->device = device;
+    if (cudaDeviceGetAttribute(&P->n_sm, cudaDevAttrMultiProcessorCount, device) != cudaSuccess || P->n_sm < 1) { cudaGetLastError(); P->n_sm = 148; }
     const int u = cfg->upsample, s = cfg->subpixel, m = u * s;
     P->m = m;
     P->nx = u * cfg->mx; P->ny = u * cfg->my;
@@ -659,7 +660,8 @@ int launch_extrude(epsgrad_plan *P, const float *e2d, float *eps, cudaStream_t s
 {
     ExtrudeParams ep;
     ep.e2d = e2d; ep.eps = eps; ep.zw = P->d_zw; ep.ncol = P->nx * P->ny; ep.nz = P->cfg.nz;
-    k_extrude<<<dim3(cdiv(ep.ncol, extrude_cols_per_cta(ep.nz)), P->cfg.batch), EX_THREADS, 0, st>>>(ep);
+    ep.nblk = cdiv(ep.ncol, extrude_cols_per_block(ep.nz));
+    k_extrude<<<dim3(3 * ep.nblk, P->cfg.batch), EX_THREADS, 0, st>>>(ep);
     return check_launch(P, "extrude", st);
 }
 
@@ -677,16 +679,20 @@ int launch_zreduce(epsgrad_plan *P, int n_pairs, const void *const *EF, const vo
         while ((1 << zp.chs[g]) < zp.nch[g]) ++zp.chs[g];
         if (zp.chs[g] > 8) return EPSGRAD_EUNSUPPORTED;     // window wider than one CTA pass (nz > 512)
     }
-    const int rows = 2 * zp.nch[0] + zp.nch[1];
-    zp.ncp = zred_cols_per_pass(rows);
-    if (zp.ncp < 1) return EPSGRAD_EUNSUPPORTED;
+    size_t smem = 0;
+    for (int g = 0; g < 2; ++g) {
+        zp.ncp[g] = zred_cols_per_pass(zp.nch[g]);
+        if (zp.ncp[g] < 1) return EPSGRAD_EUNSUPPORTED;
+        const size_t need = (size_t)2 * (zp.nch[g] | 1) * zp.ncp[g] * 16;
+        if (need > smem) smem = need;
+    }
+    zp.nblk = cdiv(zp.ncol, ZR_COLS);
     // windows of at most 128 bytes per column: ask for 64-byte fills
     const bool sparse = maxnch * 16 <= 128 && zp.nz * 8 > 128;
-    const size_t smem = (size_t)2 * rows * zp.ncp * 16 + (size_t)5 * zp.nz * 4;
     auto kern = sparse ? k_zreduce<true> : k_zreduce<false>;
     int rc = set_smem(kern, smem);
     if (rc) return rc;
-    const dim3 grid(cdiv(zp.ncol, ZR_COLS), P->cfg.batch);
+    const dim3 grid(3 * zp.nblk, P->cfg.batch);
     for (int p0 = 0; p0 < n_pairs; p0 += ZR_MAX_PAIRS) {
         const int np = n_pairs - p0 < ZR_MAX_PAIRS ? n_pairs - p0 : ZR_MAX_PAIRS;
         for (int p = 0; p < ZR_MAX_PAIRS; ++p) {

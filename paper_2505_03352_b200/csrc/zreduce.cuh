@@ -6,19 +6,21 @@
 //   planes -- full cells, lower face, upper face -- and the mask kernel applies the face factors.  This keeps the
 //   field stream independent of the 2-D chain: the kernel depends on nothing but the fields.
 // Only the 16-byte chunks (2 complex64 cells) of a z column that hold slab cells are read ("|Omega_D";
-// d eps/dC = 0 elsewhere); `dense` plans read every chunk.  A CTA owns ZR_COLS consecutive columns of one design, all
-// three components: it starts asynchronous 16-byte copies (LDGSTS) of every window of both fields into shared memory
-// -- no register staging, one pass of address arithmetic, up to 4 CTAs x 53 KB in flight per SM -- then multiplies and
-// reduces out of shared memory.  Sparse windows ask for 64-byte L2 fills: the default fill is the whole 128-byte line,
-// and 64 B is the smallest granule the part offers, so a window that straddles a line boundary costs
-// 128 B of DRAM traffic per column, component and field instead of 256 B.
+// d eps/dC = 0 elsewhere); `dense` plans read every chunk.  CTA n of the grid owns component n / nblk and ZR_COLS
+// consecutive columns: the resident CTAs read one advancing window of one component plane of E_F and of E_A (measured:
+// 37 us; 48 us when every CTA reads its columns in all three component planes).  A CTA starts asynchronous
+// 16-byte copies (LDGSTS) of every window of both fields into shared memory -- no register staging, one pass of address
+// arithmetic, up to 5 CTAs x 40 KB in flight per SM -- then each thread multiplies and reduces one column out of shared
+// memory.  Sparse windows ask for 64-byte L2 fills: the default fill is the whole 128-byte line, and 64 B is the smallest
+// granule the part offers, so a window that straddles a line boundary costs 128 B of DRAM traffic per
+// column, component and field instead of 256 B.
 #pragma once
 #include "common.cuh"
 
 namespace epsgrad {
 
-constexpr int ZR_THREADS = 256, ZR_COLS = 128, ZR_MAX_PAIRS = 8;
-constexpr int ZR_STAGE_CHUNKS = ZR_COLS * 13;   // staging capacity per field in 16-byte chunks (paper slab: 4 + 4 + 5 per column)
+constexpr int ZR_THREADS = 256, ZR_COLS = 256, ZR_MAX_PAIRS = 8;
+constexpr int ZR_STAGE_CHUNKS = ZR_COLS * 5;    // staging capacity per field in 16-byte chunks (paper slab: 4 or 5 per column)
 
 struct ZredParams {
     const float4 *ef[ZR_MAX_PAIRS];
@@ -26,15 +28,15 @@ struct ZredParams {
     float *gbar;           // [B,5,ncol]: planes x, y, z-full, z-lower-face, z-upper-face
     const float *zw;       // [7][nz] z tables (epsgrad.cu); rows 0 (wxy) and 2..4 (z-full / lower / upper indicators) are used
     int n_pairs, accumulate;
-    int ncol, nz;
+    int ncol, nz, nblk;    // nblk = ceil(ncol / ZR_COLS) column blocks per component plane
     int ch0[2], nch[2];    // chunk window (chunk = 2 cells = 16 B) for {x,y} and {z}
     int chs[2];            // log2 of the lanes per column of the copy loop: 2^chs >= nch
-    int ncp;               // columns staged per pass (<= ZR_COLS): ncp (2 nch[0] + nch[1]) <= ZR_STAGE_CHUNKS
+    int ncp[2];            // columns staged per pass (<= ZR_COLS): ncp (nch | 1) <= ZR_STAGE_CHUNKS
 };
 
-__host__ __device__ inline int zred_cols_per_pass(int rows)
+__host__ __device__ inline int zred_cols_per_pass(int nch)
 {
-    int n = ZR_STAGE_CHUNKS / (rows > 0 ? rows : 1);
+    int n = ZR_STAGE_CHUNKS / (nch | 1);
     if (n >= 32) n &= ~31;                 // whole warps of columns
     return n > ZR_COLS ? ZR_COLS : n;
 }
@@ -50,101 +52,76 @@ __device__ __forceinline__ void cp_async16(float4 *smem, const float4 *g)
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-// Issue side: copies of the z windows of columns [col0, col0+nc) of design b, all three components, fields E_F and
-// E_A of pair p.  Buffer layout per field: [chunk row][column], chunk rows = nch[0] rows of x, nch[0] of y, nch[1] of z
-// (reads of consecutive columns are conflict-free).  2^chs >= nch lanes per column (a power of two: no divisions), so a
-// warp instruction covers 32 >> chs neighbouring windows; lanes beyond the window idle.
+// Issue side: copies of the z windows of columns [col0, col0+nc) of component c of design b, fields E_F and E_A of pair p.
+// Buffer layout per field: [column][nch | 1] chunks: a column's window stays contiguous, so a returning 32-byte sector
+// lands in one shared-memory write (a [chunk][column] layout splits it in two and costs 25 % of the kernel, measured),
+// and the odd pitch makes the per-column reads of consecutive threads conflict-free.  2^chs >= nch lanes per column (a
+// power of two: no divisions), so a warp instruction covers 32 >> chs neighbouring windows; lanes beyond the window idle.
 template <bool SPARSE>
-__device__ __forceinline__ void zwindow_issue(const ZredParams &P, float4 *buf, int p, int b, int col0, int nc)
+__device__ __forceinline__ void zwindow_issue(const ZredParams &P, float4 *buf, int p, int b, int c, int col0, int nc)
 {
-    const int nzc = P.nz >> 1, rows = 2 * P.nch[0] + P.nch[1];
-    float4 *bf = buf, *ba = buf + rows * P.ncp;
-    int row0 = 0;
-    for (int c = 0; c < 3; ++c) {
-        const int grp = c == 2, nch = P.nch[grp], sh = P.chs[grp];
-        const int ch = threadIdx.x & ((1 << sh) - 1), lstep = ZR_THREADS >> sh;
-        if (ch < nch) {
-            const size_t first = (((size_t)b * 3 + c) * P.ncol + col0) * nzc + P.ch0[grp] + ch;
-            const float4 *pf = P.ef[p] + first, *pa = P.ea[p] + first;
-            float4 *df = bf + (row0 + ch) * P.ncp, *da = ba + (row0 + ch) * P.ncp;
-            for (int lc = threadIdx.x >> sh; lc < nc; lc += lstep) {
-                cp_async16<SPARSE>(df + lc, pf + lc * nzc);
-                cp_async16<SPARSE>(da + lc, pa + lc * nzc);
-            }
+    const int grp = c == 2, nzc = P.nz >> 1, nch = P.nch[grp], sh = P.chs[grp], ncp = P.ncp[grp];
+    const int ch = threadIdx.x & ((1 << sh) - 1), lstep = ZR_THREADS >> sh;
+    if (ch < nch) {
+        const size_t first = (((size_t)b * 3 + c) * P.ncol + col0) * nzc + P.ch0[grp] + ch;
+        const float4 *pf = P.ef[p] + first, *pa = P.ea[p] + first;
+        const int pitch = nch | 1;
+        float4 *df = buf + ch, *da = df + pitch * ncp;
+        for (int lc = threadIdx.x >> sh; lc < nc; lc += lstep) {
+            cp_async16<SPARSE>(df + lc * pitch, pf + lc * nzc);
+            cp_async16<SPARSE>(da + lc * pitch, pa + lc * nzc);
         }
-        row0 += nch;
     }
     cp_async_commit();
 }
 
-// Consume side: Eq. (1) cotangent of the staged window of local column lc, component c, times the extrusion weights.
-// acc[0]: x, y or z-full; acc[1], acc[2]: z lower / upper face.
-__device__ __forceinline__ void zwindow_reduce(const ZredParams &P, const float *zw, const float4 *buf, int c, int lc, float acc[3])
-{
-    const int grp = c == 2, nch = P.nch[grp], ch0 = P.ch0[grp], nz = P.nz;
-    const int rows = 2 * P.nch[0] + P.nch[1], row0 = c * P.nch[0];
-    const float4 *bf = buf + row0 * P.ncp + lc, *ba = bf + rows * P.ncp;
-    for (int ch = 0; ch < nch; ++ch) {
-        const float4 f = bf[ch * P.ncp], a = ba[ch * P.ncp];
-        const int k = 2 * (ch0 + ch);
-        const float g0 = -2.0f * (f.x * a.x - f.y * a.y);
-        const float g1 = -2.0f * (f.z * a.z - f.w * a.w);
-        if (grp == 0) {
-            acc[0] = fmaf(zw[k], g0, fmaf(zw[k + 1], g1, acc[0]));
-        } else {
-#pragma unroll
-            for (int o = 0; o < 3; ++o) acc[o] = fmaf(zw[(2 + o) * nz + k], g0, fmaf(zw[(2 + o) * nz + k + 1], g1, acc[o]));
-        }
-    }
-}
-
-// grid (ceil(ncol/ZR_COLS), B); dynamic shared memory: 5 nz floats (z tables) + 2 fields x rows x ncp chunks
+// grid (3 nblk, B); dynamic shared memory: 2 fields x ncp x (nch | 1) chunks
 template <bool SPARSE>
-__global__ void __launch_bounds__(ZR_THREADS, 4) k_zreduce(const __grid_constant__ ZredParams P)
+__global__ void __launch_bounds__(ZR_THREADS, 5) k_zreduce(const __grid_constant__ ZredParams P)
 {
-    extern __shared__ __align__(16) float4 sm4[];
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int b = blockIdx.y, colb = blockIdx.x * ZR_COLS, ncb = min(ZR_COLS, P.ncol - colb);
-    const int nz = P.nz;
-    float4 *stage = sm4;
-    float *zw = reinterpret_cast<float *>(sm4 + 2 * (2 * P.nch[0] + P.nch[1]) * P.ncp);     // [5][nz]
+    extern __shared__ __align__(16) float4 stage[];
+    const int tid = threadIdx.x;
+    const int c = blockIdx.x / P.nblk, blk = blockIdx.x - c * P.nblk, b = blockIdx.y;
+    const int grp = c == 2, nch = P.nch[grp], ch0 = P.ch0[grp], ncp = P.ncp[grp], nz = P.nz;
+    const int colb = blk * ZR_COLS, ncb = min(ZR_COLS, P.ncol - colb);
 
-    zwindow_issue<SPARSE>(P, stage, 0, b, colb, min(P.ncp, ncb));
-    for (int k = tid; k < 5 * nz; k += ZR_THREADS) zw[k] = P.zw[k];
-
-    // Warp item = (component, 32 columns of the pass): warp-uniform component; a warp owns items w and w + 8.
-    for (int c0 = 0; c0 < ncb; c0 += P.ncp) {
-        const int nc = min(P.ncp, ncb - c0), ncw = (nc + 31) >> 5, nitem = 3 * ncw;
-        float acc[2][3] = {{0.f, 0.f, 0.f}, {0.f, 0.f, 0.f}};
+    zwindow_issue<SPARSE>(P, stage, 0, b, c, colb, min(ncp, ncb));
+    // a thread reduces one column; the extrusion weights (2 cells per chunk; three rows for component z) are warp-uniform
+    // cached loads
+    for (int c0 = 0; c0 < ncb; c0 += ncp) {
+        const int nc = min(ncp, ncb - c0);
+        float acc[3] = {0.f, 0.f, 0.f};
         for (int p = 0; p < P.n_pairs; ++p) {
             if (c0 > 0 || p > 0) {
                 __syncthreads();                     // every thread is done reading the previous windows
-                zwindow_issue<SPARSE>(P, stage, p, b, colb + c0, nc);
+                zwindow_issue<SPARSE>(P, stage, p, b, c, colb + c0, nc);
             }
             cp_async_wait_all();
             __syncthreads();
+            if (tid < nc) {
+                const int pitch = nch | 1;
+                const float4 *bf = stage + tid * pitch, *ba = bf + pitch * ncp;
+                for (int ch = 0; ch < nch; ++ch) {
+                    const float4 f = bf[ch], a = ba[ch];
+                    const int k = 2 * (ch0 + ch);
+                    const float g0 = -2.0f * (f.x * a.x - f.y * a.y);       // Eq. (1): -2 Re(E_F E_A), plain product (S10)
+                    const float g1 = -2.0f * (f.z * a.z - f.w * a.w);
+                    if (grp == 0) {
+                        acc[0] = fmaf(__ldg(P.zw + k), g0, fmaf(__ldg(P.zw + k + 1), g1, acc[0]));
+                    } else {
 #pragma unroll
-            for (int u = 0; u < 2; ++u) {
-                const int item = warp + u * (ZR_THREADS / 32);
-                if (item < nitem) {
-                    const int c = item / ncw, lc = (item - c * ncw) * 32 + lane;
-                    if (lc < nc) zwindow_reduce(P, zw, stage, c, lc, acc[u]);
+                        for (int o = 0; o < 3; ++o)
+                            acc[o] = fmaf(__ldg(P.zw + (2 + o) * nz + k), g0, fmaf(__ldg(P.zw + (2 + o) * nz + k + 1), g1, acc[o]));
+                    }
                 }
             }
         }
-#pragma unroll
-        for (int u = 0; u < 2; ++u) {
-            const int item = warp + u * (ZR_THREADS / 32);
-            if (item < nitem) {
-                const int c = item / ncw, lc = (item - c * ncw) * 32 + lane;
-                if (lc < nc) {
-                    float *dst = P.gbar + (size_t)b * 5 * P.ncol + colb + c0 + lc;
-                    const int nout = c == 2 ? 3 : 1;
-                    for (int o = 0; o < nout; ++o) {
-                        float *d = dst + (size_t)(c == 2 ? 2 + o : c) * P.ncol;
-                        *d = P.accumulate ? *d + acc[u][o] : acc[u][o];
-                    }
-                }
+        if (tid < nc) {
+            float *dst = P.gbar + (size_t)b * 5 * P.ncol + colb + c0 + tid;
+            const int nout = grp ? 3 : 1;
+            for (int o = 0; o < nout; ++o) {
+                float *d = dst + (size_t)(grp ? 2 + o : c) * P.ncol;
+                *d = P.accumulate ? *d + acc[o] : acc[o];
             }
         }
     }
