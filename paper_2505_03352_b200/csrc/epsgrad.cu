@@ -528,10 +528,10 @@ int launch_filter_m(epsgrad_plan *P, const float *C, float *phi, cudaStream_t st
         fp.mx = mx; fp.my = my; fp.px = P->px; fp.py = P->py; fp.T = T; fp.NT = NT; fp.eta0 = P->eta0;
         if (M == 4 && (NT == 5 || NT == 9 || NT == 13)) {      // fast path (filter4.cuh)
             auto kern = NT == 5 ? k_filter_conic4<5> : (NT == 9 ? k_filter_conic4<9> : k_filter_conic4<13>);
-            const size_t smem4 = filter4_smem_floats(NT) * 4;
+            const size_t smem4 = (filter4_smem_floats(NT) + 4) * 4;
             int rc4 = set_smem(kern, smem4);
             if (rc4) return rc4;
-            kern<<<dim3(cdiv(my, F4_TB), cdiv(mx, F4_TA), B), F4_THREADS, smem4, st>>>(fp);
+            kern<<<dim3(cdiv(my, F4_TB), cdiv(mx, F4_TA), B), F4F_THREADS, smem4, st>>>(fp);
             return check_launch(P, "filter", st);
         }
         const size_t smem = ((size_t)NT * NT * M * M + (size_t)(TA + 2 * T) * (TB + 2 * T + 1) + 2 * NT) * 4;
@@ -577,7 +577,7 @@ int launch_filterT_conic(epsgrad_plan *P, const float *v, float *dC, cudaStream_
         const size_t smem4 = filterT4_smem_floats(NT) * 4;
         int rc4 = set_smem(kern, smem4);
         if (rc4) return rc4;
-        kern<<<dim3(cdiv(fp.my, F4_TB), cdiv(fp.mx, F4_TA), P->cfg.batch), F4_THREADS, smem4, st>>>(fp);
+        kern<<<dim3(cdiv(fp.my, F4_TB), cdiv(fp.mx, F4_TA), P->cfg.batch), F4T_THREADS, smem4, st>>>(fp);
         return check_launch(P, "filterT", st);
     }
     const size_t smem = ((size_t)NT * NT * M * M + (size_t)M * (S::TA + 2 * T) * M * (S::TB + 2 * T) + 2 * NT) * 4;

@@ -20,27 +20,32 @@ namespace epsgrad {
 
 constexpr int F4_NB = 4, F4_TA = 4, F4_TB = 8 * F4_NB, F4_THREADS = 32 * F4_TA;
 
+constexpr int F4_G = 3, F4F_THREADS = F4_THREADS * F4_G;     // forward: tap rows split over F4_G warp groups (see the transpose below)
+
 __host__ __device__ inline size_t filter4_smem_floats(int NT)
 {
     const int T = (NT - 1) / 2;
-    return (size_t)NT * NT * 16 + (size_t)(F4_TA + 2 * T) * (F4_TB + 2 * T + 1);
+    return (size_t)NT * NT * 16 + (size_t)(F4_TA + 2 * T) * (F4_TB + 2 * T + 1) + (size_t)F4_G * F4_THREADS * 16;
 }
 
-// grid (ceil(my/32), ceil(mx/4), B), 128 threads: warp <-> control row la, lane = sp*8 + lb
+// grid (ceil(my/32), ceil(mx/4), B), 384 threads: warp <-> (tap-row group g, control row la), lane = sp*8 + lb
 template <int NTC>
-__global__ void __launch_bounds__(F4_THREADS) k_filter_conic4(const FilterParams P)
+__global__ void __launch_bounds__(F4F_THREADS) k_filter_conic4(const FilterParams P)
 {
-    constexpr int T = (NTC - 1) / 2, TA = F4_TA, TB = F4_TB, NB = F4_NB, CW = TB + 2 * T + 1;
+    constexpr int T = (NTC - 1) / 2, TA = F4_TA, TB = F4_TB, NB = F4_NB, CW = TB + 2 * T + 1, G = F4_G;
+    constexpr int TXPG = (NTC + G - 1) / G;
     extern __shared__ __align__(16) float sm[];
     float *w_s = sm;                               // [NTC][NTC][4][4]
     float *c_s = w_s + NTC * NTC * 16;             // [(TA+2T)][CW]
+    float *part = c_s + (TA + 2 * T) * CW;         // [G][jb][j][F4_THREADS] partial sums
+    part += (4 - ((NTC * NTC * 16 + (TA + 2 * T) * CW) & 3)) & 3;       // 16-byte aligned (one float4 of slack is in the budget)
     const int tid = threadIdx.x;
     const int a_base = blockIdx.y * TA, b_base = blockIdx.x * TB, b = blockIdx.z;
 
-    for (int i = tid; i < NTC * NTC * 4; i += F4_THREADS)
+    for (int i = tid; i < NTC * NTC * 4; i += F4F_THREADS)
         reinterpret_cast<float4 *>(w_s)[i] = reinterpret_cast<const float4 *>(P.w)[i];
     const float *Cb = P.C + (size_t)b * P.mx * P.my;
-    for (int r = tid >> 5; r < TA + 2 * T; r += F4_THREADS / 32) {
+    for (int r = tid >> 5; r < TA + 2 * T; r += F4F_THREADS / 32) {
         const int a = a_base - T + r;
         for (int c = tid & 31; c < TB + 2 * T; c += 32) {
             const int bb = b_base - T + c;
@@ -51,15 +56,16 @@ __global__ void __launch_bounds__(F4_THREADS) k_filter_conic4(const FilterParams
     }
     __syncthreads();
 
-    const int la = tid >> 5, lane = tid & 31, sp = lane >> 3, lb = lane & 7;
+    const int warp = tid >> 5, g = warp / TA, la = warp - g * TA, lane = tid & 31, sp = lane >> 3, lb = lane & 7;
     float acc[NB][4];
 #pragma unroll
     for (int jb = 0; jb < NB; ++jb)
 #pragma unroll
         for (int j = 0; j < 4; ++j) acc[jb][j] = 0.0f;
 
+    const int tx0 = g * TXPG, tx1 = min(tx0 + TXPG, NTC);
 #pragma unroll 1
-    for (int tx = 0; tx < NTC; ++tx) {
+    for (int tx = tx0; tx < tx1; ++tx) {
         float wr[NTC][4];
 #pragma unroll
         for (int ty = 0; ty < NTC; ++ty) lds_vec<4>(w_s + ((tx * NTC + ty) * 4 + sp) * 4, wr[ty]);
@@ -77,70 +83,96 @@ __global__ void __launch_bounds__(F4_THREADS) k_filter_conic4(const FilterParams
             }
         }
     }
-    const int a0 = a_base + la;
-    if (a0 >= P.mx) return;
-    const int p = 4 * a0 + sp, nix = P.nrm.ix(a0, sp);
-    float *row = P.phi + ((size_t)b * P.px + p) * P.py;
+    // partial sums meet in shared memory: slot (la, lane) of group g, one float4 per jb; consecutive lanes, consecutive float4
+    const int slot = la * 32 + lane;
 #pragma unroll
-    for (int jb = 0; jb < NB; ++jb) {
-        const int b0 = b_base + NB * lb + jb;
-        if (b0 >= P.my) continue;
-        const int niy = P.nrm.iy(b0, 0);
-        float4 o;
-        o.x = acc[jb][0] * P.nrm.at_index(nix, niy);
-        o.y = acc[jb][1] * P.nrm.at_index(nix, niy + 1);
-        o.z = acc[jb][2] * P.nrm.at_index(nix, niy + 2);
-        o.w = acc[jb][3] * P.nrm.at_index(nix, niy + 3);
-        *reinterpret_cast<float4 *>(row + 4 * b0) = o;
+    for (int jb = 0; jb < NB; ++jb)
+        reinterpret_cast<float4 *>(part)[(g * NB + jb) * F4_THREADS + slot] = make_float4(acc[jb][0], acc[jb][1], acc[jb][2], acc[jb][3]);
+    __syncthreads();
+    // (jb, slot) pairs over all threads: sum the groups, apply the normaliser, store
+    for (int it = tid; it < NB * F4_THREADS; it += F4F_THREADS) {
+        const int jb = it / F4_THREADS, sl = it - jb * F4_THREADS;
+        const int la2 = sl >> 5, ln = sl & 31, sp2 = ln >> 3, lb2 = ln & 7;
+        const int a0 = a_base + la2, b0 = b_base + NB * lb2 + jb;
+        float4 o = reinterpret_cast<const float4 *>(part)[jb * F4_THREADS + sl];
+#pragma unroll
+        for (int gg = 1; gg < G; ++gg) {
+            const float4 t = reinterpret_cast<const float4 *>(part)[(gg * NB + jb) * F4_THREADS + sl];
+            o.x += t.x; o.y += t.y; o.z += t.z; o.w += t.w;
+        }
+        if (a0 >= P.mx || b0 >= P.my) continue;
+        const int nix = P.nrm.ix(a0, sp2), niy = P.nrm.iy(b0, 0);
+        o.x *= P.nrm.at_index(nix, niy);
+        o.y *= P.nrm.at_index(nix, niy + 1);
+        o.z *= P.nrm.at_index(nix, niy + 2);
+        o.w *= P.nrm.at_index(nix, niy + 3);
+        *reinterpret_cast<float4 *>(P.phi + ((size_t)b * P.px + 4 * a0 + sp2) * P.py + 4 * b0) = o;
     }
 }
 
 // ---------------------------------------------------------------- transpose
+// The tap rows tx are split over F4T_G warp groups (each warp of a group owns one control row of the tile), so a CTA
+// carries F4T_G * F4_TA warps instead of F4_TA: the kernel is latency bound (one wave of ~500 CTAs), and the extra warps
+// are what hides the shared-memory and FMA latencies.  Partial sums meet in shared memory.  The v tile is staged with
+// 16-byte asynchronous copies (zero-filled outside the mask), all in flight at once.
+constexpr int F4T_G = 3, F4T_THREADS = 32 * F4_TA * F4T_G;
+
 __host__ __device__ inline int filterT4_pitch(int T) { const int nb = F4_TB + 2 * T; return 4 * (nb + (nb + 3) / 4); }
 __host__ __device__ inline size_t filterT4_smem_floats(int NT)
 {
     const int T = (NT - 1) / 2;
-    return (size_t)NT * NT * 16 + (size_t)4 * (F4_TA + 2 * T) * filterT4_pitch(T);
+    return (size_t)NT * NT * 16 + (size_t)4 * (F4_TA + 2 * T) * filterT4_pitch(T) + (size_t)F4T_G * F4_TA * F4_TB;
 }
 
-// grid (ceil(my/32), ceil(mx/4), B), 128 threads
-template <int NTC>
-__global__ void __launch_bounds__(F4_THREADS) k_filterT_conic4(const FilterTParams P)
+// 16-byte asynchronous copy with zero fill: src_bytes = 16 copies, 0 writes zeros (the source address is not read)
+__device__ __forceinline__ void f4_cp_async16_zfill(float *smem, const float *g, int src_bytes)
 {
-    constexpr int T = (NTC - 1) / 2, TA = F4_TA, TB = F4_TB, NB = F4_NB;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;"
+                 :: "r"((unsigned)__cvta_generic_to_shared(smem)), "l"(g), "r"(src_bytes) : "memory");
+}
+
+// grid (ceil(my/32), ceil(mx/4), B), 384 threads
+template <int NTC>
+__global__ void __launch_bounds__(F4T_THREADS) k_filterT_conic4(const FilterTParams P)
+{
+    constexpr int T = (NTC - 1) / 2, TA = F4_TA, TB = F4_TB, NB = F4_NB, G = F4T_G;
+    constexpr int TXPG = (NTC + G - 1) / G;                       // tap rows per warp group
     constexpr int VH = 4 * (TA + 2 * T), VB = TB + 2 * T;       // v tile: rows, blocks of 4 floats per row
     extern __shared__ __align__(16) float sm[];
     const int pitch = filterT4_pitch(T);
     float *w_s = sm;                               // [NTC][NTC][4][4]
     float *v_s = w_s + NTC * NTC * 16;             // [VH][pitch], block c at 4(c + c/4)
+    float *part = v_s + VH * pitch;                // [G][TA][TB] partial sums
     const int tid = threadIdx.x;
     const int a_base = blockIdx.y * TA, b_base = blockIdx.x * TB, b = blockIdx.z;
 
-    for (int i = tid; i < NTC * NTC * 4; i += F4_THREADS)
-        reinterpret_cast<float4 *>(w_s)[i] = reinterpret_cast<const float4 *>(P.w)[i];
     const float *vb = P.v + (size_t)b * P.px * P.py;
     const int p_base = 4 * (a_base - T), q_base = 4 * (b_base - T);
-    for (int r = tid >> 5; r < VH; r += F4_THREADS / 32) {
+    for (int r = tid >> 5; r < VH; r += F4T_THREADS / 32) {
         const int p = p_base + r;
         const bool rin = p >= 0 && p < P.px;
         for (int c = tid & 31; c < VB; c += 32) {
             const int q = q_base + 4 * c;
-            float4 x = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (rin && q >= 0 && q < P.py) x = *reinterpret_cast<const float4 *>(vb + (size_t)p * P.py + q);
-            *reinterpret_cast<float4 *>(v_s + r * pitch + 4 * (c + (c >> 2))) = x;
+            const bool in = rin && q >= 0 && q < P.py;
+            f4_cp_async16_zfill(v_s + r * pitch + 4 * (c + (c >> 2)), in ? vb + (size_t)p * P.py + q : vb, in ? 16 : 0);
         }
     }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    for (int i = tid; i < NTC * NTC * 4; i += F4T_THREADS)
+        reinterpret_cast<float4 *>(w_s)[i] = reinterpret_cast<const float4 *>(P.w)[i];
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
     __syncthreads();
 
-    const int la = tid >> 5, lane = tid & 31, sp = lane >> 3, lb = lane & 7;
+    const int warp = tid >> 5, g = warp / TA, la = warp - g * TA, lane = tid & 31, sp = lane >> 3, lb = lane & 7;
     float acc[NB][4];
 #pragma unroll
     for (int jb = 0; jb < NB; ++jb)
 #pragma unroll
         for (int j = 0; j < 4; ++j) acc[jb][j] = 0.0f;
 
+    const int tx0 = g * TXPG, tx1 = min(tx0 + TXPG, NTC);
 #pragma unroll 1
-    for (int tx = 0; tx < NTC; ++tx) {
+    for (int tx = tx0; tx < tx1; ++tx) {
         float wr[NTC][4];
 #pragma unroll
         for (int ty = 0; ty < NTC; ++ty) lds_vec<4>(w_s + ((tx * NTC + ty) * 4 + sp) * 4, wr[ty]);
@@ -161,14 +193,20 @@ __global__ void __launch_bounds__(F4_THREADS) k_filterT_conic4(const FilterTPara
             }
         }
     }
-    const int a = a_base + la;
 #pragma unroll
     for (int jb = 0; jb < NB; ++jb) {
         float s = (acc[jb][0] + acc[jb][1]) + (acc[jb][2] + acc[jb][3]);
         s += __shfl_xor_sync(0xffffffffu, s, 8);
         s += __shfl_xor_sync(0xffffffffu, s, 16);
-        const int bb = b_base + NB * lb + jb;
-        if (sp == 0 && a < P.mx && bb < P.my) P.dC[((size_t)b * P.mx + a) * P.my + bb] = s;
+        if (sp == 0) part[(g * TA + la) * TB + NB * lb + jb] = s;
+    }
+    __syncthreads();
+    if (tid < TA * TB) {
+        const int a = a_base + tid / TB, bb = b_base + tid % TB;
+        float s = 0.0f;
+#pragma unroll
+        for (int gg = 0; gg < G; ++gg) s += part[gg * TA * TB + tid];
+        if (a < P.mx && bb < P.my) P.dC[((size_t)b * P.mx + a) * P.my + bb] = s;
     }
 }
 

@@ -143,35 +143,45 @@ __global__ void __launch_bounds__(MG_THREADS) k_maskgrad(const __grid_constant__
     const int TP = s * TI, TQ = s * TJ;
     const float *phib = P.phi + (size_t)b * P.px * P.py;
     float *vb = P.v + (size_t)b * P.px * P.py;
-    for (int it = tid; it < TP * TQ; it += NTH) {
-        const int tp = it / TQ, tq = it - tp * TQ;
-        const int p = s * i0 + tp, q = s * j0 + tq;
-        if (p >= P.px || q >= P.py) continue;
-        const int iz = p / s, jz = q / s;
-        float ebar = AbZ[(iz - i0) * TJ + (jz - j0)], rbar = 0.f;
-        if (p >= hs) {                                       // E_x owner
-            const int ix = (p - hs) / s;
-            const float mlt = p == P.px - 1 ? (float)(1 + hs) : 1.0f;
-            const int idx = (ix - oi) * CJ + (jz - oj);
-            ebar = fmaf(mlt, AbF[idx], ebar);
-            rbar = fmaf(mlt, R[idx], rbar);
+    for (int base = tid; base < TP * TQ; base += 4 * NTH) {
+        float ph[4];                                           // filter output of four pixels in flight
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int it = base + u * NTH, tp = it / TQ, tq = it - tp * TQ;
+            const int p = s * i0 + tp, q = s * j0 + tq;
+            if (it < TP * TQ && p < P.px && q < P.py) ph[u] = phib[p * P.py + q];
         }
-        if (q >= hs) {                                       // E_y owner
-            const int jy = (q - hs) / s;
-            const float mlt = q == P.py - 1 ? (float)(1 + hs) : 1.0f;
-            const int idx = (iz - oi) * CJ + (jy - oj);
-            ebar = fmaf(mlt, AbF[NC + idx], ebar);
-            rbar = fmaf(mlt, R[4 * NC + idx], rbar);
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int it = base + u * NTH, tp = it / TQ, tq = it - tp * TQ;
+            const int p = s * i0 + tp, q = s * j0 + tq;
+            if (it >= TP * TQ || p >= P.px || q >= P.py) continue;
+            const int iz = p / s, jz = q / s;
+            float ebar = AbZ[(iz - i0) * TJ + (jz - j0)], rbar = 0.f;
+            if (p >= hs) {                                       // E_x owner
+                const int ix = (p - hs) / s;
+                const float mlt = p == P.px - 1 ? (float)(1 + hs) : 1.0f;
+                const int idx = (ix - oi) * CJ + (jz - oj);
+                ebar = fmaf(mlt, AbF[idx], ebar);
+                rbar = fmaf(mlt, R[idx], rbar);
+            }
+            if (q >= hs) {                                       // E_y owner
+                const int jy = (q - hs) / s;
+                const float mlt = q == P.py - 1 ? (float)(1 + hs) : 1.0f;
+                const int idx = (iz - oi) * CJ + (jy - oj);
+                ebar = fmaf(mlt, AbF[NC + idx], ebar);
+                rbar = fmaf(mlt, R[4 * NC + idx], rbar);
+            }
+            // one exponential serves rho and its slope: a = exp(-2|t|), rho = 1/(1+a) or a/(1+a), slope = 2 beta a/(1+a)^2
+            const float t = P.beta * (ph[u] - P.eta_r);
+            const float a = __expf(-2.0f * fabsf(t));
+            const float d = fast_rcp(1.0f + a);
+            const float rho = t >= 0.f ? d : a * d;
+            const float r = fast_rcp(fmaf(P.deps, rho, P.eps_clad));   // 1/e
+            const float slope = 2.0f * P.beta * a * d * d;
+            const float rhobar = P.deps * inv_s2 * (ebar - rbar * r * r);
+            vb[p * P.py + q] = rhobar * slope * P.nrm.at_index(nidx[tp], nidx[TP + tq]);
         }
-        // one exponential serves rho and its slope: a = exp(-2|t|), rho = 1/(1+a) or a/(1+a), slope = 2 beta a/(1+a)^2
-        const float t = P.beta * (phib[p * P.py + q] - P.eta_r);
-        const float a = __expf(-2.0f * fabsf(t));
-        const float d = fast_rcp(1.0f + a);
-        const float rho = t >= 0.f ? d : a * d;
-        const float r = fast_rcp(fmaf(P.deps, rho, P.eps_clad));   // 1/e
-        const float slope = 2.0f * P.beta * a * d * d;
-        const float rhobar = P.deps * inv_s2 * (ebar - rbar * r * r);
-        vb[p * P.py + q] = rhobar * slope * P.nrm.at_index(nidx[tp], nidx[TP + tq]);
     }
 }
 
