@@ -26,7 +26,7 @@ __device__ __forceinline__ int border_class(int a0, int M, int T, int K)
 // SPARSE: the access touches only a 64..96-byte window of each 512-byte z column.  By default a
 // miss fills the whole 128-byte line from DRAM (measured: 256 B fetched per column for a window
 // that straddles a line boundary); the L2::64B prefetch-size qualifier halves that -- 64 B is the
-// smallest fill granularity this part honours (profiles/r1b_zreduce_granularity.md).
+// smallest fill granularity this part honours.
 template <bool SPARSE>
 __device__ __forceinline__ float4 ld_stream(const float4 *p)
 {

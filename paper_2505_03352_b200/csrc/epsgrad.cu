@@ -660,8 +660,18 @@ int launch_extrude(epsgrad_plan *P, const float *e2d, float *eps, cudaStream_t s
 {
     ExtrudeParams ep;
     ep.e2d = e2d; ep.eps = eps; ep.zw = P->d_zw; ep.ncol = P->nx * P->ny; ep.nz = P->cfg.nz;
-    ep.nblk = cdiv(ep.ncol, extrude_cols_per_block(ep.nz));
-    k_extrude<<<dim3(3 * ep.nblk, P->cfg.batch), EX_THREADS, 0, st>>>(ep);
+    ep.cpb = extrude_cols_per_block(ep.nz);
+    ep.nblk = cdiv(ep.ncol, ep.cpb);
+    const int nz4 = ep.nz >> 2;
+    ep.sh4 = -1;
+    if (EX_THREADS % nz4 == 0)
+        for (int sft = 0; sft <= 8; ++sft)
+            if ((1 << sft) == nz4) ep.sh4 = sft;
+    if (P->cfg.batch > 65535) return EPSGRAD_EUNSUPPORTED;
+    const size_t smem = (size_t)3 * ep.cpb * 4;
+    int rc = set_smem(k_extrude, smem);
+    if (rc) return rc;
+    k_extrude<<<dim3(ep.nblk, 3, P->cfg.batch), EX_THREADS, smem, st>>>(ep);
     return check_launch(P, "extrude", st);
 }
 
@@ -692,7 +702,8 @@ int launch_zreduce(epsgrad_plan *P, int n_pairs, const void *const *EF, const vo
     auto kern = sparse ? k_zreduce<true> : k_zreduce<false>;
     int rc = set_smem(kern, smem);
     if (rc) return rc;
-    const dim3 grid(3 * zp.nblk, P->cfg.batch);
+    if (P->cfg.batch > 65535) return EPSGRAD_EUNSUPPORTED;
+    const dim3 grid(zp.nblk, 3, P->cfg.batch);
     for (int p0 = 0; p0 < n_pairs; p0 += ZR_MAX_PAIRS) {
         const int np = n_pairs - p0 < ZR_MAX_PAIRS ? n_pairs - p0 : ZR_MAX_PAIRS;
         for (int p = 0; p < ZR_MAX_PAIRS; ++p) {

@@ -14,7 +14,7 @@
 
 namespace epsgrad {
 
-constexpr int EX_THREADS = 256, EX_PASSES = 8;
+constexpr int EX_THREADS = 256, EX_PASSES = 16, EX_CTAS_PER_SM = 8;
 
 struct ExtrudeParams {
     const float *e2d;      // [B,5,ncol]: eps2d_x, eps2d_y, eps2d_z, eps_zz lower face, eps_zz upper face
@@ -22,6 +22,8 @@ struct ExtrudeParams {
     const float *zw;       // [7][nz] z tables (epsgrad.cu)
     int ncol, nz;
     int nblk;              // column blocks per component plane
+    int cpb;               // columns per block (extrude_cols_per_block)
+    int sh4;               // log2(nz/4) when nz/4 is a power of two <= EX_THREADS (fast path), else -1
 };
 
 __host__ __device__ inline int extrude_cols_per_block(int nz)
@@ -30,23 +32,21 @@ __host__ __device__ inline int extrude_cols_per_block(int nz)
     return EX_THREADS % nz4 == 0 ? (EX_THREADS / nz4) * EX_PASSES : 64;
 }
 
-// grid (3 nblk, B); static shared memory
-__global__ void __launch_bounds__(EX_THREADS) k_extrude(const __grid_constant__ ExtrudeParams P)
+// grid (nblk, 3, B): x fastest, so CTAs are dispatched component by component; dynamic shared memory 3 cpb floats
+__global__ void __launch_bounds__(EX_THREADS, EX_CTAS_PER_SM) k_extrude(const __grid_constant__ ExtrudeParams P)
 {
-    __shared__ float vs[3][EX_THREADS * EX_PASSES];           // plane values of the block: [plane][column]; cols_per_block <= 256 EX_PASSES
-    const int tid = threadIdx.x, b = blockIdx.y, nz = P.nz, nz4 = nz >> 2, ncol = P.ncol;
-    const int c = blockIdx.x / P.nblk, blk = blockIdx.x - c * P.nblk;
-    const int cpb = extrude_cols_per_block(nz), col0 = blk * cpb, ncb = min(cpb, ncol - col0);
+    extern __shared__ float vsm[];                            // plane values of the block: [3][cpb]
+    const int tid = threadIdx.x, b = blockIdx.z, nz = P.nz, nz4 = nz >> 2, ncol = P.ncol;
+    const int c = blockIdx.y, blk = blockIdx.x;
+    const int cpb = P.cpb, col0 = blk * cpb, ncb = min(cpb, ncol - col0);
     const float *ed = P.e2d + (size_t)b * 5 * ncol;
     float *out = P.eps + ((size_t)b * 3 + c) * ncol * nz;
     // stage: c = x, y need their own plane; c = z needs planes 2 (full cells), 3 and 4 (face cells)
     const int npl = c == 2 ? 3 : 1;
-    for (int it = tid; it < npl * cpb; it += EX_THREADS) {
-        const int o = it / cpb, lc = it - o * cpb;
-        if (lc < ncb) vs[o][lc] = ed[(size_t)(c + o) * ncol + col0 + lc];
-    }
-    if (EX_THREADS % nz4 == 0) {
-        const int k = (tid % nz4) << 2, cq = tid / nz4, cpp = EX_THREADS / nz4;
+    for (int o = 0; o < npl; ++o)
+        for (int lc = tid; lc < ncb; lc += EX_THREADS) vsm[o * cpb + lc] = ed[(size_t)(c + o) * ncol + col0 + lc];
+    if (P.sh4 >= 0) {
+        const int k = (tid & (nz4 - 1)) << 2, cq = tid >> P.sh4, cpp = EX_THREADS >> P.sh4;
         float4 *dst = reinterpret_cast<float4 *>(out + (size_t)(col0 + cq) * nz + k);
         if (c < 2) {
             float wx[4], bx[4];
@@ -57,7 +57,7 @@ __global__ void __launch_bounds__(EX_THREADS) k_extrude(const __grid_constant__ 
             for (int pass = 0; pass < EX_PASSES; ++pass) {
                 const int lc = cq + pass * cpp;
                 if (lc < ncb) {
-                    const float v = vs[0][lc];
+                    const float v = vsm[lc];
                     float4 o;
                     o.x = fmaf(wx[0], v, bx[0]); o.y = fmaf(wx[1], v, bx[1]);
                     o.z = fmaf(wx[2], v, bx[2]); o.w = fmaf(wx[3], v, bx[3]);
@@ -76,7 +76,7 @@ __global__ void __launch_bounds__(EX_THREADS) k_extrude(const __grid_constant__ 
             for (int pass = 0; pass < EX_PASSES; ++pass) {
                 const int lc = cq + pass * cpp;
                 if (lc < ncb) {
-                    const float v = vs[0][lc], vl = vs[1][lc], vh = vs[2][lc];
+                    const float v = vsm[lc], vl = vsm[cpb + lc], vh = vsm[2 * cpb + lc];
                     float4 o;
                     o.x = fmaf(zf[0], v, fmaf(zl[0], vl, fmaf(zh[0], vh, bz[0])));
                     o.y = fmaf(zf[1], v, fmaf(zl[1], vl, fmaf(zh[1], vh, bz[1])));
@@ -92,12 +92,12 @@ __global__ void __launch_bounds__(EX_THREADS) k_extrude(const __grid_constant__ 
         __syncthreads();
         for (int f = tid; f < ncb * nz4; f += EX_THREADS) {
             const int lc = f / nz4, k = (f - lc * nz4) << 2;
-            const float v = vs[0][lc];
+            const float v = vsm[lc];
             float o[4];
 #pragma unroll
             for (int x = 0; x < 4; ++x)
                 o[x] = c < 2 ? fmaf(w_xy[k + x], v, b_xy[k + x])
-                             : fmaf(i_f[k + x], v, fmaf(i_l[k + x], vs[1][lc], fmaf(i_h[k + x], vs[2][lc], b_z[k + x])));
+                             : fmaf(i_f[k + x], v, fmaf(i_l[k + x], vsm[cpb + lc], fmaf(i_h[k + x], vsm[2 * cpb + lc], b_z[k + x])));
             __stcs(reinterpret_cast<float4 *>(out + (size_t)(col0 + lc) * nz + k), make_float4(o[0], o[1], o[2], o[3]));
         }
     }

@@ -9,7 +9,7 @@
 //     (warp-wide that is one 64-byte broadcast each), then sweeps the NTC+3 source columns, each
 //     loaded value feeding up to NB outputs:  shared-memory wavefronts per FMA drop from 1.25
 //     (reverse) / 0.31 (forward) to 0.40 / 0.15 -- the earlier kernels were shared-memory bound
-//     (profiles/r1b_ncu_full_summary.md).
+//     (profiles/r1a_ncu_full_summary.md).
 // Forward reads c' (control resolution, scalar, conflict-free); reverse reads the v tile staged with
 // one padding block after every 4 (block c at float offset 4(c + c/4)): lanes of a quarter-warp then
 // hit 8 distinct 16-byte bank groups.

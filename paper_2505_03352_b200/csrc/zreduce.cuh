@@ -6,8 +6,8 @@
 //   planes -- full cells, lower face, upper face -- and the mask kernel applies the face factors.  This keeps the
 //   field stream independent of the 2-D chain: the kernel depends on nothing but the fields.
 // Only the 16-byte chunks (2 complex64 cells) of a z column that hold slab cells are read ("|Omega_D";
-// d eps/dC = 0 elsewhere); `dense` plans read every chunk.  CTA n of the grid owns component n / nblk and ZR_COLS
-// consecutive columns: the resident CTAs read one advancing window of one component plane of E_F and of E_A (measured:
+// d eps/dC = 0 elsewhere); `dense` plans read every chunk.  a CTA owns one component and ZR_COLS
+// consecutive columns, and CTAs are dispatched component by component: the resident CTAs read one advancing window of one component plane of E_F and of E_A (measured:
 // 37 us; 48 us when every CTA reads its columns in all three component planes).  A CTA starts asynchronous
 // 16-byte copies (LDGSTS) of every window of both fields into shared memory -- no register staging, one pass of address
 // arithmetic, up to 5 CTAs x 40 KB in flight per SM -- then each thread multiplies and reduces one column out of shared
@@ -75,13 +75,13 @@ __device__ __forceinline__ void zwindow_issue(const ZredParams &P, float4 *buf, 
     cp_async_commit();
 }
 
-// grid (3 nblk, B); dynamic shared memory: 2 fields x ncp x (nch | 1) chunks
+// grid (nblk, 3, B): x fastest, so CTAs are dispatched component by component; dynamic shared memory: 2 fields x ncp x (nch | 1) chunks
 template <bool SPARSE>
 __global__ void __launch_bounds__(ZR_THREADS, 5) k_zreduce(const __grid_constant__ ZredParams P)
 {
     extern __shared__ __align__(16) float4 stage[];
     const int tid = threadIdx.x;
-    const int c = blockIdx.x / P.nblk, blk = blockIdx.x - c * P.nblk, b = blockIdx.y;
+    const int c = blockIdx.y, blk = blockIdx.x, b = blockIdx.z;
     const int grp = c == 2, nch = P.nch[grp], ch0 = P.ch0[grp], ncp = P.ncp[grp], nz = P.nz;
     const int colb = blk * ZR_COLS, ncb = min(ZR_COLS, P.ncol - colb);
 

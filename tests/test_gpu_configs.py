@@ -1,5 +1,5 @@
 """GPU parity on the five BASELINE.json configs at FULL size, in the launch configuration bench.py
-times (eps_forward_vjp, fused streams).
+times (eps_forward_vjp, two-stream schedule).
 
 Tiny, Paper-scale and Multi-wavelength are compared with the float64 oracle element by element.
 Large (2000x2000x64) and Wide batch (8 x 2048x2048x32) are too big for the oracle to finish in
