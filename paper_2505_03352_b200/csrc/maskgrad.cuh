@@ -111,7 +111,8 @@ __global__ void __launch_bounds__(MG_THREADS) k_maskgrad(const __grid_constant__
                             const int src = i_ - di * CJ - dj;
                             const float kx = (float)(di * (2 - (dj < 0 ? -dj : dj))) * 0.125f;
                             const float ky = (float)(dj * (2 - (di < 0 ? -di : di))) * 0.125f;
-                            dbar = fmaf(kx, gxs[src], fmaf(ky, gys[src], dbar));
+                            if (di != 0) dbar = fmaf(kx, gxs[src], dbar);        // the zero taps fold away (unrolled)
+                            if (dj != 0) dbar = fmaf(ky, gys[src], dbar);
                         }
                 } else {
                     // border: sources (i,di) with clamp(i+di) == ii: i = ii-di in range, plus the folded terms
@@ -143,6 +144,44 @@ __global__ void __launch_bounds__(MG_THREADS) k_maskgrad(const __grid_constant__
     const int TP = s * TI, TQ = s * TJ;
     const float *phib = P.phi + (size_t)b * P.px * P.py;
     float *vb = P.v + (size_t)b * P.px * P.py;
+    if (S == 2) {
+        // s = 2: a thread per cell owns its 2 x 2 pixels.  Rows p = 2i, 2i+1 have E_x owners i-1 and i, columns q = 2j, 2j+1
+        // have E_y owners j-1 and j: nine shared-memory values serve the four pixels; 8-byte loads and stores.
+        static_assert(TI * TJ == NTH, "one thread per cell");
+        const int ti = tid / TJ, tj = tid - ti * TJ, i = i0 + ti, j = j0 + tj;
+        if (i >= nx || j >= ny) return;
+        const int c0 = (ti + 2) * CJ + tj + 2;                      // the cell in the staged arrays
+        const float az = AbZ[tid];
+        float ex[2], hx[2], ey[2], hy[2];                           // owner values per pixel row a / column c, multiplicity folded in
+        ex[0] = i >= 1 ? AbF[c0 - CJ] : 0.f;  hx[0] = i >= 1 ? R[c0 - CJ] : 0.f;
+        ey[0] = j >= 1 ? AbF[NC + c0 - 1] : 0.f;  hy[0] = j >= 1 ? R[4 * NC + c0 - 1] : 0.f;
+        const float mx = i == nx - 1 ? 2.0f : 1.0f, my = j == ny - 1 ? 2.0f : 1.0f;   // the clamped last pixel is owned twice
+        ex[1] = mx * AbF[c0];  hx[1] = mx * R[c0];
+        ey[1] = my * AbF[NC + c0];  hy[1] = my * R[4 * NC + c0];
+        const int p = 2 * i, q = 2 * j;
+        const float2 ph0 = *reinterpret_cast<const float2 *>(phib + p * P.py + q);
+        const float2 ph1 = *reinterpret_cast<const float2 *>(phib + (p + 1) * P.py + q);
+        const float phv[2][2] = {{ph0.x, ph0.y}, {ph1.x, ph1.y}};
+        const int nq0 = nidx[TP + 2 * tj], nq1 = nidx[TP + 2 * tj + 1];
+        const float k0 = P.deps * inv_s2 * 2.0f * P.beta;
+#pragma unroll
+        for (int a = 0; a < 2; ++a) {
+            const int np = nidx[2 * ti + a];
+            float o[2];
+#pragma unroll
+            for (int c = 0; c < 2; ++c) {
+                // one exponential serves rho and its slope: e2 = exp(-2|t|), rho = 1/(1+e2) or e2/(1+e2), slope = 2 beta e2/(1+e2)^2
+                const float t = P.beta * (phv[a][c] - P.eta_r);
+                const float e2 = __expf(-2.0f * fabsf(t));
+                const float d = fast_rcp(1.0f + e2);
+                const float r = fast_rcp(fmaf(P.deps, t >= 0.f ? d : e2 * d, P.eps_clad));   // 1/e
+                const float ebar = az + ex[a] + ey[c], rbar = hx[a] + hy[c];
+                o[c] = k0 * e2 * d * d * (ebar - rbar * r * r) * P.nrm.at_index(np, c == 0 ? nq0 : nq1);
+            }
+            *reinterpret_cast<float2 *>(vb + (p + a) * P.py + q) = make_float2(o[0], o[1]);
+        }
+        return;
+    }
     for (int base = tid; base < TP * TQ; base += 4 * NTH) {
         float ph[4];                                           // filter output of four pixels in flight
 #pragma unroll
