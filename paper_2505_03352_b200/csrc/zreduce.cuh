@@ -6,14 +6,14 @@
 //   planes -- full cells, lower face, upper face -- and the mask kernel applies the face factors.  This keeps the
 //   field stream independent of the 2-D chain: the kernel depends on nothing but the fields.
 // Only the 16-byte chunks (2 complex64 cells) of a z column that hold slab cells are read ("|Omega_D";
-// d eps/dC = 0 elsewhere); `dense` plans read every chunk.  a CTA owns one component and ZR_COLS
-// consecutive columns, and CTAs are dispatched component by component: the resident CTAs read one advancing window of one component plane of E_F and of E_A (measured:
-// 37 us; 48 us when every CTA reads its columns in all three component planes).  A CTA starts asynchronous
-// 16-byte copies (LDGSTS) of every window of both fields into shared memory -- no register staging, one pass of address
-// arithmetic, up to 5 CTAs x 40 KB in flight per SM -- then each thread multiplies and reduces one column out of shared
-// memory.  Sparse windows ask for 64-byte L2 fills: the default fill is the whole 128-byte line, and 64 B is the smallest
-// granule the part offers, so a window that straddles a line boundary costs 128 B of DRAM traffic per
-// column, component and field instead of 256 B.
+// d eps/dC = 0 elsewhere); `dense` plans read every chunk.  A CTA owns one component and ZR_COLS consecutive columns, and
+// CTAs are dispatched component by component: the resident CTAs read one advancing window of one component plane of E_F
+// and of E_A (measured: 37 us; 48 us when every CTA reads its columns in all three component planes).  A
+// CTA starts asynchronous 16-byte copies (LDGSTS) of every window of both fields into shared memory -- no register
+// staging, one pass of address arithmetic, up to 5 CTAs x 40 KB in flight per SM -- then each thread multiplies and
+// reduces one column out of shared memory.  Sparse windows ask for 64-byte L2 fills: the default fill is the whole
+// 128-byte line, and 64 B is the smallest granule the part offers, so a window that straddles a line
+// boundary costs 128 B of DRAM traffic per column, component and field instead of 256 B.
 #pragma once
 #include "common.cuh"
 
