@@ -30,7 +30,8 @@
  *     never synchronise the host, never allocate, and never write an input.
  *   - *_host entry points take HOST pointers (pinned memory recommended), stage through
  *     the plan's staging buffer (epsgrad_plan_set_staging), enqueue H2D copies, the same
- *     kernels, and D2H copies on `stream`, and return without synchronising.
+ *     kernels, and D2H copies on `stream`, and return without synchronising.  Pinned field
+ *     buffers are read in place, slab windows only (epsgrad_plan_set_host_direct).
  *   - The caller owns every data buffer, the workspace and the staging buffer.  The
  *     library owns the plan: a host struct plus a few KB of device tables (filter
  *     weights, border normalisers, z weights) allocated in epsgrad_plan_create.
@@ -150,6 +151,11 @@ int eps_forward_vjp(epsgrad_plan_t *plan, const float *C, float beta, int n_pair
 int eps_forward_vjp_host(epsgrad_plan_t *plan, const float *C_host, float beta, int n_pairs,
                          const void *const *EF_host, const void *const *EA_host,
                          float *eps_host, float *dFdC_host, void *stream);
+/* Field transfer of the *_host entry points (default 1).  1: when every field buffer is pinned, mapped host memory (and the
+ * plan is not in dense-read mode), the Eq. (1) reduction copies its slab windows straight out of host memory and the rest
+ * of the fields never crosses the bus (only Omega_D enters the gradient); buffers that are not pinned fall back to
+ * 0.  0: every field is copied whole into the staging buffer first.  Results are identical.                              */
+int epsgrad_plan_set_host_direct(epsgrad_plan_t *plan, int enable);
 /* bytes the last *_host call copied host->device and device->host                       */
 int epsgrad_plan_last_copy_bytes(const epsgrad_plan_t *plan, uint64_t *h2d, uint64_t *d2h);
 

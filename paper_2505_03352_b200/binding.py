@@ -19,7 +19,7 @@ EXPORTS = (
     "epsgrad_plan_create", "epsgrad_plan_destroy", "epsgrad_workspace_bytes",
     "epsgrad_plan_set_workspace", "epsgrad_staging_bytes", "epsgrad_plan_set_staging",
     "epsgrad_plan_set_dense_reads", "epsgrad_plan_last_launches", "epsgrad_plan_last_copy_bytes",
-    "epsgrad_plan_set_profiling", "epsgrad_plan_last_kernel_times", "epsgrad_plan_set_overlap", "epsgrad_plan_set_timeline", "epsgrad_plan_read_timeline", 
+    "epsgrad_plan_set_profiling", "epsgrad_plan_last_kernel_times", "epsgrad_plan_set_overlap", "epsgrad_plan_set_host_direct", "epsgrad_plan_set_timeline", "epsgrad_plan_read_timeline", 
     "eps_forward", "eps_vjp", "eps_forward_vjp", "eps_forward_vjp_host",
     "epsgrad_stage_filter", "epsgrad_stage_eps2d", "epsgrad_stage_zreduce",
     "epsgrad_status_string", "epsgrad_version",
@@ -105,6 +105,7 @@ def lib() -> ctypes.CDLL:
     L.epsgrad_stage_filter.argtypes = [vp, vp, vp, vp]
     L.epsgrad_stage_eps2d.argtypes = [vp, vp, f32, vp, vp]
     L.epsgrad_plan_set_overlap.argtypes = [vp, i32]
+    L.epsgrad_plan_set_host_direct.argtypes = [vp, i32]
     L.epsgrad_plan_set_timeline.argtypes = [vp, i32]
     L.epsgrad_plan_read_timeline.argtypes = [vp, i32, vp, vp]
     L.epsgrad_stage_zreduce.argtypes = [vp, i32, vp, vp, vp, vp]
@@ -208,6 +209,9 @@ class Plan:
         a, b = ctypes.c_uint64(), ctypes.c_uint64()
         _check(lib().epsgrad_plan_last_copy_bytes(self._h, ctypes.byref(a), ctypes.byref(b)), "last_copy_bytes")
         return int(a.value), int(b.value)
+
+    def set_host_direct(self, enable: bool) -> None:
+        _check(lib().epsgrad_plan_set_host_direct(self._h, int(bool(enable))), "epsgrad_plan_set_host_direct")
 
     def set_overlap(self, enable: bool) -> None:
         _check(lib().epsgrad_plan_set_overlap(self._h, int(bool(enable))), "epsgrad_plan_set_overlap")

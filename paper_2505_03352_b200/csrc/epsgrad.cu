@@ -37,7 +37,7 @@ struct epsgrad_plan {
     // z windows (chunks of 2 cells) for {x,y} and {z}; face weights
     int ch0[2], nch[2];
     float w_lo, w_hi;
-    int dense;
+    int dense, host_direct, cur_host_src;   // cur_host_src: the fields of the call in flight are pinned host memory
     // scalars
     float eta0, eta_r, eps_clad, deps, delta;
     // caller-owned buffers
@@ -294,6 +294,7 @@ extern "C" int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsg
         cudaSetDevice(prev2);
         if (!ok) { cudaGetLastError(); epsgrad_plan_destroy(P); return EPSGRAD_ECUDA; }
         P->overlap = 1;
+        P->host_direct = 1;
     }
 
     // ---- workspace carve-up
@@ -391,6 +392,13 @@ extern "C" int epsgrad_plan_set_dense_reads(epsgrad_plan_t *P, int dense)
 {
     if (!P) return EPSGRAD_EINVAL;
     P->dense = dense != 0;
+    return EPSGRAD_OK;
+}
+
+extern "C" int epsgrad_plan_set_host_direct(epsgrad_plan_t *P, int enable)
+{
+    if (!P) return EPSGRAD_EINVAL;
+    P->host_direct = enable != 0;
     return EPSGRAD_OK;
 }
 
@@ -676,7 +684,8 @@ int launch_extrude(epsgrad_plan *P, const float *e2d, float *eps, cudaStream_t s
 }
 
 // ---- R1: the field read stream; more than ZR_MAX_PAIRS pairs are chained through accumulating launches
-int launch_zreduce(epsgrad_plan *P, int n_pairs, const void *const *EF, const void *const *EA, float *gbar, cudaStream_t st)
+int launch_zreduce(epsgrad_plan *P, int n_pairs, const void *const *EF, const void *const *EA, float *gbar, cudaStream_t st,
+                   bool host_src = false)
 {
     ZredParams zp;
     zp.gbar = gbar; zp.zw = P->d_zw; zp.ncol = P->nx * P->ny; zp.nz = P->cfg.nz;
@@ -699,7 +708,8 @@ int launch_zreduce(epsgrad_plan *P, int n_pairs, const void *const *EF, const vo
     zp.nblk = cdiv(zp.ncol, ZR_COLS);
     // windows of at most 128 bytes per column: ask for 64-byte fills
     const bool sparse = maxnch * 16 <= 128 && zp.nz * 8 > 128;
-    auto kern = sparse ? k_zreduce<true> : k_zreduce<false>;
+    host_src = host_src || P->cur_host_src;
+    auto kern = host_src ? k_zreduce<false, true> : (sparse ? k_zreduce<true, false> : k_zreduce<false, false>);
     int rc = set_smem(kern, smem);
     if (rc) return rc;
     if (P->cfg.batch > 65535) return EPSGRAD_EUNSUPPORTED;
@@ -874,7 +884,25 @@ extern "C" int eps_forward_vjp_host(epsgrad_plan_t *P, const float *C_host, floa
     std::vector<const void *> ef(n_pairs), ea(n_pairs);
     bool ok = cudaMemcpyAsync(dC, C_host, b_c, cudaMemcpyHostToDevice, st) == cudaSuccess;
     P->last_h2d += b_c;
-    for (int p = 0; p < n_pairs && ok; ++p) {
+    // Eq. (1) needs only the slab cells of the fields ("|Omega_D").  When every field buffer is pinned, mapped host
+    // memory, the z-reduction reads its windows straight out of it (16-byte asynchronous copies over PCIe / C2C) and the
+    // rest of the fields never crosses the bus; otherwise (pageable memory, dense plans) the fields are staged whole.
+    bool direct = P->host_direct && !P->dense && n_pairs > 0;
+    for (int p = 0; p < n_pairs && direct; ++p) {
+        const void *hp[2] = {EF_host[p], EA_host[p]};
+        const void **dp[2] = {&ef[p], &ea[p]};
+        for (int f = 0; f < 2 && direct; ++f) {
+            cudaPointerAttributes at;
+            if (cudaPointerGetAttributes(&at, hp[f]) != cudaSuccess) { cudaGetLastError(); direct = false; break; }
+            if (at.type != cudaMemoryTypeHost || !at.devicePointer || ((uintptr_t)at.devicePointer & 15)) { direct = false; break; }
+            *dp[f] = at.devicePointer;
+        }
+    }
+    if (direct) {
+        const size_t ncolB = (size_t)P->cfg.batch * P->nx * P->ny;
+        P->last_h2d += (size_t)2 * n_pairs * ncolB * ((size_t)2 * P->nch[0] + P->nch[1]) * 16;   // the chunks the kernel copies
+    }
+    for (int p = 0; p < n_pairs && ok && !direct; ++p) {
         ef[p] = base; base += align_up(b_f, 256);
         ea[p] = base; base += align_up(b_f, 256);
         ok = cudaMemcpyAsync((void *)ef[p], EF_host[p], b_f, cudaMemcpyHostToDevice, st) == cudaSuccess &&
@@ -882,7 +910,33 @@ extern "C" int eps_forward_vjp_host(epsgrad_plan_t *P, const float *C_host, floa
         P->last_h2d += 2 * b_f;
     }
     if (!ok) { cudaGetLastError(); return EPSGRAD_ECUDA; }
+    if (direct && eps_host && dFdC_host && P->overlap && !P->prof) {
+        // The bus is full duplex: eps does not depend on the fields, so it is finished first and travels to the host on the
+        // auxiliary stream while the z-reduction pulls its windows the other way.
+        cudaStream_t ax = P->aux;
+        int rc = launch_filter(P, dC, ws_phi(P), st);
+        if (!rc) rc = launch_fwd2d(P, ws_phi(P), beta, ws_e2d(P), ws_coef(P), nullptr, st);
+        if (!rc) rc = launch_extrude(P, ws_e2d(P), dE, st);
+        if (rc) return rc;
+        ok = cudaEventRecord(P->ev_2d, st) == cudaSuccess && cudaStreamWaitEvent(ax, P->ev_2d, 0) == cudaSuccess &&
+             cudaMemcpyAsync(eps_host, dE, b_e, cudaMemcpyDeviceToHost, ax) == cudaSuccess &&
+             cudaEventRecord(P->ev_join, ax) == cudaSuccess;
+        P->last_d2h += b_e;
+        if (ok) {
+            rc = launch_zreduce(P, n_pairs, ef.data(), ea.data(), ws_gbar(P), st, true);
+            if (!rc) rc = launch_maskgrad(P, ws_phi(P), beta, ws_gbar(P), ws_coef(P), ws_v(P), st);
+            if (!rc) rc = launch_filterT(P, ws_v(P), dG, st);
+            if (!rc) ok = cudaMemcpyAsync(dFdC_host, dG, b_c, cudaMemcpyDeviceToHost, st) == cudaSuccess;
+            P->last_d2h += b_c;
+        }
+        // always join
+        if (cudaStreamWaitEvent(st, P->ev_join, 0) != cudaSuccess) ok = false;
+        if (!ok) { cudaGetLastError(); return EPSGRAD_ECUDA; }
+        return rc;
+    }
+    P->cur_host_src = direct;
     int rc = run_chain(P, dC, beta, n_pairs, ef.data(), ea.data(), eps_host ? dE : nullptr, dFdC_host ? dG : nullptr, st);
+    P->cur_host_src = 0;
     if (rc) return rc;
     if (eps_host) {
         ok = ok && cudaMemcpyAsync(eps_host, dE, b_e, cudaMemcpyDeviceToHost, st) == cudaSuccess;

@@ -57,7 +57,10 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 // lands in one shared-memory write (a [chunk][column] layout splits it in two and costs 25 % of the kernel, measured),
 // and the odd pitch makes the per-column reads of consecutive threads conflict-free.  2^chs >= nch lanes per column (a
 // power of two: no divisions), so a warp instruction covers 32 >> chs neighbouring windows; lanes beyond the window idle.
-template <bool SPARSE>
+// HOSTSRC: the fields live in pinned host memory (epsgrad_plan_set_host_direct): plain 16-byte loads, four columns in
+// flight per thread, then shared-memory stores -- over PCIe these run 3x faster than LDGSTS (measured), and the bus, not
+// the SM, is the limit.
+template <bool SPARSE, bool HOSTSRC>
 __device__ __forceinline__ void zwindow_issue(const ZredParams &P, float4 *buf, int p, int b, int c, int col0, int nc)
 {
     const int grp = c == 2, nzc = P.nz >> 1, nch = P.nch[grp], sh = P.chs[grp], ncp = P.ncp[grp];
@@ -67,16 +70,32 @@ __device__ __forceinline__ void zwindow_issue(const ZredParams &P, float4 *buf, 
         const float4 *pf = P.ef[p] + first, *pa = P.ea[p] + first;
         const int pitch = nch | 1;
         float4 *df = buf + ch, *da = df + pitch * ncp;
-        for (int lc = threadIdx.x >> sh; lc < nc; lc += lstep) {
-            cp_async16<SPARSE>(df + lc * pitch, pf + lc * nzc);
-            cp_async16<SPARSE>(da + lc * pitch, pa + lc * nzc);
+        if (HOSTSRC) {
+            for (int lc0 = threadIdx.x >> sh; lc0 < nc; lc0 += 4 * lstep) {
+                float4 f[4], a[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int lc = lc0 + u * lstep;
+                    if (lc < nc) { f[u] = ld_stream<false>(pf + lc * nzc); a[u] = ld_stream<false>(pa + lc * nzc); }
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int lc = lc0 + u * lstep;
+                    if (lc < nc) { df[lc * pitch] = f[u]; da[lc * pitch] = a[u]; }
+                }
+            }
+        } else {
+            for (int lc = threadIdx.x >> sh; lc < nc; lc += lstep) {
+                cp_async16<SPARSE>(df + lc * pitch, pf + lc * nzc);
+                cp_async16<SPARSE>(da + lc * pitch, pa + lc * nzc);
+            }
         }
     }
     cp_async_commit();
 }
 
 // grid (nblk, 3, B): x fastest, so CTAs are dispatched component by component; dynamic shared memory: 2 fields x ncp x (nch | 1) chunks
-template <bool SPARSE>
+template <bool SPARSE, bool HOSTSRC>
 __global__ void __launch_bounds__(ZR_THREADS, 5) k_zreduce(const __grid_constant__ ZredParams P)
 {
     extern __shared__ __align__(16) float4 stage[];
@@ -85,7 +104,7 @@ __global__ void __launch_bounds__(ZR_THREADS, 5) k_zreduce(const __grid_constant
     const int grp = c == 2, nch = P.nch[grp], ch0 = P.ch0[grp], ncp = P.ncp[grp], nz = P.nz;
     const int colb = blk * ZR_COLS, ncb = min(ZR_COLS, P.ncol - colb);
 
-    zwindow_issue<SPARSE>(P, stage, 0, b, c, colb, min(ncp, ncb));
+    zwindow_issue<SPARSE, HOSTSRC>(P, stage, 0, b, c, colb, min(ncp, ncb));
     // a thread reduces one column; the extrusion weights (2 cells per chunk; three rows for component z) are warp-uniform
     // cached loads
     for (int c0 = 0; c0 < ncb; c0 += ncp) {
@@ -94,7 +113,7 @@ __global__ void __launch_bounds__(ZR_THREADS, 5) k_zreduce(const __grid_constant
         for (int p = 0; p < P.n_pairs; ++p) {
             if (c0 > 0 || p > 0) {
                 __syncthreads();                     // every thread is done reading the previous windows
-                zwindow_issue<SPARSE>(P, stage, p, b, c, colb + c0, nc);
+                zwindow_issue<SPARSE, HOSTSRC>(P, stage, p, b, c, colb + c0, nc);
             }
             cp_async_wait_all();
             __syncthreads();
