@@ -40,7 +40,7 @@ class _Cfg(ctypes.Structure):
         ("radius", ctypes.c_double), ("sigma", ctypes.c_double),
         ("z_lo", ctypes.c_double), ("z_hi", ctypes.c_double),
         ("eta", ctypes.c_double), ("eps_core", ctypes.c_double), ("eps_clad", ctypes.c_double),
-        ("delta", ctypes.c_double),
+        ("delta", ctypes.c_double), ("morph_diam", ctypes.c_double), ("morph_alpha", ctypes.c_double),
     ]
 
 
@@ -63,11 +63,13 @@ class OracleConfig:
     eps_core: float = 12.11
     eps_clad: float = 2.085
     delta: float = 1e-12
+    morph_diam: float = 0.0         # d of Eqs. (4)-(5) in Yee cells; 0 = morphological filters off
+    morph_alpha: float = 20.0
 
     def c(self) -> _Cfg:
         return _Cfg(self.mx, self.my, self.nx, self.ny, self.nz, self.s, self.filter_kind,
                     self.normalize, self.radius, self.sigma, self.z_lo, self.z_hi, self.eta,
-                    self.eps_core, self.eps_clad, self.delta)
+                    self.eps_core, self.eps_clad, self.delta, self.morph_diam, self.morph_alpha)
 
     @property
     def px(self) -> int:
@@ -127,6 +129,24 @@ def filter_T(cfg: OracleConfig, Phibar):
     Cbar = np.empty((cfg.mx, cfg.my))
     lib().orc_filter_T(ctypes.byref(c), _p(Phibar), _p(Cbar))
     return Cbar
+
+
+def morph(cfg: OracleConfig, x, erode: bool):
+    """Eq. (4) (dilate) or Eq. (5) (erode) on the mask grid"""
+    c = cfg.c()
+    x = _f64(x, (cfg.px, cfg.py))
+    y = np.empty_like(x)
+    lib().orc_morph(ctypes.byref(c), _p(x), ctypes.c_int(int(erode)), _p(y))
+    return y
+
+
+def morph_T(cfg: OracleConfig, x, erode: bool, ybar):
+    c = cfg.c()
+    x = _f64(x, (cfg.px, cfg.py))
+    ybar = _f64(ybar, (cfg.px, cfg.py))
+    xbar = np.zeros_like(x)
+    lib().orc_morph_T(ctypes.byref(c), _p(x), ctypes.c_int(int(erode)), _p(ybar), _p(xbar))
+    return xbar
 
 
 def project(Phi, beta: float, eta: float):

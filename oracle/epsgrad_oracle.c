@@ -49,6 +49,8 @@ typedef struct {
     double  eta;             /* 0.5 -> Eq. (6) form, 0 -> Eq. (3) form (S9)       */
     double  eps_core, eps_clad;
     double  delta;           /* guard in the normal normalisation (S6)            */
+    double  morph_diam;      /* d of Eqs. (4)-(5) in Yee cells; 0 = filters off   */
+    double  morph_alpha;     /* alpha of Eqs. (4)-(5) (App. B: 20)                */
 } orc_cfg;
 
 static int clampi(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); }
@@ -368,12 +370,77 @@ void orc_extrude_T(const orc_cfg *g, const double *eps2d, const double *epsbar, 
 }
 
 /* ------------------------------------------------------------------ */
+/* Morphological filters, Eqs. (4)-(5), on the mask grid.   */
+/*   dilate  y = (1/alpha) log  sum K_m exp(alpha x)                   */
+/*   erode   y = 1 - (1/alpha) log sum K_m exp(alpha (1 - x))          */
+/* K_m = 1 inside a circle of diameter d: the mask pixels whose */
+/* centre offset (dp,dq) has dp^2 + dq^2 <= (d s / 2)^2, d in cells.   */
+/* K_m is normalised to unit sum over the pixels that lie inside the   */
+/* region (G5, S18): otherwise dilate(c) != c.  Finite sums replace    */
+/* the integrals, as in Eq. (8).                               */
+/* ------------------------------------------------------------------ */
+void orc_morph(const orc_cfg *g, const double *x, int erode, double *y)
+{
+    const int px = g->s * g->nx, py = g->s * g->ny;
+    const double rp = 0.5 * g->morph_diam * g->s, al = g->morph_alpha;
+    const int R = (int)floor(rp);
+#pragma omp parallel for schedule(static)
+    for (int p = 0; p < px; ++p)
+        for (int q = 0; q < py; ++q) {
+            double S = 0.0;
+            int N = 0;
+            for (int dp = -R; dp <= R; ++dp)
+                for (int dq = -R; dq <= R; ++dq) {
+                    if ((double)(dp * dp + dq * dq) > rp * rp) continue;
+                    const int pp = p + dp, qq = q + dq;
+                    if (pp < 0 || pp >= px || qq < 0 || qq >= py) continue;
+                    const double v = x[(size_t)pp * py + qq];
+                    S += exp(al * (erode ? 1.0 - v : v));
+                    ++N;
+                }
+            const double l = log(S / (double)N) / al;
+            y[(size_t)p * py + q] = erode ? 1.0 - l : l;
+        }
+}
+
+/* transpose of orc_morph at x: xbar += J^T ybar (scatter form, serial).
+ * d y[p,q] / d x[p',q'] = exp(alpha x') / S[p,q] (dilate), exp(alpha (1-x')) / S[p,q] (erode). */
+void orc_morph_T(const orc_cfg *g, const double *x, int erode, const double *ybar, double *xbar)
+{
+    const int px = g->s * g->nx, py = g->s * g->ny;
+    const double rp = 0.5 * g->morph_diam * g->s, al = g->morph_alpha;
+    const int R = (int)floor(rp);
+    for (int p = 0; p < px; ++p)
+        for (int q = 0; q < py; ++q) {
+            double S = 0.0;
+            for (int dp = -R; dp <= R; ++dp)
+                for (int dq = -R; dq <= R; ++dq) {
+                    if ((double)(dp * dp + dq * dq) > rp * rp) continue;
+                    const int pp = p + dp, qq = q + dq;
+                    if (pp < 0 || pp >= px || qq < 0 || qq >= py) continue;
+                    const double v = x[(size_t)pp * py + qq];
+                    S += exp(al * (erode ? 1.0 - v : v));
+                }
+            const double yb = ybar[(size_t)p * py + q];
+            for (int dp = -R; dp <= R; ++dp)
+                for (int dq = -R; dq <= R; ++dq) {
+                    if ((double)(dp * dp + dq * dq) > rp * rp) continue;
+                    const int pp = p + dp, qq = q + dq;
+                    if (pp < 0 || pp >= px || qq < 0 || qq >= py) continue;
+                    const double v = x[(size_t)pp * py + qq];
+                    xbar[(size_t)pp * py + qq] += yb * exp(al * (erode ? 1.0 - v : v)) / S;
+                }
+        }
+}
+
+/* ------------------------------------------------------------------ */
 /* Whole forward chain, steps 1-7 in order.  C is the fp32 buffer the  */
 /* GPU sees, converted to double.  eps: [3,nx,ny,nz] double.           */
 /* eps2d_out: optional [3,nx,ny].                                      */
 /* ------------------------------------------------------------------ */
 typedef struct {
     double *Phi, *rho, *e, *r;          /* mask arrays [px*py]                */
+    double *mx[5];                      /* morphological chain: rho0, dilate, erode, erode, dilate (S17) */
     double *A[3], *H[3], *D[3];         /* cell averages per component        */
     double *gx[2], *gy[2];              /* Sobel gradients of D_x, D_y        */
     double *eps2d;                      /* [3,nx,ny]                          */
@@ -383,6 +450,7 @@ static void work_alloc(const orc_cfg *g, orc_work *w)
 {
     size_t nm = (size_t)g->s * g->nx * g->s * g->ny, nc = (size_t)g->nx * g->ny;
     w->Phi = malloc(8 * nm); w->rho = malloc(8 * nm); w->e = malloc(8 * nm); w->r = malloc(8 * nm);
+    for (int k = 0; k < 5; ++k) w->mx[k] = g->morph_diam > 0.0 ? malloc(8 * nm) : NULL;
     for (int c = 0; c < 3; ++c) { w->A[c] = malloc(8 * nc); w->H[c] = malloc(8 * nc); w->D[c] = malloc(8 * nc); }
     for (int c = 0; c < 2; ++c) { w->gx[c] = malloc(8 * nc); w->gy[c] = malloc(8 * nc); }
     w->eps2d = malloc(8 * 3 * nc);
@@ -391,6 +459,7 @@ static void work_alloc(const orc_cfg *g, orc_work *w)
 static void work_free(orc_work *w)
 {
     free(w->Phi); free(w->rho); free(w->e); free(w->r);
+    for (int k = 0; k < 5; ++k) free(w->mx[k]);
     for (int c = 0; c < 3; ++c) { free(w->A[c]); free(w->H[c]); free(w->D[c]); }
     for (int c = 0; c < 2; ++c) { free(w->gx[c]); free(w->gy[c]); }
     free(w->eps2d);
@@ -403,7 +472,15 @@ static void forward_2d(const orc_cfg *g, const float *C32, double beta, orc_work
     for (int64_t i = 0; i < (int64_t)g->mx * g->my; ++i) C[i] = (double)C32[i];
     orc_filter(g, C, w->Phi, NULL);                                 /* steps 1-2 */
     free(C);
-    orc_project(nm, w->Phi, beta, g->eta, w->rho);                  /* step 3    */
+    if (g->morph_diam > 0.0) {
+        /* P:L64-74 (S17): first projection, then "dilate and erode and erode and dilate" (close, then open),
+         * then the second projection, Eq. (6), with its threshold 1/2 */
+        static const int is_erode[4] = {0, 1, 1, 0};
+        orc_project(nm, w->Phi, beta, g->eta, w->mx[0]);
+        for (int k = 0; k < 4; ++k) orc_morph(g, w->mx[k], is_erode[k], w->mx[k + 1]);
+        orc_project(nm, w->mx[4], beta, 0.5, w->rho);
+    } else
+        orc_project(nm, w->Phi, beta, g->eta, w->rho);              /* step 3    */
     orc_mix(g, nm, w->rho, w->e, w->r);
     for (int c = 0; c < 3; ++c) {                                   /* step 4    */
         orc_average(g, w->e, c, w->A[c]);
@@ -478,7 +555,19 @@ static void reverse_2d(const orc_cfg *g, double beta, const orc_work *w,
         orc_average_T(g, Dbar, c, rhobar);
     }
     orc_mix_T(g, (int64_t)nm, w->e, ebar, rbar, rhobar);            /* step 3^T */
-    orc_project_T((int64_t)nm, w->Phi, beta, g->eta, rhobar, Phibar);
+    if (g->morph_diam > 0.0) {
+        static const int is_erode[4] = {0, 1, 1, 0};
+        double *cur = malloc(8 * nm), *nxt = malloc(8 * nm);
+        orc_project_T((int64_t)nm, w->mx[4], beta, 0.5, rhobar, cur);
+        for (int k = 3; k >= 0; --k) {
+            memset(nxt, 0, 8 * nm);
+            orc_morph_T(g, w->mx[k], is_erode[k], cur, nxt);
+            double *t = cur; cur = nxt; nxt = t;
+        }
+        orc_project_T((int64_t)nm, w->Phi, beta, g->eta, cur, Phibar);
+        free(cur); free(nxt);
+    } else
+        orc_project_T((int64_t)nm, w->Phi, beta, g->eta, rhobar, Phibar);
     orc_filter_T(g, Phibar, dFdC);                                  /* step 2^T */
     free(ebar); free(rbar); free(rhobar); free(Abar); free(Hbar); free(Dbar);
     free(gxbar); free(gybar); free(Phibar);

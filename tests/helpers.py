@@ -61,9 +61,29 @@ def torch_sobel(D):
     return F.conv2d(Dp, kx[None, None])[0, 0], F.conv2d(Dp, kx.t().contiguous()[None, None])[0, 0]
 
 
+def torch_morph(cfg, x, erode):
+    """Eqs. (4)-(5) from library primitives: unfold the mask into disk neighbourhoods (outside = -inf, i.e. weight 0),
+    torch.logsumexp, minus log of the in-range count (unit-sum kernel, S18)."""
+    rp = 0.5 * cfg.morph_diam * cfg.s
+    R = int(math.floor(rp))
+    d = torch.arange(-R, R + 1, dtype=torch.float64)
+    disk = ((d[:, None] ** 2 + d[None, :] ** 2) <= rp * rp).reshape(-1)
+    z = cfg.morph_alpha * ((1.0 - x) if erode else x)
+    zp = F.pad(z[None, None], (R, R, R, R), value=float("-inf"))
+    cols = F.unfold(zp, 2 * R + 1)[0]                                  # [(2R+1)^2, px*py]
+    cols = cols[disk]
+    n = torch.isfinite(cols).sum(0).to(torch.float64)
+    l = ((torch.logsumexp(cols, 0) - torch.log(n)) / cfg.morph_alpha).reshape(x.shape)
+    return 1.0 - l if erode else l
+
+
 def torch_eps2d(cfg, C, beta):
     Phi = torch_filter(cfg, C)
     rho = 0.5 * (1 + torch.tanh(beta * (Phi - cfg.eta)))
+    if cfg.morph_diam > 0:                                             # P:L64-74 (S17): dilate, erode, erode, dilate, Eq. (6)
+        for erode in (False, True, True, False):
+            rho = torch_morph(cfg, rho, erode)
+        rho = 0.5 * (1 + torch.tanh(beta * (rho - 0.5)))
     e = rho * cfg.eps_core + (1 - rho) * cfg.eps_clad
     r = 1.0 / e
     out = []
