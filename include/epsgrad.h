@@ -9,6 +9,7 @@
  *     Eq. (2)  Phi  = sum_ab C_ab b(x-x_a, y-y_b)   on a mask with `subpixel` pixels per
  *              Yee cell (normalised density-filter form by default, S2)
  *     Eq. (3)/(6)  rho = 1/2 (1 + tanh(beta (Phi - eta)))
+ *     Eq. (4)/(5)  optional morphological dilate / erode of rho, then Eq. (6)
  *     mixing   eps = rho eps_core + (1-rho) eps_clad
  *     Eq. (8)  cell averages <eps>, <1/eps> on the half-cell-shifted E_x/E_y/E_z
  *              footprints (finite sums on the mask)
@@ -51,7 +52,8 @@ extern "C" {
 
 #define EPSGRAD_OK             0
 #define EPSGRAD_EINVAL        -1   /* null / misaligned pointer, bad size, beta <= 0, eps <= 0, ... */
-#define EPSGRAD_EUNSUPPORTED  -2   /* upsample*subpixel not in {2,4,6,8}, Nz % 4 != 0, tables too large */
+#define EPSGRAD_EUNSUPPORTED  -2   /* upsample*subpixel not in {2,4,6,8}, Nz % 4 != 0, tables too large,
+                                      morphological disk radius > 16 mask pixels or wider than the mask */
 #define EPSGRAD_ENOWORKSPACE  -3   /* workspace / staging buffer missing or too small */
 #define EPSGRAD_ECUDA         -4   /* CUDA runtime error (no device, launch failure) */
 #define EPSGRAD_ENOMEM        -5   /* host allocation failed */
@@ -78,6 +80,10 @@ typedef struct {
     double  eta;              /* projection threshold: 0.5 -> Eq. (6), 0 -> Eq. (3) (S9)     */
     double  eps_core, eps_clad;
     double  normal_delta;     /* guard in n_c^2 = g_c^2/(|g|^2 + delta) (S6; default 1e-12)  */
+    double  morph_diameter;   /* d of Eqs. (4)-(5) in Yee cells (minimum feature size); 0 = morphological
+                                 filters off.  On: rho0 = projection(Phi), "dilate, erode, erode, dilate" (
+                                 S17) with the disk K_m normalised over the in-region pixels (S18), then Eq. (6) */
+    double  morph_alpha;      /* alpha of Eqs. (4)-(5) (App. B: 20); used when morph_diameter > 0                */
 } epsgrad_config_t;
 
 /* ---- plan -------------------------------------------------------------------------- */
@@ -114,7 +120,7 @@ int epsgrad_plan_last_launches(const epsgrad_plan_t *plan);
 
 /* Per-kernel timing for roofline accounting.  When enabled, every eps_* / stage call also
  * records a CUDA event on `stream` before its first and after each of its kernels (at most
- * 16).  epsgrad_plan_last_kernel_times waits (host-blocking: the one exception to "never
+ * 24).  epsgrad_plan_last_kernel_times waits (host-blocking: the one exception to "never
  * synchronises") for the last call's events and returns the number n of kernels it
  * launched, writing ms[i] = device time between the events around kernel i (it includes
  * the launch gap before it) and names[i] = a static string naming the kernel; ms[i] = -1
@@ -124,7 +130,7 @@ int epsgrad_plan_last_kernel_times(epsgrad_plan_t *plan, int max_n, float *ms, c
 
 /* Timeline of one call (diagnostic; default off).  When enabled, a one-thread kernel that stores the device clock
  * (%globaltimer, ns) is enqueued at the start of a two-stream call and after each kernel on that kernel's stream (up to
- * 32 stamps), so the stamps show when each kernel of either stream ended.  epsgrad_plan_read_timeline synchronises the
+ * 48 stamps), so the stamps show when each kernel of either stream ended.  epsgrad_plan_read_timeline synchronises the
  * device (host-blocking) and returns the number n of stamps of the last call with their names ("begin" or the kernel
  * whose end they mark).  The extra kernels perturb the schedule slightly; not for timed runs.                          */
 int epsgrad_plan_set_timeline(epsgrad_plan_t *plan, int enable);

@@ -41,7 +41,7 @@ class Config(ctypes.Structure):
         ("z_lo", ctypes.c_double), ("z_hi", ctypes.c_double),
         ("filter_radius", ctypes.c_double), ("filter_sigma", ctypes.c_double),
         ("eta", ctypes.c_double), ("eps_core", ctypes.c_double), ("eps_clad", ctypes.c_double),
-        ("normal_delta", ctypes.c_double),
+        ("normal_delta", ctypes.c_double), ("morph_diameter", ctypes.c_double), ("morph_alpha", ctypes.c_double),
     ]
 
     @property
@@ -55,9 +55,9 @@ class Config(ctypes.Structure):
 
 def make_config(*, batch=1, mx, my, nz, z_lo, z_hi, upsample=2, subpixel=2, filter_kind=FILTER_CONIC,
                 filter_radius=4.0, filter_sigma=1.0, filter_normalize=1, eta=0.5, eps_core=12.11,
-                eps_clad=2.085, normal_delta=1e-12) -> Config:
+                eps_clad=2.085, normal_delta=1e-12, morph_diameter=0.0, morph_alpha=20.0) -> Config:
     return Config(batch, mx, my, upsample, subpixel, nz, filter_kind, filter_normalize, z_lo, z_hi,
-                  filter_radius, filter_sigma, eta, eps_core, eps_clad, normal_delta)
+                  filter_radius, filter_sigma, eta, eps_core, eps_clad, normal_delta, morph_diameter, morph_alpha)
 
 
 def config_of(w) -> Config:
@@ -65,7 +65,8 @@ def config_of(w) -> Config:
     return make_config(batch=w.batch, mx=w.mx, my=w.my, nz=w.nz, z_lo=w.z_lo, z_hi=w.z_hi, upsample=w.upsample,
                        subpixel=w.subpixel, filter_kind=w.filter_kind, filter_radius=w.radius,
                        filter_sigma=w.sigma if w.sigma > 0 else 1.0, eta=w.eta, eps_core=w.eps_core,
-                       eps_clad=w.eps_clad, normal_delta=w.normal_delta)
+                       eps_clad=w.eps_clad, normal_delta=w.normal_delta,
+                       morph_diameter=getattr(w, "morph_diameter", 0.0), morph_alpha=getattr(w, "morph_alpha", 20.0))
 
 
 _lib = None
@@ -221,9 +222,9 @@ class Plan:
 
     def read_timeline(self):
         """[(name, ns since the first stamp)] of the last call (synchronises the device)"""
-        ns = (ctypes.c_uint64 * 32)()
-        names = (ctypes.c_char_p * 32)()
-        n = lib().epsgrad_plan_read_timeline(self._h, 32, ns, names)
+        ns = (ctypes.c_uint64 * 48)()
+        names = (ctypes.c_char_p * 48)()
+        n = lib().epsgrad_plan_read_timeline(self._h, 48, ns, names)
         _check(min(n, 0), "epsgrad_plan_read_timeline")
         return [(names[i].decode(), int(ns[i]) - int(ns[0])) for i in range(n)]
 
@@ -232,9 +233,9 @@ class Plan:
 
     def last_kernel_times(self):
         """[(kernel name, ms)] of the last call (blocks until its events have completed)."""
-        ms = (ctypes.c_float * 16)()
-        names = (ctypes.c_char_p * 16)()
-        n = lib().epsgrad_plan_last_kernel_times(self._h, 16, ms, names)
+        ms = (ctypes.c_float * 24)()
+        names = (ctypes.c_char_p * 24)()
+        n = lib().epsgrad_plan_last_kernel_times(self._h, 24, ms, names)
         if n < 0:
             raise EpsgradError(n, "epsgrad_plan_last_kernel_times")
         return [(names[i].decode(), float(ms[i])) for i in range(n)]

@@ -16,11 +16,12 @@
 #include "extrude.cuh"
 #include "zreduce.cuh"
 #include "maskgrad.cuh"
+#include "morph.cuh"
 
 using namespace epsgrad;
 
 #define EPSGRAD_VERSION 100   /* 0.1.0 */
-#define EPSGRAD_MAX_KERNELS 16
+#define EPSGRAD_MAX_KERNELS 24
 
 struct epsgrad_plan {
     epsgrad_config_t cfg;
@@ -37,6 +38,12 @@ struct epsgrad_plan {
     // z windows (chunks of 2 cells) for {x,y} and {z}; face weights
     int ch0[2], nch[2];
     float w_lo, w_hi;
+    // morphological filters (Eqs. (4)-(5)): disk radius in mask pixels (0 = off), alpha, device tables
+    int morph_R;
+    float morph_alpha;
+    int *d_hl;                 // [2R+1] half-lengths of the disk rows
+    float *d_invn;             // [(2R+1)^2] 1/N by border class
+    size_t off_m[4], off_mc, off_cot;
     int dense, host_direct, cur_host_src;   // cur_host_src: the fields of the call in flight are pinned host memory
     // scalars
     float eta0, eta_r, eps_clad, deps, delta;
@@ -109,6 +116,13 @@ static int validate(const epsgrad_config_t *c)
     if (c->filter_kind == EPSGRAD_FILTER_GAUSSIAN && !(c->filter_sigma > 0.0)) return EPSGRAD_EINVAL;
     if (!(c->eps_core > 0.0) || !(c->eps_clad > 0.0) || c->eps_core == c->eps_clad) return EPSGRAD_EINVAL;
     if (!(c->normal_delta >= 0.0)) return EPSGRAD_EINVAL;
+    if (!(c->morph_diameter >= 0.0)) return EPSGRAD_EINVAL;
+    if (c->morph_diameter > 0.0) {
+        if (!(c->morph_alpha > 0.0)) return EPSGRAD_EINVAL;
+        const int R = (int)std::floor(0.5 * c->morph_diameter * c->subpixel);
+        if (R > MO_MAX_R) return EPSGRAD_EUNSUPPORTED;
+        if (c->subpixel * c->upsample * c->mx < 2 * R + 1 || c->subpixel * c->upsample * c->my < 2 * R + 1) return EPSGRAD_EUNSUPPORTED;
+    }
     const int m = c->upsample * c->subpixel;
     if (m != 2 && m != 4 && m != 6 && m != 8) return EPSGRAD_EUNSUPPORTED;
     if (c->nz % 4) return EPSGRAD_EUNSUPPORTED;
@@ -278,6 +292,37 @@ extern "C" int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsg
         return EPSGRAD_ECUDA;
     }
 
+    // ---- morphological disk: K_m = 1 for dp^2 + dq^2 <= (d s / 2)^2, unit sum over the in-region pixels (S18)
+    if (cfg->morph_diameter > 0.0) {
+        const double rp = 0.5 * cfg->morph_diameter * s;
+        const int R = (int)std::floor(rp), NI = 2 * R + 1;
+        P->morph_R = R;
+        P->morph_alpha = (float)cfg->morph_alpha;
+        std::vector<int> hl(NI);
+        for (int dp = -R; dp <= R; ++dp) hl[dp + R] = (int)std::floor(std::sqrt(rp * rp - (double)dp * dp) + 1e-9);
+        std::vector<float> invn((size_t)NI * NI);
+        for (int cp = 0; cp < NI; ++cp)
+            for (int cq = 0; cq < NI; ++cq) {
+                // class c < R: c pixels from the low edge; c > R: 2R - c pixels from the high edge; R: interior
+                const int lo_p = cp < R ? cp : R, hi_p = cp > R ? 2 * R - cp : R;
+                const int lo_q = cq < R ? cq : R, hi_q = cq > R ? 2 * R - cq : R;
+                int n = 0;
+                for (int dp = -lo_p; dp <= hi_p; ++dp)
+                    for (int dq = -lo_q; dq <= hi_q; ++dq)
+                        if ((double)(dp * dp + dq * dq) <= rp * rp) ++n;
+                invn[(size_t)cp * NI + cq] = (float)(1.0 / n);
+            }
+        int prevd = 0;
+        cudaGetDevice(&prevd);
+        cudaSetDevice(device);
+        bool okm = cudaMalloc(&P->d_hl, NI * sizeof(int)) == cudaSuccess &&
+                   cudaMalloc(&P->d_invn, invn.size() * sizeof(float)) == cudaSuccess &&
+                   cudaMemcpy(P->d_hl, hl.data(), NI * sizeof(int), cudaMemcpyHostToDevice) == cudaSuccess &&
+                   cudaMemcpy(P->d_invn, invn.data(), invn.size() * sizeof(float), cudaMemcpyHostToDevice) == cudaSuccess;
+        cudaSetDevice(prevd);
+        if (!okm) { cudaGetLastError(); epsgrad_plan_destroy(P); return EPSGRAD_ECUDA; }
+    }
+
     // ---- auxiliary stream and fork/join events (no timing) for the two-stream schedule
     {
         int prev2 = 0;
@@ -305,6 +350,11 @@ extern "C" int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsg
     P->off_gbar = off; off += align_up(n_cell * 5 * 4, 256);
     P->off_e2d = off;  off += align_up(n_cell * F2_NE2D * 4, 256);
     P->off_coef = off; off += align_up(n_cell * F2_NCOEF * 4, 256);
+    if (P->morph_R > 0) {
+        for (int k = 0; k < 4; ++k) { P->off_m[k] = off; off += align_up(n_mask * 4, 256); }
+        P->off_mc = off;  off += align_up(n_mask * 4, 256);
+        P->off_cot = off; off += align_up(n_mask * 4, 256);
+    }
     P->off_tmp = off;  off += P->separable ? align_up((size_t)cfg->batch * cfg->mx * P->py * 4, 256) : 0;
     P->ws_need = off;
     *out = P;
@@ -316,6 +366,8 @@ extern "C" int epsgrad_plan_destroy(epsgrad_plan_t *P)
     if (!P) return EPSGRAD_EINVAL;
     if (P->d_tables) cudaFree(P->d_tables);
     if (P->d_tl) cudaFree(P->d_tl);
+    if (P->d_hl) cudaFree(P->d_hl);
+    if (P->d_invn) cudaFree(P->d_invn);
     if (P->aux) cudaStreamDestroy(P->aux);
     if (P->ev_fork) cudaEventDestroy(P->ev_fork);
     if (P->ev_r) cudaEventDestroy(P->ev_r);
@@ -519,6 +571,9 @@ Normaliser make_nrm(const epsgrad_plan *P)
 
 float *ws_phi(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_phi); }
 float *ws_v(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_v); }
+float *ws_m(const epsgrad_plan *P, int k) { return (float *)((char *)P->ws + P->off_m[k]); }
+float *ws_mc(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_mc); }
+float *ws_cot(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_cot); }
 float *ws_gbar(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_gbar); }
 float *ws_e2d(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_e2d); }
 float *ws_coef(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_coef); }
@@ -654,6 +709,7 @@ int launch_fwd2d(epsgrad_plan *P, const float *phi, float beta, float *e2d, floa
     fp.phi = phi; fp.e2d = e2d; fp.coef = coef; fp.eps2d = eps2d;
     fp.nx = P->nx; fp.ny = P->ny; fp.px = P->px; fp.py = P->py; fp.s = P->cfg.subpixel;
     fp.beta = beta; fp.eta_r = P->eta_r; fp.eps_clad = P->eps_clad; fp.deps = P->deps; fp.delta = P->delta;
+    if (P->morph_R > 0) { fp.phi = ws_mc(P); fp.eta_r = 0.0f; }     // Eq. (6) on the filtered mask, centred at 1/2
     fp.w_lo = P->w_lo; fp.w_hi = P->w_hi;
     const size_t smem = fwd2d_smem_floats(fp.s) * 4;
     auto kern = fp.s == 2 ? k_fwd2d<2> : (fp.s == 4 ? k_fwd2d<4> : k_fwd2d<0>);
@@ -728,6 +784,72 @@ int launch_zreduce(epsgrad_plan *P, int n_pairs, const void *const *EF, const vo
     return EPSGRAD_OK;
 }
 
+// ---- Eqs. (4)-(5): "dilate, erode, erode, dilate" (S17) between the first projection and Eq. (6)
+int launch_morph_one(epsgrad_plan *P, const MorphParams &mp, cudaStream_t st, const char *name)
+{
+    const size_t smem = morph_smem_floats(P->morph_R) * 4;
+    int rc = set_smem(k_morph, smem);
+    if (rc) return rc;
+    k_morph<<<dim3(cdiv(P->py, MO_T), cdiv(P->px, MO_T), P->cfg.batch), MO_THREADS, smem, st>>>(mp);
+    return check_launch(P, name, st);
+}
+
+MorphParams morph_base(const epsgrad_plan *P, float beta)
+{
+    MorphParams mp;
+    std::memset(&mp, 0, sizeof(mp));
+    mp.hl = P->d_hl; mp.invn = P->d_invn; mp.nrm = make_nrm(P);
+    mp.px = P->px; mp.py = P->py; mp.R = P->morph_R;
+    mp.beta = beta; mp.eta_r = P->eta_r;
+    return mp;
+}
+
+// forward: Phi' -> rho0 (kept in m[0]) -> m[1] -> m[2] -> m[3] -> rho~ - 1/2 (mc)
+int launch_morph_forward(epsgrad_plan *P, const float *phi, float beta, cudaStream_t st)
+{
+    static const float sign[4] = {1.f, -1.f, -1.f, 1.f};
+    for (int k = 0; k < 4; ++k) {
+        MorphParams mp = morph_base(P, beta);
+        mp.x = k == 0 ? phi : ws_m(P, k);
+        mp.out = k == 3 ? ws_mc(P) : ws_m(P, k + 1);
+        mp.rho0 = ws_m(P, 0);
+        mp.first = k == 0; mp.last = k == 3; mp.transposed = 0;
+        mp.a = sign[k] * P->morph_alpha;
+        int rc = launch_morph_one(P, mp, st, "morph");
+        if (rc) return rc;
+    }
+    return EPSGRAD_OK;
+}
+
+// transposed: cotangent of rho~ (cot) -> ... -> v (the last op applies projection^T and 1/den); buffers alternate
+int launch_morph_reverse(epsgrad_plan *P, const float *phi, float beta, float *v, cudaStream_t st)
+{
+    static const float sign[4] = {1.f, -1.f, -1.f, 1.f};
+    float *src = v, *dst = ws_cot(P);                  // maskgrad left the cotangent of rho~ in v; four ops later the result is back in v
+    for (int k = 3; k >= 0; --k) {
+        MorphParams mp = morph_base(P, beta);
+        mp.x = k == 0 ? phi : ws_m(P, k);
+        mp.y = k == 3 ? ws_mc(P) : ws_m(P, k + 1);
+        mp.ybar = src;
+        mp.out = dst;
+        mp.rho0 = ws_m(P, 0);
+        mp.first = k == 0; mp.last = k == 3; mp.transposed = 1;
+        mp.a = sign[k] * P->morph_alpha;
+        int rc = launch_morph_one(P, mp, st, "morphT");
+        if (rc) return rc;
+        float *t = src; src = dst; dst = t;
+    }
+    return EPSGRAD_OK;
+}
+
+// F1 and, when they are on, the first projection and the morphological filters
+int launch_front(epsgrad_plan *P, const float *C, float beta, cudaStream_t st)
+{
+    int rc = launch_filter(P, C, ws_phi(P), st);
+    if (!rc && P->morph_R > 0) rc = launch_morph_forward(P, ws_phi(P), beta, st);
+    return rc;
+}
+
 // ---- R2..R5
 int launch_maskgrad(epsgrad_plan *P, const float *phi, float beta, const float *gbar, const float *coef, float *v, cudaStream_t st)
 {
@@ -735,6 +857,8 @@ int launch_maskgrad(epsgrad_plan *P, const float *phi, float beta, const float *
     mp.phi = phi; mp.gbar = gbar; mp.coef = coef; mp.v = v; mp.nrm = make_nrm(P);
     mp.nx = P->nx; mp.ny = P->ny; mp.px = P->px; mp.py = P->py; mp.s = P->cfg.subpixel;
     mp.beta = beta; mp.eta_r = P->eta_r; mp.eps_clad = P->eps_clad; mp.deps = P->deps;
+    mp.use_den = 1;
+    if (P->morph_R > 0) { mp.phi = ws_mc(P); mp.eta_r = 0.0f; mp.use_den = 0; }   // v holds the cotangent of rho~: the filters^T follow
     const size_t smem = maskgrad_smem_floats(mp.s) * 4;
     auto kern = mp.s == 2 ? k_maskgrad<2> : (mp.s == 4 ? k_maskgrad<4> : k_maskgrad<0>);
     int rc = set_smem(kern, smem);
@@ -780,11 +904,12 @@ int run_chain(epsgrad_plan *P, const float *C, float beta, int n_pairs, const vo
 {
     int rc = EPSGRAD_OK;
     if (!dFdC || !P->overlap || P->prof) {
-        rc = launch_filter(P, C, ws_phi(P), st);
+        rc = launch_front(P, C, beta, st);
         if (!rc) rc = launch_fwd2d(P, ws_phi(P), beta, eps ? ws_e2d(P) : nullptr, dFdC ? ws_coef(P) : nullptr, nullptr, st);
         if (!rc && dFdC) rc = launch_zreduce(P, n_pairs, EF, EA, ws_gbar(P), st);
         if (!rc && eps) rc = launch_extrude(P, ws_e2d(P), eps, st);
         if (!rc && dFdC) rc = launch_maskgrad(P, ws_phi(P), beta, ws_gbar(P), ws_coef(P), ws_v(P), st);
+        if (!rc && dFdC && P->morph_R > 0) rc = launch_morph_reverse(P, ws_phi(P), beta, ws_v(P), st);
         if (!rc && dFdC) rc = launch_filterT(P, ws_v(P), dFdC, st);
         return rc;
     }
@@ -794,7 +919,7 @@ int run_chain(epsgrad_plan *P, const float *C, float beta, int n_pairs, const vo
         cudaGetLastError();
         return EPSGRAD_ECUDA;
     }
-    rc = launch_filter(P, C, ws_phi(P), ax);
+    rc = launch_front(P, C, beta, ax);
     if (!rc) rc = launch_zreduce(P, n_pairs, EF, EA, ws_gbar(P), st);
     if (!rc && cudaEventRecord(P->ev_r, st) != cudaSuccess) rc = EPSGRAD_ECUDA;
     if (!rc) rc = launch_fwd2d(P, ws_phi(P), beta, eps ? ws_e2d(P) : nullptr, ws_coef(P), nullptr, ax);
@@ -805,6 +930,7 @@ int run_chain(epsgrad_plan *P, const float *C, float beta, int n_pairs, const vo
         if (cudaStreamWaitEvent(st, P->ev_2d, 0) != cudaSuccess) rc = EPSGRAD_ECUDA;
         if (!rc) rc = launch_extrude(P, ws_e2d(P), eps, st);
     }
+    if (!rc && P->morph_R > 0) rc = launch_morph_reverse(P, ws_phi(P), beta, ws_v(P), ax);
     if (!rc) rc = launch_filterT(P, ws_v(P), dFdC, ax);
     // always join, even on error, so that the auxiliary stream never outlives the call
     if (cudaEventRecord(P->ev_join, ax) != cudaSuccess || cudaStreamWaitEvent(st, P->ev_join, 0) != cudaSuccess) {
@@ -914,7 +1040,7 @@ extern "C" int eps_forward_vjp_host(epsgrad_plan_t *P, const float *C_host, floa
         // The bus is full duplex: eps does not depend on the fields, so it is finished first and travels to the host on the
         // auxiliary stream while the z-reduction pulls its windows the other way.
         cudaStream_t ax = P->aux;
-        int rc = launch_filter(P, dC, ws_phi(P), st);
+        int rc = launch_front(P, dC, beta, st);
         if (!rc) rc = launch_fwd2d(P, ws_phi(P), beta, ws_e2d(P), ws_coef(P), nullptr, st);
         if (!rc) rc = launch_extrude(P, ws_e2d(P), dE, st);
         if (rc) return rc;
@@ -925,6 +1051,7 @@ extern "C" int eps_forward_vjp_host(epsgrad_plan_t *P, const float *C_host, floa
         if (ok) {
             rc = launch_zreduce(P, n_pairs, ef.data(), ea.data(), ws_gbar(P), st, true);
             if (!rc) rc = launch_maskgrad(P, ws_phi(P), beta, ws_gbar(P), ws_coef(P), ws_v(P), st);
+            if (!rc && P->morph_R > 0) rc = launch_morph_reverse(P, ws_phi(P), beta, ws_v(P), st);
             if (!rc) rc = launch_filterT(P, ws_v(P), dG, st);
             if (!rc) ok = cudaMemcpyAsync(dFdC_host, dG, b_c, cudaMemcpyDeviceToHost, st) == cudaSuccess;
             P->last_d2h += b_c;
@@ -969,7 +1096,7 @@ extern "C" int epsgrad_stage_eps2d(epsgrad_plan_t *P, const float *C, float beta
     DeviceGuard g(P->device);
     cudaStream_t st = (cudaStream_t)stream;
     begin_call(P, st);
-    rc = launch_filter(P, C, ws_phi(P), st);
+    rc = launch_front(P, C, beta, st);
     if (!rc) rc = launch_fwd2d(P, ws_phi(P), beta, nullptr, nullptr, eps2d, st);
     return rc;
 }

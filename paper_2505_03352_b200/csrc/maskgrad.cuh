@@ -17,12 +17,13 @@
 namespace epsgrad {
 
 struct MaskGradParams {
-    const float *phi;      // [B,px,py]
+    const float *phi;      // [B,px,py] centred input of the last projection: Phi' or, with morphological filters, rho~ - 1/2
     const float *gbar;     // [B,5,nx,ny]  z-reduced cotangent: x, y, z-full, z-lower-face, z-upper-face
     const float *coef;     // [B,10,nx,ny] [hbk, abk, gxk, gyk] for c = x, for c = y, flo, fhi
     float *v;              // [B,px,py]
     Normaliser nrm;
     int nx, ny, px, py, s;
+    int use_den;           // 1: v carries 1/den of Eq. (2); 0: the morphological filters^T follow and the last one applies it
     float beta, eta_r, eps_clad, deps;
 };
 
@@ -176,7 +177,7 @@ __global__ void __launch_bounds__(MG_THREADS) k_maskgrad(const __grid_constant__
                 const float d = fast_rcp(1.0f + e2);
                 const float r = fast_rcp(fmaf(P.deps, t >= 0.f ? d : e2 * d, P.eps_clad));   // 1/e
                 const float ebar = az + ex[a] + ey[c], rbar = hx[a] + hy[c];
-                o[c] = k0 * e2 * d * d * (ebar - rbar * r * r) * P.nrm.at_index(np, c == 0 ? nq0 : nq1);
+                o[c] = k0 * e2 * d * d * (ebar - rbar * r * r) * (P.use_den ? P.nrm.at_index(np, c == 0 ? nq0 : nq1) : 1.0f);
             }
             *reinterpret_cast<float2 *>(vb + (p + a) * P.py + q) = make_float2(o[0], o[1]);
         }
@@ -219,7 +220,7 @@ __global__ void __launch_bounds__(MG_THREADS) k_maskgrad(const __grid_constant__
             const float r = fast_rcp(fmaf(P.deps, rho, P.eps_clad));   // 1/e
             const float slope = 2.0f * P.beta * a * d * d;
             const float rhobar = P.deps * inv_s2 * (ebar - rbar * r * r);
-            vb[p * P.py + q] = rhobar * slope * P.nrm.at_index(nidx[tp], nidx[TP + tq]);
+            vb[p * P.py + q] = rhobar * slope * (P.use_den ? P.nrm.at_index(nidx[tp], nidx[TP + tq]) : 1.0f);
         }
     }
 }

@@ -1,0 +1,126 @@
+// morph.cuh -- morphological filters of the design mask, Eqs. (4)-(5), forward and transposed.
+//   dilate  y = (1/alpha) log sum K_m exp(alpha x)              erode  y = 1 - (1/alpha) log sum K_m exp(alpha (1 - x))
+// K_m = 1 inside a circle of diameter d, normalised to unit sum over the pixels inside the region (G5, S18), finite
+// sums on the mask grid as in Eq. (8).  With a signed alpha both are ONE formula,
+//   y_i = (1/a) log( (1/N_i) sum_{j in disk(i)} exp(a x_j) ),      a = +alpha: dilate,  a = -alpha: erode,
+// and so is the transpose (the disk is symmetric, N cancels out of d y_i / d x_j = exp(a x_j) / S_i):
+//   xbar_j = sum_{i in disk(j)} ybar_i exp(a (x_j - y_i)) / N_i    (exponent bounded by log N: no overflow).
+// Both directions are the same skeleton -- stage f(pixel) for a tile plus a halo of R pixels (0 outside the region), sum it
+// over the disk, finish per pixel -- so one kernel serves the four forward and the four transposed operations of the chain
+// "dilate, erode, erode, dilate" (S17), with the neighbouring pointwise steps folded in at the chain ends:
+//   first forward op  stages exp(a rho0) with rho0 = projection (Eq. (3)/(6) form, S9) of the filter output, and keeps rho0;
+//   last forward op   writes y - 1/2, the centred input of the second projection, Eq. (6);
+//   last transposed op multiplies by the slope of the first projection and by 1/den (S2): the mask cotangent v of filterT.
+// A thread owns four neighbouring pixels of a row: every staged value it loads feeds up to four disk sums (plain adds: no
+// sliding-window subtraction, the staged values span e^-20..e^20).  Bound: shared-memory reads and FADD issue; L2-resident.
+#pragma once
+#include "common.cuh"
+
+namespace epsgrad {
+
+constexpr int MO_T = 32, MO_THREADS = 256, MO_MAX_R = 16;
+
+struct MorphParams {
+    const float *x;        // [B,px,py] input of the forward op (first op: centred filter output Phi')
+    const float *y;        // transposed op: output of the forward op (last op of the chain: centred, y - 1/2)
+    const float *ybar;     // transposed op: cotangent of y
+    float *out;            // forward: y (last op: y - 1/2); transposed: xbar (first op of the chain: v)
+    float *rho0;           // first forward op: keeps rho0 = projection(Phi') for the transposed pass
+    const int *hl;         // [2R+1] half-lengths of the disk rows
+    const float *invn;     // [(2R+1)^2] 1/N by border class (rows, columns)
+    Normaliser nrm;        // first op of the chain, transposed: 1/den of Eq. (2)
+    int px, py, R;
+    int transposed, first, last;
+    float a;               // signed alpha
+    float beta, eta_r;     // first projection (first op only)
+};
+
+__host__ __device__ inline size_t morph_smem_floats(int R) { return (size_t)(MO_T + 2 * R) * (MO_T + 2 * R + 1) + 2 * R + 1; }
+
+// border class of pixel p along an axis of n pixels (n >= 2R+1): distance to the nearer edge, capped at R
+__device__ __forceinline__ int morph_class(int p, int n, int R)
+{
+    if (p < R) return p;
+    const int d = n - 1 - p;
+    return d < R ? 2 * R - d : R;
+}
+
+// grid (ceil(py/32), ceil(px/32), B)
+__global__ void __launch_bounds__(MO_THREADS) k_morph(const __grid_constant__ MorphParams P)
+{
+    extern __shared__ __align__(16) float sm[];
+    const int R = P.R, W = MO_T + 2 * R, pitch = W + 1;
+    float *f_s = sm;                                       // [W][pitch]
+    int *hl_s = reinterpret_cast<int *>(f_s + W * pitch);  // [2R+1]
+    const int tid = threadIdx.x, b = blockIdx.z;
+    const int p0 = blockIdx.y * MO_T, q0 = blockIdx.x * MO_T;
+    const size_t plane = (size_t)b * P.px * P.py;
+    const float a = P.a;
+    const int NI = 2 * R + 1;
+
+    for (int k = tid; k < NI; k += MO_THREADS) hl_s[k] = P.hl[k];
+    // ---- stage f over the tile + halo
+    for (int it = tid; it < W * W; it += MO_THREADS) {
+        const int lp = it / W, lq = it - lp * W;
+        const int p = p0 - R + lp, q = q0 - R + lq;
+        float f = 0.0f;
+        if (p >= 0 && p < P.px && q >= 0 && q < P.py) {
+            const size_t idx = plane + (size_t)p * P.py + q;
+            if (!P.transposed) {
+                float xv = P.x[idx];
+                if (P.first) {
+                    // rho0 = 1/2 (1 + tanh(beta (Phi - eta))) = 1/(1 + exp(-2t))
+                    const float t = P.beta * (xv - P.eta_r);
+                    xv = fast_rcp(1.0f + __expf(-2.0f * t));
+                    if (lp >= R && lp < R + MO_T && lq >= R && lq < R + MO_T) P.rho0[idx] = xv;
+                }
+                f = __expf(a * xv);
+            } else {
+                const float yv = P.y[idx] + (P.last ? 0.5f : 0.0f);
+                f = P.ybar[idx] * __expf(-a * yv) *
+                    P.invn[morph_class(p, P.px, R) * NI + morph_class(q, P.py, R)];
+            }
+        }
+        f_s[lp * pitch + lq] = f;
+    }
+    __syncthreads();
+
+    // ---- disk sums: thread -> row r, columns 4 c4 .. 4 c4 + 3
+    const int r = tid >> 3, c4 = (tid & 7) << 2;
+    float acc[4] = {0.f, 0.f, 0.f, 0.f};
+    for (int dp = -R; dp <= R; ++dp) {
+        const int h = hl_s[dp + R];
+        const float *row = f_s + (r + R + dp) * pitch + c4 + R - h;     // first element of the run of pixel c4
+        const int n = 2 * h + 1;
+        for (int k = 0; k < n + 3; ++k) {
+            const float v = row[k];
+            if (k < n) acc[0] += v;
+            if (k >= 1 && k < n + 1) acc[1] += v;
+            if (k >= 2 && k < n + 2) acc[2] += v;
+            if (k >= 3) acc[3] += v;
+        }
+    }
+    // ---- finish per pixel
+    const int p = p0 + r;
+    if (p >= P.px) return;
+    const float inv_a = 1.0f / a;
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const int q = q0 + c4 + u;
+        if (q >= P.py) continue;
+        const size_t idx = plane + (size_t)p * P.py + q;
+        if (!P.transposed) {
+            const float invn = P.invn[morph_class(p, P.px, R) * NI + morph_class(q, P.py, R)];
+            const float y = __logf(acc[u] * invn) * inv_a;
+            P.out[idx] = P.last ? y - 0.5f : y;
+        } else {
+            const float xv = P.first ? P.rho0[idx] : P.x[idx];
+            float o = acc[u] * __expf(a * xv);
+            // first op of the chain: projection^T in the overflow-free analytic form, then 1/den (S2)
+            if (P.first) o *= project_slope(P.x[idx], P.beta, P.eta_r) * P.nrm.at(p, q);
+            P.out[idx] = o;
+        }
+    }
+}
+
+}  // namespace epsgrad

@@ -19,7 +19,8 @@ def oracle_cfg(cfg: B.Config) -> O.OracleConfig:
     return O.OracleConfig(mx=cfg.mx, my=cfg.my, nx=cfg.nx, ny=cfg.ny, nz=cfg.nz, z_lo=cfg.z_lo, z_hi=cfg.z_hi,
                           s=cfg.subpixel, filter_kind=cfg.filter_kind, radius=cfg.filter_radius,
                           sigma=cfg.filter_sigma, normalize=cfg.filter_normalize, eta=cfg.eta,
-                          eps_core=cfg.eps_core, eps_clad=cfg.eps_clad, delta=cfg.normal_delta)
+                          eps_core=cfg.eps_core, eps_clad=cfg.eps_clad, delta=cfg.normal_delta,
+                          morph_diam=cfg.morph_diameter, morph_alpha=cfg.morph_alpha)
 
 
 def rand_C(cfg: B.Config, seed: int) -> np.ndarray:

@@ -40,7 +40,7 @@ def test_status_strings():
 
 def test_config_struct_layout_matches_header():
     # 8 int32 then 8 doubles, no padding
-    assert ctypes.sizeof(B.Config) == 8 * 4 + 8 * 8
+    assert ctypes.sizeof(B.Config) == 8 * 4 + 10 * 8
     assert B.Config.z_lo.offset == 32 and B.Config.normal_delta.offset == 32 + 7 * 8
 
 
