@@ -115,7 +115,8 @@ def oracle_cfg(w, mx=None, my=None):
     mx, my = mx or w.mx, my or w.my
     return O.OracleConfig(mx=mx, my=my, nx=w.upsample * mx, ny=w.upsample * my, nz=w.nz, z_lo=w.z_lo, z_hi=w.z_hi,
                           s=w.subpixel, filter_kind=w.filter_kind, radius=w.radius, sigma=w.sigma or 1.0, eta=w.eta,
-                          eps_core=w.eps_core, eps_clad=w.eps_clad, delta=w.normal_delta)
+                          eps_core=w.eps_core, eps_clad=w.eps_clad, delta=w.normal_delta,
+                          morph_diam=w.morph_diameter, morph_alpha=w.morph_alpha)
 
 
 def oracle_step_inputs(w, mx, my):
@@ -174,7 +175,8 @@ def base_line(w, args, n_gpus):
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "data": "synthetic",
         "config": {"workload": f"{w.name}: C {w.batch}x{w.mx}x{w.my} -> Yee {w.nx}x{w.ny}x{w.nz}, "
                                f"{'conic' if w.filter_kind == 0 else 'gaussian'} R={w.radius:g}, beta={list(w.betas)}, "
-                               f"{w.n_pairs} field pair(s), slab [{w.z_lo},{w.z_hi}]",
+                               f"{w.n_pairs} field pair(s), slab [{w.z_lo},{w.z_hi}]"
+                               + (f", morphological filters d={w.morph_diameter:g} cells alpha={w.morph_alpha:g}" if w.morph_diameter > 0 else ""),
                    "per_gpu": "one such design batch per GPU (independent designs, no collective)",
                    "launch": "CUDA graph replay of eps_forward_vjp (captured through the C ABI)" if getattr(args, "graph", True)
                              else "eager eps_forward_vjp calls",

@@ -11,8 +11,8 @@
 //   first forward op  stages exp(a rho0) with rho0 = projection (Eq. (3)/(6) form, S9) of the filter output, and keeps rho0;
 //   last forward op   writes y - 1/2, the centred input of the second projection, Eq. (6);
 //   last transposed op multiplies by the slope of the first projection and by 1/den (S2): the mask cotangent v of filterT.
-// A thread owns four neighbouring pixels of a row: every staged value it loads feeds up to four disk sums (plain adds: no
-// sliding-window subtraction, the staged values span e^-20..e^20).  Bound: shared-memory reads and FADD issue; L2-resident.
+// A thread owns four neighbouring pixels of a row: the part of a disk row that their four windows share is summed once
+// (plain adds: no sliding-window subtraction, the staged values span e^-20..e^20).  Bound: shared-memory reads and FADD issue; L2-resident.
 #pragma once
 #include "common.cuh"
 
@@ -59,29 +59,34 @@ __global__ void __launch_bounds__(MO_THREADS) k_morph(const __grid_constant__ Mo
     const int NI = 2 * R + 1;
 
     for (int k = tid; k < NI; k += MO_THREADS) hl_s[k] = P.hl[k];
-    // ---- stage f over the tile + halo
-    for (int it = tid; it < W * W; it += MO_THREADS) {
-        const int lp = it / W, lq = it - lp * W;
-        const int p = p0 - R + lp, q = q0 - R + lq;
-        float f = 0.0f;
-        if (p >= 0 && p < P.px && q >= 0 && q < P.py) {
-            const size_t idx = plane + (size_t)p * P.py + q;
-            if (!P.transposed) {
-                float xv = P.x[idx];
-                if (P.first) {
-                    // rho0 = 1/2 (1 + tanh(beta (Phi - eta))) = 1/(1 + exp(-2t))
-                    const float t = P.beta * (xv - P.eta_r);
-                    xv = fast_rcp(1.0f + __expf(-2.0f * t));
-                    if (lp >= R && lp < R + MO_T && lq >= R && lq < R + MO_T) P.rho0[idx] = xv;
+    // ---- stage f over the tile + halo (flat index, advanced without divisions)
+    {
+        int lp = tid / W, lq = tid - lp * W;
+        const int dlp = MO_THREADS / W, dlq = MO_THREADS - dlp * W;
+        for (int it = tid; it < W * W; it += MO_THREADS) {
+            const int p = p0 - R + lp, q = q0 - R + lq;
+            float f = 0.0f;
+            if (p >= 0 && p < P.px && q >= 0 && q < P.py) {
+                const size_t idx = plane + (size_t)p * P.py + q;
+                if (!P.transposed) {
+                    float xv = P.x[idx];
+                    if (P.first) {
+                        // rho0 = 1/2 (1 + tanh(beta (Phi - eta))) = 1/(1 + exp(-2t))
+                        const float t = P.beta * (xv - P.eta_r);
+                        xv = fast_rcp(1.0f + __expf(-2.0f * t));
+                        if (lp >= R && lp < R + MO_T && lq >= R && lq < R + MO_T) P.rho0[idx] = xv;
+                    }
+                    f = __expf(a * xv);
+                } else {
+                    const float yv = P.y[idx] + (P.last ? 0.5f : 0.0f);
+                    f = P.ybar[idx] * __expf(-a * yv) *
+                        P.invn[morph_class(p, P.px, R) * NI + morph_class(q, P.py, R)];
                 }
-                f = __expf(a * xv);
-            } else {
-                const float yv = P.y[idx] + (P.last ? 0.5f : 0.0f);
-                f = P.ybar[idx] * __expf(-a * yv) *
-                    P.invn[morph_class(p, P.px, R) * NI + morph_class(q, P.py, R)];
             }
+            f_s[lp * pitch + lq] = f;
+            lp += dlp; lq += dlq;
+            if (lq >= W) { lq -= W; ++lp; }
         }
-        f_s[lp * pitch + lq] = f;
     }
     __syncthreads();
 
@@ -92,12 +97,19 @@ __global__ void __launch_bounds__(MO_THREADS) k_morph(const __grid_constant__ Mo
         const int h = hl_s[dp + R];
         const float *row = f_s + (r + R + dp) * pitch + c4 + R - h;     // first element of the run of pixel c4
         const int n = 2 * h + 1;
-        for (int k = 0; k < n + 3; ++k) {
-            const float v = row[k];
-            if (k < n) acc[0] += v;
-            if (k >= 1 && k < n + 1) acc[1] += v;
-            if (k >= 2 && k < n + 2) acc[2] += v;
-            if (k >= 3) acc[3] += v;
+        if (n >= 4) {
+            // the four windows [u, u+n) share the elements 3 .. n-1: sum them once, then add each window's own three
+            float c = 0.f;
+            for (int k = 3; k < n; ++k) c += row[k];
+            const float v0 = row[0], v1 = row[1], v2 = row[2], w0 = row[n], w1 = row[n + 1], w2 = row[n + 2];
+            acc[0] += c + ((v0 + v1) + v2);
+            acc[1] += c + ((v1 + v2) + w0);
+            acc[2] += c + ((v2 + w0) + w1);
+            acc[3] += c + ((w0 + w1) + w2);
+        } else {
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                for (int k = 0; k < n; ++k) acc[u] += row[u + k];
         }
     }
     // ---- finish per pixel

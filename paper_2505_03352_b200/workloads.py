@@ -35,6 +35,8 @@ class Workload:
     eps_core: float = 12.11     # Si
     eps_clad: float = 2.085     # SiO2
     normal_delta: float = 1e-12
+    morph_diameter: float = 0.0 # d of Eqs. (4)-(5) in Yee cells; 0 = morphological filters off (as in Fig. 4)
+    morph_alpha: float = 20.0   # App. B
 
     @property
     def nx(self) -> int:
@@ -60,7 +62,12 @@ CONFIGS = (
     Workload("large", 3, 1, 1000, 1000, 64, 28.25, 35.75, 0, 12.0, 0.0, (32.0,), 1, "blurred"),
     Workload("widebatch", 4, 8, 1024, 1024, 32, 14.25, 17.75, 1, 32.0, 10.0, (8.0,), 1, "uniform"),
 )
-BY_NAME = {w.name: w for w in CONFIGS}
+# Not a BASELINE.json config: the paper-scale workload with the morphological filters on (minimum feature size d = 4 cells
+# = 100 nm at the 25 nm cells of Fig. 4, alpha = 20 of App. B), for `bench.py --config paper_morph`.
+EXTRA = (
+    Workload("paper_morph", 1, 1, 250, 250, 64, 28.25, 35.75, 0, 8.0, 0.0, (16.0,), 1, "uniform", morph_diameter=4.0),
+)
+BY_NAME = {w.name: w for w in CONFIGS + EXTRA}
 
 
 def make_C(w: Workload) -> np.ndarray:

@@ -16,7 +16,8 @@ import oracle as O
 def cfg_of(w, **over) -> O.OracleConfig:
     kw = dict(mx=w.mx, my=w.my, nx=w.nx, ny=w.ny, nz=w.nz, z_lo=w.z_lo, z_hi=w.z_hi, s=w.subpixel,
               filter_kind=w.filter_kind, radius=w.radius, sigma=w.sigma, eta=w.eta,
-              eps_core=w.eps_core, eps_clad=w.eps_clad, delta=w.normal_delta)
+              eps_core=w.eps_core, eps_clad=w.eps_clad, delta=w.normal_delta,
+              morph_diam=getattr(w, "morph_diameter", 0.0), morph_alpha=getattr(w, "morph_alpha", 20.0))
     kw.update(over)
     return O.OracleConfig(**kw)
 
