@@ -112,7 +112,7 @@ template <int M>
 __global__ void __launch_bounds__(FilterTShape<M>::NTHR) k_filterT_conic(const FilterTParams P)
 {
     using S = FilterTShape<M>;
-    constexpr int TA = S::TA, TB = S::TB, SP = S::SP, ROWS = S::ROWS, nthr = S::NTHR;
+    constexpr int TA = S::TA, TB = S::TB, ROWS = S::ROWS, nthr = S::NTHR;
     extern __shared__ __align__(16) float sm[];
     const int T = P.T, NT = P.NT;
     const int VH = M * (TA + 2 * T), VW = M * (TB + 2 * T);   // v tile
