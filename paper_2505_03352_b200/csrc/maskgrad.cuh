@@ -145,7 +145,7 @@ __global__ void __launch_bounds__(MG_THREADS) k_maskgrad(const __grid_constant__
     const int TP = s * TI, TQ = s * TJ;
     const float *phib = P.phi + (size_t)b * P.px * P.py;
     float *vb = P.v + (size_t)b * P.px * P.py;
-    if (S == 2) {
+    if constexpr (S == 2) {
         // s = 2: a thread per cell owns its 2 x 2 pixels.  Rows p = 2i, 2i+1 have E_x owners i-1 and i, columns q = 2j, 2j+1
         // have E_y owners j-1 and j: nine shared-memory values serve the four pixels; 8-byte loads and stores.
         static_assert(TI * TJ == NTH, "one thread per cell");
@@ -181,8 +181,7 @@ __global__ void __launch_bounds__(MG_THREADS) k_maskgrad(const __grid_constant__
             }
             *reinterpret_cast<float2 *>(vb + (p + a) * P.py + q) = make_float2(o[0], o[1]);
         }
-        return;
-    }
+    } else {
     for (int base = tid; base < TP * TQ; base += 4 * NTH) {
         float ph[4];                                           // filter output of four pixels in flight
 #pragma unroll
@@ -222,6 +221,7 @@ __global__ void __launch_bounds__(MG_THREADS) k_maskgrad(const __grid_constant__
             const float rhobar = P.deps * inv_s2 * (ebar - rbar * r * r);
             vb[p * P.py + q] = rhobar * slope * (P.use_den ? P.nrm.at_index(nidx[tp], nidx[TP + tq]) : 1.0f);
         }
+    }
     }
 }
 
