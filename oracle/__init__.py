@@ -306,6 +306,55 @@ def vjp_real(cfg: OracleConfig, C, beta: float, epsbar):
     return out
 
 
+def vjp_real_beta(cfg: OracleConfig, C, beta: float, epsbar):
+    """((d eps/dC)^T epsbar [mx,my], epsbar . d eps/d beta) for a real cotangent."""
+    c = cfg.c()
+    C = _c32(C, cfg)
+    epsbar = _f64(epsbar, (3, cfg.nx, cfg.ny, cfg.nz))
+    out = np.empty((cfg.mx, cfg.my))
+    db = ctypes.c_double(0.0)
+    lib().orc_vjp_real_beta(ctypes.byref(c), _p(C), ctypes.c_double(beta), _p(epsbar), _p(out), ctypes.byref(db))
+    return out, float(db.value)
+
+
+def unbinarity(cfg: OracleConfig, C, beta: float) -> float:
+    """u(beta): mean of 4 rho (1 - rho) over the projected design mask (S20)."""
+    c = cfg.c()
+    lib().orc_unbinarity.restype = ctypes.c_double
+    return float(lib().orc_unbinarity(ctypes.byref(c), _p(_c32(C, cfg)), ctypes.c_double(beta)))
+
+
+def beta_schedule(beta_min: float, beta_max: float, i: int, n_iter: int) -> float:
+    """Eq. (14)."""
+    lib().orc_beta_schedule.restype = ctypes.c_double
+    return float(lib().orc_beta_schedule(ctypes.c_double(beta_min), ctypes.c_double(beta_max), ctypes.c_int(i), ctypes.c_int(n_iter)))
+
+
+def beta_update(t: float, beta_max: float, gamma: float, u: float, u0: float, beta: float):
+    """Eq. (15): returns the new (t, beta_max)."""
+    ct, cb = ctypes.c_double(t), ctypes.c_double(beta_max)
+    lib().orc_beta_update(ctypes.byref(ct), ctypes.byref(cb), ctypes.c_double(gamma), ctypes.c_double(u),
+                          ctypes.c_double(u0), ctypes.c_double(beta))
+    return float(ct.value), float(cb.value)
+
+
+def vjp_beta(cfg: OracleConfig, C, beta: float, EF: list, EA: list):
+    """Eq. (1) gradient and d F/d beta from field pairs (complex64 [3,nx,ny,nz])."""
+    c = cfg.c()
+    C = _c32(C, cfg)
+    n = len(EF)
+    assert n == len(EA) and n >= 1
+    keep = [[np.ascontiguousarray(a, dtype=np.complex64) for a in lst] for lst in (EF, EA)]
+    for a in keep[0] + keep[1]:
+        assert a.shape == (3, cfg.nx, cfg.ny, cfg.nz)
+    pf = (ctypes.c_void_p * n)(*[a.ctypes.data for a in keep[0]])
+    pa = (ctypes.c_void_p * n)(*[a.ctypes.data for a in keep[1]])
+    out = np.empty((cfg.mx, cfg.my))
+    db = ctypes.c_double(0.0)
+    lib().orc_vjp_beta(ctypes.byref(c), _p(C), ctypes.c_double(beta), ctypes.c_int(n), pf, pa, _p(out), ctypes.byref(db))
+    return out, float(db.value)
+
+
 def vjp(cfg: OracleConfig, C, beta: float, EF: list, EA: list):
     """Eq. (1): -2 Re((d eps/dC)^T (E_F . E_A)) summed over the pairs; fields complex64 [3,nx,ny,nz]."""
     c = cfg.c()

@@ -159,6 +159,18 @@ void orc_project_T(int64_t n, const double *Phi, double beta, double eta,
     }
 }
 
+/* eps_hat is differentiable in beta too: d rho / d beta = (Phi - eta)/2 / cosh^2(beta (Phi - eta));
+ * returns sum_i rhobar_i d rho_i / d beta. */
+double orc_project_dbeta(int64_t n, const double *Phi, double beta, double eta, const double *rhobar)
+{
+    double acc = 0.0;
+    for (int64_t i = 0; i < n; ++i) {
+        double c = cosh(beta * (Phi[i] - eta));
+        acc += rhobar[i] * 0.5 * (Phi[i] - eta) / (c * c);
+    }
+    return acc;
+}
+
 /* ------------------------------------------------------------------ */
 /* Step 3b. Mixing rule: e = rho eps_core + (1-rho) eps_clad;  */
 /* r = 1/e is the integrand of <eps^-1> in Eq. (7).                    */
@@ -539,7 +551,7 @@ int orc_forward_stages(const orc_cfg *g, const float *C32, double beta,
 /* the transpose of its forward loop.                                  */
 /* ------------------------------------------------------------------ */
 static void reverse_2d(const orc_cfg *g, double beta, const orc_work *w,
-                       const double *eps2dbar, double *dFdC)
+                       const double *eps2dbar, double *dFdC, double *dFdbeta)
 {
     const size_t nm = (size_t)g->s * g->nx * g->s * g->ny, nc = (size_t)g->nx * g->ny;
     double *ebar = calloc(nm, 8), *rbar = calloc(nm, 8), *rhobar = calloc(nm, 8);
@@ -558,30 +570,41 @@ static void reverse_2d(const orc_cfg *g, double beta, const orc_work *w,
     if (g->morph_diam > 0.0) {
         static const int is_erode[4] = {0, 1, 1, 0};
         double *cur = malloc(8 * nm), *nxt = malloc(8 * nm);
+        if (dFdbeta) *dFdbeta = orc_project_dbeta((int64_t)nm, w->mx[4], beta, 0.5, rhobar);
         orc_project_T((int64_t)nm, w->mx[4], beta, 0.5, rhobar, cur);
         for (int k = 3; k >= 0; --k) {
             memset(nxt, 0, 8 * nm);
             orc_morph_T(g, w->mx[k], is_erode[k], cur, nxt);
             double *t = cur; cur = nxt; nxt = t;
         }
+        if (dFdbeta) *dFdbeta += orc_project_dbeta((int64_t)nm, w->Phi, beta, g->eta, cur);   /* both projections use beta (S17) */
         orc_project_T((int64_t)nm, w->Phi, beta, g->eta, cur, Phibar);
         free(cur); free(nxt);
-    } else
+    } else {
+        if (dFdbeta) *dFdbeta = orc_project_dbeta((int64_t)nm, w->Phi, beta, g->eta, rhobar);
         orc_project_T((int64_t)nm, w->Phi, beta, g->eta, rhobar, Phibar);
+    }
     orc_filter_T(g, Phibar, dFdC);                                  /* step 2^T */
     free(ebar); free(rbar); free(rhobar); free(Abar); free(Hbar); free(Dbar);
     free(gxbar); free(gybar); free(Phibar);
 }
 
 /* VJP with an arbitrary real cotangent epsbar [3,nx,ny,nz]. */
+int orc_vjp_real_beta(const orc_cfg *g, const float *C32, double beta, const double *epsbar, double *dFdC, double *dFdbeta);
 int orc_vjp_real(const orc_cfg *g, const float *C32, double beta, const double *epsbar, double *dFdC)
+{
+    return orc_vjp_real_beta(g, C32, beta, epsbar, dFdC, NULL);
+}
+
+/* the same with d F / d beta = epsbar . d eps_hat / d beta; dFdbeta may be NULL */
+int orc_vjp_real_beta(const orc_cfg *g, const float *C32, double beta, const double *epsbar, double *dFdC, double *dFdbeta)
 {
     orc_work w;
     work_alloc(g, &w);
     forward_2d(g, C32, beta, &w);
     double *e2bar = malloc(8 * 3 * (size_t)g->nx * g->ny);
     orc_extrude_T(g, w.eps2d, epsbar, e2bar);                       /* step 7^T */
-    reverse_2d(g, beta, &w, e2bar, dFdC);
+    reverse_2d(g, beta, &w, e2bar, dFdC, dFdbeta);
     free(e2bar);
     work_free(&w);
     return 0;
@@ -593,8 +616,16 @@ int orc_vjp_real(const orc_cfg *g, const float *C32, double beta, const double *
  * conjugate (S10).  Fields are complex64 [3,nx,ny,nz], interleaved
  * (re,im) floats, converted to double.
  */
+int orc_vjp_beta(const orc_cfg *g, const float *C32, double beta, int n_pairs,
+                 const float *const *EF, const float *const *EA, double *dFdC, double *dFdbeta);
 int orc_vjp(const orc_cfg *g, const float *C32, double beta, int n_pairs,
             const float *const *EF, const float *const *EA, double *dFdC)
+{
+    return orc_vjp_beta(g, C32, beta, n_pairs, EF, EA, dFdC, NULL);
+}
+
+int orc_vjp_beta(const orc_cfg *g, const float *C32, double beta, int n_pairs,
+                 const float *const *EF, const float *const *EA, double *dFdC, double *dFdbeta)
 {
     const size_t n3 = 3 * (size_t)g->nx * g->ny * g->nz;
     double *G3 = calloc(n3, 8);
@@ -606,9 +637,41 @@ int orc_vjp(const orc_cfg *g, const float *C32, double beta, int n_pairs,
             G3[i] += -2.0 * (ar * br - ai * bi);
         }
     }
-    int rc = orc_vjp_real(g, C32, beta, G3, dFdC);
+    int rc = orc_vjp_real_beta(g, C32, beta, G3, dFdC, dFdbeta);
     free(G3);
     return rc;
+}
+
+/* ------------------------------------------------------------------ */
+/* "Unbinarity" u(beta), the relative number of gray pixels.  */
+/* Reading S20: the measure of non-discreteness, the mean over the     */
+/* design mask of 4 rho (1 - rho) (1 for rho = 1/2, 0 for a binary     */
+/* pixel), rho being the final projected mask.                          */
+/* ------------------------------------------------------------------ */
+double orc_unbinarity(const orc_cfg *g, const float *C32, double beta)
+{
+    const int64_t nm = (int64_t)g->s * g->nx * g->s * g->ny;
+    orc_work w;
+    work_alloc(g, &w);
+    forward_2d(g, C32, beta, &w);
+    double acc = 0.0;
+    for (int64_t i = 0; i < nm; ++i) acc += 4.0 * w.rho[i] * (1.0 - w.rho[i]);
+    work_free(&w);
+    return acc / (double)nm;
+}
+
+/* Eq. (14): beta_i = beta_min + (beta_max - beta_min) (exp((i/N)^2) - 1)/(e - 1) */
+double orc_beta_schedule(double beta_min, double beta_max, int i, int n_iter)
+{
+    const double x = (double)i / (double)n_iter;
+    return beta_min + (beta_max - beta_min) * (exp(x * x) - 1.0) / (exp(1.0) - 1.0);
+}
+
+/* Eq. (15): t <- gamma t + (1-gamma)(1/u - 1)/beta;  beta_max <- gamma beta_max + (1-gamma)(1/u0 - 1)/t */
+void orc_beta_update(double *t, double *beta_max, double gamma, double u, double u0, double beta)
+{
+    *t = gamma * *t + (1.0 - gamma) * (1.0 / u - 1.0) / beta;
+    *beta_max = gamma * *beta_max + (1.0 - gamma) * (1.0 / u0 - 1.0) / *t;
 }
 
 int orc_num_threads(void)

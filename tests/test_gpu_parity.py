@@ -100,6 +100,28 @@ def test_dense_reads_give_the_same_gradient():
     check_vjp(cfg, C, 16.0, EF, EA, plan=plan)
 
 
+def test_profiling_and_timeline_hooks_name_every_kernel():
+    cfg = B.make_config(mx=23, my=18, nz=16, z_lo=6.25, z_hi=9.75, filter_radius=4.0)
+    C = dev(rand_C(cfg, 4))
+    EFn, EAn = rand_fields(cfg, 1, 9)
+    EF, EA = [dev(f) for f in EFn], [dev(f) for f in EAn]
+    plan = B.Plan(cfg)
+    eps0, g0 = plan.eps_forward_vjp(C, 8.0, EF, EA)
+    plan.set_profiling(True)                                  # serial schedule, one event after each kernel
+    eps1, g1 = plan.eps_forward_vjp(C, 8.0, EF, EA)
+    times = plan.last_kernel_times()
+    plan.set_profiling(False)
+    assert [n for n, _ in times] == ["filter", "fwd2d", "zreduce", "extrude", "maskgrad", "filterT"]
+    assert all(ms > 0 for _, ms in times)
+    plan.set_timeline(True)                                   # device-clock stamps on both streams
+    eps2, g2 = plan.eps_forward_vjp(C, 8.0, EF, EA)
+    tl = plan.read_timeline()
+    plan.set_timeline(False)
+    assert sorted(n for n, _ in tl) == sorted(["begin", "filter", "fwd2d", "zreduce", "extrude", "maskgrad", "filterT"])
+    assert all(t >= 0 for _, t in tl)
+    assert torch.equal(eps0, eps1) and torch.equal(g0, g1) and torch.equal(eps0, eps2) and torch.equal(g0, g2)
+
+
 def test_forward_vjp_equals_separate_calls_and_keeps_inputs():
     cfg = B.make_config(mx=30, my=26, nz=16, z_lo=6.25, z_hi=9.75, filter_radius=4.0)
     C = dev(rand_C(cfg, 6))
