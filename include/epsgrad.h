@@ -147,6 +147,24 @@ int eps_forward(epsgrad_plan_t *plan, const float *C, float beta, float *eps, vo
 int eps_vjp(epsgrad_plan_t *plan, const float *C, float beta, int n_pairs,
             const void *const *EF, const void *const *EA, float *dFdC, void *stream);
 
+/* eps_vjp plus d F/d beta: eps_hat(C, beta) is differentiable with respect to the projection strength too;
+ * dFdbeta: DEVICE array of B floats, dFdbeta[b] = -2 Re( (d eps_hat_b/d beta)^T (E_F (.) E_A) ) summed over the pairs.  With the
+ * morphological filters on both projections contribute (S17).  Deterministic (two-stage sums, no atomics).               */
+int eps_vjp_beta(epsgrad_plan_t *plan, const float *C, float beta, int n_pairs,
+                 const void *const *EF, const void *const *EA, float *dFdC, float *dFdbeta, void *stream);
+
+/* "Unbinarity" u(beta), the relative number of gray pixels of the design, read as the measure of non-discreteness
+ * (S20): the mean over the design mask of 4 rho (1 - rho), rho the final projected mask; u: DEVICE array of B floats.   */
+int eps_unbinarity(epsgrad_plan_t *plan, const float *C, float beta, float *u, void *stream);
+
+/* The paper's update rule for the projection strength (host scalars).  Eq. (14), P:L150:
+ *   beta_i = beta_min + (beta_max - beta_min) (exp((i/N)^2) - 1)/(e - 1);
+ * Eq. (15), moving averages with decay gamma that steer beta_max so that u reaches u0 at the last iteration:
+ *   t <- gamma t + (1-gamma)(1/u - 1)/beta,   beta_max <- gamma beta_max + (1-gamma)(1/u0 - 1)/t.
+ * epsgrad_beta_update returns EPSGRAD_EINVAL (and changes nothing) for u, u0, beta <= 0, gamma outside [0,1] or t <= 0.   */
+double epsgrad_beta_schedule(double beta_min, double beta_max, int i, int n_iter);
+int    epsgrad_beta_update(double *t, double *beta_max, double gamma, double u, double u0, double beta);
+
 /* Both in one call; the filter output (Phi) is computed once and shared.                */
 int eps_forward_vjp(epsgrad_plan_t *plan, const float *C, float beta, int n_pairs,
                     const void *const *EF, const void *const *EA,

@@ -20,7 +20,8 @@ EXPORTS = (
     "epsgrad_plan_set_workspace", "epsgrad_staging_bytes", "epsgrad_plan_set_staging",
     "epsgrad_plan_set_dense_reads", "epsgrad_plan_last_launches", "epsgrad_plan_last_copy_bytes",
     "epsgrad_plan_set_profiling", "epsgrad_plan_last_kernel_times", "epsgrad_plan_set_overlap", "epsgrad_plan_set_host_direct", "epsgrad_plan_set_timeline", "epsgrad_plan_read_timeline", 
-    "eps_forward", "eps_vjp", "eps_forward_vjp", "eps_forward_vjp_host",
+    "eps_forward", "eps_vjp", "eps_forward_vjp", "eps_forward_vjp_host", "eps_vjp_beta", "eps_unbinarity",
+    "epsgrad_beta_schedule", "epsgrad_beta_update",
     "epsgrad_stage_filter", "epsgrad_stage_eps2d", "epsgrad_stage_zreduce",
     "epsgrad_status_string", "epsgrad_version",
 )
@@ -72,6 +73,18 @@ def config_of(w) -> Config:
 _lib = None
 
 
+def beta_schedule(beta_min: float, beta_max: float, i: int, n_iter: int) -> float:
+    """Eq. (14) (P:L150)."""
+    return float(lib().epsgrad_beta_schedule(beta_min, beta_max, i, n_iter))
+
+
+def beta_update(t: float, beta_max: float, gamma: float, u: float, u0: float, beta: float):
+    """Eq. (15): the new (t, beta_max)."""
+    ct, cb = ctypes.c_double(t), ctypes.c_double(beta_max)
+    _check(lib().epsgrad_beta_update(ctypes.byref(ct), ctypes.byref(cb), gamma, u, u0, beta), "epsgrad_beta_update")
+    return float(ct.value), float(cb.value)
+
+
 def lib() -> ctypes.CDLL:
     """Load (building if stale and nvcc is present) libepsgrad.so; raises if it cannot be had."""
     global _lib
@@ -101,6 +114,11 @@ def lib() -> ctypes.CDLL:
     L.epsgrad_plan_last_kernel_times.argtypes = [vp, i32, ctypes.POINTER(f32), ctypes.POINTER(ctypes.c_char_p)]
     L.eps_forward.argtypes = [vp, vp, f32, vp, vp]
     L.eps_vjp.argtypes = [vp, vp, f32, i32, vp, vp, vp, vp]
+    L.eps_vjp_beta.argtypes = [vp, vp, f32, i32, vp, vp, vp, vp, vp]
+    L.eps_unbinarity.argtypes = [vp, vp, f32, vp, vp]
+    L.epsgrad_beta_schedule.restype = ctypes.c_double
+    L.epsgrad_beta_schedule.argtypes = [ctypes.c_double, ctypes.c_double, i32, i32]
+    L.epsgrad_beta_update.argtypes = [vp, vp, ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_double]
     L.eps_forward_vjp.argtypes = [vp, vp, f32, i32, vp, vp, vp, vp, vp]
     L.eps_forward_vjp_host.argtypes = [vp, vp, f32, i32, vp, vp, vp, vp, vp]
     L.epsgrad_stage_filter.argtypes = [vp, vp, vp, vp]
@@ -245,6 +263,21 @@ class Plan:
         eps = self._out(out, self.eps_shape)
         _check(lib().eps_forward(self._h, self._c(C).data_ptr(), beta, eps.data_ptr(), self._stream()), "eps_forward")
         return eps
+
+    def eps_vjp_beta(self, C, beta: float, EF: Sequence, EA: Sequence, out=None):
+        """(dF/dC [B,Mx,My], dF/dbeta [B]) (P:L148)"""
+        pf, pa = self._fields(EF, EA)
+        g = self._out(out, self.ctrl_shape)
+        db = self._torch.empty(self.ctrl_shape[0], dtype=self._torch.float32, device=self.device)
+        _check(lib().eps_vjp_beta(self._h, self._c(C).data_ptr(), beta, len(EF), pf, pa, g.data_ptr(), db.data_ptr(),
+                                  self._stream()), "eps_vjp_beta")
+        return g, db
+
+    def unbinarity(self, C, beta: float):
+        """u(beta) [B]: mean over the design mask of 4 rho (1 - rho) (S20)"""
+        u = self._torch.empty(self.ctrl_shape[0], dtype=self._torch.float32, device=self.device)
+        _check(lib().eps_unbinarity(self._h, self._c(C).data_ptr(), beta, u.data_ptr(), self._stream()), "eps_unbinarity")
+        return u
 
     def eps_vjp(self, C, beta: float, EF: Sequence, EA: Sequence, out=None):
         pf, pa = self._fields(EF, EA)

@@ -17,6 +17,7 @@
 #include "zreduce.cuh"
 #include "maskgrad.cuh"
 #include "morph.cuh"
+#include "reduce.cuh"
 
 using namespace epsgrad;
 
@@ -44,6 +45,9 @@ struct epsgrad_plan {
     int *d_hl;                 // [2R+1] half-lengths of the disk rows
     float *d_invn;             // [(2R+1)^2] 1/N by border class
     size_t off_m[4], off_mc, off_cot;
+    // beta-related outputs (NEXT-2): per-CTA partial sums, the d F/d beta output of the call in flight
+    size_t off_part; int n_part_mg, n_part_mo, n_part_ub;
+    float *cur_dbeta;
     int dense, host_direct, cur_host_src;   // cur_host_src: the fields of the call in flight are pinned host memory
     // scalars
     float eta0, eta_r, eps_clad, deps, delta;
@@ -355,6 +359,13 @@ extern "C" int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsg
         P->off_mc = off;  off += align_up(n_mask * 4, 256);
         P->off_cot = off; off += align_up(n_mask * 4, 256);
     }
+    P->n_part_mg = ((P->ny + MG_TJ - 1) / MG_TJ) * ((P->nx + MG_TI - 1) / MG_TI);
+    P->n_part_mo = P->morph_R > 0 ? ((P->py + MO_T - 1) / MO_T) * ((P->px + MO_T - 1) / MO_T) : 0;
+    P->n_part_ub = (int)(((size_t)P->px * P->py + UB_THREADS * UB_PER_THREAD - 1) / (UB_THREADS * UB_PER_THREAD));
+    {
+        const size_t a = (size_t)P->n_part_mg + P->n_part_mo, b = (size_t)P->n_part_ub;
+        P->off_part = off; off += align_up((size_t)cfg->batch * (a > b ? a : b) * 4, 256);
+    }
     P->off_tmp = off;  off += P->separable ? align_up((size_t)cfg->batch * cfg->mx * P->py * 4, 256) : 0;
     P->ws_need = off;
     *out = P;
@@ -574,6 +585,7 @@ float *ws_v(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_v);
 float *ws_m(const epsgrad_plan *P, int k) { return (float *)((char *)P->ws + P->off_m[k]); }
 float *ws_mc(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_mc); }
 float *ws_cot(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_cot); }
+float *ws_part(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_part); }
 float *ws_gbar(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_gbar); }
 float *ws_e2d(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_e2d); }
 float *ws_coef(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_coef); }
@@ -834,12 +846,22 @@ int launch_morph_reverse(epsgrad_plan *P, const float *phi, float beta, float *v
         mp.out = dst;
         mp.rho0 = ws_m(P, 0);
         mp.first = k == 0; mp.last = k == 3; mp.transposed = 1;
+        mp.dbeta_part = k == 0 && P->cur_dbeta ? ws_part(P) + (size_t)P->cfg.batch * P->n_part_mg : nullptr;   // [B][n_part_mo]
         mp.a = sign[k] * P->morph_alpha;
         int rc = launch_morph_one(P, mp, st, "morphT");
         if (rc) return rc;
         float *t = src; src = dst; dst = t;
     }
     return EPSGRAD_OK;
+}
+
+// d F/d beta: add the per-CTA partial sums maskgrad (and, with the filters on, the last morph^T op) left
+int launch_dbeta_sum(epsgrad_plan *P, cudaStream_t st)
+{
+    if (!P->cur_dbeta) return EPSGRAD_OK;
+    const float *pa = ws_part(P);
+    k_sum_partials<<<P->cfg.batch, 256, 0, st>>>(pa, P->n_part_mg, pa + (size_t)P->cfg.batch * P->n_part_mg, P->n_part_mo, 1.0f, P->cur_dbeta);
+    return check_launch(P, "dbeta", st);
 }
 
 // F1 and, when they are on, the first projection and the morphological filters
@@ -858,6 +880,7 @@ int launch_maskgrad(epsgrad_plan *P, const float *phi, float beta, const float *
     mp.nx = P->nx; mp.ny = P->ny; mp.px = P->px; mp.py = P->py; mp.s = P->cfg.subpixel;
     mp.beta = beta; mp.eta_r = P->eta_r; mp.eps_clad = P->eps_clad; mp.deps = P->deps;
     mp.use_den = 1;
+    mp.dbeta_part = P->cur_dbeta ? ws_part(P) : nullptr;               // [B][n_part_mg]
     if (P->morph_R > 0) { mp.phi = ws_mc(P); mp.eta_r = 0.0f; mp.use_den = 0; }   // v holds the cotangent of rho~: the filters^T follow
     const size_t smem = maskgrad_smem_floats(mp.s) * 4;
     auto kern = mp.s == 2 ? k_maskgrad<2> : (mp.s == 4 ? k_maskgrad<4> : k_maskgrad<0>);
@@ -911,6 +934,7 @@ int run_chain(epsgrad_plan *P, const float *C, float beta, int n_pairs, const vo
         if (!rc && dFdC) rc = launch_maskgrad(P, ws_phi(P), beta, ws_gbar(P), ws_coef(P), ws_v(P), st);
         if (!rc && dFdC && P->morph_R > 0) rc = launch_morph_reverse(P, ws_phi(P), beta, ws_v(P), st);
         if (!rc && dFdC) rc = launch_filterT(P, ws_v(P), dFdC, st);
+        if (!rc && dFdC) rc = launch_dbeta_sum(P, st);
         return rc;
     }
     cudaStream_t ax = P->aux;
@@ -932,6 +956,7 @@ int run_chain(epsgrad_plan *P, const float *C, float beta, int n_pairs, const vo
     }
     if (!rc && P->morph_R > 0) rc = launch_morph_reverse(P, ws_phi(P), beta, ws_v(P), ax);
     if (!rc) rc = launch_filterT(P, ws_v(P), dFdC, ax);
+    if (!rc) rc = launch_dbeta_sum(P, ax);
     // always join, even on error, so that the auxiliary stream never outlives the call
     if (cudaEventRecord(P->ev_join, ax) != cudaSuccess || cudaStreamWaitEvent(st, P->ev_join, 0) != cudaSuccess) {
         cudaGetLastError();
@@ -965,6 +990,58 @@ extern "C" int eps_vjp(epsgrad_plan_t *P, const float *C, float beta, int n_pair
     cudaStream_t st = (cudaStream_t)stream;
     begin_call(P, st);
     return run_chain(P, C, beta, n_pairs, EF, EA, nullptr, dFdC, st);
+}
+
+extern "C" int eps_vjp_beta(epsgrad_plan_t *P, const float *C, float beta, int n_pairs,
+                            const void *const *EF, const void *const *EA, float *dFdC, float *dFdbeta, void *stream)
+{
+    int rc = check_common(P, C, beta);
+    if (!rc) rc = check_pairs(n_pairs, EF, EA);
+    if (rc) return rc;
+    if (!aligned16(dFdC) || !dFdbeta) return EPSGRAD_EINVAL;
+    DeviceGuard g(P->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    begin_call(P, st);
+    P->cur_dbeta = dFdbeta;
+    rc = run_chain(P, C, beta, n_pairs, EF, EA, nullptr, dFdC, st);
+    P->cur_dbeta = nullptr;
+    return rc;
+}
+
+extern "C" int eps_unbinarity(epsgrad_plan_t *P, const float *C, float beta, float *u, void *stream)
+{
+    int rc = check_common(P, C, beta);
+    if (rc) return rc;
+    if (!u) return EPSGRAD_EINVAL;
+    DeviceGuard g(P->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    begin_call(P, st);
+    rc = launch_front(P, C, beta, st);
+    if (rc) return rc;
+    const size_t n_mask = (size_t)P->px * P->py;
+    const bool morph = P->morph_R > 0;
+    k_unbinarity<<<dim3(P->n_part_ub, P->cfg.batch), UB_THREADS, 0, st>>>(morph ? ws_mc(P) : ws_phi(P), n_mask, beta,
+                                                                         morph ? 0.0f : P->eta_r, ws_part(P));
+    rc = check_launch(P, "unbinarity", st);
+    if (rc) return rc;
+    k_sum_partials<<<P->cfg.batch, 256, 0, st>>>(ws_part(P), P->n_part_ub, nullptr, 0, (float)(1.0 / (double)n_mask), u);
+    return check_launch(P, "unbinarity_sum", st);
+}
+
+extern "C" double epsgrad_beta_schedule(double beta_min, double beta_max, int i, int n_iter)
+{
+    const double x = n_iter > 0 ? (double)i / (double)n_iter : 1.0;
+    return beta_min + (beta_max - beta_min) * std::expm1(x * x) / std::expm1(1.0);
+}
+
+extern "C" int epsgrad_beta_update(double *t, double *beta_max, double gamma, double u, double u0, double beta)
+{
+    if (!t || !beta_max || !(u > 0.0) || !(u0 > 0.0) || !(beta > 0.0) || !(gamma >= 0.0 && gamma <= 1.0)) return EPSGRAD_EINVAL;
+    const double tn = gamma * *t + (1.0 - gamma) * (1.0 / u - 1.0) / beta;
+    if (!(tn > 0.0)) return EPSGRAD_EINVAL;
+    *t = tn;
+    *beta_max = gamma * *beta_max + (1.0 - gamma) * (1.0 / u0 - 1.0) / tn;
+    return EPSGRAD_OK;
 }
 
 extern "C" int eps_forward_vjp(epsgrad_plan_t *P, const float *C, float beta, int n_pairs,

@@ -13,6 +13,7 @@
 // Sobel^T sources on [i0-2, i0+TI].
 #pragma once
 #include "common.cuh"
+#include "reduce.cuh"
 
 namespace epsgrad {
 
@@ -21,6 +22,7 @@ struct MaskGradParams {
     const float *gbar;     // [B,5,nx,ny]  z-reduced cotangent: x, y, z-full, z-lower-face, z-upper-face
     const float *coef;     // [B,10,nx,ny] [hbk, abk, gxk, gyk] for c = x, for c = y, flo, fhi
     float *v;              // [B,px,py]
+    float *dbeta_part;     // nullptr, or one partial sum of d F/d beta per CTA: [B][gridDim.y * gridDim.x] (reduce.cuh)
     Normaliser nrm;
     int nx, ny, px, py, s;
     int use_den;           // 1: v carries 1/den of Eq. (2); 0: the morphological filters^T follow and the last one applies it
@@ -150,7 +152,8 @@ __global__ void __launch_bounds__(MG_THREADS) k_maskgrad(const __grid_constant__
         // have E_y owners j-1 and j: nine shared-memory values serve the four pixels; 8-byte loads and stores.
         static_assert(TI * TJ == NTH, "one thread per cell");
         const int ti = tid / TJ, tj = tid - ti * TJ, i = i0 + ti, j = j0 + tj;
-        if (i >= nx || j >= ny) return;
+        float db = 0.f;                                             // sum of Phibar (x - eta) over this thread's pixels
+        if (i < nx && j < ny) {
         const int c0 = (ti + 2) * CJ + tj + 2;                      // the cell in the staged arrays
         const float az = AbZ[tid];
         float ex[2], hx[2], ey[2], hy[2];                           // owner values per pixel row a / column c, multiplicity folded in
@@ -177,11 +180,19 @@ __global__ void __launch_bounds__(MG_THREADS) k_maskgrad(const __grid_constant__
                 const float d = fast_rcp(1.0f + e2);
                 const float r = fast_rcp(fmaf(P.deps, t >= 0.f ? d : e2 * d, P.eps_clad));   // 1/e
                 const float ebar = az + ex[a] + ey[c], rbar = hx[a] + hy[c];
-                o[c] = k0 * e2 * d * d * (ebar - rbar * r * r) * (P.use_den ? P.nrm.at_index(np, c == 0 ? nq0 : nq1) : 1.0f);
+                const float pb = k0 * e2 * d * d * (ebar - rbar * r * r);          // Phibar
+                db = fmaf(pb, phv[a][c] - P.eta_r, db);
+                o[c] = pb * (P.use_den ? P.nrm.at_index(np, c == 0 ? nq0 : nq1) : 1.0f);
             }
             *reinterpret_cast<float2 *>(vb + (p + a) * P.py + q) = make_float2(o[0], o[1]);
         }
+        }
+        if (P.dbeta_part) {                                         // block-uniform
+            const float sdb = block_sum(db, reinterpret_cast<float *>(nidx));      // nidx is dead for every thread past block_sum's first barrier
+            if (tid == 0) P.dbeta_part[(size_t)b * gridDim.y * gridDim.x + blockIdx.y * gridDim.x + blockIdx.x] = sdb / P.beta;
+        }
     } else {
+    float db = 0.f;
     for (int base = tid; base < TP * TQ; base += 4 * NTH) {
         float ph[4];                                           // filter output of four pixels in flight
 #pragma unroll
@@ -219,8 +230,13 @@ __global__ void __launch_bounds__(MG_THREADS) k_maskgrad(const __grid_constant__
             const float r = fast_rcp(fmaf(P.deps, rho, P.eps_clad));   // 1/e
             const float slope = 2.0f * P.beta * a * d * d;
             const float rhobar = P.deps * inv_s2 * (ebar - rbar * r * r);
+            db = fmaf(rhobar * slope, ph[u] - P.eta_r, db);
             vb[p * P.py + q] = rhobar * slope * (P.use_den ? P.nrm.at_index(nidx[tp], nidx[TP + tq]) : 1.0f);
         }
+    }
+    if (P.dbeta_part) {
+        const float sdb = block_sum(db, reinterpret_cast<float *>(nidx));
+        if (tid == 0) P.dbeta_part[(size_t)b * gridDim.y * gridDim.x + blockIdx.y * gridDim.x + blockIdx.x] = sdb / P.beta;
     }
     }
 }

@@ -15,6 +15,7 @@
 // (plain adds: no sliding-window subtraction, the staged values span e^-20..e^20).  Bound: shared-memory reads and FADD issue; L2-resident.
 #pragma once
 #include "common.cuh"
+#include "reduce.cuh"
 
 namespace epsgrad {
 
@@ -26,6 +27,7 @@ struct MorphParams {
     const float *ybar;     // transposed op: cotangent of y
     float *out;            // forward: y (last op: y - 1/2); transposed: xbar (first op of the chain: v)
     float *rho0;           // first forward op: keeps rho0 = projection(Phi') for the transposed pass
+    float *dbeta_part;     // first op, transposed: nullptr, or one partial sum of d F/d beta per CTA (first projection; reduce.cuh)
     const int *hl;         // [2R+1] half-lengths of the disk rows
     const float *invn;     // [(2R+1)^2] 1/N by border class (rows, columns)
     Normaliser nrm;        // first op of the chain, transposed: 1/den of Eq. (2)
@@ -114,12 +116,12 @@ __global__ void __launch_bounds__(MO_THREADS) k_morph(const __grid_constant__ Mo
     }
     // ---- finish per pixel
     const int p = p0 + r;
-    if (p >= P.px) return;
     const float inv_a = 1.0f / a;
+    float db = 0.f;
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
         const int q = q0 + c4 + u;
-        if (q >= P.py) continue;
+        if (p >= P.px || q >= P.py) continue;
         const size_t idx = plane + (size_t)p * P.py + q;
         if (!P.transposed) {
             const float invn = P.invn[morph_class(p, P.px, R) * NI + morph_class(q, P.py, R)];
@@ -128,10 +130,20 @@ __global__ void __launch_bounds__(MO_THREADS) k_morph(const __grid_constant__ Mo
         } else {
             const float xv = P.first ? P.rho0[idx] : P.x[idx];
             float o = acc[u] * __expf(a * xv);
-            // first op of the chain: projection^T in the overflow-free analytic form, then 1/den (S2)
-            if (P.first) o *= project_slope(P.x[idx], P.beta, P.eta_r) * P.nrm.at(p, q);
+            if (P.first) {
+                // first op of the chain: projection^T in the overflow-free analytic form, then 1/den (S2);
+                // the same cotangent gives the first projection's share of d F/d beta: Phibar (Phi - eta)/beta
+                const float phi = P.x[idx];
+                o *= project_slope(phi, P.beta, P.eta_r);
+                db = fmaf(o, phi - P.eta_r, db);
+                o *= P.nrm.at(p, q);
+            }
             P.out[idx] = o;
         }
+    }
+    if (P.dbeta_part) {                                        // block-uniform; first transposed op only
+        const float sdb = block_sum(db, f_s);                  // f_s is dead past block_sum's first barrier
+        if (tid == 0) P.dbeta_part[(size_t)b * gridDim.y * gridDim.x + blockIdx.y * gridDim.x + blockIdx.x] = sdb / P.beta;
     }
 }
 
