@@ -165,6 +165,12 @@ int eps_unbinarity(epsgrad_plan_t *plan, const float *C, float beta, float *u, v
 double epsgrad_beta_schedule(double beta_min, double beta_max, int i, int n_iter);
 int    epsgrad_beta_update(double *t, double *beta_max, double gamma, double u, double u0, double beta);
 
+/* Adam, Eqs. (10)-(11): one step `step` >= 1, in place, on n control variables (DEVICE pointers; M, V the
+ * moment buffers, zero before step 1; G the gradient of Eq. (1)).  Defaults of App. B: b1 .9, b2 .999, lr .001.
+ *   M = b1 M + (1-b1) G,  V = b2 V + (1-b2) G^2,  C -= lr (M/(1-b1^step)) / (sqrt(V/(1-b2^step)) + eps)                     */
+int epsgrad_adam_step(float *C, float *M, float *V, const float *G, size_t n, int step,
+                      double b1, double b2, double lr, double eps, void *stream);
+
 /* Both in one call; the filter output (Phi) is computed once and shared.                */
 int eps_forward_vjp(epsgrad_plan_t *plan, const float *C, float beta, int n_pairs,
                     const void *const *EF, const void *const *EA,

@@ -355,6 +355,15 @@ def vjp_beta(cfg: OracleConfig, C, beta: float, EF: list, EA: list):
     return out, float(db.value)
 
 
+def adam_step(C, M, V, G, i: int, b1=0.9, b2=0.999, lr=1e-3, eps=1e-8):
+    """Eqs. (10)-(11): one Adam step i >= 1 on float64 copies; returns (C, M, V)."""
+    C, M, V = (np.array(a, dtype=np.float64, order="C") for a in (C, M, V))
+    G = _f64(G)
+    lib().orc_adam_step(ctypes.c_int64(C.size), _p(C), _p(M), _p(V), _p(G), ctypes.c_int(i), ctypes.c_double(b1),
+                        ctypes.c_double(b2), ctypes.c_double(lr), ctypes.c_double(eps))
+    return C, M, V
+
+
 def vjp(cfg: OracleConfig, C, beta: float, EF: list, EA: list):
     """Eq. (1): -2 Re((d eps/dC)^T (E_F . E_A)) summed over the pairs; fields complex64 [3,nx,ny,nz]."""
     c = cfg.c()

@@ -674,6 +674,22 @@ void orc_beta_update(double *t, double *beta_max, double gamma, double u, double
     *beta_max = gamma * *beta_max + (1.0 - gamma) * (1.0 / u0 - 1.0) / *t;
 }
 
+/* ------------------------------------------------------------------ */
+/* Adam, Eqs. (10)-(11), one step i >= 1, in place:       */
+/*   M = b1 M + (1-b1) G,  V = b2 V + (1-b2) G^2,                      */
+/*   Mh = M/(1-b1^i),  Vh = V/(1-b2^i),  C = C - lr Mh/(sqrt(Vh)+eps)  */
+/* ------------------------------------------------------------------ */
+void orc_adam_step(int64_t n, double *C, double *M, double *V, const double *G,
+                   int i, double b1, double b2, double lr, double eps)
+{
+    const double c1 = 1.0 - pow(b1, (double)i), c2 = 1.0 - pow(b2, (double)i);
+    for (int64_t k = 0; k < n; ++k) {
+        M[k] = b1 * M[k] + (1.0 - b1) * G[k];
+        V[k] = b2 * V[k] + (1.0 - b2) * G[k] * G[k];
+        C[k] -= lr * (M[k] / c1) / (sqrt(V[k] / c2) + eps);
+    }
+}
+
 int orc_num_threads(void)
 {
     int n = 1;

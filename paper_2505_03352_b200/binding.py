@@ -21,7 +21,7 @@ EXPORTS = (
     "epsgrad_plan_set_dense_reads", "epsgrad_plan_last_launches", "epsgrad_plan_last_copy_bytes",
     "epsgrad_plan_set_profiling", "epsgrad_plan_last_kernel_times", "epsgrad_plan_set_overlap", "epsgrad_plan_set_host_direct", "epsgrad_plan_set_timeline", "epsgrad_plan_read_timeline", 
     "eps_forward", "eps_vjp", "eps_forward_vjp", "eps_forward_vjp_host", "eps_vjp_beta", "eps_unbinarity",
-    "epsgrad_beta_schedule", "epsgrad_beta_update",
+    "epsgrad_beta_schedule", "epsgrad_beta_update", "epsgrad_adam_step",
     "epsgrad_stage_filter", "epsgrad_stage_eps2d", "epsgrad_stage_zreduce",
     "epsgrad_status_string", "epsgrad_version",
 )
@@ -73,6 +73,15 @@ def config_of(w) -> Config:
 _lib = None
 
 
+def adam_step(C, M, V, G, step: int, b1=0.9, b2=0.999, lr=1e-3, eps=1e-8) -> None:
+    """Eqs. (10)-(11) in place on CUDA float32 tensors of one shape (current stream)."""
+    import torch
+    for x in (C, M, V, G):
+        assert x.is_cuda and x.dtype == torch.float32 and x.is_contiguous() and x.shape == C.shape
+    _check(lib().epsgrad_adam_step(C.data_ptr(), M.data_ptr(), V.data_ptr(), G.data_ptr(), C.numel(), step, b1, b2, lr, eps,
+                                   torch.cuda.current_stream(C.device).cuda_stream), "epsgrad_adam_step")
+
+
 def beta_schedule(beta_min: float, beta_max: float, i: int, n_iter: int) -> float:
     """Eq. (14) (P:L150)."""
     return float(lib().epsgrad_beta_schedule(beta_min, beta_max, i, n_iter))
@@ -118,6 +127,7 @@ def lib() -> ctypes.CDLL:
     L.eps_unbinarity.argtypes = [vp, vp, f32, vp, vp]
     L.epsgrad_beta_schedule.restype = ctypes.c_double
     L.epsgrad_beta_schedule.argtypes = [ctypes.c_double, ctypes.c_double, i32, i32]
+    L.epsgrad_adam_step.argtypes = [vp, vp, vp, vp, sz, i32, ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_double, vp]
     L.epsgrad_beta_update.argtypes = [vp, vp, ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_double]
     L.eps_forward_vjp.argtypes = [vp, vp, f32, i32, vp, vp, vp, vp, vp]
     L.eps_forward_vjp_host.argtypes = [vp, vp, f32, i32, vp, vp, vp, vp, vp]

@@ -1028,6 +1028,18 @@ extern "C" int eps_unbinarity(epsgrad_plan_t *P, const float *C, float beta, flo
     return check_launch(P, "unbinarity_sum", st);
 }
 
+extern "C" int epsgrad_adam_step(float *C, float *M, float *V, const float *G, size_t n, int step,
+                                 double b1, double b2, double lr, double eps, void *stream)
+{
+    if (!C || !M || !V || !G || step < 1) return EPSGRAD_EINVAL;
+    if (!(b1 >= 0.0 && b1 < 1.0) || !(b2 >= 0.0 && b2 < 1.0) || !(lr > 0.0) || !(eps >= 0.0)) return EPSGRAD_EINVAL;
+    if (n == 0) return EPSGRAD_OK;
+    const double c1 = 1.0 - std::pow(b1, (double)step), c2 = 1.0 - std::pow(b2, (double)step);
+    k_adam<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(C, M, V, G, n, (float)b1, (float)b2, (float)(1.0 - b1), (float)(1.0 - b2), (float)(1.0 / c1),
+                                                                        (float)(1.0 / c2), (float)lr, (float)eps);
+    return cudaGetLastError() == cudaSuccess ? EPSGRAD_OK : EPSGRAD_ECUDA;
+}
+
 extern "C" double epsgrad_beta_schedule(double beta_min, double beta_max, int i, int n_iter)
 {
     const double x = n_iter > 0 ? (double)i / (double)n_iter : 1.0;

@@ -57,3 +57,19 @@ def test_beta_schedule_matches_oracle():
         assert abs(t - to) < 1e-13 and abs(bm - bo) < 1e-10
     with pytest.raises(B.EpsgradError):
         B.beta_update(1.0, 50.0, 0.95, 0.0, 0.01, 10.0)
+
+
+def test_adam_steps_match_oracle():
+    rng = np.random.default_rng(51)
+    shape = (2, 37, 29)
+    C0 = rng.random(shape).astype(np.float32)
+    C, M, V = dev(C0.copy()), torch.zeros(shape, device="cuda"), torch.zeros(shape, device="cuda")
+    Co, Mo, Vo = C0.astype(np.float64), np.zeros(shape), np.zeros(shape)
+    for i in range(1, 21):
+        G = (rng.standard_normal(shape) * (0.01 + 0.1 * i)).astype(np.float32)
+        B.adam_step(C, M, V, dev(G), i)
+        Co, Mo, Vo = O.adam_step(Co, Mo, Vo, G, i)
+        assert np.max(np.abs(C.cpu().numpy() - Co)) < 2e-6
+        assert rel_inf(M.cpu().numpy().astype(np.float64), Mo) < 1e-5 and rel_inf(V.cpu().numpy().astype(np.float64), Vo) < 1e-5
+    with pytest.raises(B.EpsgradError):
+        B.adam_step(C, M, V, C, 0)

@@ -83,3 +83,23 @@ def test_beta_update_eq15_fixed_point():
     assert abs(t - tstar) < 1e-9 and abs(bmax - (1.0 / u0 - 1.0) / tstar) < 1e-6
     t1, b1 = O.beta_update(2.0, 80.0, gamma, 0.2, u0, 16.0)          # one step, by hand
     assert abs(t1 - (0.95 * 2.0 + 0.05 * 4.0 / 16.0)) < 1e-15 and abs(b1 - (0.95 * 80.0 + 0.05 * 99.0 / t1)) < 1e-12
+
+
+def test_adam_first_step_closed_form_and_library():
+    # step 1 from zero moments: Mh = G, Vh = G^2, so C moves by -lr G/(|G| + eps) (Eqs. (10)-(11))
+    rng = np.random.default_rng(21)
+    C0 = rng.random((7, 9))
+    G = rng.standard_normal((7, 9))
+    C1, M1, V1 = O.adam_step(C0, np.zeros_like(C0), np.zeros_like(C0), G, 1, lr=1e-3, eps=1e-8)
+    assert np.max(np.abs(C1 - (C0 - 1e-3 * G / (np.abs(G) + 1e-8)))) < 1e-15
+    assert np.allclose(M1, 0.1 * G, rtol=1e-14) and np.allclose(V1, 0.001 * G * G, rtol=1e-12)
+    # 25 steps with fresh gradients against torch.optim.Adam in float64 (same update rule, App. B defaults)
+    Ct = torch.tensor(C0.copy(), requires_grad=True)
+    opt = torch.optim.Adam([Ct], lr=1e-3, betas=(0.9, 0.999), eps=1e-8)
+    C, M, V = C0.copy(), np.zeros_like(C0), np.zeros_like(C0)
+    for i in range(1, 26):
+        G = rng.standard_normal(C0.shape) * (1.0 + i)
+        Ct.grad = torch.tensor(G.copy())
+        opt.step()
+        C, M, V = O.adam_step(C, M, V, G, i)
+        assert np.max(np.abs(C - Ct.detach().numpy())) < 1e-13
