@@ -65,6 +65,12 @@ extern "C" {
 
 typedef struct epsgrad_plan epsgrad_plan_t;   /* opaque, library-owned */
 
+/* Position of the design region inside a simulation domain (cells); see epsgrad_plan_set_embedding. */
+typedef struct {
+    int32_t nx_full, ny_full, nz_full;   /* the solver's grid                                         */
+    int32_t i0, j0, k0;                  /* first cell of the design region in it (k0 % 4 == 0)       */
+} epsgrad_embedding_t;
+
 /* Geometry, filter and materials of a batch of B identical design regions (cell units). */
 typedef struct {
     int32_t batch;            /* B >= 1 independent designs                                  */
@@ -181,6 +187,15 @@ int eps_forward_vjp(epsgrad_plan_t *plan, const float *C, float beta, int n_pair
 int eps_forward_vjp_host(epsgrad_plan_t *plan, const float *C_host, float beta, int n_pairs,
                          const void *const *EF_host, const void *const *EA_host,
                          float *eps_host, float *dFdC_host, void *stream);
+/* Embedding in a simulation domain (Eq. (1) restricts the fields to Omega_D; Fig. 4: a 210x210-cell design
+ * region in a 430x450x64 model).  After this call the DEVICE entry points take eps, E_F and E_A as the solver's full arrays
+ * [B, 3, nx_full, ny_full, nz_full]: the fields are read, and eps is written, only inside the block
+ * [i0, i0+Nx) x [j0, j0+Ny) x [k0, k0+Nz); the rest of eps is not touched (it belongs to the solver).  z_lo, z_hi stay relative
+ * to k0.  NULL switches back to region-sized arrays.  Needs nz_full % 4 == 0 and k0 % 4 == 0 (16-byte pieces), else
+ * EPSGRAD_EUNSUPPORTED; a block that sticks out of the domain is EPSGRAD_EINVAL.  The *_host entry points and the stage
+ * taps keep region-sized buffers (eps_forward_vjp_host returns EPSGRAD_EUNSUPPORTED while an embedding is set).          */
+int epsgrad_plan_set_embedding(epsgrad_plan_t *plan, const epsgrad_embedding_t *embedding);
+
 /* Field transfer of the *_host entry points (default 1).  1: when every field buffer is pinned, mapped host memory (and the
  * plan is not in dense-read mode), the Eq. (1) reduction copies its slab windows straight out of host memory and the rest
  * of the fields never crosses the bus (only Omega_D enters the gradient); buffers that are not pinned fall back to

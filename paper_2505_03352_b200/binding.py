@@ -19,7 +19,7 @@ EXPORTS = (
     "epsgrad_plan_create", "epsgrad_plan_destroy", "epsgrad_workspace_bytes",
     "epsgrad_plan_set_workspace", "epsgrad_staging_bytes", "epsgrad_plan_set_staging",
     "epsgrad_plan_set_dense_reads", "epsgrad_plan_last_launches", "epsgrad_plan_last_copy_bytes",
-    "epsgrad_plan_set_profiling", "epsgrad_plan_last_kernel_times", "epsgrad_plan_set_overlap", "epsgrad_plan_set_host_direct", "epsgrad_plan_set_timeline", "epsgrad_plan_read_timeline", 
+    "epsgrad_plan_set_profiling", "epsgrad_plan_last_kernel_times", "epsgrad_plan_set_overlap", "epsgrad_plan_set_host_direct", "epsgrad_plan_set_embedding", "epsgrad_plan_set_timeline", "epsgrad_plan_read_timeline", 
     "eps_forward", "eps_vjp", "eps_forward_vjp", "eps_forward_vjp_host", "eps_vjp_beta", "eps_unbinarity",
     "epsgrad_beta_schedule", "epsgrad_beta_update", "epsgrad_adam_step",
     "epsgrad_stage_filter", "epsgrad_stage_eps2d", "epsgrad_stage_zreduce",
@@ -31,6 +31,11 @@ class EpsgradError(RuntimeError):
     def __init__(self, status: int, where: str):
         self.status = status
         super().__init__(f"{where}: {status_string(status)} ({status})")
+
+
+class Embedding(ctypes.Structure):
+    """epsgrad_embedding_t (include/epsgrad.h)."""
+    _fields_ = [(n, ctypes.c_int32) for n in ("nx_full", "ny_full", "nz_full", "i0", "j0", "k0")]
 
 
 class Config(ctypes.Structure):
@@ -135,6 +140,7 @@ def lib() -> ctypes.CDLL:
     L.epsgrad_stage_eps2d.argtypes = [vp, vp, f32, vp, vp]
     L.epsgrad_plan_set_overlap.argtypes = [vp, i32]
     L.epsgrad_plan_set_host_direct.argtypes = [vp, i32]
+    L.epsgrad_plan_set_embedding.argtypes = [vp, vp]
     L.epsgrad_plan_set_timeline.argtypes = [vp, i32]
     L.epsgrad_plan_read_timeline.argtypes = [vp, i32, vp, vp]
     L.epsgrad_stage_zreduce.argtypes = [vp, i32, vp, vp, vp, vp]
@@ -176,6 +182,7 @@ class Plan:
                "epsgrad_plan_set_workspace")
         self._stg = None
         self._stg_pairs = -1
+        self._field_shape = None          # set_embedding: shape of the solver's arrays
 
     def close(self) -> None:
         if getattr(self, "_h", None):
@@ -193,6 +200,11 @@ class Plan:
     def eps_shape(self):
         c = self.cfg
         return (c.batch, 3, c.nx, c.ny, c.nz)
+
+    @property
+    def field_shape(self):
+        """shape of eps / E_F / E_A as the device entry points take them (the solver's arrays when an embedding is set)"""
+        return self._field_shape or self.eps_shape
 
     @property
     def ctrl_shape(self):
@@ -216,8 +228,8 @@ class Plan:
         t = self._torch
         assert len(EF) == len(EA) and len(EF) >= 1
         for f in list(EF) + list(EA):
-            assert f.is_cuda and f.dtype == t.complex64 and f.is_contiguous() and tuple(f.shape) == self.eps_shape, \
-                (f.shape, f.dtype, self.eps_shape)
+            assert f.is_cuda and f.dtype == t.complex64 and f.is_contiguous() and tuple(f.shape) == self.field_shape, \
+                (f.shape, f.dtype, self.field_shape)
         return _ptr_array(EF), _ptr_array(EA)
 
     def _out(self, out, shape):
@@ -238,6 +250,16 @@ class Plan:
         a, b = ctypes.c_uint64(), ctypes.c_uint64()
         _check(lib().epsgrad_plan_last_copy_bytes(self._h, ctypes.byref(a), ctypes.byref(b)), "last_copy_bytes")
         return int(a.value), int(b.value)
+
+    def set_embedding(self, nx_full=None, ny_full=None, nz_full=None, i0=0, j0=0, k0=0) -> None:
+        """eps / E_F / E_A become the solver's full arrays [B,3,nx_full,ny_full,nz_full]; no arguments: back to region-sized arrays"""
+        if nx_full is None:
+            _check(lib().epsgrad_plan_set_embedding(self._h, None), "epsgrad_plan_set_embedding")
+            self._field_shape = None
+        else:
+            e = Embedding(nx_full, ny_full, nz_full, i0, j0, k0)
+            _check(lib().epsgrad_plan_set_embedding(self._h, ctypes.byref(e)), "epsgrad_plan_set_embedding")
+            self._field_shape = (self.eps_shape[0], 3, nx_full, ny_full, nz_full)
 
     def set_host_direct(self, enable: bool) -> None:
         _check(lib().epsgrad_plan_set_host_direct(self._h, int(bool(enable))), "epsgrad_plan_set_host_direct")
@@ -270,7 +292,7 @@ class Plan:
 
     # ---- hot path (device tensors)
     def eps_forward(self, C, beta: float, out=None):
-        eps = self._out(out, self.eps_shape)
+        eps = self._out(out, self.field_shape)
         _check(lib().eps_forward(self._h, self._c(C).data_ptr(), beta, eps.data_ptr(), self._stream()), "eps_forward")
         return eps
 
@@ -298,7 +320,7 @@ class Plan:
 
     def eps_forward_vjp(self, C, beta: float, EF: Sequence, EA: Sequence, eps_out=None, grad_out=None):
         pf, pa = self._fields(EF, EA)
-        eps = self._out(eps_out, self.eps_shape)
+        eps = self._out(eps_out, self.field_shape)
         g = self._out(grad_out, self.ctrl_shape)
         _check(lib().eps_forward_vjp(self._h, self._c(C).data_ptr(), beta, len(EF), pf, pa, eps.data_ptr(),
                                      g.data_ptr(), self._stream()), "eps_forward_vjp")

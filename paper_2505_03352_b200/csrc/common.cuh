@@ -22,6 +22,23 @@ __device__ __forceinline__ int border_class(int a0, int M, int T, int K)
     return d < T ? 2 * T - d : T;
 }
 
+// Where the z columns of the design region sit in the caller's 4-D arrays, in 16-byte pieces of the array's element type
+// (2 complex64 cells of a field, 4 floats of eps).  Dense region arrays [B,3,nx,ny,nz]: column col = i*ny + j of plane (b,c)
+// starts at ((b*3+c)*ncol + col) * col_pitch.  Embedded in a simulation domain [B,3,NXf,NYf,NZf] with the design region at
+// (i0,j0,k0) (epsgrad_plan_set_embedding; "|Omega_D"): at (((b*3+c)*NXf + i0+i)*NYf + j0+j)*col_pitch + k0 (pieces).
+struct ColumnMap {
+    int embedded, ny;
+    unsigned col_pitch;                 // pieces per z column of the caller's array
+    size_t row_pitch, plane_pitch, base;
+    __device__ __forceinline__ size_t plane(int b, int c) const { return ((size_t)b * 3 + c) * plane_pitch + base; }
+    __device__ __forceinline__ size_t col(int idx) const
+    {
+        if (!embedded) return (size_t)idx * col_pitch;
+        const int i = idx / ny, j = idx - i * ny;
+        return (size_t)i * row_pitch + (size_t)j * col_pitch;
+    }
+};
+
 // streaming 16-byte load that does not allocate in L1 (fields are read exactly once).
 // SPARSE: the access touches only a 64..96-byte window of each 512-byte z column.  By default a
 // miss fills the whole 128-byte line from DRAM (measured: 256 B fetched per column for a window

@@ -48,6 +48,8 @@ struct epsgrad_plan {
     // beta-related outputs (NEXT-2): per-CTA partial sums, the d F/d beta output of the call in flight
     size_t off_part; int n_part_mg, n_part_mo, n_part_ub;
     float *cur_dbeta;
+    // embedding of the design region in the caller's simulation-domain arrays (epsgrad_plan_set_embedding); emb.nx_full = 0: none
+    epsgrad_embedding_t emb;
     int dense, host_direct, cur_host_src;   // cur_host_src: the fields of the call in flight are pinned host memory
     // scalars
     float eta0, eta_r, eps_clad, deps, delta;
@@ -458,6 +460,18 @@ extern "C" int epsgrad_plan_set_dense_reads(epsgrad_plan_t *P, int dense)
     return EPSGRAD_OK;
 }
 
+extern "C" int epsgrad_plan_set_embedding(epsgrad_plan_t *P, const epsgrad_embedding_t *e)
+{
+    if (!P) return EPSGRAD_EINVAL;
+    if (!e) { std::memset(&P->emb, 0, sizeof(P->emb)); return EPSGRAD_OK; }
+    if (e->nx_full < 1 || e->ny_full < 1 || e->nz_full < 1 || e->i0 < 0 || e->j0 < 0 || e->k0 < 0) return EPSGRAD_EINVAL;
+    if (e->i0 + P->nx > e->nx_full || e->j0 + P->ny > e->ny_full || e->k0 + P->cfg.nz > e->nz_full) return EPSGRAD_EINVAL;
+    if (e->nz_full % 4 || e->k0 % 4) return EPSGRAD_EUNSUPPORTED;          // 16-byte pieces of eps (4 cells) and of the fields (2 cells)
+    if ((double)P->cfg.batch * 3.0 * e->nx_full * e->ny_full > 2.0e9) return EPSGRAD_EUNSUPPORTED;
+    P->emb = *e;
+    return EPSGRAD_OK;
+}
+
 extern "C" int epsgrad_plan_set_host_direct(epsgrad_plan_t *P, int enable)
 {
     if (!P) return EPSGRAD_EINVAL;
@@ -731,11 +745,34 @@ int launch_fwd2d(epsgrad_plan *P, const float *phi, float beta, float *e2d, floa
     return check_launch(P, "fwd2d", st);
 }
 
+// Column addressing of eps (cells_per_piece = 4) or of a field (2) in 16-byte pieces (common.cuh ColumnMap)
+ColumnMap make_colmap(const epsgrad_plan *P, int cells_per_piece)
+{
+    ColumnMap cm;
+    const epsgrad_embedding_t &e = P->emb;
+    cm.ny = P->ny;
+    if (e.nx_full > 0) {
+        cm.embedded = 1;
+        cm.col_pitch = (unsigned)(e.nz_full / cells_per_piece);
+        cm.row_pitch = (size_t)e.ny_full * cm.col_pitch;
+        cm.plane_pitch = (size_t)e.nx_full * cm.row_pitch;
+        cm.base = (size_t)e.i0 * cm.row_pitch + (size_t)e.j0 * cm.col_pitch + (size_t)(e.k0 / cells_per_piece);
+    } else {
+        cm.embedded = 0;
+        cm.col_pitch = (unsigned)(P->cfg.nz / cells_per_piece);
+        cm.row_pitch = (size_t)P->ny * cm.col_pitch;
+        cm.plane_pitch = (size_t)P->nx * cm.row_pitch;
+        cm.base = 0;
+    }
+    return cm;
+}
+
 // ---- F6: the eps store stream
 int launch_extrude(epsgrad_plan *P, const float *e2d, float *eps, cudaStream_t st)
 {
     ExtrudeParams ep;
     ep.e2d = e2d; ep.eps = eps; ep.zw = P->d_zw; ep.ncol = P->nx * P->ny; ep.nz = P->cfg.nz;
+    ep.cm = make_colmap(P, 4);
     ep.cpb = extrude_cols_per_block(ep.nz);
     ep.nblk = cdiv(ep.ncol, ep.cpb);
     const int nz4 = ep.nz >> 2;
@@ -757,6 +794,7 @@ int launch_zreduce(epsgrad_plan *P, int n_pairs, const void *const *EF, const vo
 {
     ZredParams zp;
     zp.gbar = gbar; zp.zw = P->d_zw; zp.ncol = P->nx * P->ny; zp.nz = P->cfg.nz;
+    zp.cm = make_colmap(P, 2);
     int maxnch = 1;
     for (int g = 0; g < 2; ++g) {
         zp.ch0[g] = P->dense ? 0 : P->ch0[g];
@@ -1084,6 +1122,7 @@ extern "C" int eps_forward_vjp_host(epsgrad_plan_t *P, const float *C_host, floa
     } else {
         n_pairs = 0;
     }
+    if (P->emb.nx_full > 0) return EPSGRAD_EUNSUPPORTED;     // host buffers are region-sized: no embedding here
     if (!P->ws) return EPSGRAD_ENOWORKSPACE;
     if (!P->stg || P->stg_bytes < epsgrad_staging_bytes(P, n_pairs)) return EPSGRAD_ENOWORKSPACE;
     DeviceGuard g(P->device);

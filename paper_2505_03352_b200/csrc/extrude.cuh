@@ -19,7 +19,8 @@ constexpr int EX_THREADS = 256, EX_PASSES = 16, EX_CTAS_PER_SM = 8;
 
 struct ExtrudeParams {
     const float *e2d;      // [B,5,ncol]: eps2d_x, eps2d_y, eps2d_z, eps_zz lower face, eps_zz upper face
-    float *eps;            // [B,3,ncol,nz]
+    float *eps;            // [B,3,ncol,nz], or the simulation domain's array when embedded (cm)
+    ColumnMap cm;          // where the columns sit in eps (16-byte pieces = 4 cells)
     const float *zw;       // [7][nz] z tables (epsgrad.cu)
     int ncol, nz;
     int nblk;              // column blocks per component plane
@@ -41,14 +42,14 @@ __global__ void __launch_bounds__(EX_THREADS, EX_CTAS_PER_SM) k_extrude(const __
     const int c = blockIdx.y, blk = blockIdx.x;
     const int cpb = P.cpb, col0 = blk * cpb, ncb = min(cpb, ncol - col0);
     const float *ed = P.e2d + (size_t)b * 5 * ncol;
-    float *out = P.eps + ((size_t)b * 3 + c) * ncol * nz;
+    float4 *out = reinterpret_cast<float4 *>(P.eps) + P.cm.plane(b, c);
     // stage: c = x, y need their own plane; c = z needs planes 2 (full cells), 3 and 4 (face cells)
     const int npl = c == 2 ? 3 : 1;
     for (int o = 0; o < npl; ++o)
         for (int lc = tid; lc < ncb; lc += EX_THREADS) vsm[o * cpb + lc] = ed[(size_t)(c + o) * ncol + col0 + lc];
     if (P.sh4 >= 0) {
-        const int k = (tid & (nz4 - 1)) << 2, cq = tid >> P.sh4, cpp = EX_THREADS >> P.sh4;
-        float4 *dst = reinterpret_cast<float4 *>(out + (size_t)(col0 + cq) * nz + k);
+        const int kq = tid & (nz4 - 1), k = kq << 2, cq = tid >> P.sh4, cpp = EX_THREADS >> P.sh4;
+        float4 *dst = out + kq;
         if (c < 2) {
             float wx[4], bx[4];
 #pragma unroll
@@ -62,7 +63,7 @@ __global__ void __launch_bounds__(EX_THREADS, EX_CTAS_PER_SM) k_extrude(const __
                     float4 o;
                     o.x = fmaf(wx[0], v, bx[0]); o.y = fmaf(wx[1], v, bx[1]);
                     o.z = fmaf(wx[2], v, bx[2]); o.w = fmaf(wx[3], v, bx[3]);
-                    __stcs(dst + (size_t)pass * cpp * nz4, o);
+                    __stcs(dst + P.cm.col(col0 + lc), o);
                 }
             }
         } else {
@@ -83,7 +84,7 @@ __global__ void __launch_bounds__(EX_THREADS, EX_CTAS_PER_SM) k_extrude(const __
                     o.y = fmaf(zf[1], v, fmaf(zl[1], vl, fmaf(zh[1], vh, bz[1])));
                     o.z = fmaf(zf[2], v, fmaf(zl[2], vl, fmaf(zh[2], vh, bz[2])));
                     o.w = fmaf(zf[3], v, fmaf(zl[3], vl, fmaf(zh[3], vh, bz[3])));
-                    __stcs(dst + (size_t)pass * cpp * nz4, o);
+                    __stcs(dst + P.cm.col(col0 + lc), o);
                 }
             }
         }
@@ -99,7 +100,7 @@ __global__ void __launch_bounds__(EX_THREADS, EX_CTAS_PER_SM) k_extrude(const __
             for (int x = 0; x < 4; ++x)
                 o[x] = c < 2 ? fmaf(w_xy[k + x], v, b_xy[k + x])
                              : fmaf(i_f[k + x], v, fmaf(i_l[k + x], vsm[cpb + lc], fmaf(i_h[k + x], vsm[2 * cpb + lc], b_z[k + x])));
-            __stcs(reinterpret_cast<float4 *>(out + (size_t)(col0 + lc) * nz + k), make_float4(o[0], o[1], o[2], o[3]));
+            __stcs(out + P.cm.col(col0 + lc) + (k >> 2), make_float4(o[0], o[1], o[2], o[3]));
         }
     }
 }

@@ -31,6 +31,7 @@ struct ZredParams {
     int ncol, nz, nblk;    // nblk = ceil(ncol / ZR_COLS) column blocks per component plane
     int ch0[2], nch[2];    // chunk window (chunk = 2 cells = 16 B) for {x,y} and {z}
     int chs[2];            // log2 of the lanes per column of the copy loop: 2^chs >= nch
+    ColumnMap cm;          // where the columns sit in E_F / E_A (16-byte pieces = 2 cells)
     int ncp[2];            // columns staged per pass (<= ZR_COLS): ncp (nch | 1) <= ZR_STAGE_CHUNKS
 };
 
@@ -63,10 +64,10 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 template <bool SPARSE, bool HOSTSRC>
 __device__ __forceinline__ void zwindow_issue(const ZredParams &P, float4 *buf, int p, int b, int c, int col0, int nc)
 {
-    const int grp = c == 2, nzc = P.nz >> 1, nch = P.nch[grp], sh = P.chs[grp], ncp = P.ncp[grp];
+    const int grp = c == 2, nch = P.nch[grp], sh = P.chs[grp], ncp = P.ncp[grp];
     const int ch = threadIdx.x & ((1 << sh) - 1), lstep = ZR_THREADS >> sh;
     if (ch < nch) {
-        const size_t first = (((size_t)b * 3 + c) * P.ncol + col0) * nzc + P.ch0[grp] + ch;
+        const size_t first = P.cm.plane(b, c) + P.ch0[grp] + ch;
         const float4 *pf = P.ef[p] + first, *pa = P.ea[p] + first;
         const int pitch = nch | 1;
         float4 *df = buf + ch, *da = df + pitch * ncp;
@@ -76,7 +77,7 @@ __device__ __forceinline__ void zwindow_issue(const ZredParams &P, float4 *buf, 
 #pragma unroll
                 for (int u = 0; u < 4; ++u) {
                     const int lc = lc0 + u * lstep;
-                    if (lc < nc) { f[u] = ld_stream<false>(pf + lc * nzc); a[u] = ld_stream<false>(pa + lc * nzc); }
+                    if (lc < nc) { const size_t o = P.cm.col(col0 + lc); f[u] = ld_stream<false>(pf + o); a[u] = ld_stream<false>(pa + o); }
                 }
 #pragma unroll
                 for (int u = 0; u < 4; ++u) {
@@ -86,8 +87,9 @@ __device__ __forceinline__ void zwindow_issue(const ZredParams &P, float4 *buf, 
             }
         } else {
             for (int lc = threadIdx.x >> sh; lc < nc; lc += lstep) {
-                cp_async16<SPARSE>(df + lc * pitch, pf + lc * nzc);
-                cp_async16<SPARSE>(da + lc * pitch, pa + lc * nzc);
+                const size_t o = P.cm.col(col0 + lc);
+                cp_async16<SPARSE>(df + lc * pitch, pf + o);
+                cp_async16<SPARSE>(da + lc * pitch, pa + o);
             }
         }
     }
