@@ -90,20 +90,25 @@ __global__ void __launch_bounds__(F2_THREADS) k_fwd2d(const __grid_constant__ Fw
     const int nx = P.nx, ny = P.ny, ncol = nx * ny;
     const float inv_s2 = 1.0f / (float)(s * s);
 
-    // ---- stage 1: mask tile (replicate outside the region, S5): e and r = 1/e; loads batched four deep
+    // ---- stage 1: mask tile (replicate outside the region, S5): e and r = 1/e; loads batched four deep.  The flat index
+    // advances by NTH without divisions; tiles whose ring lies inside the mask skip the clamps (block-uniform).
     {
         const float *phib = P.phi + (size_t)b * P.px * P.py;
         const int p_base = s * (i0 - 1), q_base = s * (j0 - 1);
+        const bool inside = p_base >= 0 && q_base >= 0 && p_base + MP <= P.px && q_base + MQ <= P.py;
+        const int dlp = NTH / MQ, dlq = NTH - dlp * MQ;
+        int lp = tid / MQ, lq = tid - lp * MQ;
         for (int base = tid; base < MP * MQ; base += 4 * NTH) {
             float ph[4];
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
-                const int i = base + u * NTH;
-                if (i < MP * MQ) {
-                    const int lp = i / MQ, lq = i - lp * MQ;
-                    const int p = clampi(p_base + lp, 0, P.px - 1), q = clampi(q_base + lq, 0, P.py - 1);
+                if (base + u * NTH < MP * MQ) {
+                    const int p = inside ? p_base + lp : clampi(p_base + lp, 0, P.px - 1);
+                    const int q = inside ? q_base + lq : clampi(q_base + lq, 0, P.py - 1);
                     ph[u] = phib[p * P.py + q];
                 }
+                lp += dlp; lq += dlq;
+                if (lq >= MQ) { lq -= MQ; ++lp; }
             }
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
