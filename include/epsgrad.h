@@ -39,6 +39,8 @@
  *   - Every function returns an int status: 0 = EPSGRAD_OK, negative = error (below).
  *     No exceptions, no abort.  Asynchronous faults surface at the caller's next sync.
  *   - There is no CPU path.  Without a CUDA device plan creation fails with EPSGRAD_ECUDA.
+ *   - A plan carries per-call state (launch accounting, the schedule's events): use one plan
+ *     from one host thread at a time; different plans are independent.
  */
 #ifndef EPSGRAD_H_
 #define EPSGRAD_H_
@@ -192,8 +194,9 @@ int eps_forward_vjp_host(epsgrad_plan_t *plan, const float *C_host, float beta, 
  * [B, 3, nx_full, ny_full, nz_full]: the fields are read, and eps is written, only inside the block
  * [i0, i0+Nx) x [j0, j0+Ny) x [k0, k0+Nz); the rest of eps is not touched (it belongs to the solver).  z_lo, z_hi stay relative
  * to k0.  NULL switches back to region-sized arrays.  Needs nz_full % 4 == 0 and k0 % 4 == 0 (16-byte pieces), else
- * EPSGRAD_EUNSUPPORTED; a block that sticks out of the domain is EPSGRAD_EINVAL.  The *_host entry points and the stage
- * taps keep region-sized buffers (eps_forward_vjp_host returns EPSGRAD_EUNSUPPORTED while an embedding is set).          */
+ * EPSGRAD_EUNSUPPORTED; a block that sticks out of the domain is EPSGRAD_EINVAL.  epsgrad_stage_zreduce follows the embedding
+ * (its fields are the solver's arrays); the *_host entry points keep region-sized buffers and return EPSGRAD_EUNSUPPORTED
+ * while an embedding is set.                                                                                              */
 int epsgrad_plan_set_embedding(epsgrad_plan_t *plan, const epsgrad_embedding_t *embedding);
 
 /* Field transfer of the *_host entry points (default 1).  1: when every field buffer is pinned, mapped host memory (and the
