@@ -643,11 +643,11 @@ int launch_filter_m(epsgrad_plan *P, const float *C, float *phi, cudaStream_t st
     }
     {
         sp.in = ws_tmp(P); sp.out = phi;
-        const size_t smem = ((size_t)NT * M + (size_t)(8 + 2 * T) * 128) * 4;
+        const size_t smem = sepx_smem_floats(NT, M) * 4;
         if (smem > 200 * 1024) return EPSGRAD_EUNSUPPORTED;
         int rc = set_smem(k_sep_up_x<M>, smem);
         if (rc) return rc;
-        k_sep_up_x<M><<<dim3(cdiv(P->py, 128), cdiv(mx, 8), B), SEP_THREADS, smem, st>>>(sp);
+        k_sep_up_x<M><<<dim3(cdiv(P->py, SEPX_THREADS), cdiv(mx, SEPX_NBA), B), SEPX_THREADS, smem, st>>>(sp);
         return check_launch(P, "filter_up_x", st);
     }
 }
@@ -688,11 +688,11 @@ int launch_filterT_m(epsgrad_plan *P, const float *v, float *dC, cudaStream_t st
     sp.mx = mx; sp.my = my; sp.px = P->px; sp.py = P->py; sp.T = T; sp.NT = NT; sp.eta0 = 0.0f;
     {
         sp.in = v; sp.out = ws_tmp(P);
-        const size_t smem = ((size_t)NT * M + (size_t)M * (8 + 2 * T) * 64) * 4;
+        const size_t smem = sepx_smem_floats(NT, M) * 4;
         if (smem > 200 * 1024) return EPSGRAD_EUNSUPPORTED;
         int rc = set_smem(k_sep_down_x<M>, smem);
         if (rc) return rc;
-        k_sep_down_x<M><<<dim3(cdiv(P->py, 64), cdiv(mx, 8), B), SEP_THREADS, smem, st>>>(sp);
+        k_sep_down_x<M><<<dim3(cdiv(P->py, SEPX_THREADS), cdiv(mx, SEPX_NBA), B), SEPX_THREADS, smem, st>>>(sp);
         if ((rc = check_launch(P, "filterT_down_x", st))) return rc;
     }
     {
