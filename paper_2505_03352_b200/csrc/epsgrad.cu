@@ -854,7 +854,7 @@ MorphParams morph_base(const epsgrad_plan *P, float beta)
     return mp;
 }
 
-// forward: Phi' -> rho0 (kept in m[0]) -> m[1] -> m[2] -> m[3] -> rho~ - 1/2 (mc)
+// forward: Phi' -> rho0 (kept in m[0]) -> z_1 (m[1]) -> z_2 (m[2]) -> z_3 (m[3]) -> rho~ - 1/2 (mc); z-space: morph.cuh
 int launch_morph_forward(epsgrad_plan *P, const float *phi, float beta, cudaStream_t st)
 {
     static const float sign[4] = {1.f, -1.f, -1.f, 1.f};
@@ -864,6 +864,7 @@ int launch_morph_forward(epsgrad_plan *P, const float *phi, float beta, cudaStre
         mp.out = k == 3 ? ws_mc(P) : ws_m(P, k + 1);
         mp.rho0 = ws_m(P, 0);
         mp.first = k == 0; mp.last = k == 3; mp.transposed = 0;
+        mp.x_inv = k > 0 && sign[k] != sign[k - 1];
         mp.a = sign[k] * P->morph_alpha;
         int rc = launch_morph_one(P, mp, st, "morph");
         if (rc) return rc;
@@ -884,6 +885,7 @@ int launch_morph_reverse(epsgrad_plan *P, const float *phi, float beta, float *v
         mp.out = dst;
         mp.rho0 = ws_m(P, 0);
         mp.first = k == 0; mp.last = k == 3; mp.transposed = 1;
+        mp.x_inv = k > 0 && sign[k] != sign[k - 1];
         mp.dbeta_part = k == 0 && P->cur_dbeta ? ws_part(P) + (size_t)P->cfg.batch * P->n_part_mg : nullptr;   // [B][n_part_mo]
         mp.a = sign[k] * P->morph_alpha;
         int rc = launch_morph_one(P, mp, st, "morphT");

@@ -11,6 +11,10 @@
 //   first forward op  stages exp(a rho0) with rho0 = projection (Eq. (3)/(6) form, S9) of the filter output, and keeps rho0;
 //   last forward op   writes y - 1/2, the centred input of the second projection, Eq. (6);
 //   last transposed op multiplies by the slope of the first projection and by 1/den (S2): the mask cotangent v of filterT.
+// Between the ops of the chain the masks are kept in "z-space": op k stores z_k = (1/N) sum exp(a_k x) instead of
+// y_k = log(z_k)/a_k, because the next op only needs exp(a_{k+1} y_k) = z_k^(a_{k+1}/a_k) = z_k or 1/z_k (|a| = alpha for all
+// four ops), and the transposed ops only exp(-a_k y_k) = 1/z_k: six of the eight launches run without exp or log, and the
+// log/exp round trip's rounding disappears.  Only the chain's first input (rho0) and last output (rho~) are real masks.
 // A thread owns four neighbouring pixels of a row: the part of a disk row that their four windows share is summed once
 // (plain adds: no sliding-window subtraction, the staged values span e^-20..e^20).  Bound: shared-memory reads and FADD issue; L2-resident.
 #pragma once
@@ -22,10 +26,10 @@ namespace epsgrad {
 constexpr int MO_T = 32, MO_THREADS = 256, MO_MAX_R = 16;
 
 struct MorphParams {
-    const float *x;        // [B,px,py] input of the forward op (first op: centred filter output Phi')
-    const float *y;        // transposed op: output of the forward op (last op of the chain: centred, y - 1/2)
+    const float *x;        // [B,px,py] input of the forward op: first op: centred filter output Phi'; later ops: z of the previous op
+    const float *y;        // transposed op: output of the forward op: z of this op; last op of the chain: the centred mask y - 1/2
     const float *ybar;     // transposed op: cotangent of y
-    float *out;            // forward: y (last op: y - 1/2); transposed: xbar (first op of the chain: v)
+    float *out;            // forward: z of this op (last op: y - 1/2); transposed: xbar (first op of the chain: v)
     float *rho0;           // first forward op: keeps rho0 = projection(Phi') for the transposed pass
     float *dbeta_part;     // first op, transposed: nullptr, or one partial sum of d F/d beta per CTA (first projection; reduce.cuh)
     const int *hl;         // [2R+1] half-lengths of the disk rows
@@ -33,6 +37,7 @@ struct MorphParams {
     Normaliser nrm;        // first op of the chain, transposed: 1/den of Eq. (2)
     int px, py, R;
     int transposed, first, last;
+    int x_inv;             // ops after the first: exp(a x) = 1/z_prev (the sign of alpha flipped) instead of z_prev
     float a;               // signed alpha
     float beta, eta_r;     // first projection (first op only)
 };
@@ -77,12 +82,14 @@ __global__ void __launch_bounds__(MO_THREADS) k_morph(const __grid_constant__ Mo
                         const float t = P.beta * (xv - P.eta_r);
                         xv = fast_rcp(1.0f + __expf(-2.0f * t));
                         if (lp >= R && lp < R + MO_T && lq >= R && lq < R + MO_T) P.rho0[idx] = xv;
+                        f = __expf(a * xv);
+                    } else {
+                        f = P.x_inv ? fast_rcp(xv) : xv;          // exp(a y_prev) = z_prev^(+-1)
                     }
-                    f = __expf(a * xv);
                 } else {
-                    const float yv = P.y[idx] + (P.last ? 0.5f : 0.0f);
-                    f = P.ybar[idx] * __expf(-a * yv) *
-                        P.invn[morph_class(p, P.px, R) * NI + morph_class(q, P.py, R)];
+                    // exp(-a y) = 1/z of this op; the last op kept the real mask (centred): one exponential
+                    const float iz = P.last ? __expf(-a * (P.y[idx] + 0.5f)) : fast_rcp(P.y[idx]);
+                    f = P.ybar[idx] * iz * P.invn[morph_class(p, P.px, R) * NI + morph_class(q, P.py, R)];
                 }
             }
             f_s[lp * pitch + lq] = f;
@@ -125,11 +132,11 @@ __global__ void __launch_bounds__(MO_THREADS) k_morph(const __grid_constant__ Mo
         const size_t idx = plane + (size_t)p * P.py + q;
         if (!P.transposed) {
             const float invn = P.invn[morph_class(p, P.px, R) * NI + morph_class(q, P.py, R)];
-            const float y = __logf(acc[u] * invn) * inv_a;
-            P.out[idx] = P.last ? y - 0.5f : y;
+            const float z = acc[u] * invn;
+            P.out[idx] = P.last ? __logf(z) * inv_a - 0.5f : z;
         } else {
             const float xv = P.first ? P.rho0[idx] : P.x[idx];
-            float o = acc[u] * __expf(a * xv);
+            float o = acc[u] * (P.first ? __expf(a * xv) : (P.x_inv ? fast_rcp(xv) : xv));     // exp(a x) as in the forward staging
             if (P.first) {
                 // first op of the chain: projection^T in the overflow-free analytic form, then 1/den (S2);
                 // the same cotangent gives the first projection's share of d F/d beta: Phibar (Phi - eta)/beta
