@@ -199,6 +199,12 @@ int eps_forward_vjp_host(epsgrad_plan_t *plan, const float *C_host, float beta, 
  * while an embedding is set.                                                                                              */
 int epsgrad_plan_set_embedding(epsgrad_plan_t *plan, const epsgrad_embedding_t *embedding);
 
+/* How the device-resident field windows are fetched (default 0).  1: by the tensor memory accelerator, one bulk tensor
+ * copy per field and 256 columns, persistent CTAs (region-sized fields with sparse windows only; other cases fall back).
+ * 0: by 16-byte asynchronous copies (LDGSTS), 2 us faster at paper scale.  Same bytes, same results; a measurement switch.
+ * EPSGRAD_EUNSUPPORTED when TMA descriptors cannot be built on this driver.                                               */
+int epsgrad_plan_set_tma(epsgrad_plan_t *plan, int enable);
+
 /* Field transfer of the *_host entry points (default 1).  1: when every field buffer is pinned, mapped host memory (and the
  * plan is not in dense-read mode), the Eq. (1) reduction copies its slab windows straight out of host memory and the rest
  * of the fields never crosses the bus (only Omega_D enters the gradient); buffers that are not pinned fall back to

@@ -50,6 +50,8 @@ struct epsgrad_plan {
     float *cur_dbeta;
     // embedding of the design region in the caller's simulation-domain arrays (epsgrad_plan_set_embedding); emb.nx_full = 0: none
     epsgrad_embedding_t emb;
+    int use_tma;               // field windows by TMA bulk tensor copies where possible (epsgrad_plan_set_tma)
+    void *tma_encode;          // cuTensorMapEncodeTiled, fetched through the runtime (no link against libcuda)
     int dense, host_direct, cur_host_src;   // cur_host_src: the fields of the call in flight are pinned host memory
     // scalars
     float eta0, eta_r, eps_clad, deps, delta;
@@ -346,6 +348,13 @@ extern "C" int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsg
         if (!ok) { cudaGetLastError(); epsgrad_plan_destroy(P); return EPSGRAD_ECUDA; }
         P->overlap = 1;
         P->host_direct = 1;
+        {
+            cudaDriverEntryPointQueryResult qres;
+            void *fn = nullptr;
+            if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess) { cudaGetLastError(); fn = nullptr; }
+            P->tma_encode = fn;
+            P->use_tma = 0;              // measured: 39 us against 37 us for the LDGSTS kernel at paper scale
+        }
     }
 
     // ---- workspace carve-up
@@ -469,6 +478,14 @@ extern "C" int epsgrad_plan_set_embedding(epsgrad_plan_t *P, const epsgrad_embed
     if (e->nz_full % 4 || e->k0 % 4) return EPSGRAD_EUNSUPPORTED;          // 16-byte pieces of eps (4 cells) and of the fields (2 cells)
     if ((double)P->cfg.batch * 3.0 * e->nx_full * e->ny_full > 2.0e9) return EPSGRAD_EUNSUPPORTED;
     P->emb = *e;
+    return EPSGRAD_OK;
+}
+
+extern "C" int epsgrad_plan_set_tma(epsgrad_plan_t *P, int enable)
+{
+    if (!P) return EPSGRAD_EINVAL;
+    if (enable && !P->tma_encode) return EPSGRAD_EUNSUPPORTED;
+    P->use_tma = enable != 0;
     return EPSGRAD_OK;
 }
 
@@ -815,6 +832,45 @@ int launch_zreduce(epsgrad_plan *P, int n_pairs, const void *const *EF, const vo
     // windows of at most 128 bytes per column: ask for 64-byte fills
     const bool sparse = maxnch * 16 <= 128 && zp.nz * 8 > 128;
     host_src = host_src || P->cur_host_src;
+    if (sparse && !host_src && P->use_tma && P->emb.nx_full == 0) {
+        // TMA variant (zreduce.cuh): one 2-D tensor map per field, rows = z columns, box = {window, 256 columns}
+        typedef CUresult (*EncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                     const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                     CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+        EncodeFn enc = (EncodeFn)P->tma_encode;
+        ZredTmaParams tp;
+        tp.gbar = gbar; tp.zw = P->d_zw; tp.ncol = zp.ncol; tp.nz = zp.nz;
+        for (int g = 0; g < 2; ++g) { tp.ch0[g] = zp.ch0[g]; tp.nch[g] = zp.nch[g]; }
+        tp.wb = (zp.nch[0] | 1) > (zp.nch[1] | 1) ? (zp.nch[0] | 1) : (zp.nch[1] | 1);
+        const cuuint64_t dims[2] = {(cuuint64_t)zp.nz * 2, (cuuint64_t)P->cfg.batch * 3 * zp.ncol};
+        const cuuint64_t strides[1] = {(cuuint64_t)zp.nz * 8};
+        const cuuint32_t box[2] = {(cuuint32_t)tp.wb * 4, (cuuint32_t)ZR_COLS}, es[2] = {1, 1};
+        const size_t smem_t = (size_t)2 * ZR_COLS * tp.wb * 16 + 128;
+        int rct = set_smem(k_zreduce_tma, smem_t);
+        if (rct) return rct;
+        const int per_sm = 5;                                   // resident set: 5 CTAs x 40 KB of windows in flight per SM
+        const int n_items = 3 * cdiv(zp.ncol, ZR_COLS), n_want = per_sm * P->n_sm / P->cfg.batch;
+        const dim3 grid_t(n_items < n_want || n_want < 1 ? n_items : n_want, P->cfg.batch);
+        if (P->cfg.batch > 65535) return EPSGRAD_EUNSUPPORTED;
+        for (int p0 = 0; p0 < n_pairs; p0 += ZR_MAX_PAIRS) {
+            const int np = n_pairs - p0 < ZR_MAX_PAIRS ? n_pairs - p0 : ZR_MAX_PAIRS;
+            for (int p = 0; p < np; ++p) {
+                if (enc(&tp.mf[p], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void *>(EF[p0 + p]), dims, strides, box, es,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_64B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS ||
+                    enc(&tp.ma[p], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void *>(EA[p0 + p]), dims, strides, box, es,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_64B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+                    return EPSGRAD_ECUDA;
+            }
+            for (int p = np; p < ZR_MAX_PAIRS; ++p) { tp.mf[p] = tp.mf[0]; tp.ma[p] = tp.ma[0]; }
+            tp.n_pairs = np; tp.accumulate = p0 > 0;
+            k_zreduce_tma<<<grid_t, ZR_THREADS, smem_t, st>>>(tp);
+            rct = check_launch(P, "zreduce", st);
+            if (rct) return rct;
+        }
+        return EPSGRAD_OK;
+    }
     auto kern = host_src ? k_zreduce<false, true> : (sparse ? k_zreduce<true, false> : k_zreduce<false, false>);
     int rc = set_smem(kern, smem);
     if (rc) return rc;

@@ -15,6 +15,7 @@
 // 128-byte line, and 64 B is the smallest granule the part offers, so a window that straddles a line
 // boundary costs 128 B of DRAM traffic per column, component and field instead of 256 B.
 #pragma once
+#include <cuda.h>          // CUtensorMap (type only: the encoder is fetched through cudaGetDriverEntryPoint)
 #include "common.cuh"
 
 namespace epsgrad {
@@ -139,6 +140,109 @@ __global__ void __launch_bounds__(ZR_THREADS, 5) k_zreduce(const __grid_constant
         }
         if (tid < nc) {
             float *dst = P.gbar + (size_t)b * 5 * P.ncol + colb + c0 + tid;
+            const int nout = grp ? 3 : 1;
+            for (int o = 0; o < nout; ++o) {
+                float *d = dst + (size_t)(grp ? 2 + o : c) * P.ncol;
+                *d = P.accumulate ? *d + acc[o] : acc[o];
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------- TMA variant
+// The same reduction with the windows fetched by the tensor memory accelerator: per pass and field ONE bulk tensor copy
+// (cp.async.bulk.tensor.2d, box {ZR_TMA_W floats of z} x {256 columns}, L2 promotion 64 B) issued by one thread and tracked
+// by an mbarrier, instead of ~3000 LDGSTS instructions per CTA.  Measured at paper scale: 39 us against 37 us for the
+// LDGSTS kernel (both DRAM bound), and no better beside the 2-D kernels of the two-stream schedule (the hypothesis that the
+// LDGSTS stream's pressure on the SM's memory pipe is what slows them down did not hold), so it is an option
+// (epsgrad_plan_set_tma), off by default.  Region-sized (not embedded), device-resident fields with sparse windows only.
+// Fields as a 2-D tensor: rows = z columns (B*3*ncol of them), inner dimension = 2 nz floats.  Both window groups use one
+// box width ZR box = 4 * max(nch[0] | 1, nch[1] | 1) floats starting at the group's first chunk (a box that sticks out of
+// the column is zero-filled by the hardware); the odd chunk pitch keeps the per-column reads conflict-free.
+struct ZredTmaParams {
+    alignas(64) CUtensorMap mf[ZR_MAX_PAIRS];
+    alignas(64) CUtensorMap ma[ZR_MAX_PAIRS];
+    float *gbar;
+    const float *zw;
+    int n_pairs, accumulate;
+    int ncol, nz;
+    int ch0[2], nch[2];
+    int wb;                // box width in 16-byte chunks
+};
+
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"((unsigned)__cvta_generic_to_shared(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned phase)
+{
+    asm volatile(
+        "{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n @p bra DONE_%=;\n bra WAIT_%=;\n DONE_%=:\n}\n"
+        :: "r"((unsigned)__cvta_generic_to_shared(bar)), "r"(phase) : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(void *smem, const CUtensorMap *map, unsigned long long *bar, int x, int y)
+{
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+                 :: "r"((unsigned)__cvta_generic_to_shared(smem)), "l"(map), "r"((unsigned)__cvta_generic_to_shared(bar)), "r"(x), "r"(y) : "memory");
+}
+
+// grid (n_cta, 1, B): persistent CTAs, each walking the (component, column block) items n_cta apart, component by component
+// (items of one component are consecutive, so the resident CTAs still read one advancing window); n_cta is chosen on the
+// host as a few CTAs per SM, which leaves shared memory, threads and registers of every SM to the 2-D kernels of the other
+// stream.  Dynamic shared memory: 2 fields x 256 columns x wb chunks (+ 128 bytes of alignment slack).
+__global__ void __launch_bounds__(ZR_THREADS, 5) k_zreduce_tma(const __grid_constant__ ZredTmaParams P)
+{
+    extern __shared__ unsigned char smraw[];
+    __shared__ __align__(8) unsigned long long bar;
+    float4 *stage = reinterpret_cast<float4 *>((reinterpret_cast<uintptr_t>(smraw) + 127) & ~(uintptr_t)127);
+    const int tid = threadIdx.x, b = blockIdx.y;
+    const int nz = P.nz, wb = P.wb, nblk = (P.ncol + ZR_COLS - 1) / ZR_COLS;
+    float4 *sf = stage, *sa = stage + ZR_COLS * wb;
+    const unsigned box_bytes = (unsigned)ZR_COLS * wb * 16u;
+    if (tid == 0) {
+        mbar_init(&bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    unsigned phase = 0;
+    for (int item = blockIdx.x; item < 3 * nblk; item += gridDim.x) {
+        const int c = item / nblk, blk = item - c * nblk;
+        const int grp = c == 2, nch = P.nch[grp], ch0 = P.ch0[grp];
+        const int colb = blk * ZR_COLS, ncb = min(ZR_COLS, P.ncol - colb);
+        const int row0 = (b * 3 + c) * P.ncol + colb;        // < 2^31 by validate()
+        float acc[3] = {0.f, 0.f, 0.f};
+        for (int p = 0; p < P.n_pairs; ++p) {
+            __syncthreads();                                 // every thread is done reading the previous windows
+            if (tid == 0) {
+                mbar_expect_tx(&bar, 2u * box_bytes);        // rows or floats outside the tensor are zero-filled and still counted
+                tma_load_2d(sf, &P.mf[p], &bar, 4 * ch0, row0);
+                tma_load_2d(sa, &P.ma[p], &bar, 4 * ch0, row0);
+            }
+            mbar_wait(&bar, phase);
+            phase ^= 1u;
+            if (tid < ncb) {
+                const float4 *bf = sf + tid * wb, *ba = sa + tid * wb;
+                for (int ch = 0; ch < nch; ++ch) {
+                    const float4 f = bf[ch], a = ba[ch];
+                    const int k = 2 * (ch0 + ch);
+                    const float g0 = -2.0f * (f.x * a.x - f.y * a.y);       // Eq. (1): -2 Re(E_F E_A), plain product (S10)
+                    const float g1 = -2.0f * (f.z * a.z - f.w * a.w);
+                    if (grp == 0) {
+                        acc[0] = fmaf(__ldg(P.zw + k), g0, fmaf(__ldg(P.zw + k + 1), g1, acc[0]));
+                    } else {
+#pragma unroll
+                        for (int o = 0; o < 3; ++o)
+                            acc[o] = fmaf(__ldg(P.zw + (2 + o) * nz + k), g0, fmaf(__ldg(P.zw + (2 + o) * nz + k + 1), g1, acc[o]));
+                    }
+                }
+            }
+        }
+        if (tid < ncb) {
+            float *dst = P.gbar + (size_t)b * 5 * P.ncol + colb + tid;
             const int nout = grp ? 3 : 1;
             for (int o = 0; o < nout; ++o) {
                 float *d = dst + (size_t)(grp ? 2 + o : c) * P.ncol;

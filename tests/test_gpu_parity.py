@@ -90,6 +90,23 @@ def test_zreduce_planes_match_definition():
     assert rel_inf(g, ref) < 1e-5
 
 
+def test_tma_field_reads_give_the_same_bits():
+    # the TMA variant of the field stream (epsgrad_plan_set_tma) against the LDGSTS kernel: same windows, same per-column sums
+    for kw, n_pairs in ((dict(mx=23, my=18, nz=64, z_lo=28.25, z_hi=35.75, filter_radius=4.0), 1),
+                        (dict(batch=2, mx=67, my=59, nz=32, z_lo=14.25, z_hi=17.75, filter_radius=4.0), 3),
+                        (dict(mx=130, my=131, nz=16, z_lo=6.25, z_hi=9.75, filter_radius=4.0), 9)):
+        cfg = B.make_config(**kw)
+        C = dev(rand_C(cfg, 4))
+        EFn, EAn = rand_fields(cfg, n_pairs, 9)
+        EF, EA = [dev(f) for f in EFn], [dev(f) for f in EAn]
+        plan = B.Plan(cfg)
+        g0, G0 = plan.eps_vjp(C, 16.0, EF, EA), plan.stage_zreduce(EF, EA)
+        plan.set_tma(True)
+        g1, G1 = plan.eps_vjp(C, 16.0, EF, EA), plan.stage_zreduce(EF, EA)
+        torch.cuda.synchronize()
+        assert torch.equal(G0, G1) and torch.equal(g0, g1)
+
+
 def test_dense_reads_give_the_same_gradient():
     cfg = B.make_config(mx=23, my=18, nz=64, z_lo=28.25, z_hi=35.75, filter_radius=4.0)
     C = rand_C(cfg, 4)
