@@ -200,6 +200,29 @@ def test_calls_are_cuda_graph_capturable():
         assert torch.equal(eps, eps_ref) and torch.equal(g, g_ref)
 
 
+@pytest.mark.parametrize("z", [
+    (3.2, 3.6),        # slab inside one cell: no full E_x/E_y cell, two fractional E_z cells
+    (0.0, 8.0),        # slab = the whole grid: every cell full, no face inside the grid for E_x/E_y
+    (-1.0, 2.5),       # sticks out below: clipped at the grid
+    (6.3, 11.0),       # sticks out above
+    (3.0, 5.0),        # faces on cell boundaries: no fractional E_x/E_y cell, two half-filled E_z cells
+    (9.0, 10.0),       # entirely outside the grid: eps = eps_clad, dF/dC = 0
+])
+def test_degenerate_slabs(z):
+    cfg = B.make_config(mx=14, my=11, nz=8, z_lo=z[0], z_hi=z[1], filter_radius=3.0)
+    C = rand_C(cfg, 71)
+    EF, EA = rand_fields(cfg, 2, 72)
+    plan = B.Plan(cfg)
+    check_forward(cfg, C, 8.0, plan)
+    g = plan.eps_vjp(dev(C), 8.0, [dev(f) for f in EF], [dev(f) for f in EA]).cpu().numpy().astype(np.float64)
+    ref = O.vjp(oracle_cfg(cfg), C[0], 8.0, [f[0] for f in EF], [f[0] for f in EA])
+    if z[0] >= cfg.nz:
+        assert np.all(ref == 0.0) and np.all(g == 0.0)
+        assert np.all(plan.eps_forward(dev(C), 8.0).cpu().numpy() == np.float32(cfg.eps_clad))
+    else:
+        assert rel_inf(g[0], ref) < TOL_GRAD and rel_l2(g[0], ref) < TOL_GRAD
+
+
 def test_real_cotangent_special_case():
     # VJP with an arbitrary (real) field w: E_F = -w/2, E_A = 1
     cfg = B.make_config(mx=12, my=14, nz=8, z_lo=2.25, z_hi=5.75, filter_radius=3.0)
