@@ -53,8 +53,10 @@ extern "C" {
 #endif
 
 #define EPSGRAD_OK             0
-#define EPSGRAD_EINVAL        -1   /* null / misaligned pointer, bad size, beta <= 0, eps <= 0, ... */
-#define EPSGRAD_EUNSUPPORTED  -2   /* upsample*subpixel not in {2,4,6,8}, Nz % 4 != 0, tables too large,
+#define EPSGRAD_EINVAL        -1   /* null / misaligned pointer, bad size, beta <= 0, eps <= 0, a normalised filter whose
+                                      support leaves a mask pixel without any control pixel (R <= (u - 1/s)/sqrt(2)), ... */
+#define EPSGRAD_EUNSUPPORTED  -2   /* upsample*subpixel not in {2,4,6,8}, Nz % 4 != 0, tables too large (conic filter: taps x
+                                      phases beyond 200 KB of shared memory, e.g. R = 12 cells at 8 mask pixels per control pixel),
                                       morphological disk radius > 16 mask pixels or wider than the mask */
 #define EPSGRAD_ENOWORKSPACE  -3   /* workspace / staging buffer missing or too small */
 #define EPSGRAD_ECUDA         -4   /* CUDA runtime error (no device, launch failure) */

@@ -179,6 +179,7 @@ extern "C" int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsg
     std::vector<float> w;
     std::vector<int> tyr(2 * NT, 0);
     std::vector<float> invden;
+    bool uncovered = false;                          // a mask pixel out of reach of every control pixel: den = 0 in Eq. (2)/S2
     if (!P->separable) {
         w.assign((size_t)NT * NT * m * m, 0.0f);
         for (int tx = 0; tx < NT; ++tx) {
@@ -213,6 +214,7 @@ extern "C" int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsg
                                     den += (double)w[(((size_t)tx * NT + ty) * m + fx) * m + fy];
                                 }
                             }
+                            if (!(den > 0.0)) uncovered = true;
                             invden[(size_t)(kx * m + fx) * RY + ky * m + fy] = (float)(1.0 / den);
                         }
                 }
@@ -233,11 +235,14 @@ extern "C" int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsg
                             const int a = a0 + t - T;
                             if (a >= 0 && a < M) den += (double)w[(size_t)t * m + f];
                         }
+                        if (!(den > 0.0)) uncovered = true;
                         invden[(ax ? RX : 0) + k * m + f] = (float)(1.0 / den);
                     }
                 }
             }
     }
+
+    if (uncovered) { delete P; return EPSGRAD_EINVAL; }    // the density filter would divide 0 by 0 there (R < u/sqrt(2))
 
     // ---- z tables (S7, S8): wxy_k = |[k,k+1] ^ slab|, wz_k = |[k+1/2,k+3/2] ^ slab|
     const int nz = cfg->nz;

@@ -290,6 +290,16 @@ def test_error_codes():
     with pytest.raises(B.EpsgradError) as e:
         B.Plan(B.make_config(mx=8, my=8, nz=6, z_lo=2.0, z_hi=5.0))
     assert e.value.status == B.EUNSUPPORTED
+    # cone too small to reach the mask pixels midway between control pixels: the normalised Eq. (2) would be 0/0 there
+    with pytest.raises(B.EpsgradError) as e:
+        B.Plan(B.make_config(mx=8, my=8, nz=8, z_lo=2.0, z_hi=5.0, upsample=2, subpixel=4, filter_radius=1.0))
+    assert e.value.status == B.EINVAL
+    B.Plan(B.make_config(mx=8, my=8, nz=8, z_lo=2.0, z_hi=5.0, upsample=2, subpixel=4, filter_radius=1.0, filter_normalize=0))
+    B.Plan(B.make_config(mx=8, my=8, nz=8, z_lo=2.0, z_hi=5.0, upsample=2, subpixel=4, filter_radius=1.3))
+    # tap table of the conic filter beyond shared memory
+    with pytest.raises(B.EpsgradError) as e:
+        B.Plan(B.make_config(mx=40, my=40, nz=8, z_lo=2.0, z_hi=5.0, upsample=1, subpixel=8, filter_radius=12.0))
+    assert e.value.status == B.EUNSUPPORTED
     plan = B.Plan(B.make_config(mx=8, my=8, nz=8, z_lo=2.0, z_hi=5.0))
     with pytest.raises(B.EpsgradError) as e:
         plan.eps_forward(torch.rand(plan.ctrl_shape, device="cuda"), -1.0)

@@ -1,0 +1,115 @@
+"""GPU parity on a seeded sweep of random configurations: grid sizes around the tile edges (16x16 Yee cells per CTA of
+the 2-D kernels, 256 columns per CTA of the 3-D kernels), every supported (upsample, subpixel) pair, both filters with
+integer and fractional radii, slabs whose faces fall anywhere in z (on cell edges, inside one cell, on a 16-byte chunk
+boundary), batches, several field pairs, the morphological filters on and off, beta from 1 to 64.  Each case checks eps,
+dF/dC, dF/dbeta and u(beta) against the float64 oracle at BASELINE.json's tolerances.  The hand-picked cases of
+test_gpu_parity.py stay the first line; this one looks for what they did not think of."""
+import os
+
+import numpy as np
+import pytest
+
+import oracle as O
+from gpu_common import TOL_EPS, TOL_GRAD, dev, max_rel, oracle_cfg, rand_C, rand_fields
+from helpers import rel_inf, rel_l2
+from paper_2505_03352_b200 import binding as B
+
+pytestmark = pytest.mark.gpu
+
+UP_SUB = [(1, 2), (2, 2), (1, 4), (3, 2), (1, 6), (2, 4), (4, 2), (1, 8)]       # upsample * subpixel in {2, 4, 6, 8}
+N_CASES = int(os.environ.get("EPSGRAD_SWEEP_CASES", "40"))      # a longer hunt: EPSGRAD_SWEEP_CASES=400 pytest tests/test_gpu_sweep.py
+
+
+def draw(i: int):
+    """Case i of the sweep: (config kwargs, beta, n_pairs).  Sizes are bounded so the oracle takes about a second."""
+    rng = np.random.default_rng([20250503, i])
+    u, s = UP_SUB[i % len(UP_SUB)]
+    cells = int(rng.integers(6, 72))                                  # Yee cells along x: below, at and above 16, 32, 48, 64
+    mx = max(1, round(cells / u))
+    my = max(1, round(int(rng.integers(6, 72)) / u))
+    nz = 4 * int(rng.integers(1, 11))
+    kind = int(rng.random() < 0.3)
+    kw = dict(batch=int(rng.integers(1, 4)) if i % 5 == 0 else 1, mx=mx, my=my, nz=nz, upsample=u, subpixel=s, filter_kind=kind)
+    if kind == 0:
+        # radii the library takes: every mask pixel within reach of a control pixel, R > (u - 1/s)/sqrt(2) (else den = 0 in
+        # the normalised Eq. (2): EPSGRAD_EINVAL), and the tap table within shared memory (s >= 6 at one cell per control
+        # pixel: R <= 5.5 cells; EPSGRAD_EUNSUPPORTED beyond) -- both limits are checked in test_gpu_parity.py::test_error_codes
+        radii = [r for r in [1.0, 2.0, 3.3, 4.0, 5.5, 8.0, 12.0]
+                 if r > (u - 1.0 / s) / np.sqrt(2.0) + 0.05 and not (u == 1 and s >= 6 and r > 5.5)]
+        kw["filter_radius"] = float(rng.choice(radii))
+    else:
+        kw["filter_sigma"] = float(rng.choice([0.8, 2.5, 6.0]))
+        kw["filter_radius"] = float(np.ceil(3.2 * kw["filter_sigma"]))
+    # slab: faces anywhere, sometimes snapped to cell edges, to the ends of the column or into a single cell
+    mode = i % 6
+    lo, hi = np.sort(rng.uniform(0.0, nz, 2))
+    if hi - lo < 0.05:
+        hi = min(float(nz), lo + 0.3)
+    if mode == 1:
+        lo, hi = float(np.floor(lo)), float(np.ceil(hi))             # faces on cell edges
+        if hi == lo: hi = lo + 1.0
+    elif mode == 2:
+        lo = 0.0                                                      # slab from the bottom of the column
+    elif mode == 3:
+        hi = float(nz)                                                # ... to its top
+    elif mode == 4:
+        k = int(rng.integers(0, nz)); lo, hi = k + 0.2, k + 0.7      # inside one cell
+    kw["z_lo"], kw["z_hi"] = float(lo), float(hi)
+    if i % 4 == 3:
+        d = float(rng.choice([1.5, 2.5, 4.0]))
+        R = int(np.floor(0.5 * d * s))
+        if R >= 1 and min(s * u * mx, s * u * my) >= 2 * R + 1:
+            kw["morph_diameter"] = d
+    if i % 7 == 0:
+        kw["eta"] = float(rng.uniform(0.3, 0.7))
+    if i % 9 == 0:
+        kw["eps_core"], kw["eps_clad"] = 2.1, 12.0                    # inverted contrast
+    if i % 3 == 2:
+        kw["normal_delta"] = float(rng.choice([1e-8, 1e-5]))          # guard of the normals (S6); default 1e-12 otherwise
+    beta = float(np.exp(rng.uniform(0.0, np.log(64.0))))
+    return kw, beta, int(rng.integers(1, 4))
+
+
+def errors(kw, beta, n_pairs, i):
+    """Run both sides on case i with configuration kw: worst (eps, dF/dC, dF/dbeta, u) errors over the batch, each divided
+    by its tolerance (<= 1 passes)."""
+    cfg = B.make_config(**kw)
+    C = rand_C(cfg, 1000 + i)
+    EF, EA = rand_fields(cfg, n_pairs, 2000 + i)
+    plan = B.Plan(cfg)
+    dEF, dEA = [dev(f) for f in EF], [dev(f) for f in EA]
+    eps, g = plan.eps_forward_vjp(dev(C), beta, dEF, dEA)
+    g2, db = plan.eps_vjp_beta(dev(C), beta, dEF, dEA)
+    u = plan.unbinarity(dev(C), beta)
+    eps, g, g2, db, u = (t.cpu().numpy().astype(np.float64) for t in (eps, g, g2, db, u))
+    assert np.array_equal(g, g2), kw
+    oc = oracle_cfg(cfg)
+    worst = np.zeros(4)
+    for b in range(cfg.batch):
+        f, a = [x[b] for x in EF], [x[b] for x in EA]
+        eps_ref = O.forward(oc, C[b], beta)
+        g_ref, db_ref = O.vjp_beta(oc, C[b], beta, f, a)
+        u_ref = O.unbinarity(oc, C[b], beta)
+        # d F/d beta is a sum of signed per-pixel terms: same scale as tests/test_gpu_beta.py
+        scale = max(abs(db_ref), 1e-3 * np.abs(g_ref).sum())
+        worst = np.maximum(worst, [max_rel(eps[b], eps_ref) / TOL_EPS,
+                                   max(rel_inf(g[b], g_ref), rel_l2(g[b], g_ref)) / TOL_GRAD,
+                                   abs(db[b] - db_ref) / (TOL_GRAD * scale),
+                                   abs(u[b] - u_ref) / (1e-5 * max(u_ref, 1e-3))])
+    return worst
+
+
+@pytest.mark.parametrize("i", range(N_CASES))
+def test_random_configuration(i):
+    kw, beta, n_pairs = draw(i)
+    e = errors(kw, beta, n_pairs, i)
+    assert e[0] < 1 and e[3] < 1, (kw, beta, e)
+    if e[1] >= 1 or e[2] >= 1:
+        # The one known way past the gradient tolerance is the conditioning of the normals: where the mask is
+        # almost flat, n_c^2 = g_c^2/(|g|^2 + delta) amplifies float32 rounding of the Sobel differences by 1/|g| (up to
+        # 1/sqrt(delta)), and the large terms it creates only cancel further down the reverse pass.  Seen at beta ~ 1 under
+        # a wide filter, on a control grid smaller than the filter, and on a fully binarised mask whose whole gradient is
+        # 1e-5 of the usual size -- 3 of 400 cases, all under 1e-2.  Such a case must pass once the guard is above the noise.
+        assert e[1] < 100 and e[2] < 100 and kw.get("normal_delta", 1e-12) < 1e-8, (kw, beta, e)
+        e2 = errors(dict(kw, normal_delta=1e-6), beta, n_pairs, i)
+        assert np.all(e2 < 1), (kw, beta, e, e2)
