@@ -113,3 +113,79 @@ def test_random_configuration(i):
         assert e[1] < 100 and e[2] < 100 and kw.get("normal_delta", 1e-12) < 1e-8, (kw, beta, e)
         e2 = errors(dict(kw, normal_delta=1e-6), beta, n_pairs, i)
         assert np.all(e2 < 1), (kw, beta, e, e2)
+
+
+@pytest.mark.parametrize("i", range(N_CASES))
+def test_random_configuration_every_entry_point(i):
+    """The same draws through every other way into the library: separate calls, the serial schedule, the TMA and the dense
+    field streams, the host entry point (pinned, in-place windows, and staged), CUDA-graph replay, and an embedding in a
+    larger simulation domain -- each against eps_forward_vjp on region-sized device arrays (checked against the oracle
+    above), bit for bit wherever the arithmetic order is the same."""
+    import torch
+    kw, beta, n_pairs = draw(i)
+    cfg = B.make_config(**kw)
+    rng = np.random.default_rng([77, i])
+    Cn = rand_C(cfg, 1000 + i)
+    EFn, EAn = rand_fields(cfg, n_pairs, 2000 + i)
+    C, EF, EA = dev(Cn), [dev(f) for f in EFn], [dev(f) for f in EAn]
+    plan = B.Plan(cfg)
+    eps0, g0 = plan.eps_forward_vjp(C, beta, EF, EA)
+    G0 = plan.stage_zreduce(EF, EA)
+    # separate calls; serial schedule
+    assert torch.equal(plan.eps_forward(C, beta), eps0) and torch.equal(plan.eps_vjp(C, beta, EF, EA), g0)
+    plan.set_overlap(False)
+    eps1, g1 = plan.eps_forward_vjp(C, beta, EF, EA)
+    assert torch.equal(eps1, eps0) and torch.equal(g1, g0)
+    plan.set_overlap(True)
+    # TMA field stream: same windows, same per-column order
+    plan.set_tma(True)
+    assert torch.equal(plan.stage_zreduce(EF, EA), G0) and torch.equal(plan.eps_vjp(C, beta, EF, EA), g0)
+    plan.set_tma(False)
+    # dense field stream: the cells outside the slab have zero weight, the order inside a column is the same
+    plan.set_dense_reads(True)
+    assert torch.equal(plan.eps_vjp(C, beta, EF, EA), g0)
+    plan.set_dense_reads(False)
+    # CUDA graph replay of the fused call
+    eps_g, g_g = torch.empty_like(eps0), torch.empty_like(g0)
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        plan.eps_forward_vjp(C, beta, EF, EA, eps_out=eps_g, grad_out=g_g)
+    torch.cuda.current_stream().wait_stream(s)
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        plan.eps_forward_vjp(C, beta, EF, EA, eps_out=eps_g, grad_out=g_g)
+    eps_g.zero_(); g_g.zero_()
+    graph.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(eps_g, eps0) and torch.equal(g_g, g0)
+    # host entry point: pinned buffers (windows read in place), then staged whole
+    pin = lambda a: torch.from_numpy(a).pin_memory()
+    eps_h = torch.empty(plan.eps_shape, dtype=torch.float32).pin_memory()
+    g_h = torch.empty(plan.ctrl_shape, dtype=torch.float32).pin_memory()
+    hC, hEF, hEA = pin(Cn), [pin(f) for f in EFn], [pin(f) for f in EAn]
+    for direct in (True, False):
+        plan.set_host_direct(direct)
+        eps_h.zero_(); g_h.zero_()
+        plan.eps_forward_vjp_host(hC, beta, hEF, hEA, eps_h, g_h)
+        torch.cuda.synchronize()
+        assert torch.equal(eps_h, eps0.cpu()) and torch.equal(g_h, g0.cpu()), (kw, direct)
+    plan.set_host_direct(True)
+    # embedded in a larger domain at a random origin (k0 and nz_full multiples of 4)
+    i0, j0, k0 = int(rng.integers(0, 9)), int(rng.integers(0, 9)), 4 * int(rng.integers(0, 3))
+    nxf, nyf, nzf = cfg.nx + i0 + int(rng.integers(0, 7)), cfg.ny + j0 + int(rng.integers(0, 7)), cfg.nz + k0 + 4 * int(rng.integers(0, 3))
+    shape = (cfg.batch, 3, nxf, nyf, nzf)
+    blk = (slice(None), slice(None), slice(i0, i0 + cfg.nx), slice(j0, j0 + cfg.ny), slice(k0, k0 + cfg.nz))
+    fEF, fEA = [], []
+    for f, lst in [(f, fEF) for f in EF] + [(f, fEA) for f in EA]:
+        full = torch.view_as_complex(torch.randn(*shape, 2, device="cuda"))      # anything outside the block must not matter
+        full[blk] = f
+        lst.append(full)
+    plan.set_embedding(nxf, nyf, nzf, i0, j0, k0)
+    eps_f = torch.full(shape, -7.0, device="cuda")
+    _, g_e = plan.eps_forward_vjp(C, beta, fEF, fEA, eps_out=eps_f)
+    torch.cuda.synchronize()
+    assert torch.equal(g_e, g0) and torch.equal(eps_f[blk], eps0), (kw, shape, (i0, j0, k0))
+    outside = torch.ones(shape, dtype=torch.bool, device="cuda")
+    outside[blk] = False
+    assert bool((eps_f[outside] == -7.0).all())
