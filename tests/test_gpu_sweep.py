@@ -72,7 +72,11 @@ def draw(i: int):
 
 def errors(kw, beta, n_pairs, i):
     """Run both sides on case i with configuration kw: worst (eps, dF/dC, dF/dbeta, u) errors over the batch, each divided
-    by its tolerance (<= 1 passes)."""
+    by its tolerance (<= 1 passes).  The tolerances are BASELINE.json's up to beta = 17 and grow with beta beyond: float32
+    leaves delta Phi ~ 4 roundings at |Phi'| <= 1/2 = 2.4e-7 on the filter output, the projection turns it into
+    delta eps/eps <= (|eps_core - eps_clad|/eps_min) (beta/2) delta Phi = 5.8e-7 beta for Si/SiO2, which is
+    1e-5 at beta = 17.  (The BASELINE configs stay at 7e-7 even at beta = 64: their filters average 200 control pixels and
+    |Phi'| is ten times smaller; a filter of radius 1 does not smooth at all.)"""
     cfg = B.make_config(**kw)
     C = rand_C(cfg, 1000 + i)
     EF, EA = rand_fields(cfg, n_pairs, 2000 + i)
@@ -84,6 +88,7 @@ def errors(kw, beta, n_pairs, i):
     eps, g, g2, db, u = (t.cpu().numpy().astype(np.float64) for t in (eps, g, g2, db, u))
     assert np.array_equal(g, g2), kw
     oc = oracle_cfg(cfg)
+    amp = max(1.0, beta / 17.0)
     worst = np.zeros(4)
     for b in range(cfg.batch):
         f, a = [x[b] for x in EF], [x[b] for x in EA]
@@ -92,25 +97,31 @@ def errors(kw, beta, n_pairs, i):
         u_ref = O.unbinarity(oc, C[b], beta)
         # d F/d beta is a sum of signed per-pixel terms: same scale as tests/test_gpu_beta.py
         scale = max(abs(db_ref), 1e-3 * np.abs(g_ref).sum())
-        worst = np.maximum(worst, [max_rel(eps[b], eps_ref) / TOL_EPS,
-                                   max(rel_inf(g[b], g_ref), rel_l2(g[b], g_ref)) / TOL_GRAD,
-                                   abs(db[b] - db_ref) / (TOL_GRAD * scale),
+        worst = np.maximum(worst, [max_rel(eps[b], eps_ref) / (TOL_EPS * amp),
+                                   max(rel_inf(g[b], g_ref), rel_l2(g[b], g_ref)) / (TOL_GRAD * amp),
+                                   abs(db[b] - db_ref) / (TOL_GRAD * amp * scale),
                                    abs(u[b] - u_ref) / (1e-5 * max(u_ref, 1e-3))])
     return worst
 
 
-@pytest.mark.parametrize("i", range(N_CASES))
+# the cases of the 1300-case hunt that needed the rules below always run
+HARD = [183, 214, 239, 547, 1092, 1239]
+
+
+@pytest.mark.parametrize("i", list(range(N_CASES)) + [i for i in HARD if i >= N_CASES])
 def test_random_configuration(i):
     kw, beta, n_pairs = draw(i)
     e = errors(kw, beta, n_pairs, i)
-    assert e[0] < 1 and e[3] < 1, (kw, beta, e)
-    if e[1] >= 1 or e[2] >= 1:
-        # The one known way past the gradient tolerance is the conditioning of the normals: where the mask is
-        # almost flat, n_c^2 = g_c^2/(|g|^2 + delta) amplifies float32 rounding of the Sobel differences by 1/|g| (up to
-        # 1/sqrt(delta)), and the large terms it creates only cancel further down the reverse pass.  Seen at beta ~ 1 under
-        # a wide filter, on a control grid smaller than the filter, and on a fully binarised mask whose whole gradient is
-        # 1e-5 of the usual size -- 3 of 400 cases, all under 1e-2.  Such a case must pass once the guard is above the noise.
-        assert e[1] < 100 and e[2] < 100 and kw.get("normal_delta", 1e-12) < 1e-8, (kw, beta, e)
+    assert e[3] < 1, (kw, beta, e)
+    if np.any(e[:3] >= 1):
+        # The one known way past the tolerances is the conditioning of the normals: where the mask is flat
+        # to float32 rounding, n_c^2 = g_c^2/(|g|^2 + delta) turns the rounding noise of the Sobel differences (noise^2 ~
+        # 1e-14 against the default delta = 1e-12) into an error of n^2, and its derivative, ~ 1/|g|, into large terms of the
+        # reverse pass that only cancel further down.  Seen in 6 of 1300 cases: gray plateaus left by the morphological
+        # filters (eps off by 1.4e-4), beta ~ 1 under a wide filter, a control grid smaller than the filter, and fully
+        # binarised masks whose whole gradient is 1e-5 ... 1e-10 of the usual size.  Such a case must pass once the guard is
+        # well above the noise.
+        assert kw.get("normal_delta", 1e-12) < 1e-8, (kw, beta, e)
         e2 = errors(dict(kw, normal_delta=1e-6), beta, n_pairs, i)
         assert np.all(e2 < 1), (kw, beta, e, e2)
 
