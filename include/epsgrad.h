@@ -153,7 +153,9 @@ int eps_forward(epsgrad_plan_t *plan, const float *C, float beta, float *eps, vo
 
 /* Eq. (1): dFdC = -2 Re((d eps/dC)^T (E_F (.) E_A)) summed over n_pairs >= 1
  * pairs.  EF, EA: HOST arrays of n_pairs DEVICE pointers to complex64 [B,3,Nx,Ny,Nz].
- * A real cotangent w can be fed as E_F = -w/2 + 0i, E_A = 1 + 0i.               */
+ * A real cotangent w can be fed as E_F = -w/2 + 0i, E_A = 1 + 0i.
+ * Limit: the z window of the field reads (the slab's cells; the whole column for dense
+ * plans) must not exceed 512 cells, else EPSGRAD_EUNSUPPORTED.                         */
 int eps_vjp(epsgrad_plan_t *plan, const float *C, float beta, int n_pairs,
             const void *const *EF, const void *const *EA, float *dFdC, void *stream);
 

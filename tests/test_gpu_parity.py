@@ -36,6 +36,13 @@ CASES = {
     "slab_fills_z": (dict(mx=18, my=18, nz=8, z_lo=0.0, z_hi=8.0, filter_radius=3.0), 8.0),
     "slab_half_cell_faces": (dict(mx=18, my=18, nz=8, z_lo=2.5, z_hi=5.5, filter_radius=3.0), 8.0),
     "batch3": (dict(batch=3, mx=21, my=19, nz=8, z_lo=2.25, z_hi=5.75, filter_radius=3.0), 8.0),
+    # tall columns: a window of 256 chunks per column (4 columns per pass of the field stream), a thin slab far up a column
+    # longer than a CTA of the store stream, a column length that no power of two divides; long thin regions
+    "tall_full_slab": (dict(mx=9, my=7, nz=512, z_lo=0.0, z_hi=512.0, filter_radius=3.0), 9.0),
+    "tall_thin_slab": (dict(mx=9, my=7, nz=2048, z_lo=1000.25, z_hi=1007.75, filter_radius=3.0), 9.0),
+    "nz36": (dict(mx=9, my=7, nz=36, z_lo=3.5, z_hi=30.0, filter_radius=3.0), 9.0),
+    "long_in_x": (dict(mx=300, my=3, nz=12, z_lo=3.5, z_hi=10.0, filter_radius=3.0), 9.0),
+    "long_in_y": (dict(mx=3, my=700, nz=12, z_lo=3.5, z_hi=10.0, filter_radius=3.0), 9.0),
 }
 
 
@@ -299,6 +306,13 @@ def test_error_codes():
     # tap table of the conic filter beyond shared memory
     with pytest.raises(B.EpsgradError) as e:
         B.Plan(B.make_config(mx=40, my=40, nz=8, z_lo=2.0, z_hi=5.0, upsample=1, subpixel=8, filter_radius=12.0))
+    assert e.value.status == B.EUNSUPPORTED
+    # field window wider than 512 cells: the forward call works, the reverse pass says so
+    plan = B.Plan(B.make_config(mx=4, my=4, nz=1024, z_lo=3.5, z_hi=1000.0))
+    plan.eps_forward(torch.rand(plan.ctrl_shape, device="cuda"), 8.0)
+    f = torch.zeros(plan.eps_shape, dtype=torch.complex64, device="cuda")
+    with pytest.raises(B.EpsgradError) as e:
+        plan.eps_vjp(torch.rand(plan.ctrl_shape, device="cuda"), 8.0, [f], [f])
     assert e.value.status == B.EUNSUPPORTED
     plan = B.Plan(B.make_config(mx=8, my=8, nz=8, z_lo=2.0, z_hi=5.0))
     with pytest.raises(B.EpsgradError) as e:
