@@ -382,3 +382,7 @@ def vjp(cfg: OracleConfig, C, beta: float, EF: list, EA: list):
     out = np.empty((cfg.mx, cfg.my))
     lib().orc_vjp(ctypes.byref(c), _p(C), ctypes.c_double(beta), ctypes.c_int(n), pf, pa, _p(out))
     return out
+
+
+# ---- SOAP, Eqs. (12)-(13): plain numpy, see soap.py
+from .soap import soap_accumulate, soap_eigenbasis, soap_step  # noqa: E402,F401
