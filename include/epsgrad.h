@@ -183,6 +183,32 @@ int    epsgrad_beta_update(double *t, double *beta_max, double gamma, double u, 
 int epsgrad_adam_step(float *C, float *M, float *V, const float *G, size_t n, int step,
                       double b1, double b2, double lr, double eps, void *stream);
 
+/* SOAP, Eqs. (12)-(13) (readings S21-S23 in DESIGN.md), on ONE [mx,my] matrix of control variables (a batch:
+ * one set of buffers and calls per design).  All pointers DEVICE, row-major float32:
+ *   C, M, G [mx,my]   control variables, first moment of Eq. (10) in the original basis (zero before step 1), gradient;
+ *   Vp [mx,my]        second moment in the rotated basis (zero before step 1);
+ *   L [mx,mx], R [my,my]   the accumulators of Eq. (12) (zero before step 1);
+ *   QL [mx,mx], QR [my,my] their orthonormal eigenvectors as COLUMNS, Q[r][j] = component r of eigenvector j.
+ * One optimizer iteration is: epsgrad_soap_accumulate; epsgrad_soap_eigh on L and on R (every iteration or every few: the
+ * caller's choice, S23); epsgrad_soap_step.
+ *   epsgrad_soap_accumulate   L <- b2 L + (1-b2) G G^T,  R <- b2 R + (1-b2) G^T G                              (Eq. (12))
+ *   epsgrad_soap_eigh         Q, w <- eigenvectors / ascending eigenvalues [n] of the symmetric A [n,n] (A is not
+ *                             written).  The library's one LIBRARY step (cuSOLVER syevd), loaded with dlopen on first use:
+ *                             EPSGRAD_EUNSUPPORTED (and workspace_bytes = 0) when cuSOLVER is not on the machine.  Uses the
+ *                             current device; one host thread at a time.  Eigenvector signs are the solver's: they do not
+ *                             change the update (S23).
+ *   epsgrad_soap_step         M <- b1 M + (1-b1) G;  G' = QL^T G QR;  M' = QL^T M QR;  V' <- b2 V' + (1-b2) G'^2;
+ *                             N' = (M'/(1-b1^step)) / sqrt(V'/(1-b2^step) + eps)  (eps inside the root, as printed);
+ *                             C <- C - lr QL N' QR^T                                                           (Eq. (13))
+ * `work` is caller-owned device scratch of at least the matching *_workspace_bytes.  Errors: EPSGRAD_EINVAL (null pointer,
+ * size < 1, step < 1, b outside [0,1), lr <= 0, eps < 0), EPSGRAD_ENOWORKSPACE, EPSGRAD_ECUDA.  No host synchronisation.   */
+int    epsgrad_soap_accumulate(float *L, float *R, const float *G, int mx, int my, double b2, void *stream);
+size_t epsgrad_soap_eigh_workspace_bytes(int n);
+int    epsgrad_soap_eigh(const float *A, float *Q, float *w, int n, void *work, size_t work_bytes, void *stream);
+size_t epsgrad_soap_step_workspace_bytes(int mx, int my);
+int    epsgrad_soap_step(float *C, float *M, float *Vp, const float *G, const float *QL, const float *QR, int mx, int my,
+                         int step, double b1, double b2, double lr, double eps, void *work, size_t work_bytes, void *stream);
+
 /* Both in one call; the filter output (Phi) is computed once and shared.                */
 int eps_forward_vjp(epsgrad_plan_t *plan, const float *C, float beta, int n_pairs,
                     const void *const *EF, const void *const *EA,

@@ -22,6 +22,8 @@ EXPORTS = (
     "epsgrad_plan_set_profiling", "epsgrad_plan_last_kernel_times", "epsgrad_plan_set_overlap", "epsgrad_plan_set_host_direct", "epsgrad_plan_set_embedding", "epsgrad_plan_set_tma", "epsgrad_plan_set_timeline", "epsgrad_plan_read_timeline", 
     "eps_forward", "eps_vjp", "eps_forward_vjp", "eps_forward_vjp_host", "eps_vjp_beta", "eps_unbinarity",
     "epsgrad_beta_schedule", "epsgrad_beta_update", "epsgrad_adam_step",
+    "epsgrad_soap_accumulate", "epsgrad_soap_eigh_workspace_bytes", "epsgrad_soap_eigh",
+    "epsgrad_soap_step_workspace_bytes", "epsgrad_soap_step",
     "epsgrad_stage_filter", "epsgrad_stage_eps2d", "epsgrad_stage_zreduce",
     "epsgrad_status_string", "epsgrad_version",
 )
@@ -87,6 +89,70 @@ def adam_step(C, M, V, G, step: int, b1=0.9, b2=0.999, lr=1e-3, eps=1e-8) -> Non
                                    torch.cuda.current_stream(C.device).cuda_stream), "epsgrad_adam_step")
 
 
+class Soap:
+    """State and calls of the SOAP optimizer, Eqs. (12)-(13), for one [mx,my] matrix of control variables on a
+    CUDA device: owns M, V', L, R, Q_L, Q_R and the scratch buffers; every step of the arithmetic is a library call."""
+
+    def __init__(self, mx: int, my: int, device=None):
+        import torch
+        self._torch = torch
+        self.device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+        z = lambda *shape: torch.zeros(*shape, dtype=torch.float32, device=self.device)
+        self.mx, self.my = mx, my
+        self.M, self.Vp, self.L, self.R = z(mx, my), z(mx, my), z(mx, mx), z(my, my)
+        self.QL, self.QR = torch.eye(mx, dtype=torch.float32, device=self.device), torch.eye(my, dtype=torch.float32, device=self.device)
+        self.wL, self.wR = z(mx), z(my)
+        self._work = torch.empty(lib().epsgrad_soap_step_workspace_bytes(mx, my), dtype=torch.uint8, device=self.device)
+        self._ework = None
+        self.step = 0
+
+    def _stream(self):
+        return self._torch.cuda.current_stream(self.device).cuda_stream
+
+    def _chk(self, *ts):
+        t = self._torch
+        for x in ts:
+            assert x.is_cuda and x.dtype == t.float32 and x.is_contiguous()
+
+    def accumulate(self, G, b2=0.999) -> None:
+        """Eq. (12)"""
+        self._chk(G)
+        assert tuple(G.shape) == (self.mx, self.my)
+        with self._torch.cuda.device(self.device):
+            _check(lib().epsgrad_soap_accumulate(self.L.data_ptr(), self.R.data_ptr(), G.data_ptr(), self.mx, self.my, b2,
+                                                 self._stream()), "epsgrad_soap_accumulate")
+
+    def eigh(self, A, Q, w) -> None:
+        """Q, w <- eigenvectors (columns) and ascending eigenvalues of the symmetric A"""
+        t = self._torch
+        self._chk(A, Q, w)
+        n = A.shape[0]
+        assert tuple(A.shape) == (n, n) and tuple(Q.shape) == (n, n) and tuple(w.shape) == (n,)
+        with t.cuda.device(self.device):
+            need = lib().epsgrad_soap_eigh_workspace_bytes(n)
+            if need == 0:
+                raise EpsgradError(EUNSUPPORTED, "epsgrad_soap_eigh_workspace_bytes")
+            if self._ework is None or self._ework.numel() < need:
+                self._ework = t.empty(need, dtype=t.uint8, device=self.device)
+            _check(lib().epsgrad_soap_eigh(A.data_ptr(), Q.data_ptr(), w.data_ptr(), n, self._ework.data_ptr(), self._ework.numel(),
+                                           self._stream()), "epsgrad_soap_eigh")
+
+    def refresh(self) -> None:
+        """Q_L, Q_R <- eigenvectors of L, R"""
+        self.eigh(self.L, self.QL, self.wL)
+        self.eigh(self.R, self.QR, self.wR)
+
+    def update(self, C, G, b1=0.9, b2=0.999, lr=1e-3, eps=1e-8) -> None:
+        """Eq. (13) in place on C with the current bases; counts the step"""
+        self._chk(C, G)
+        assert tuple(C.shape) == (self.mx, self.my) and tuple(G.shape) == (self.mx, self.my)
+        self.step += 1
+        with self._torch.cuda.device(self.device):
+            _check(lib().epsgrad_soap_step(C.data_ptr(), self.M.data_ptr(), self.Vp.data_ptr(), G.data_ptr(), self.QL.data_ptr(),
+                                           self.QR.data_ptr(), self.mx, self.my, self.step, b1, b2, lr, eps,
+                                           self._work.data_ptr(), self._work.numel(), self._stream()), "epsgrad_soap_step")
+
+
 def beta_schedule(beta_min: float, beta_max: float, i: int, n_iter: int) -> float:
     """Eq. (14) (P:L150)."""
     return float(lib().epsgrad_beta_schedule(beta_min, beta_max, i, n_iter))
@@ -134,6 +200,14 @@ def lib() -> ctypes.CDLL:
     L.epsgrad_beta_schedule.argtypes = [ctypes.c_double, ctypes.c_double, i32, i32]
     L.epsgrad_adam_step.argtypes = [vp, vp, vp, vp, sz, i32, ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_double, vp]
     L.epsgrad_beta_update.argtypes = [vp, vp, ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_double]
+    L.epsgrad_soap_accumulate.argtypes = [vp, vp, vp, i32, i32, ctypes.c_double, vp]
+    L.epsgrad_soap_eigh_workspace_bytes.restype = sz
+    L.epsgrad_soap_eigh_workspace_bytes.argtypes = [i32]
+    L.epsgrad_soap_eigh.argtypes = [vp, vp, vp, i32, vp, sz, vp]
+    L.epsgrad_soap_step_workspace_bytes.restype = sz
+    L.epsgrad_soap_step_workspace_bytes.argtypes = [i32, i32]
+    L.epsgrad_soap_step.argtypes = [vp, vp, vp, vp, vp, vp, i32, i32, i32, ctypes.c_double, ctypes.c_double, ctypes.c_double,
+                                    ctypes.c_double, vp, sz, vp]
     L.eps_forward_vjp.argtypes = [vp, vp, f32, i32, vp, vp, vp, vp, vp]
     L.eps_forward_vjp_host.argtypes = [vp, vp, f32, i32, vp, vp, vp, vp, vp]
     L.epsgrad_stage_filter.argtypes = [vp, vp, vp, vp]

@@ -86,7 +86,7 @@ __global__ void __launch_bounds__(SEPX_THREADS) k_sep_up_x(const SepParams P)
     extern __shared__ __align__(16) float w_pad[];
     constexpr int NBA = SEPX_NBA;
     sepx_load_weights<M>(P, w_pad);
-    const int T = P.T, NT = P.NT;
+    const int T = P.T;
     const int q = blockIdx.x * SEPX_THREADS + threadIdx.x, a_base = blockIdx.y * NBA, b = blockIdx.z;
     if (q >= P.py) return;
     const float *tb = P.in + (size_t)b * P.mx * P.py + q;
