@@ -142,11 +142,14 @@ def test_random_configuration_every_entry_point(i):
     plan = B.Plan(cfg)
     eps0, g0 = plan.eps_forward_vjp(C, beta, EF, EA)
     G0 = plan.stage_zreduce(EF, EA)
+    gb0, db0 = plan.eps_vjp_beta(C, beta, EF, EA)
+    assert torch.equal(gb0, g0)
     # separate calls; serial schedule
     assert torch.equal(plan.eps_forward(C, beta), eps0) and torch.equal(plan.eps_vjp(C, beta, EF, EA), g0)
     plan.set_overlap(False)
     eps1, g1 = plan.eps_forward_vjp(C, beta, EF, EA)
-    assert torch.equal(eps1, eps0) and torch.equal(g1, g0)
+    gb1, db1 = plan.eps_vjp_beta(C, beta, EF, EA)
+    assert torch.equal(eps1, eps0) and torch.equal(g1, g0) and torch.equal(gb1, g0) and torch.equal(db1, db0)
     plan.set_overlap(True)
     # TMA field stream: same windows, same per-column order
     plan.set_tma(True)
@@ -195,8 +198,10 @@ def test_random_configuration_every_entry_point(i):
     plan.set_embedding(nxf, nyf, nzf, i0, j0, k0)
     eps_f = torch.full(shape, -7.0, device="cuda")
     _, g_e = plan.eps_forward_vjp(C, beta, fEF, fEA, eps_out=eps_f)
+    gb_e, db_e = plan.eps_vjp_beta(C, beta, fEF, fEA)
     torch.cuda.synchronize()
     assert torch.equal(g_e, g0) and torch.equal(eps_f[blk], eps0), (kw, shape, (i0, j0, k0))
+    assert torch.equal(gb_e, g0) and torch.equal(db_e, db0)
     outside = torch.ones(shape, dtype=torch.bool, device="cuda")
     outside[blk] = False
     assert bool((eps_f[outside] == -7.0).all())
