@@ -235,10 +235,15 @@ int epsgrad_plan_set_embedding(epsgrad_plan_t *plan, const epsgrad_embedding_t *
  * EPSGRAD_EUNSUPPORTED when TMA descriptors cannot be built on this driver.                                               */
 int epsgrad_plan_set_tma(epsgrad_plan_t *plan, int enable);
 
-/* Field transfer of the *_host entry points (default 1).  1: when every field buffer is pinned, mapped host memory (and the
- * plan is not in dense-read mode), the Eq. (1) reduction copies its slab windows straight out of host memory and the rest
- * of the fields never crosses the bus (only Omega_D enters the gradient); buffers that are not pinned fall back to
- * 0.  0: every field is copied whole into the staging buffer first.  Results are identical.                              */
+/* Field transfer of the *_host entry points (mode; default 2).  Eq. (1) needs only the slab cells of the fields (P:L27:
+ * only Omega_D enters the gradient), so when every field buffer is pinned, mapped host memory (and the plan is not in
+ * dense-read mode) the rest of the fields never crosses the bus:
+ *   1: the Eq. (1) reduction reads its slab windows straight out of host memory;
+ *   2: as 1 for calls that return the gradient only; calls that also return eps gather the union slab window of every z
+ *      column into the staging buffer with one strided copy per field on the copy engine, beside the eps transfer in the
+ *      other direction (4 % faster than 1 at paper scale);
+ *   0: every field is copied whole into the staging buffer first (also the fallback for buffers that are not pinned).
+ * Results are identical in all modes.                                                                                    */
 int epsgrad_plan_set_host_direct(epsgrad_plan_t *plan, int enable);
 /* bytes the last *_host call copied host->device and device->host                       */
 int epsgrad_plan_last_copy_bytes(const epsgrad_plan_t *plan, uint64_t *h2d, uint64_t *d2h);

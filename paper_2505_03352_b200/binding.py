@@ -339,8 +339,9 @@ class Plan:
     def set_tma(self, enable: bool) -> None:
         _check(lib().epsgrad_plan_set_tma(self._h, int(bool(enable))), "epsgrad_plan_set_tma")
 
-    def set_host_direct(self, enable: bool) -> None:
-        _check(lib().epsgrad_plan_set_host_direct(self._h, int(bool(enable))), "epsgrad_plan_set_host_direct")
+    def set_host_direct(self, mode) -> None:
+        """0 / False: fields staged whole; 1 / True: slab windows read in place by the kernel; 2: gathered by the copy engine"""
+        _check(lib().epsgrad_plan_set_host_direct(self._h, int(mode)), "epsgrad_plan_set_host_direct")
 
     def set_overlap(self, enable: bool) -> None:
         _check(lib().epsgrad_plan_set_overlap(self._h, int(bool(enable))), "epsgrad_plan_set_overlap")

@@ -356,7 +356,7 @@ extern "C" int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsg
         cudaSetDevice(prev2);
         if (!ok) { cudaGetLastError(); epsgrad_plan_destroy(P); return EPSGRAD_ECUDA; }
         P->overlap = 1;
-        P->host_direct = 1;
+        P->host_direct = 2;
         {
             cudaDriverEntryPointQueryResult qres;
             void *fn = nullptr;
@@ -501,7 +501,7 @@ extern "C" int epsgrad_plan_set_tma(epsgrad_plan_t *P, int enable)
 extern "C" int epsgrad_plan_set_host_direct(epsgrad_plan_t *P, int enable)
 {
     if (!P) return EPSGRAD_EINVAL;
-    P->host_direct = enable != 0;
+    P->host_direct = enable < 0 ? 0 : (enable > 2 ? 2 : enable);
     return EPSGRAD_OK;
 }
 
@@ -815,12 +815,34 @@ int launch_extrude(epsgrad_plan *P, const float *e2d, float *eps, cudaStream_t s
 }
 
 // ---- R1: the field read stream; more than ZR_MAX_PAIRS pairs are chained through accumulating launches
+// first chunk and number of chunks of the union of the two slab windows (x|y and z) of a field column
+void window_union(const epsgrad_plan *P, int *first, int *count)
+{
+    int lo = P->cfg.nz / 2, hi = 0;
+    for (int g = 0; g < 2; ++g)
+        if (P->nch[g] > 0) { lo = std::min(lo, P->ch0[g]); hi = std::max(hi, P->ch0[g] + P->nch[g]); }
+    *first = hi > lo ? lo : 0;
+    *count = hi > lo ? hi - lo : 0;
+}
+
+// packed: EF / EA hold only the union window of every column, [B,3,ncol][count] chunks (the host entry point's gather)
 int launch_zreduce(epsgrad_plan *P, int n_pairs, const void *const *EF, const void *const *EA, float *gbar, cudaStream_t st,
-                   bool host_src = false)
+                   bool host_src = false, bool packed = false)
 {
     ZredParams zp;
     zp.gbar = gbar; zp.zw = P->d_zw; zp.ncol = P->nx * P->ny; zp.nz = P->cfg.nz;
     zp.cm = make_colmap(P, 2);
+    int u0 = 0, un = 0;
+    zp.choff = 0;
+    if (packed) {
+        window_union(P, &u0, &un);
+        zp.cm.embedded = 0;
+        zp.cm.col_pitch = (unsigned)un;
+        zp.cm.row_pitch = (size_t)P->ny * un;
+        zp.cm.plane_pitch = (size_t)P->nx * zp.cm.row_pitch;
+        zp.cm.base = 0;
+        zp.choff = u0;
+    }
     int maxnch = 1;
     for (int g = 0; g < 2; ++g) {
         zp.ch0[g] = P->dense ? 0 : P->ch0[g];
@@ -839,7 +861,7 @@ int launch_zreduce(epsgrad_plan *P, int n_pairs, const void *const *EF, const vo
     }
     zp.nblk = cdiv(zp.ncol, ZR_COLS);
     // windows of at most 128 bytes per column: ask for 64-byte fills
-    const bool sparse = maxnch * 16 <= 128 && zp.nz * 8 > 128;
+    const bool sparse = maxnch * 16 <= 128 && zp.nz * 8 > 128 && !packed;     // packed windows are one dense stream
     host_src = host_src || P->cur_host_src;
     if (sparse && !host_src && P->use_tma && P->emb.nx_full == 0) {
         // TMA variant (zreduce.cuh): one 2-D tensor map per field, rows = z columns, box = {window, 256 columns}
@@ -1357,6 +1379,51 @@ extern "C" int eps_forward_vjp_host(epsgrad_plan_t *P, const float *C_host, floa
         P->last_h2d += 2 * b_f;
     }
     if (!ok) { cudaGetLastError(); return EPSGRAD_ECUDA; }
+    if (direct && P->host_direct == 2 && eps_host && dFdC_host && P->overlap && !P->prof) {
+        // Copy-engine gather: one strided 2-D copy per field moves the union slab window of every z column into a packed
+        // staging buffer on the auxiliary stream, while eps is computed and sent to the host on the caller's stream -- the
+        // two transfers use the two copy engines, and no SM waits on the bus (at paper scale 7.0 ms against 7.9 ms for the
+        // in-place reads beside the same eps transfer).
+        int u0 = 0, un = 0;
+        window_union(P, &u0, &un);
+        const size_t rows = (size_t)P->cfg.batch * 3 * P->nx * P->ny, wbytes = (size_t)un * 16, b_p = align_up(rows * wbytes, 256);
+        cudaStream_t ax = P->aux;
+        ok = cudaEventRecord(P->ev_fork, st) == cudaSuccess && cudaStreamWaitEvent(ax, P->ev_fork, 0) == cudaSuccess;
+        for (int p = 0; p < n_pairs && ok; ++p) {
+            ef[p] = base; base += b_p;
+            ea[p] = base; base += b_p;
+            if (un > 0)
+                ok = cudaMemcpy2DAsync((void *)ef[p], wbytes, (const char *)EF_host[p] + (size_t)u0 * 16, (size_t)P->cfg.nz * 8, wbytes, rows,
+                                       cudaMemcpyHostToDevice, ax) == cudaSuccess &&
+                     cudaMemcpy2DAsync((void *)ea[p], wbytes, (const char *)EA_host[p] + (size_t)u0 * 16, (size_t)P->cfg.nz * 8, wbytes, rows,
+                                       cudaMemcpyHostToDevice, ax) == cudaSuccess;
+        }
+        ok = ok && cudaEventRecord(P->ev_r, ax) == cudaSuccess;
+        P->last_h2d = b_c + (size_t)2 * n_pairs * rows * wbytes;
+        int rc = EPSGRAD_OK;
+        if (ok) {
+            rc = launch_front(P, dC, beta, st);
+            if (!rc) rc = launch_fwd2d(P, ws_phi(P), beta, ws_e2d(P), ws_coef(P), nullptr, st);
+            if (!rc && eps_host) {
+                rc = launch_extrude(P, ws_e2d(P), dE, st);
+                if (!rc) ok = cudaMemcpyAsync(eps_host, dE, b_e, cudaMemcpyDeviceToHost, st) == cudaSuccess;
+                P->last_d2h += b_e;
+            }
+        }
+        // always join the auxiliary stream
+        if (cudaStreamWaitEvent(st, P->ev_r, 0) != cudaSuccess) ok = false;
+        if (!ok) { cudaGetLastError(); return EPSGRAD_ECUDA; }
+        if (rc) return rc;
+        rc = launch_zreduce(P, n_pairs, ef.data(), ea.data(), ws_gbar(P), st, false, true);
+        if (!rc) rc = launch_maskgrad(P, ws_phi(P), beta, ws_gbar(P), ws_coef(P), ws_v(P), st);
+        if (!rc && P->morph_R > 0) rc = launch_morph_reverse(P, ws_phi(P), beta, ws_v(P), st);
+        if (!rc) rc = launch_filterT(P, ws_v(P), dG, st);
+        if (rc) return rc;
+        ok = cudaMemcpyAsync(dFdC_host, dG, b_c, cudaMemcpyDeviceToHost, st) == cudaSuccess;
+        P->last_d2h += b_c;
+        if (!ok) { cudaGetLastError(); return EPSGRAD_ECUDA; }
+        return EPSGRAD_OK;
+    }
     if (direct && eps_host && dFdC_host && P->overlap && !P->prof) {
         // The bus is full duplex: eps does not depend on the fields, so it is finished first and travels to the host on the
         // auxiliary stream while the z-reduction pulls its windows the other way.

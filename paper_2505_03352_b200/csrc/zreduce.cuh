@@ -34,6 +34,7 @@ struct ZredParams {
     int chs[2];            // log2 of the lanes per column of the copy loop: 2^chs >= nch
     ColumnMap cm;          // where the columns sit in E_F / E_A (16-byte pieces = 2 cells)
     int ncp[2];            // columns staged per pass (<= ZR_COLS): ncp (nch | 1) <= ZR_STAGE_CHUNKS
+    int choff;             // chunk the stored columns start at: 0, or the first chunk of the union window for packed fields
 };
 
 __host__ __device__ inline int zred_cols_per_pass(int nch)
@@ -68,7 +69,7 @@ __device__ __forceinline__ void zwindow_issue(const ZredParams &P, float4 *buf, 
     const int grp = c == 2, nch = P.nch[grp], sh = P.chs[grp], ncp = P.ncp[grp];
     const int ch = threadIdx.x & ((1 << sh) - 1), lstep = ZR_THREADS >> sh;
     if (ch < nch) {
-        const size_t first = P.cm.plane(b, c) + P.ch0[grp] + ch;
+        const size_t first = P.cm.plane(b, c) + (P.ch0[grp] - P.choff) + ch;
         const float4 *pf = P.ef[p] + first, *pa = P.ea[p] + first;
         const int pitch = nch | 1;
         float4 *df = buf + ch, *da = df + pitch * ncp;

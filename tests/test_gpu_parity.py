@@ -267,10 +267,24 @@ def test_host_entry_point_matches_device_entry_point():
     plan.eps_forward_vjp_host(pin(Cn), 8.0, [pin(f) for f in EFn], [pin(f) for f in EAn], eps_h, g_h)
     torch.cuda.synchronize()
     assert torch.equal(eps_h, eps_d.cpu()) and torch.equal(g_h, g_d.cpu())
-    # pinned fields are read in place, slab windows only: cells 6..9 for x, y (2 chunks of 16 B), 5..9 for z (3 chunks)
+    # only the slab windows of pinned fields cross the bus: cells 6..9 for x, y (2 chunks of 16 B), 5..9 for z (3 chunks).
+    # Default (mode 2): the union window (3 chunks) of every column of every component, gathered by the copy engine
     h2d, d2h = plan.last_copy_bytes()
     ncol = cfg.batch * cfg.nx * cfg.ny
-    assert h2d == Cn.nbytes + 2 * 2 * ncol * (2 + 2 + 3) * 16 and d2h == eps_h.numel() * 4 + g_h.numel() * 4
+    assert h2d == Cn.nbytes + 2 * 2 * ncol * 3 * 3 * 16 and d2h == eps_h.numel() * 4 + g_h.numel() * 4
+    # mode 1: read in place by the kernel, exactly the chunks of each component's window
+    plan.set_host_direct(1)
+    eps_h.zero_(); g_h.zero_()
+    plan.eps_forward_vjp_host(pin(Cn), 8.0, [pin(f) for f in EFn], [pin(f) for f in EAn], eps_h, g_h)
+    torch.cuda.synchronize()
+    assert torch.equal(eps_h, eps_d.cpu()) and torch.equal(g_h, g_d.cpu())
+    assert plan.last_copy_bytes()[0] == Cn.nbytes + 2 * 2 * ncol * (2 + 2 + 3) * 16
+    # gradient only: mode 2 behaves as mode 1
+    plan.set_host_direct(2)
+    g_h.zero_()
+    plan.eps_forward_vjp_host(pin(Cn), 8.0, [pin(f) for f in EFn], [pin(f) for f in EAn], None, g_h)
+    torch.cuda.synchronize()
+    assert torch.equal(g_h, g_d.cpu()) and plan.last_copy_bytes()[0] == Cn.nbytes + 2 * 2 * ncol * (2 + 2 + 3) * 16
     # whole-field staging (also the fallback for pageable buffers) gives the same bits
     plan.set_host_direct(False)
     eps_h.zero_(); g_h.zero_()
@@ -279,7 +293,7 @@ def test_host_entry_point_matches_device_entry_point():
     assert torch.equal(eps_h, eps_d.cpu()) and torch.equal(g_h, g_d.cpu())
     h2d, d2h = plan.last_copy_bytes()
     assert h2d == Cn.nbytes + sum(f.nbytes for f in EFn + EAn)
-    plan.set_host_direct(True)
+    plan.set_host_direct(2)
     eps_h.zero_(); g_h.zero_()
     plan.eps_forward_vjp_host(torch.from_numpy(Cn), 8.0, [torch.from_numpy(f) for f in EFn], [torch.from_numpy(f) for f in EAn], eps_h, g_h)
     torch.cuda.synchronize()

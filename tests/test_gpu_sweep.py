@@ -173,18 +173,18 @@ def test_random_configuration_every_entry_point(i):
     graph.replay()
     torch.cuda.synchronize()
     assert torch.equal(eps_g, eps0) and torch.equal(g_g, g0)
-    # host entry point: pinned buffers (windows read in place), then staged whole
+    # host entry point: pinned buffers (windows gathered by the copy engine; read in place), then staged whole
     pin = lambda a: torch.from_numpy(a).pin_memory()
     eps_h = torch.empty(plan.eps_shape, dtype=torch.float32).pin_memory()
     g_h = torch.empty(plan.ctrl_shape, dtype=torch.float32).pin_memory()
     hC, hEF, hEA = pin(Cn), [pin(f) for f in EFn], [pin(f) for f in EAn]
-    for direct in (True, False):
+    for direct in (2, 1, 0):
         plan.set_host_direct(direct)
         eps_h.zero_(); g_h.zero_()
         plan.eps_forward_vjp_host(hC, beta, hEF, hEA, eps_h, g_h)
         torch.cuda.synchronize()
         assert torch.equal(eps_h, eps0.cpu()) and torch.equal(g_h, g0.cpu()), (kw, direct)
-    plan.set_host_direct(True)
+    plan.set_host_direct(2)
     # embedded in a larger domain at a random origin (k0 and nz_full multiples of 4)
     i0, j0, k0 = int(rng.integers(0, 9)), int(rng.integers(0, 9)), 4 * int(rng.integers(0, 3))
     nxf, nyf, nzf = cfg.nx + i0 + int(rng.integers(0, 7)), cfg.ny + j0 + int(rng.integers(0, 7)), cfg.nz + k0 + 4 * int(rng.integers(0, 3))
