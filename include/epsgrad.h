@@ -229,6 +229,15 @@ int eps_forward_vjp_host(epsgrad_plan_t *plan, const float *C_host, float beta, 
  * while an embedding is set.                                                                                              */
 int epsgrad_plan_set_embedding(epsgrad_plan_t *plan, const epsgrad_embedding_t *embedding);
 
+/* x-slab of a region shared by several GPUs (default off).  The plan's region is this rank's rows of a larger
+ * design plus a halo wide enough for the dependency cone (filter radius + 3 cells on either side), but the
+ * caller's eps / E_F / E_A hold only the rows it owns: [B,3,x_count,Ny,Nz] = Yee rows [x_first, x_first + x_count) of the
+ * region.  eps is written and the fields are read on those rows only; every other row of the region contributes nothing to
+ * dFdC, which stays region-sized (partial: the ranks' gradients add; the halo parts overlap the neighbours' controls).
+ * (0, 0) switches back.  EPSGRAD_EINVAL for a range outside the region; EPSGRAD_EUNSUPPORTED together with an embedding and
+ * in the *_host entry points.                                                                                              */
+int epsgrad_plan_set_slab(epsgrad_plan_t *plan, int x_first, int x_count);
+
 /* How the device-resident field windows are fetched (default 0).  1: by the tensor memory accelerator, one bulk tensor
  * copy per field and 256 columns, persistent CTAs (region-sized fields with sparse windows only; other cases fall back).
  * 0: by 16-byte asynchronous copies (LDGSTS), 2 us faster at paper scale.  Same bytes, same results; a measurement switch.

@@ -19,7 +19,7 @@ EXPORTS = (
     "epsgrad_plan_create", "epsgrad_plan_destroy", "epsgrad_workspace_bytes",
     "epsgrad_plan_set_workspace", "epsgrad_staging_bytes", "epsgrad_plan_set_staging",
     "epsgrad_plan_set_dense_reads", "epsgrad_plan_last_launches", "epsgrad_plan_last_copy_bytes",
-    "epsgrad_plan_set_profiling", "epsgrad_plan_last_kernel_times", "epsgrad_plan_set_overlap", "epsgrad_plan_set_host_direct", "epsgrad_plan_set_embedding", "epsgrad_plan_set_tma", "epsgrad_plan_set_timeline", "epsgrad_plan_read_timeline", 
+    "epsgrad_plan_set_profiling", "epsgrad_plan_last_kernel_times", "epsgrad_plan_set_overlap", "epsgrad_plan_set_host_direct", "epsgrad_plan_set_embedding", "epsgrad_plan_set_slab", "epsgrad_plan_set_tma", "epsgrad_plan_set_timeline", "epsgrad_plan_read_timeline", 
     "eps_forward", "eps_vjp", "eps_forward_vjp", "eps_forward_vjp_host", "eps_vjp_beta", "eps_unbinarity",
     "epsgrad_beta_schedule", "epsgrad_beta_update", "epsgrad_adam_step",
     "epsgrad_soap_accumulate", "epsgrad_soap_eigh_workspace_bytes", "epsgrad_soap_eigh",
@@ -214,6 +214,7 @@ def lib() -> ctypes.CDLL:
     L.epsgrad_stage_eps2d.argtypes = [vp, vp, f32, vp, vp]
     L.epsgrad_plan_set_overlap.argtypes = [vp, i32]
     L.epsgrad_plan_set_host_direct.argtypes = [vp, i32]
+    L.epsgrad_plan_set_slab.argtypes = [vp, i32, i32]
     L.epsgrad_plan_set_embedding.argtypes = [vp, vp]
     L.epsgrad_plan_set_tma.argtypes = [vp, i32]
     L.epsgrad_plan_set_timeline.argtypes = [vp, i32]
@@ -335,6 +336,11 @@ class Plan:
             e = Embedding(nx_full, ny_full, nz_full, i0, j0, k0)
             _check(lib().epsgrad_plan_set_embedding(self._h, ctypes.byref(e)), "epsgrad_plan_set_embedding")
             self._field_shape = (self.eps_shape[0], 3, nx_full, ny_full, nz_full)
+
+    def set_slab(self, x_first: int = 0, x_count: int = 0) -> None:
+        """eps / E_F / E_A hold only Yee rows [x_first, x_first + x_count) of the region: [B,3,x_count,Ny,Nz]; (0, 0): off"""
+        _check(lib().epsgrad_plan_set_slab(self._h, x_first, x_count), "epsgrad_plan_set_slab")
+        self._field_shape = (self.eps_shape[0], 3, x_count, self.eps_shape[3], self.eps_shape[4]) if x_count > 0 else None
 
     def set_tma(self, enable: bool) -> None:
         _check(lib().epsgrad_plan_set_tma(self._h, int(bool(enable))), "epsgrad_plan_set_tma")

@@ -56,6 +56,7 @@ struct epsgrad_plan {
     epsgrad_embedding_t emb;
     int use_tma;               // field windows by TMA bulk tensor copies where possible (epsgrad_plan_set_tma)
     void *tma_encode;          // cuTensorMapEncodeTiled, fetched through the runtime (no link against libcuda)
+    int slab_x0, slab_nx;                   // x-slab: the caller's arrays hold Yee rows [slab_x0, slab_x0 + slab_nx) only; 0, 0 = off
     int dense, host_direct, cur_host_src;   // cur_host_src: the fields of the call in flight are pinned host memory
     // scalars
     float eta0, eta_r, eps_clad, deps, delta;
@@ -486,6 +487,7 @@ extern "C" int epsgrad_plan_set_embedding(epsgrad_plan_t *P, const epsgrad_embed
     if (e->i0 + P->nx > e->nx_full || e->j0 + P->ny > e->ny_full || e->k0 + P->cfg.nz > e->nz_full) return EPSGRAD_EINVAL;
     if (e->nz_full % 4 || e->k0 % 4) return EPSGRAD_EUNSUPPORTED;          // 16-byte pieces of eps (4 cells) and of the fields (2 cells)
     if ((double)P->cfg.batch * 3.0 * e->nx_full * e->ny_full > 2.0e9) return EPSGRAD_EUNSUPPORTED;
+    if (P->slab_nx > 0) return EPSGRAD_EUNSUPPORTED;                        // one addressing option at a time
     P->emb = *e;
     return EPSGRAD_OK;
 }
@@ -495,6 +497,16 @@ extern "C" int epsgrad_plan_set_tma(epsgrad_plan_t *P, int enable)
     if (!P) return EPSGRAD_EINVAL;
     if (enable && !P->tma_encode) return EPSGRAD_EUNSUPPORTED;
     P->use_tma = enable != 0;
+    return EPSGRAD_OK;
+}
+
+extern "C" int epsgrad_plan_set_slab(epsgrad_plan_t *P, int x_first, int x_count)
+{
+    if (!P) return EPSGRAD_EINVAL;
+    if (x_first == 0 && x_count == 0) { P->slab_x0 = P->slab_nx = 0; return EPSGRAD_OK; }
+    if (x_first < 0 || x_count < 1 || x_first + x_count > P->nx) return EPSGRAD_EINVAL;
+    if (P->emb.nx_full > 0) return EPSGRAD_EUNSUPPORTED;         // one addressing option at a time
+    P->slab_x0 = x_first; P->slab_nx = x_count;
     return EPSGRAD_OK;
 }
 
@@ -787,7 +799,7 @@ ColumnMap make_colmap(const epsgrad_plan *P, int cells_per_piece)
         cm.embedded = 0;
         cm.col_pitch = (unsigned)(P->cfg.nz / cells_per_piece);
         cm.row_pitch = (size_t)P->ny * cm.col_pitch;
-        cm.plane_pitch = (size_t)P->nx * cm.row_pitch;
+        cm.plane_pitch = (size_t)(P->slab_nx > 0 ? P->slab_nx : P->nx) * cm.row_pitch;
         cm.base = 0;
     }
     return cm;
@@ -798,6 +810,8 @@ int launch_extrude(epsgrad_plan *P, const float *e2d, float *eps, cudaStream_t s
 {
     ExtrudeParams ep;
     ep.e2d = e2d; ep.eps = eps; ep.zw = P->d_zw; ep.ncol = P->nx * P->ny; ep.nz = P->cfg.nz;
+    ep.pstride = ep.ncol;
+    if (P->slab_nx > 0) { ep.ncol = P->slab_nx * P->ny; ep.e2d += (size_t)P->slab_x0 * P->ny; }     // the slab's rows are one run of columns
     ep.cm = make_colmap(P, 4);
     ep.cpb = extrude_cols_per_block(ep.nz);
     ep.nblk = cdiv(ep.ncol, ep.cpb);
@@ -831,6 +845,13 @@ int launch_zreduce(epsgrad_plan *P, int n_pairs, const void *const *EF, const vo
 {
     ZredParams zp;
     zp.gbar = gbar; zp.zw = P->d_zw; zp.ncol = P->nx * P->ny; zp.nz = P->cfg.nz;
+    zp.pstride = zp.ncol;
+    if (P->slab_nx > 0) {
+        // x-slab: only the slab's rows have fields; the cotangent of every other column of the region is zero
+        if (cudaMemsetAsync(gbar, 0, (size_t)P->cfg.batch * 5 * zp.pstride * sizeof(float), st) != cudaSuccess) { cudaGetLastError(); return EPSGRAD_ECUDA; }
+        zp.ncol = P->slab_nx * P->ny;
+        zp.gbar += (size_t)P->slab_x0 * P->ny;
+    }
     zp.cm = make_colmap(P, 2);
     int u0 = 0, un = 0;
     zp.choff = 0;
@@ -863,7 +884,7 @@ int launch_zreduce(epsgrad_plan *P, int n_pairs, const void *const *EF, const vo
     // windows of at most 128 bytes per column: ask for 64-byte fills
     const bool sparse = maxnch * 16 <= 128 && zp.nz * 8 > 128 && !packed;     // packed windows are one dense stream
     host_src = host_src || P->cur_host_src;
-    if (sparse && !host_src && P->use_tma && P->emb.nx_full == 0) {
+    if (sparse && !host_src && P->use_tma && P->emb.nx_full == 0 && P->slab_nx == 0) {
         // TMA variant (zreduce.cuh): one 2-D tensor map per field, rows = z columns, box = {window, 256 columns}
         typedef CUresult (*EncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
                                      const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -1337,7 +1358,7 @@ extern "C" int eps_forward_vjp_host(epsgrad_plan_t *P, const float *C_host, floa
     } else {
         n_pairs = 0;
     }
-    if (P->emb.nx_full > 0) return EPSGRAD_EUNSUPPORTED;     // host buffers are region-sized: no embedding here
+    if (P->emb.nx_full > 0 || P->slab_nx > 0) return EPSGRAD_EUNSUPPORTED;     // host buffers are region-sized: no embedding or slab here
     if (!P->ws) return EPSGRAD_ENOWORKSPACE;
     if (!P->stg || P->stg_bytes < epsgrad_staging_bytes(P, n_pairs)) return EPSGRAD_ENOWORKSPACE;
     DeviceGuard g(P->device);

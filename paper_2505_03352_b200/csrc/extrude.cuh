@@ -22,7 +22,8 @@ struct ExtrudeParams {
     float *eps;            // [B,3,ncol,nz], or the simulation domain's array when embedded (cm)
     ColumnMap cm;          // where the columns sit in eps (16-byte pieces = 4 cells)
     const float *zw;       // [7][nz] z tables (epsgrad.cu)
-    int ncol, nz;
+    int ncol, nz;          // columns written (the whole region, or the rows of an x-slab: epsgrad_plan_set_slab)
+    int pstride;           // columns per plane of e2d (the whole region)
     int nblk;              // column blocks per component plane
     int cpb;               // columns per block (extrude_cols_per_block)
     int sh4;               // log2(nz/4) when nz/4 is a power of two <= EX_THREADS (fast path), else -1
@@ -41,12 +42,12 @@ __global__ void __launch_bounds__(EX_THREADS, EX_CTAS_PER_SM) k_extrude(const __
     const int tid = threadIdx.x, b = blockIdx.z, nz = P.nz, nz4 = nz >> 2, ncol = P.ncol;
     const int c = blockIdx.y, blk = blockIdx.x;
     const int cpb = P.cpb, col0 = blk * cpb, ncb = min(cpb, ncol - col0);
-    const float *ed = P.e2d + (size_t)b * 5 * ncol;
+    const float *ed = P.e2d + (size_t)b * 5 * P.pstride;
     float4 *out = reinterpret_cast<float4 *>(P.eps) + P.cm.plane(b, c);
     // stage: c = x, y need their own plane; c = z needs planes 2 (full cells), 3 and 4 (face cells)
     const int npl = c == 2 ? 3 : 1;
     for (int o = 0; o < npl; ++o)
-        for (int lc = tid; lc < ncb; lc += EX_THREADS) vsm[o * cpb + lc] = ed[(size_t)(c + o) * ncol + col0 + lc];
+        for (int lc = tid; lc < ncb; lc += EX_THREADS) vsm[o * cpb + lc] = ed[(size_t)(c + o) * P.pstride + col0 + lc];
     if (P.sh4 >= 0) {
         const int kq = tid & (nz4 - 1), k = kq << 2, cq = tid >> P.sh4, cpp = EX_THREADS >> P.sh4;
         float4 *dst = out + kq;

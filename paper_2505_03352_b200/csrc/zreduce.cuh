@@ -29,7 +29,8 @@ struct ZredParams {
     float *gbar;           // [B,5,ncol]: planes x, y, z-full, z-lower-face, z-upper-face
     const float *zw;       // [7][nz] z tables (epsgrad.cu); rows 0 (wxy) and 2..4 (z-full / lower / upper indicators) are used
     int n_pairs, accumulate;
-    int ncol, nz, nblk;    // nblk = ceil(ncol / ZR_COLS) column blocks per component plane
+    int ncol, nz, nblk;    // columns read (the whole region, or the rows of an x-slab); nblk = ceil(ncol / ZR_COLS) column blocks per plane
+    int pstride;           // columns per plane of gbar (the whole region)
     int ch0[2], nch[2];    // chunk window (chunk = 2 cells = 16 B) for {x,y} and {z}
     int chs[2];            // log2 of the lanes per column of the copy loop: 2^chs >= nch
     ColumnMap cm;          // where the columns sit in E_F / E_A (16-byte pieces = 2 cells)
@@ -140,10 +141,10 @@ __global__ void __launch_bounds__(ZR_THREADS, 5) k_zreduce(const __grid_constant
             }
         }
         if (tid < nc) {
-            float *dst = P.gbar + (size_t)b * 5 * P.ncol + colb + c0 + tid;
+            float *dst = P.gbar + (size_t)b * 5 * P.pstride + colb + c0 + tid;
             const int nout = grp ? 3 : 1;
             for (int o = 0; o < nout; ++o) {
-                float *d = dst + (size_t)(grp ? 2 + o : c) * P.ncol;
+                float *d = dst + (size_t)(grp ? 2 + o : c) * P.pstride;
                 *d = P.accumulate ? *d + acc[o] : acc[o];
             }
         }

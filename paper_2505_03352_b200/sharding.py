@@ -36,3 +36,24 @@ def max_over_ranks(value: float, device=None, group=None) -> float:
 def job_throughput(units_per_rank: int, steps: int, ms_max: float, world: int) -> float:
     """Whole-job units/s when every rank processed units_per_rank per step (weak scaling)."""
     return world * units_per_rank * steps / (ms_max * 1e-3)
+
+
+def slab_halo_cells(filter_radius: float, morph_diameter: float = 0.0) -> int:
+    """Yee cells of halo an x-slab needs on either side so that eps on its own rows, and their share of dF/dC, come out as in
+    the undivided region: half-cell shift + Sobel ring + averages reach 3 cells, each mask pixel reaches the
+    filter radius R -- and must itself sit R cells inside the slab to get the interior normaliser --, and the four morphological
+    operations reach 2 d cells more."""
+    import math
+    return int(math.ceil(filter_radius + 3.0 + 2.0 * morph_diameter))
+
+
+def slab_partition(mx: int, upsample: int, rank: int, world: int, halo_cells: int) -> dict:
+    """Third way to shard: one design split along x.  Returns the control rows this rank owns [a0, a1), the rows
+    its plan covers [e0, e1) (own rows plus the halo, clipped at the true borders of the region, where the plan's own border
+    handling is the right one) and, in Yee rows of that plan's region, the window of the rows it owns -- the arguments of
+    ``Plan.set_slab``."""
+    own = shard_range(mx, rank, world)
+    a0, a1 = own.start, own.stop
+    h = -(-halo_cells // upsample)                     # control rows
+    e0, e1 = max(0, a0 - h), min(mx, a1 + h)
+    return dict(a0=a0, a1=a1, e0=e0, e1=e1, x_first=upsample * (a0 - e0), x_count=upsample * (a1 - a0))

@@ -69,3 +69,62 @@ def test_pair_sharded_gradient_sums_to_the_full_gradient(tmp_path):
     err, t = np.load(tmp_path / "res.npy")
     assert err < 1e-12            # linearity of Eq. (1) in the pairs
     assert t == 11.0              # max over ranks
+
+
+def _slab_worker(rank, world, port, out_dir, morph):
+    """x-slab sharding with the oracle as the compute: every rank runs the chain on its own rows plus the halo."""
+    import dataclasses
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    sys.path[:0] = [root, os.path.join(root, "tests")]
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import oracle as O
+    from helpers import small_cfg
+    cfg = small_cfg(mx=26, my=7, nz=8, z_lo=2.25, z_hi=5.75, radius=3.0, morph_diam=morph)
+    u = cfg.nx // cfg.mx
+    rng = np.random.default_rng(9)
+    C = rng.random((cfg.mx, cfg.my)).astype(np.float32)
+    shape = (3, cfg.nx, cfg.ny, cfg.nz)
+    mk = lambda: (rng.standard_normal(shape) + 1j * rng.standard_normal(shape)).astype(np.complex64)
+    EF, EA = [mk()], [mk()]
+    p = sharding.slab_partition(cfg.mx, u, rank, world, sharding.slab_halo_cells(3.0, morph))
+    sub = dataclasses.replace(cfg, mx=p["e1"] - p["e0"], nx=u * (p["e1"] - p["e0"]))
+    rows = slice(p["x_first"], p["x_first"] + p["x_count"])                 # own Yee rows inside the slab's region
+    own = slice(u * p["a0"], u * p["a1"])                                  # the same rows in the undivided region
+    eps = O.forward(sub, C[p["e0"]:p["e1"]], 8.0)[:, rows]
+    # fields: only the own rows exist on this rank; every other row of the slab's region contributes nothing
+    f, a = np.zeros((3, sub.nx, sub.ny, sub.nz), np.complex64), np.zeros((3, sub.nx, sub.ny, sub.nz), np.complex64)
+    f[:, rows], a[:, rows] = EF[0][:, own], EA[0][:, own]
+    part = np.zeros((cfg.mx, cfg.my))
+    part[p["e0"]:p["e1"]] = O.vjp(sub, C[p["e0"]:p["e1"]], 8.0, [f], [a])
+    g = sharding.sum_gradients(torch.from_numpy(part))
+    full_eps = O.forward(cfg, C, 8.0)
+    err_eps = np.max(np.abs(eps - full_eps[:, own]) / full_eps[:, own])
+    worst = torch.tensor([err_eps])
+    dist.all_reduce(worst, op=dist.ReduceOp.MAX)
+    if rank == 0:
+        full = O.vjp(cfg, C, 8.0, EF, EA)
+        np.save(os.path.join(out_dir, "res.npy"), np.array([float(worst), np.max(np.abs(g.numpy() - full)) / np.max(np.abs(full))]))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world,morph", [(2, 0.0), (3, 0.0), (2, 1.5)])
+def test_x_slabs_with_halo_reproduce_the_undivided_region(tmp_path, world, morph):
+    mp.spawn(_slab_worker, args=(world, _free_port(), str(tmp_path), morph), nprocs=world, join=True)
+    err_eps, err_g = np.load(tmp_path / "res.npy")
+    assert err_eps < 1e-12 and err_g < 1e-12, (err_eps, err_g)
+
+
+def test_slab_partition_covers_the_region_once():
+    for mx, u, world, halo in [(26, 2, 3, 6), (250, 2, 8, 11), (5, 1, 4, 7), (1000, 2, 7, 15)]:
+        parts = [sharding.slab_partition(mx, u, r, world, halo) for r in range(world)]
+        assert parts[0]["a0"] == 0 and parts[-1]["a1"] == mx
+        for p, q in zip(parts, parts[1:]):
+            assert p["a1"] == q["a0"]
+        for p in parts:
+            h = -(-halo // u)
+            assert p["e0"] == max(0, p["a0"] - h) and p["e1"] == min(mx, p["a1"] + h)
+            assert p["x_first"] == u * (p["a0"] - p["e0"]) and p["x_count"] == u * (p["a1"] - p["a0"])
+            assert 0 <= p["x_first"] and p["x_first"] + p["x_count"] <= u * (p["e1"] - p["e0"])
