@@ -332,3 +332,45 @@ def test_error_codes():
     with pytest.raises(B.EpsgradError) as e:
         plan.eps_forward(torch.rand(plan.ctrl_shape, device="cuda"), -1.0)
     assert e.value.status == B.EINVAL
+
+
+def test_two_plans_on_two_streams_do_not_interfere():
+    # a plan carries its own workspace, auxiliary stream and events: calls of different plans interleaved on different streams
+    # give the bits each gives alone
+    kws = [dict(mx=37, my=29, nz=16, z_lo=6.25, z_hi=9.75, filter_radius=4.0),
+           dict(batch=2, mx=45, my=38, nz=32, z_lo=14.25, z_hi=17.75, filter_kind=1, filter_radius=8.0, filter_sigma=2.5)]
+    plans, ins, ref = [], [], []
+    for k, kw in enumerate(kws):
+        cfg = B.make_config(**kw)
+        EF, EA = rand_fields(cfg, 2, 70 + k)
+        plans.append(B.Plan(cfg))
+        ins.append((dev(rand_C(cfg, 60 + k)), [dev(f) for f in EF], [dev(f) for f in EA]))
+        ref.append(plans[k].eps_forward_vjp(ins[k][0], 8.0 + k, ins[k][1], ins[k][2]))
+    torch.cuda.synchronize()
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    outs = [[], []]
+    for rep in range(6):
+        for k in (0, 1):
+            with torch.cuda.stream(streams[k]):
+                outs[k].append(plans[k].eps_forward_vjp(ins[k][0], 8.0 + k, ins[k][1], ins[k][2]))
+    torch.cuda.synchronize()
+    for k in (0, 1):
+        for eps, g in outs[k]:
+            assert torch.equal(eps, ref[k][0]) and torch.equal(g, ref[k][1])
+
+
+def test_plans_are_released():
+    cfg = B.make_config(mx=64, my=64, nz=16, z_lo=6.25, z_hi=9.75, filter_radius=4.0, morph_diameter=2.0)
+    C = dev(rand_C(cfg, 3))
+    torch.cuda.synchronize()
+    free0 = None
+    for i in range(60):
+        plan = B.Plan(cfg)
+        plan.eps_forward(C, 8.0)
+        del plan
+        torch.cuda.synchronize()
+        if i == 9:
+            torch.cuda.empty_cache()
+            free0 = torch.cuda.mem_get_info()[0]
+    torch.cuda.empty_cache()
+    assert torch.cuda.mem_get_info()[0] >= free0 - (8 << 20)          # device tables, streams and events go with the plan
