@@ -205,3 +205,40 @@ def test_random_configuration_every_entry_point(i):
     outside = torch.ones(shape, dtype=torch.bool, device="cuda")
     outside[blk] = False
     assert bool((eps_f[outside] == -7.0).all())
+
+
+@pytest.mark.parametrize("i", range(N_CASES))
+def test_random_configuration_in_x_slabs(i):
+    """The same draws split along x into 2 or 3 slabs with halos: eps of every slab and the sum of the slabs'
+    partial gradients against the undivided plan."""
+    import torch
+    from paper_2505_03352_b200 import sharding
+    kw, beta, n_pairs = draw(i)
+    cfg = B.make_config(**kw)
+    world = 2 + i % 2
+    if cfg.mx < world:
+        pytest.skip("fewer control rows than slabs")
+    C = dev(rand_C(cfg, 1000 + i))
+    EFn, EAn = rand_fields(cfg, n_pairs, 2000 + i)
+    EF, EA = [dev(f) for f in EFn], [dev(f) for f in EAn]
+    eps0, g0 = B.Plan(cfg).eps_forward_vjp(C, beta, EF, EA)
+    u = cfg.upsample
+    halo = sharding.slab_halo_cells(cfg.filter_radius, cfg.morph_diameter)
+    g_sum = torch.zeros_like(g0)
+    for rank in range(world):
+        p = sharding.slab_partition(cfg.mx, u, rank, world, halo)
+        sub = dict(kw, mx=p["e1"] - p["e0"])
+        try:
+            plan = B.Plan(B.make_config(**sub))
+        except B.EpsgradError as e:                    # a slab narrower than the morphological disk
+            assert e.status == B.EUNSUPPORTED and cfg.morph_diameter > 0
+            pytest.skip("slab narrower than the morphological disk")
+        plan.set_slab(p["x_first"], p["x_count"])
+        own = slice(u * p["a0"], u * p["a1"])
+        eps_r, g_r = plan.eps_forward_vjp(C[:, p["e0"]:p["e1"]].clone(), beta, [f[:, :, own].clone() for f in EF],
+                                          [f[:, :, own].clone() for f in EA])
+        ref = eps0[:, :, own]
+        assert float(((eps_r - ref).abs() / ref).max()) < 1e-6 * max(1.0, beta / 17.0), (kw, rank, p)
+        g_sum[:, p["e0"]:p["e1"]] += g_r
+    a, b = g_sum.cpu().numpy().astype(np.float64), g0.cpu().numpy().astype(np.float64)
+    assert rel_inf(a, b) < 1e-5 * max(1.0, beta / 17.0), (kw, rel_inf(a, b))
