@@ -119,8 +119,9 @@ int epsgrad_plan_set_dense_reads(epsgrad_plan_t *plan, int dense);
 
 /* Two-stream schedule (default on).  The path has two HBM-bound kernels -- the Eq. (1) field reads, which depend
  * on nothing, and the eps stores -- and four small L2-resident ones.  Calls that compute dF/dC fork the plan's auxiliary
- * stream from `stream` (event), run the field reads there beside filter -> 2-D chain, then the 2-D reverse chain and the
- * transposed filter there beside the eps stores, and join it back (event) before returning: to the caller everything is
+ * (high-priority) stream from `stream` (event) and run the small kernels there: filter -> 2-D chain beside the field reads,
+ * then the 2-D reverse chain and the transposed filter beside the eps stores; the two HBM-bound kernels stay on `stream`,
+ * which the auxiliary stream joins (event) before the call returns: to the caller everything is
  * still ordered on `stream`, with no host synchronisation, and the calls remain CUDA-graph capturable.  0 = one stream,
  * strictly serial (also used while per-kernel profiling is on).  Results are bitwise identical.                        */
 int epsgrad_plan_set_overlap(epsgrad_plan_t *plan, int enable);
