@@ -57,14 +57,16 @@ def test_design_loop_follows_the_oracle_loop(optimizer):
             # eps well above the square of float32 noise on G' (~1e-7 |G|): the rotated gradient is nearly diagonal in the first
             # iterations and Eq. (13) divides its noise entries by sqrt(noise^2 + eps)
             if i == 1:
-                eps_soap = 1e-4 * float(np.mean(go ** 2))
+                eps_soap = 1e-2 * float(np.mean(go ** 2))
             soap.accumulate(g[0], 0.95)
             soap.refresh()
             soap.update(C[0], g[0], b2=0.95, lr=LR, eps=eps_soap)
             Lo, Ro = O.soap_accumulate(Lo, Ro, go, 0.95)
             Co, Mo, Vo = O.soap_step(Co, Mo, Vo, go, O.soap_eigenbasis(Lo)[0], O.soap_eigenbasis(Ro)[0], i, 0.9, 0.95, LR, eps_soap)
-        # the control variables stay together: steps are ~ LR per iteration, so this is ~1e-3 of the distance travelled
-        assert np.max(np.abs(C[0].cpu().numpy().astype(np.float64) - Co)) < 2e-5 * i, (optimizer, i)
+        # the control variables stay together: steps are ~ LR = 2e-2 per iteration.  SOAP's rotated update N' = M'/sqrt(V' + eps) has
+        # slope 1/sqrt(eps) at the entries that are zero in exact arithmetic, so the 1e-6 parity error of dF/dC shows more there
+        err = np.max(np.abs(C[0].cpu().numpy().astype(np.float64) - Co))
+        assert err < (2e-6 if optimizer == "adam" else 2e-5 * i), (optimizer, i, err)    # measured: 2.7e-7 / 9e-6 after 8 iterations
     assert abs(bmax - bmaxo) < 1e-3 * bmaxo and abs(t - to) < 1e-3 * to
     # both minimise F: for a fixed beta the first-order change is -LR * sum|g|-like, so F falls from the first iteration to the second
     assert F[1] < F[0]

@@ -359,6 +359,7 @@ def test_two_plans_on_two_streams_do_not_interfere():
             assert torch.equal(eps, ref[k][0]) and torch.equal(g, ref[k][1])
 
 
+@pytest.mark.skipif("PYTEST_XDIST_WORKER" in __import__("os").environ, reason="free device memory is shared with the other workers")
 def test_plans_are_released():
     cfg = B.make_config(mx=64, my=64, nz=16, z_lo=6.25, z_hi=9.75, filter_radius=4.0, morph_diameter=2.0)
     C = dev(rand_C(cfg, 3))
