@@ -49,16 +49,18 @@ template <int CJ>
 __device__ __forceinline__ void sobel_at(const float *A, int ci, int cj, int i, int j, int oi, int oj, int nx, int ny,
                                          bool inner, float &gx, float &gy)
 {
-    // one formula for both cases (differences of neighbours first: exact for nearly equal values), so that a cell gets the
-    // same bits whether its tile touches the border of the region or not
-    int rm = -CJ, rp = CJ, cm = -1, cp = 1;
-    if (!inner) {
-        rm = (clampi(i - 1, 0, nx - 1) - i) * CJ; rp = (clampi(i + 1, 0, nx - 1) - i) * CJ;
-        cm = clampi(j - 1, 0, ny - 1) - j;        cp = clampi(j + 1, 0, ny - 1) - j;
+    // one formula for both cases (differences of opposite neighbours first: exact for nearly equal values), so that a cell gets
+    // the same bits whether its tile touches the border of the region or not; only the addressing differs
+    const float *q1 = A + ci * CJ + cj;
+    float a00, a01, a02, a10, a12, a20, a21, a22;
+    if (inner) {
+        const float *q0 = q1 - CJ, *q2 = q1 + CJ;
+        a00 = q0[-1]; a01 = q0[0]; a02 = q0[1]; a10 = q1[-1]; a12 = q1[1]; a20 = q2[-1]; a21 = q2[0]; a22 = q2[1];
+    } else {
+        const float *q0 = q1 + (clampi(i - 1, 0, nx - 1) - i) * CJ, *q2 = q1 + (clampi(i + 1, 0, nx - 1) - i) * CJ;
+        const int cm = clampi(j - 1, 0, ny - 1) - j, cp = clampi(j + 1, 0, ny - 1) - j;
+        a00 = q0[cm]; a01 = q0[0]; a02 = q0[cp]; a10 = q1[cm]; a12 = q1[cp]; a20 = q2[cm]; a21 = q2[0]; a22 = q2[cp];
     }
-    const float *q1 = A + (i - oi) * CJ + (j - oj), *q0 = q1 + rm, *q2 = q1 + rp;
-    const float a00 = q0[cm], a01 = q0[0], a02 = q0[cp], a10 = q1[cm], a12 = q1[cp];
-    const float a20 = q2[cm], a21 = q2[0], a22 = q2[cp];
     gx = ((a20 - a00) + 2.0f * (a21 - a01) + (a22 - a02)) * 0.125f;
     gy = ((a02 - a00) + 2.0f * (a12 - a10) + (a22 - a20)) * 0.125f;
 }
