@@ -69,3 +69,47 @@ def check_vjp(cfg: B.Config, C: np.ndarray, beta: float, EF, EA, plan: B.Plan | 
         worst = max(worst, rel_inf(g[b], ref), rel_l2(g[b], ref))
     assert worst < tol, f"dF/dC relative error {worst:.3e} >= {tol}"
     return worst
+
+
+def check_guard_bands(cfg: B.Config, C, EF, EA, beta: float, guard: int = 4096):
+    """Outputs and workspace between guard bands of `guard` bytes (a multiple of 256: alignment kept) filled with a sentinel:
+    every kind of call must leave the bands untouched and give the bits it gives with plain buffers."""
+    SENT = 0x5A
+    n_pairs = len(EF)
+    plan = B.Plan(cfg)
+    eps0, g0 = plan.eps_forward_vjp(C, beta, EF, EA)
+    gb0, db0 = plan.eps_vjp_beta(C, beta, EF, EA)
+    u0 = plan.unbinarity(C, beta)
+
+    def banded(nbytes):
+        raw = torch.full((nbytes + 2 * guard,), SENT, dtype=torch.uint8, device="cuda")
+        return raw, raw[guard:guard + nbytes]
+
+    def intact(raw, nbytes):
+        return bool((raw[:guard] == SENT).all()) and bool((raw[guard + nbytes:] == SENT).all())
+
+    nws = B.lib().epsgrad_workspace_bytes(plan._h)
+    ws_raw, ws = banded(nws)
+    B._check(B.lib().epsgrad_plan_set_workspace(plan._h, ws.data_ptr(), nws), "epsgrad_plan_set_workspace")
+    e_raw, e_mid = banded(eps0.numel() * 4)
+    g_raw, g_mid = banded(g0.numel() * 4)
+    d_raw, d_mid = banded(db0.numel() * 4)
+    eps = e_mid.view(torch.float32).view(eps0.shape)
+    g = g_mid.view(torch.float32).view(g0.shape)
+    db = d_mid.view(torch.float32).view(db0.shape)
+    plan.eps_forward_vjp(C, beta, EF, EA, eps_out=eps, grad_out=g)
+    torch.cuda.synchronize()
+    assert torch.equal(eps, eps0) and torch.equal(g, g0)
+    eps.zero_(); g.zero_()
+    plan.eps_forward(C, beta, out=eps)
+    plan.eps_vjp(C, beta, EF, EA, out=g)
+    assert torch.equal(eps, eps0) and torch.equal(g, g0)
+    g.zero_()
+    B._check(B.lib().eps_vjp_beta(plan._h, C.data_ptr(), beta, n_pairs, *plan._fields(EF, EA), g.data_ptr(), db.data_ptr(),
+                                  plan._stream()), "eps_vjp_beta")
+    u = plan.unbinarity(C, beta)
+    torch.cuda.synchronize()
+    assert torch.equal(g, g0) and torch.equal(db, db0) and torch.equal(u, u0)
+    for raw, n in ((ws_raw, nws), (e_raw, eps0.numel() * 4), (g_raw, g0.numel() * 4), (d_raw, db0.numel() * 4)):
+        assert intact(raw, n), cfg
+    plan._ws = ws_raw                                          # keep the banded workspace alive as long as the plan

@@ -126,3 +126,15 @@ def test_widebatch_full_size_sampled_windows():
     w = W.BY_NAME["widebatch"]                                  # 8 x 1024x1024 -> 2048x2048x32, Gaussian R = 32
     K = 112
     _check_windows(w, [(0, 0, 0), (3, 400, 512), (7, w.mx - K, w.my - K), (5, w.mx - K, 0)], K)
+
+
+@pytest.mark.parametrize("name", ["paper", "paper_morph"])
+def test_paper_scale_writes_stay_inside_their_buffers(name):
+    # compute-sanitizer is closed on this pool: guard bands around the outputs and the workspace instead (gpu_common)
+    from gpu_common import check_guard_bands
+    w = W.BY_NAME[name]
+    cfg = B.config_of(w)
+    shape = (cfg.batch, 3, cfg.nx, cfg.ny, cfg.nz)
+    gen = torch.Generator(device="cuda").manual_seed(5)
+    mk = lambda: torch.view_as_complex(torch.randn(*shape, 2, device="cuda", generator=gen))
+    check_guard_bands(cfg, dev(W.make_C(w)), [mk()], [mk()], w.betas[0], guard=1 << 20)

@@ -241,3 +241,15 @@ def test_random_configuration_in_x_slabs(i):
         g_sum[:, p["e0"]:p["e1"]] += g_r
     a, b = g_sum.cpu().numpy().astype(np.float64), g0.cpu().numpy().astype(np.float64)
     assert rel_inf(a, b) < 1e-5 * max(1.0, beta / 17.0), (kw, rel_inf(a, b))
+
+
+@pytest.mark.parametrize("i", range(N_CASES))
+def test_random_configuration_writes_stay_inside_their_buffers(i):
+    """compute-sanitizer is closed on this GPU pool, so out-of-bounds writes are looked for directly: the
+    outputs and the plan's workspace sit between guard bands filled with a sentinel, and the bands must come back untouched
+    (and the results unchanged) after every kind of call (gpu_common.check_guard_bands)."""
+    from gpu_common import check_guard_bands
+    kw, beta, n_pairs = draw(i)
+    cfg = B.make_config(**kw)
+    EFn, EAn = rand_fields(cfg, n_pairs, 2000 + i)
+    check_guard_bands(cfg, dev(rand_C(cfg, 1000 + i)), [dev(f) for f in EFn], [dev(f) for f in EAn], beta)
