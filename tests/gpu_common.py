@@ -73,8 +73,10 @@ def check_vjp(cfg: B.Config, C: np.ndarray, beta: float, EF, EA, plan: B.Plan | 
 
 def check_guard_bands(cfg: B.Config, C, EF, EA, beta: float, guard: int = 4096):
     """Outputs and workspace between guard bands of `guard` bytes (a multiple of 256: alignment kept) filled with a sentinel:
-    every kind of call must leave the bands untouched and give the bits it gives with plain buffers."""
-    SENT = 0x5A
+    every kind of call must leave the bands untouched and give the bits it gives with plain buffers.  The sentinel byte 0xFF
+    makes every float a NaN, and the workspace is refilled with it before each call: a kernel that read workspace memory no
+    kernel of the same call had written (the initcheck case) would propagate NaNs into the result."""
+    SENT = 0xFF
     n_pairs = len(EF)
     plan = B.Plan(cfg)
     eps0, g0 = plan.eps_forward_vjp(C, beta, EF, EA)
@@ -100,13 +102,15 @@ def check_guard_bands(cfg: B.Config, C, EF, EA, beta: float, guard: int = 4096):
     plan.eps_forward_vjp(C, beta, EF, EA, eps_out=eps, grad_out=g)
     torch.cuda.synchronize()
     assert torch.equal(eps, eps0) and torch.equal(g, g0)
-    eps.zero_(); g.zero_()
+    eps.zero_(); g.zero_(); ws.fill_(SENT)
     plan.eps_forward(C, beta, out=eps)
+    ws.fill_(SENT)
     plan.eps_vjp(C, beta, EF, EA, out=g)
     assert torch.equal(eps, eps0) and torch.equal(g, g0)
-    g.zero_()
+    g.zero_(); ws.fill_(SENT)
     B._check(B.lib().eps_vjp_beta(plan._h, C.data_ptr(), beta, n_pairs, *plan._fields(EF, EA), g.data_ptr(), db.data_ptr(),
                                   plan._stream()), "eps_vjp_beta")
+    ws.fill_(SENT)
     u = plan.unbinarity(C, beta)
     torch.cuda.synchronize()
     assert torch.equal(g, g0) and torch.equal(db, db0) and torch.equal(u, u0)
