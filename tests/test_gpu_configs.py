@@ -138,3 +138,28 @@ def test_paper_scale_writes_stay_inside_their_buffers(name):
     gen = torch.Generator(device="cuda").manual_seed(5)
     mk = lambda: torch.view_as_complex(torch.randn(*shape, 2, device="cuda", generator=gen))
     check_guard_bands(cfg, dev(W.make_C(w)), [mk()], [mk()], w.betas[0], guard=1 << 20)
+
+
+@pytest.mark.parametrize("name", ["paper", "paper_morph"])
+def test_repeated_calls_give_the_same_bits(name):
+    # a race between the kernels of the two-stream schedule (or inside one) would show as run-to-run differences: 60 calls
+    # back to back, half of them with a second plan hammering the GPU on another stream
+    w = W.BY_NAME[name]
+    cfg = B.config_of(w)
+    shape = (cfg.batch, 3, cfg.nx, cfg.ny, cfg.nz)
+    gen = torch.Generator(device="cuda").manual_seed(6)
+    mk = lambda: torch.view_as_complex(torch.randn(*shape, 2, device="cuda", generator=gen))
+    C, EF, EA = dev(W.make_C(w)), [mk()], [mk()]
+    plan, other = B.Plan(cfg), B.Plan(cfg)
+    eps0, g0 = plan.eps_forward_vjp(C, w.betas[0], EF, EA)
+    gb0, db0 = plan.eps_vjp_beta(C, w.betas[0], EF, EA)
+    side = torch.cuda.Stream()
+    eps, g = torch.empty_like(eps0), torch.empty_like(g0)
+    for rep in range(60):
+        if rep % 2:
+            with torch.cuda.stream(side):
+                other.eps_forward_vjp(C, w.betas[0], EF, EA)
+        plan.eps_forward_vjp(C, w.betas[0], EF, EA, eps_out=eps, grad_out=g)
+        gb, db = plan.eps_vjp_beta(C, w.betas[0], EF, EA)
+        assert torch.equal(eps, eps0) and torch.equal(g, g0) and torch.equal(gb, gb0) and torch.equal(db, db0), rep
+    torch.cuda.synchronize()
