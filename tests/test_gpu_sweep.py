@@ -17,16 +17,18 @@ from paper_2505_03352_b200 import binding as B
 pytestmark = pytest.mark.gpu
 
 UP_SUB = [(1, 2), (2, 2), (1, 4), (3, 2), (1, 6), (2, 4), (4, 2), (1, 8)]       # upsample * subpixel in {2, 4, 6, 8}
+SCALE = int(os.environ.get("EPSGRAD_SWEEP_SCALE", "1"))          # 3: grids up to 216 cells (mask pixels per control pixel <= 4 only: oracle time)
 N_CASES = int(os.environ.get("EPSGRAD_SWEEP_CASES", "40"))      # a longer hunt: EPSGRAD_SWEEP_CASES=400 pytest tests/test_gpu_sweep.py
 
 
 def draw(i: int):
     """Case i of the sweep: (config kwargs, beta, n_pairs).  Sizes are bounded so the oracle takes about a second."""
     rng = np.random.default_rng([20250503, i])
-    u, s = UP_SUB[i % len(UP_SUB)]
-    cells = int(rng.integers(6, 72))                                  # Yee cells along x: below, at and above 16, 32, 48, 64
+    pairs = UP_SUB if SCALE == 1 else [(1, 2), (2, 2), (1, 4)]
+    u, s = pairs[i % len(pairs)]
+    cells = int(rng.integers(6, 72)) * SCALE                          # Yee cells along x: below, at and above 16, 32, 48, 64
     mx = max(1, round(cells / u))
-    my = max(1, round(int(rng.integers(6, 72)) / u))
+    my = max(1, round(int(rng.integers(6, 72)) * SCALE / u))
     nz = 4 * int(rng.integers(1, 11))
     kind = int(rng.random() < 0.3)
     kw = dict(batch=int(rng.integers(1, 4)) if i % 5 == 0 else 1, mx=mx, my=my, nz=nz, upsample=u, subpixel=s, filter_kind=kind)
