@@ -328,7 +328,18 @@ def test_error_codes():
     with pytest.raises(B.EpsgradError) as e:
         plan.eps_vjp(torch.rand(plan.ctrl_shape, device="cuda"), 8.0, [f], [f])
     assert e.value.status == B.EUNSUPPORTED
+    # empty inputs: no design, no control pixel, no field pair
+    for kw in (dict(batch=0, mx=8, my=8), dict(mx=0, my=8), dict(mx=8, my=0)):
+        with pytest.raises(B.EpsgradError) as e:
+            B.Plan(B.make_config(**dict(dict(nz=8, z_lo=2.0, z_hi=5.0), **kw)))
+        assert e.value.status == B.EINVAL
     plan = B.Plan(B.make_config(mx=8, my=8, nz=8, z_lo=2.0, z_hi=5.0))
+    Cd, gd = torch.rand(plan.ctrl_shape, device="cuda"), torch.empty(plan.ctrl_shape, device="cuda")
+    assert B.lib().eps_vjp(plan._h, Cd.data_ptr(), 8.0, 0, None, None, gd.data_ptr(), None) == B.EINVAL
+    assert B.lib().eps_vjp(plan._h, Cd.data_ptr(), 8.0, 1, None, None, gd.data_ptr(), None) == B.EINVAL
+    assert B.lib().eps_forward(plan._h, None, 8.0, gd.data_ptr(), None) == B.EINVAL
+    assert B.lib().eps_forward(plan._h, Cd.data_ptr(), float("nan"), gd.data_ptr(), None) == B.EINVAL
+    assert B.lib().eps_forward(plan._h, Cd.data_ptr() + 4, 8.0, gd.data_ptr(), None) == B.EINVAL      # misaligned
     with pytest.raises(B.EpsgradError) as e:
         plan.eps_forward(torch.rand(plan.ctrl_shape, device="cuda"), -1.0)
     assert e.value.status == B.EINVAL
