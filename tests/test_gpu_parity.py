@@ -328,6 +328,10 @@ def test_error_codes():
     with pytest.raises(B.EpsgradError) as e:
         plan.eps_vjp(torch.rand(plan.ctrl_shape, device="cuda"), 8.0, [f], [f])
     assert e.value.status == B.EUNSUPPORTED
+    # beyond the 32-bit plane indices: refused at plan creation, before anything is allocated
+    with pytest.raises(B.EpsgradError) as e:
+        B.Plan(B.make_config(batch=64, mx=4096, my=4096, nz=32, z_lo=14.25, z_hi=17.75))
+    assert e.value.status == B.EUNSUPPORTED
     # empty inputs: no design, no control pixel, no field pair
     for kw in (dict(batch=0, mx=8, my=8), dict(mx=0, my=8), dict(mx=8, my=0)):
         with pytest.raises(B.EpsgradError) as e:
