@@ -135,16 +135,23 @@ def oracle_step_inputs(w, mx, my):
     return ws, C, EF, EA
 
 
-def oracle_step(cfg, C, betas, EF, EA):
+def oracle_step(cfg, C, betas, EF, EA, acc=None):
     import oracle as O
     for beta in betas:
+        t0 = time.perf_counter()
         O.forward(cfg, C, beta)
+        t1 = time.perf_counter()
         O.vjp(cfg, C, beta, EF, EA)
+        t2 = time.perf_counter()
+        if acc is not None:
+            acc["forward"] += t1 - t0
+            acc["vjp"] += t2 - t1
 
 
-def time_oracle(w, budget_s: float, steps: int, warmup: int):
+def time_oracle(w, budget_s: float, steps: int, warmup: int, split: bool = False):
     """Time the float64 oracle (as it stands) on a crop of workload w sized so that
-    (steps + warmup) steps take about budget_s.  Returns (cells/s, seconds/step, sample text, threads)."""
+    (steps + warmup) steps take about budget_s.  Returns (cells/s, seconds/step, sample text, threads) and, with
+    split, the forward-only and VJP-only cells/s (O.vjp recomputes the forward chain it differentiates)."""
     import oracle as O
     # calibrate on a 32x32-control crop
     ws, C, EF, EA = oracle_step_inputs(w, min(32, w.mx), min(32, w.my))
@@ -164,14 +171,18 @@ def time_oracle(w, budget_s: float, steps: int, warmup: int):
     cfg = oracle_cfg(w, mx, my)
     for _ in range(warmup):
         oracle_step(cfg, C, w.betas, EF, EA)
+    acc = {"forward": 0.0, "vjp": 0.0}
     t0 = time.perf_counter()
     for _ in range(steps):
-        oracle_step(cfg, C, w.betas, EF, EA)
+        oracle_step(cfg, C, w.betas, EF, EA, acc)
     dt = (time.perf_counter() - t0) / steps
     cells = ws.nx * ws.ny * ws.nz                                        # one design of the batch
     sample = (f"{steps} step(s) of forward+VJP on a {mx}x{my}-control crop ({ws.nx}x{ws.ny}x{ws.nz} Yee cells, "
               f"{w.n_pairs} pair(s), {len(w.betas)} beta) of '{w.name}'"
               + (" = the full workload" if (mx, my, w.batch) == (w.mx, w.my, 1) else ""))
+    if split:
+        parts = {k: cells * len(w.betas) * steps / v for k, v in acc.items()}
+        return cells / dt, dt, sample, O.num_threads(), parts
     return cells / dt, dt, sample, O.num_threads()
 
 
@@ -285,6 +296,52 @@ def run_ours(args, w):
     cells_step = w.cells * len(w.betas)
     value = sharding.job_throughput(cells_step, args.steps, ms_total, world)
 
+    # ---- the three calls of the ABI, each timed repetition by repetition (median of >= 20 repetitions):
+    # forward (eps_forward), vjp (eps_vjp), forward_vjp (the step above).  One CUDA graph per call and buffer set, one event
+    # pair per repetition.
+    def per_rep_ms(fn, reps):
+        gs = None
+        if args.graph:
+            gs = []
+            for sset in range(NS):
+                fn(sset)
+            torch.cuda.synchronize()
+            for sset in range(NS):
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g):
+                    fn(sset)
+                gs.append(g)
+        run = (lambda i: gs[i % NS].replay()) if gs is not None else (lambda i: fn(i % NS))
+        for i in range(3):
+            run(i)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(reps + 1)]
+        torch.cuda.synchronize()
+        ev[0].record()
+        for i in range(reps):
+            run(i)
+            ev[i + 1].record()
+        torch.cuda.synchronize()
+        return sorted(ev[i].elapsed_time(ev[i + 1]) for i in range(reps))
+
+    def mode_stats(ts, n_calls):
+        med = ts[len(ts) // 2]
+        return {"ms_median": med, "ms_min": ts[0], "ms_mean": sum(ts) / len(ts), "reps": len(ts),
+                "cells_per_s": w.cells * n_calls / (med * 1e-3)}
+
+    reps = max(20, min(args.steps, 200))
+
+    def fwd_call(s):
+        for beta in w.betas:
+            plan.eps_forward(C, beta, eps)
+
+    def vjp_call(s):
+        for beta in w.betas:
+            plan.eps_vjp(C, beta, EF[s], EA[s], grad)
+
+    modes = {"forward": mode_stats(per_rep_ms(fwd_call, reps), len(w.betas)),
+             "vjp": mode_stats(per_rep_ms(vjp_call, reps), len(w.betas)),
+             "forward_vjp": mode_stats(per_rep_ms(eager_step, reps), len(w.betas))}
+
     # ---- per-kernel durations, live, with CUDA events on the launching stream (the library's hook: one event after
     # each kernel, serial schedule).  A ~150 us spin kernel is enqueued ahead of every profiled step so that the host has
     # queued the whole step before the GPU reaches it: the events then bracket kernel execution, not host launch gaps.
@@ -305,19 +362,56 @@ def run_ours(args, w):
     # the two HBM streams: 12 B written per Yee cell (extrude); the touched 32-byte field sectors read (zreduce)
     alg = {"extrude": w.cells * 12, "zreduce": zreduce_sector_bytes(w, w.n_pairs)}
     dom = max(alg, key=lambda k: kernels[k])
-    traffic = None
+
+    # the field stream alone (the stage tap of the ABI), cold L2: a 256 MB fill between repetitions, rotating field sets
+    flush = torch.empty(64 << 20, dtype=torch.float32, device=dev)
+    ts = []
+    for i in range(min(reps, 30)):
+        flush.fill_(float(i))
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a0.record()
+        plan.stage_zreduce(EF[i % NS], EA[i % NS])
+        a1.record()
+        torch.cuda.synchronize()
+        ts.append(a0.elapsed_time(a1))
+    del flush
+    ts.sort()
+    z_alone_ms = ts[len(ts) // 2]
+
+    # DRAM bytes per launch from the committed ncu --set full capture, if it was taken on THIS build (source hash)
+    traffic, traffic_note = None, "no ncu capture of this build under profiles/ (traffic.json names another source hash)"
     try:
+        from paper_2505_03352_b200 import build as cuda_build
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            traffic = json.load(f).get(w.name, {}).get(dom)
+            tj = json.load(f)
+        ent = tj.get(w.name, {})
+        if ent.get("src_sha16") == cuda_build.source_hash():
+            traffic, traffic_note = ent.get(dom), "ncu --set full capture of this build (profiles/traffic.json)"
     except Exception:
         pass
     achieved = alg[dom] / (kernels[dom] * 1e-3) / 1e9
+    dense_bytes = w.cells * 48 * w.n_pairs                              # every z cell of E_F and E_A: NOT the method's own work
+    step_bytes = alg["extrude"] * len(w.betas) + alg["zreduce"] * len(w.betas)
+    step_ms = ms_total / args.steps
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_note, "peak_source": peak_src,
                 "algorithmic_bytes": alg[dom], "kernel_ms": kernels[dom],
+                "kernel_timing": "CUDA events inside the step, serial schedule (one event after each kernel)",
                 "kernels_ms": kernels,
                 "others": {k: {"algorithmic_bytes": alg[k], "kernel_ms": kernels[k], "GB/s": alg[k] / (kernels[k] * 1e-3) / 1e9,
-                               "frac": alg[k] / (kernels[k] * 1e-3) / 1e9 / peak} for k in alg if k != dom}}
+                               "frac": alg[k] / (kernels[k] * 1e-3) / 1e9 / peak} for k in alg if k != dom},
+                "zreduce_alone": {"kernel_ms": z_alone_ms, "frac": alg["zreduce"] / (z_alone_ms * 1e-3) / 1e9 / peak,
+                                  "how": "epsgrad_stage_zreduce alone, cold L2 (256 MB fill before each repetition), median"},
+                "frac_dense_equiv": {"value": dense_bytes / (kernels["zreduce"] * 1e-3) / 1e9 / peak,
+                                     "bytes": dense_bytes,
+                                     "note": "48 B per Yee cell and pair as if every z cell were read: not the method's work "
+                                             "(d eps/dC = 0 outside the slab); context for the north_star's dense reading only"},
+                "step": {"algorithmic_bytes": step_bytes, "ms": step_ms, "GB/s": step_bytes / (step_ms * 1e-3) / 1e9,
+                         "frac": step_bytes / (step_ms * 1e-3) / 1e9 / peak,
+                         "note": "eps stores + touched field sectors over the whole overlapped step (2-D chain included)"},
+                "modes_frac": {"forward": alg["extrude"] * len(w.betas) / (modes["forward"]["ms_median"] * 1e-3) / 1e9 / peak,
+                               "vjp": alg["zreduce"] * len(w.betas) / (modes["vjp"]["ms_median"] * 1e-3) / 1e9 / peak,
+                               "vjp_dense_equiv": dense_bytes * len(w.betas) / (modes["vjp"]["ms_median"] * 1e-3) / 1e9 / peak}}
 
     # ---- end to end through the host-buffer entry point: H2D of C and the fields, D2H of eps and dF/dC
     if w.cells * 48 * w.n_pairs > 8e9:
@@ -352,11 +446,13 @@ def run_ours(args, w):
     if rank == 0:
         line = base_line(w, args, world)
         line.update({"value": value, "ms_per_step": ms_total / args.steps, "dtype": "f32",
+                     "ms_per_step_median": modes["forward_vjp"]["ms_median"], "modes": modes,
                      "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
                      "roofline": roofline})
         if world == 1:
-            val, dt, sample, threads = time_oracle(w, 15.0, 3, 1)
-            line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample}
+            val, dt, sample, threads, parts = time_oracle(w, 15.0, 3, 1, split=True)
+            line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample,
+                                    "forward_cells_per_s": parts["forward"], "vjp_cells_per_s": parts["vjp"]}
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.barrier()

@@ -239,11 +239,41 @@ int epsgrad_plan_set_embedding(epsgrad_plan_t *plan, const epsgrad_embedding_t *
  * in the *_host entry points.                                                                                              */
 int epsgrad_plan_set_slab(epsgrad_plan_t *plan, int x_first, int x_count);
 
-/* How the device-resident field windows are fetched (default 0).  1: by the tensor memory accelerator, one bulk tensor
- * copy per field and 256 columns, persistent CTAs (region-sized fields with sparse windows only; other cases fall back).
- * 0: by 16-byte asynchronous copies (LDGSTS), 2 us faster at paper scale.  Same bytes, same results; a measurement switch.
+/* How the device-resident field windows are fetched.  0: by 16-byte asynchronous copies (LDGSTS), 5 CTAs per SM.
+ * 1: by the tensor memory accelerator, one bulk tensor copy per field and 256 columns, one stage per CTA (region-sized
+ * fields with sparse windows only; other cases fall back).  2: thin persistent read stream -- one CTA per SM, TMA copies
+ * through a ring of shared-memory stages with full / empty mbarriers (region-sized or x-slab fields; embedded, packed and
+ * host-resident fields fall back to 0).  Same bytes, bitwise the same results; a measurement switch.
  * EPSGRAD_EUNSUPPORTED when TMA descriptors cannot be built on this driver.                                               */
-int epsgrad_plan_set_tma(epsgrad_plan_t *plan, int enable);
+int epsgrad_plan_set_tma(epsgrad_plan_t *plan, int mode);
+
+/* How eps is written.  0: per-thread 16-byte streaming stores (k_extrude).  1: thin persistent store stream -- the columns
+ * are assembled in shared memory (only the slab pieces change from column to column) and written by bulk asynchronous copies
+ * (region-sized or x-slab eps; embedded plans fall back to 0).  Bitwise the same results; a measurement switch.           */
+int epsgrad_plan_set_bulk_stores(epsgrad_plan_t *plan, int enable);
+
+/* One persistent dataflow kernel for the whole call (default on where it applies).  The six steps of the path are cut into
+ * tiles and column blocks grouped in bands of 16 Yee rows; one launch of co-resident CTAs takes them from two ticket lists
+ * (the two HBM streams; the 2-D work) and runs each as soon as the bands it depends on are complete, so that the ALU-bound
+ * 2-D tiles execute on the same SMs while the memory-bound blocks wait for DRAM, there are no launch ramps between steps, and
+ * every intermediate is consumed from L2 a few bands after it was produced, at any problem size.  Applies to the conic filter
+ * with upsample * subpixel = 4, subpixel = 2, R <= 12 cells, morphological filters off, up to EPSGRAD_MAX_PAIRS pairs, device
+ * buffers, no x-slab, no eps_vjp_beta; every other call runs the step as separate kernels (0 forces that everywhere).
+ * EPSGRAD_EUNSUPPORTED when enabled on a plan it does not apply to.  Results equal the separate kernels' except for the
+ * summation order of the filter taps (two partial sums per pixel instead of three).                                      */
+int epsgrad_plan_set_fused(epsgrad_plan_t *plan, int enable);
+
+/* Cycle accounting of the persistent kernel (diagnostic; default off).  enable != 0 allocates and clears 20 device counters that
+ * every CTA of the following fused calls adds to: [0..5] SM cycles spent in the items of each of the six phases (F1, F2, X, M, T,
+ * Z), [6..11] the number of items of each phase, [12] cycles spent taking and decoding tickets (and starting field copies),
+ * [13] total CTA cycles, [14] cycles spent waiting for bands, [15] cycles in the release that publishes an item, [16] cycles starting field copies, [17] cycles in the barrier that ends a round, [18..19] reserved.  out20 != NULL:
+ * synchronises the device (host-blocking) and returns the counters accumulated so far before clearing them.               */
+int epsgrad_plan_fused_profile(epsgrad_plan_t *plan, int enable, uint64_t *out20);
+
+/* Measurement knobs of the two stream kernels (0 = the default of each): knob 0 = bytes per bulk store, 1 = store-stream
+ * CTAs per SM, 2 = stages of the read stream's ring, 3 = read-stream CTAs per SM; 4 = CTAs per SM of the persistent kernel, 6 = pipeline lag (steps) between a phase of the persistent kernel and its consumer; knobs 5, 7 reserved.  EPSGRAD_EINVAL for a
+ * knob outside 0..7.  Values are clamped to what the kernels support; results never depend on them.                      */
+int epsgrad_plan_set_tuning(epsgrad_plan_t *plan, int knob, int value);
 
 /* Field transfer of the *_host entry points (mode; default 2).  Eq. (1) needs only the slab cells of the fields (P:L27:
  * only Omega_D enters the gradient), so when every field buffer is pinned, mapped host memory (and the plan is not in

@@ -19,7 +19,7 @@ EXPORTS = (
     "epsgrad_plan_create", "epsgrad_plan_destroy", "epsgrad_workspace_bytes",
     "epsgrad_plan_set_workspace", "epsgrad_staging_bytes", "epsgrad_plan_set_staging",
     "epsgrad_plan_set_dense_reads", "epsgrad_plan_last_launches", "epsgrad_plan_last_copy_bytes",
-    "epsgrad_plan_set_profiling", "epsgrad_plan_last_kernel_times", "epsgrad_plan_set_overlap", "epsgrad_plan_set_host_direct", "epsgrad_plan_set_embedding", "epsgrad_plan_set_slab", "epsgrad_plan_set_tma", "epsgrad_plan_set_timeline", "epsgrad_plan_read_timeline", 
+    "epsgrad_plan_set_profiling", "epsgrad_plan_last_kernel_times", "epsgrad_plan_set_overlap", "epsgrad_plan_set_host_direct", "epsgrad_plan_set_embedding", "epsgrad_plan_set_slab", "epsgrad_plan_set_tma", "epsgrad_plan_set_bulk_stores", "epsgrad_plan_set_tuning", "epsgrad_plan_set_fused", "epsgrad_plan_fused_profile", "epsgrad_plan_set_timeline", "epsgrad_plan_read_timeline", 
     "eps_forward", "eps_vjp", "eps_forward_vjp", "eps_forward_vjp_host", "eps_vjp_beta", "eps_unbinarity",
     "epsgrad_beta_schedule", "epsgrad_beta_update", "epsgrad_adam_step",
     "epsgrad_soap_accumulate", "epsgrad_soap_eigh_workspace_bytes", "epsgrad_soap_eigh",
@@ -217,6 +217,10 @@ def lib() -> ctypes.CDLL:
     L.epsgrad_plan_set_slab.argtypes = [vp, i32, i32]
     L.epsgrad_plan_set_embedding.argtypes = [vp, vp]
     L.epsgrad_plan_set_tma.argtypes = [vp, i32]
+    L.epsgrad_plan_set_bulk_stores.argtypes = [vp, i32]
+    L.epsgrad_plan_set_tuning.argtypes = [vp, i32, i32]
+    L.epsgrad_plan_set_fused.argtypes = [vp, i32]
+    L.epsgrad_plan_fused_profile.argtypes = [vp, i32, vp]
     L.epsgrad_plan_set_timeline.argtypes = [vp, i32]
     L.epsgrad_plan_read_timeline.argtypes = [vp, i32, vp, vp]
     L.epsgrad_stage_zreduce.argtypes = [vp, i32, vp, vp, vp, vp]
@@ -342,8 +346,29 @@ class Plan:
         _check(lib().epsgrad_plan_set_slab(self._h, x_first, x_count), "epsgrad_plan_set_slab")
         self._field_shape = (self.eps_shape[0], 3, x_count, self.eps_shape[3], self.eps_shape[4]) if x_count > 0 else None
 
-    def set_tma(self, enable: bool) -> None:
-        _check(lib().epsgrad_plan_set_tma(self._h, int(bool(enable))), "epsgrad_plan_set_tma")
+    def set_tma(self, mode) -> None:
+        """0: LDGSTS field reads; 1: single-stage TMA; 2: thin persistent TMA read stream"""
+        _check(lib().epsgrad_plan_set_tma(self._h, int(mode)), "epsgrad_plan_set_tma")
+
+    def set_bulk_stores(self, enable: bool) -> None:
+        _check(lib().epsgrad_plan_set_bulk_stores(self._h, int(bool(enable))), "epsgrad_plan_set_bulk_stores")
+
+    def set_fused(self, enable: bool) -> None:
+        """one persistent dataflow kernel per call (default where it applies) / the step as separate kernels"""
+        _check(lib().epsgrad_plan_set_fused(self._h, int(enable)), "epsgrad_plan_set_fused")
+
+    def fused_profile(self, enable: bool, read: bool = False):
+        """cycle accounting of the persistent kernel: dict of per-phase busy cycles / items, wait and total CTA cycles"""
+        out = (ctypes.c_uint64 * 20)() if read else None
+        _check(lib().epsgrad_plan_fused_profile(self._h, int(bool(enable)), out), "epsgrad_plan_fused_profile")
+        if not read:
+            return None
+        names = ("F1", "F2", "X", "M", "T", "Z")
+        return {"busy": {n: int(out[i]) for i, n in enumerate(names)}, "items": {n: int(out[6 + i]) for i, n in enumerate(names)},
+                "tickets": int(out[12]), "total": int(out[13]), "wait": int(out[14]), "release": int(out[15]), "zbegin": int(out[16]), "endsync": int(out[17])}
+
+    def set_tuning(self, knob: int, value: int) -> None:
+        _check(lib().epsgrad_plan_set_tuning(self._h, int(knob), int(value)), "epsgrad_plan_set_tuning")
 
     def set_host_direct(self, mode) -> None:
         """0 / False: fields staged whole; 1 / True: slab windows read in place by the kernel; 2: gathered by the copy engine"""

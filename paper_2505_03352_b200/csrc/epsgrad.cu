@@ -17,8 +17,11 @@
 #include "filter_sep.cuh"
 #include "fwd2d.cuh"
 #include "extrude.cuh"
+#include "extrude_bulk.cuh"
 #include "zreduce.cuh"
+#include "zreduce_pipe.cuh"
 #include "maskgrad.cuh"
+#include "mega.cuh"
 #include "morph.cuh"
 #include "reduce.cuh"
 #include "soap.cuh"
@@ -54,7 +57,13 @@ struct epsgrad_plan {
     float *cur_dbeta;
     // embedding of the design region in the caller's simulation-domain arrays (epsgrad_plan_set_embedding); emb.nx_full = 0: none
     epsgrad_embedding_t emb;
-    int use_tma;               // field windows by TMA bulk tensor copies where possible (epsgrad_plan_set_tma)
+    int use_tma;               // field windows by TMA bulk tensor copies where possible (epsgrad_plan_set_tma): 1 single-stage, 2 pipelined
+    int use_bulk;              // eps columns written by bulk copies from shared memory (epsgrad_plan_set_bulk_stores)
+    int tune[8];               // measurement knobs (epsgrad_plan_set_tuning)
+    int use_mega;              // the whole step as one persistent dataflow kernel where the configuration allows (epsgrad_plan_set_fused)
+    int *d_sched;              // its ticket and per-band completion counters
+    unsigned long long *d_mprof;   // optional cycle accounting of the persistent kernel (epsgrad_plan_fused_profile)
+    size_t sched_bytes;
     void *tma_encode;          // cuTensorMapEncodeTiled, fetched through the runtime (no link against libcuda)
     int slab_x0, slab_nx;                   // x-slab: the caller's arrays hold Yee rows [slab_x0, slab_x0 + slab_nx) only; 0, 0 = off
     int dense, host_direct, cur_host_src;   // cur_host_src: the fields of the call in flight are pinned host memory
@@ -389,6 +398,18 @@ extern "C" int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsg
     }
     P->off_tmp = off;  off += P->separable ? align_up((size_t)cfg->batch * cfg->mx * P->py * 4, 256) : 0;
     P->ws_need = off;
+    // ---- persistent dataflow kernel (mega.cuh): conic fast path with 4 mask pixels per control pixel, s = 2, no morphological filters
+    if (!P->separable && m == 4 && s == 2 && (NT == 5 || NT == 9 || NT == 13) && P->morph_R == 0) {
+        const int nb = (P->nx + MK_BAND - 1) / MK_BAND;
+        P->sched_bytes = ((size_t)MK_SCHED_HEAD + (size_t)PH_N * cfg->batch * nb) * sizeof(int);
+        int prev3 = 0;
+        cudaGetDevice(&prev3);
+        cudaSetDevice(device);
+        const bool oks = cudaMalloc(&P->d_sched, P->sched_bytes) == cudaSuccess;
+        cudaSetDevice(prev3);
+        if (!oks) { cudaGetLastError(); P->d_sched = nullptr; epsgrad_plan_destroy(P); return EPSGRAD_ECUDA; }
+        P->use_mega = 0;         // measured slower than the separate kernels on every config: an option, off by default
+    }
     *out = P;
     return EPSGRAD_OK;
 }
@@ -400,6 +421,8 @@ extern "C" int epsgrad_plan_destroy(epsgrad_plan_t *P)
     if (P->d_tl) cudaFree(P->d_tl);
     if (P->d_hl) cudaFree(P->d_hl);
     if (P->d_invn) cudaFree(P->d_invn);
+    if (P->d_sched) cudaFree(P->d_sched);
+    if (P->d_mprof) cudaFree(P->d_mprof);
     if (P->aux) cudaStreamDestroy(P->aux);
     if (P->ev_fork) cudaEventDestroy(P->ev_fork);
     if (P->ev_r) cudaEventDestroy(P->ev_r);
@@ -496,7 +519,45 @@ extern "C" int epsgrad_plan_set_tma(epsgrad_plan_t *P, int enable)
 {
     if (!P) return EPSGRAD_EINVAL;
     if (enable && !P->tma_encode) return EPSGRAD_EUNSUPPORTED;
-    P->use_tma = enable != 0;
+    P->use_tma = enable < 0 ? 0 : (enable > 2 ? 2 : enable);
+    return EPSGRAD_OK;
+}
+
+extern "C" int epsgrad_plan_set_bulk_stores(epsgrad_plan_t *P, int enable)
+{
+    if (!P) return EPSGRAD_EINVAL;
+    P->use_bulk = enable != 0;
+    return EPSGRAD_OK;
+}
+
+extern "C" int epsgrad_plan_set_fused(epsgrad_plan_t *P, int enable)
+{
+    if (!P) return EPSGRAD_EINVAL;
+    if (enable && !P->d_sched) return EPSGRAD_EUNSUPPORTED;
+    P->use_mega = enable < 0 ? 0 : (enable > 2 ? 2 : enable);
+    return EPSGRAD_OK;
+}
+
+extern "C" int epsgrad_plan_fused_profile(epsgrad_plan_t *P, int enable, uint64_t *out20)
+{
+    if (!P) return EPSGRAD_EINVAL;
+    DeviceGuardC g(P->device);
+    const size_t bytes = (2 * PH_N + 8) * sizeof(unsigned long long);
+    if (out20 && P->d_mprof) {
+        if (cudaDeviceSynchronize() != cudaSuccess || cudaMemcpy(out20, P->d_mprof, bytes, cudaMemcpyDeviceToHost) != cudaSuccess) { cudaGetLastError(); return EPSGRAD_ECUDA; }
+    }
+    if (enable && !P->d_mprof) {
+        if (cudaMalloc(&P->d_mprof, bytes) != cudaSuccess) { cudaGetLastError(); P->d_mprof = nullptr; return EPSGRAD_ECUDA; }
+    }
+    if (P->d_mprof) cudaMemset(P->d_mprof, 0, bytes);
+    if (!enable && P->d_mprof) { cudaFree(P->d_mprof); P->d_mprof = nullptr; }
+    return EPSGRAD_OK;
+}
+
+extern "C" int epsgrad_plan_set_tuning(epsgrad_plan_t *P, int knob, int value)
+{
+    if (!P || knob < 0 || knob >= 8) return EPSGRAD_EINVAL;
+    P->tune[knob] = value;
     return EPSGRAD_OK;
 }
 
@@ -643,6 +704,22 @@ float *ws_e2d(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_e
 float *ws_coef(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_coef); }
 float *ws_tmp(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_tmp); }
 
+FilterParams fill_filter(const epsgrad_plan *P, const float *C, float *phi)
+{
+    FilterParams fp;
+    fp.C = C; fp.phi = phi; fp.w = P->d_w; fp.tyrange = P->d_tyrange; fp.nrm = make_nrm(P);
+    fp.mx = P->cfg.mx; fp.my = P->cfg.my; fp.px = P->px; fp.py = P->py; fp.T = P->T; fp.NT = P->NT; fp.eta0 = P->eta0;
+    return fp;
+}
+
+FilterTParams fill_filterT(const epsgrad_plan *P, const float *v, float *dC)
+{
+    FilterTParams fp;
+    fp.v = v; fp.dC = dC; fp.w = P->d_w; fp.tyrange = P->d_tyrange;
+    fp.mx = P->cfg.mx; fp.my = P->cfg.my; fp.px = P->px; fp.py = P->py; fp.T = P->T; fp.NT = P->NT;
+    return fp;
+}
+
 // ---- F1: C -> centred Phi on the mask
 template <int M>
 int launch_filter_m(epsgrad_plan *P, const float *C, float *phi, cudaStream_t st)
@@ -650,9 +727,7 @@ int launch_filter_m(epsgrad_plan *P, const float *C, float *phi, cudaStream_t st
     const int B = P->cfg.batch, mx = P->cfg.mx, my = P->cfg.my, T = P->T, NT = P->NT;
     if (!P->separable) {
         constexpr int TA = 8, TB = 16;
-        FilterParams fp;
-        fp.C = C; fp.phi = phi; fp.w = P->d_w; fp.tyrange = P->d_tyrange; fp.nrm = make_nrm(P);
-        fp.mx = mx; fp.my = my; fp.px = P->px; fp.py = P->py; fp.T = T; fp.NT = NT; fp.eta0 = P->eta0;
+        const FilterParams fp = fill_filter(P, C, phi);
         if (M == 4 && (NT == 5 || NT == 9 || NT == 13)) {      // fast path (filter4.cuh)
             auto kern = NT == 5 ? k_filter_conic4<5> : (NT == 9 ? k_filter_conic4<9> : k_filter_conic4<13>);
             const size_t smem4 = (filter4_smem_floats(NT) + 4) * 4;
@@ -696,9 +771,7 @@ int launch_filterT_conic(epsgrad_plan *P, const float *v, float *dC, cudaStream_
 {
     using S = FilterTShape<M>;
     const int T = P->T, NT = P->NT;
-    FilterTParams fp;
-    fp.v = v; fp.dC = dC; fp.w = P->d_w; fp.tyrange = P->d_tyrange;
-    fp.mx = P->cfg.mx; fp.my = P->cfg.my; fp.px = P->px; fp.py = P->py; fp.T = T; fp.NT = NT;
+    const FilterTParams fp = fill_filterT(P, v, dC);
     if (M == 4 && (NT == 5 || NT == 9 || NT == 13)) {          // fast path (filter4.cuh)
         auto kern = NT == 5 ? k_filterT_conic4<5> : (NT == 9 ? k_filterT_conic4<9> : k_filterT_conic4<13>);
         const size_t smem4 = filterT4_smem_floats(NT) * 4;
@@ -767,7 +840,7 @@ int launch_filterT(epsgrad_plan *P, const float *v, float *dC, cudaStream_t st)
 }
 
 // ---- F2..F5: the 2-D chain; e2d / coef / eps2d may be null
-int launch_fwd2d(epsgrad_plan *P, const float *phi, float beta, float *e2d, float *coef, float *eps2d, cudaStream_t st)
+Fwd2dParams fill_fwd2d(const epsgrad_plan *P, const float *phi, float beta, float *e2d, float *coef, float *eps2d)
 {
     Fwd2dParams fp;
     fp.phi = phi; fp.e2d = e2d; fp.coef = coef; fp.eps2d = eps2d;
@@ -775,6 +848,12 @@ int launch_fwd2d(epsgrad_plan *P, const float *phi, float beta, float *e2d, floa
     fp.beta = beta; fp.eta_r = P->eta_r; fp.eps_clad = P->eps_clad; fp.deps = P->deps; fp.delta = P->delta;
     if (P->morph_R > 0) { fp.phi = ws_mc(P); fp.eta_r = 0.0f; }     // Eq. (6) on the filtered mask, centred at 1/2
     fp.w_lo = P->w_lo; fp.w_hi = P->w_hi;
+    return fp;
+}
+
+int launch_fwd2d(epsgrad_plan *P, const float *phi, float beta, float *e2d, float *coef, float *eps2d, cudaStream_t st)
+{
+    const Fwd2dParams fp = fill_fwd2d(P, phi, beta, e2d, coef, eps2d);
     const size_t smem = fwd2d_smem_floats(fp.s) * 4;
     auto kern = fp.s == 2 ? k_fwd2d<2> : (fp.s == 4 ? k_fwd2d<4> : k_fwd2d<0>);
     int rc = set_smem(kern, smem);
@@ -806,7 +885,7 @@ ColumnMap make_colmap(const epsgrad_plan *P, int cells_per_piece)
 }
 
 // ---- F6: the eps store stream
-int launch_extrude(epsgrad_plan *P, const float *e2d, float *eps, cudaStream_t st)
+ExtrudeParams fill_extrude(const epsgrad_plan *P, const float *e2d, float *eps)
 {
     ExtrudeParams ep;
     ep.e2d = e2d; ep.eps = eps; ep.zw = P->d_zw; ep.ncol = P->nx * P->ny; ep.nz = P->cfg.nz;
@@ -820,7 +899,38 @@ int launch_extrude(epsgrad_plan *P, const float *e2d, float *eps, cudaStream_t s
     if (EX_THREADS % nz4 == 0)
         for (int sft = 0; sft <= 8; ++sft)
             if ((1 << sft) == nz4) ep.sh4 = sft;
+    return ep;
+}
+
+int launch_extrude(epsgrad_plan *P, const float *e2d, float *eps, cudaStream_t st)
+{
+    const ExtrudeParams ep = fill_extrude(P, e2d, eps);
     if (P->cfg.batch > 65535) return EPSGRAD_EUNSUPPORTED;
+    if (P->use_bulk && P->emb.nx_full == 0) {
+        // thin persistent store stream (extrude_bulk.cuh): columns of a plane are one contiguous run
+        ExtrudeBulkParams bp;
+        bp.e2d = ep.e2d; bp.eps = eps; bp.zw = P->d_zw; bp.ncol = ep.ncol; bp.nz = ep.nz; bp.pstride = ep.pstride;
+        bp.eps_clad = P->eps_clad;
+        int lo = ep.nz, hi = -1;                                  // union of the two slab windows in 16-byte pieces of eps (4 cells)
+        for (int g = 0; g < 2; ++g)
+            if (P->nch[g] > 0) { lo = std::min(lo, 2 * P->ch0[g]); hi = std::max(hi, 2 * (P->ch0[g] + P->nch[g]) - 1); }
+        bp.q0 = hi >= lo ? lo / 4 : 0;
+        bp.nq = hi >= lo ? std::min(hi, ep.nz - 1) / 4 - bp.q0 + 1 : 0;
+        const int blk_bytes = P->tune[0] > 0 ? P->tune[0] : 16384;
+        int cols = blk_bytes / (ep.nz * 4);
+        if (bp.nq > 0 && cols * bp.nq > 4 * EXB_THREADS) cols = 4 * EXB_THREADS / bp.nq;
+        if (cols >= 1) {
+            bp.cols = cols;
+            bp.nblk = cdiv(bp.ncol, cols);
+            const size_t smem_b = (size_t)EXB_NBUF * cols * ep.nz * 4;
+            int rcb = set_smem(k_extrude_bulk, smem_b);
+            if (rcb) return rcb;
+            const int per_sm = P->tune[1] > 0 ? P->tune[1] : 2;
+            const int n_items = 3 * bp.nblk, n_want = std::max(1, per_sm * P->n_sm / P->cfg.batch);
+            k_extrude_bulk<<<dim3(std::min(n_items, n_want), 1, P->cfg.batch), EXB_THREADS, smem_b, st>>>(bp);
+            return check_launch(P, "extrude", st);
+        }
+    }
     const size_t smem = (size_t)3 * ep.cpb * 4;
     int rc = set_smem(k_extrude, smem);
     if (rc) return rc;
@@ -839,16 +949,13 @@ void window_union(const epsgrad_plan *P, int *first, int *count)
     *count = hi > lo ? hi - lo : 0;
 }
 
-// packed: EF / EA hold only the union window of every column, [B,3,ncol][count] chunks (the host entry point's gather)
-int launch_zreduce(epsgrad_plan *P, int n_pairs, const void *const *EF, const void *const *EA, float *gbar, cudaStream_t st,
-                   bool host_src = false, bool packed = false)
+// everything of ZredParams but the field pointers; smem: bytes of staging a CTA needs; sparse: windows worth 64-byte fills
+int fill_zreduce(const epsgrad_plan *P, float *gbar, bool packed, ZredParams &zp, size_t &smem, bool &sparse, int &maxnch,
+                 int max_cols = ZR_COLS, int stage_chunks = ZR_STAGE_CHUNKS)
 {
-    ZredParams zp;
     zp.gbar = gbar; zp.zw = P->d_zw; zp.ncol = P->nx * P->ny; zp.nz = P->cfg.nz;
     zp.pstride = zp.ncol;
     if (P->slab_nx > 0) {
-        // x-slab: only the slab's rows have fields; the cotangent of every other column of the region is zero
-        if (cudaMemsetAsync(gbar, 0, (size_t)P->cfg.batch * 5 * zp.pstride * sizeof(float), st) != cudaSuccess) { cudaGetLastError(); return EPSGRAD_ECUDA; }
         zp.ncol = P->slab_nx * P->ny;
         zp.gbar += (size_t)P->slab_x0 * P->ny;
     }
@@ -864,7 +971,7 @@ int launch_zreduce(epsgrad_plan *P, int n_pairs, const void *const *EF, const vo
         zp.cm.base = 0;
         zp.choff = u0;
     }
-    int maxnch = 1;
+    maxnch = 1;
     for (int g = 0; g < 2; ++g) {
         zp.ch0[g] = P->dense ? 0 : P->ch0[g];
         zp.nch[g] = P->dense ? P->cfg.nz / 2 : P->nch[g];
@@ -873,18 +980,76 @@ int launch_zreduce(epsgrad_plan *P, int n_pairs, const void *const *EF, const vo
         while ((1 << zp.chs[g]) < zp.nch[g]) ++zp.chs[g];
         if (zp.chs[g] > 8) return EPSGRAD_EUNSUPPORTED;     // window wider than one CTA pass (nz > 512)
     }
-    size_t smem = 0;
+    smem = 0;
     for (int g = 0; g < 2; ++g) {
-        zp.ncp[g] = zred_cols_per_pass(zp.nch[g]);
+        zp.ncp[g] = zred_cols_per_pass(zp.nch[g], max_cols, stage_chunks);
         if (zp.ncp[g] < 1) return EPSGRAD_EUNSUPPORTED;
         const size_t need = (size_t)2 * (zp.nch[g] | 1) * zp.ncp[g] * 16;
         if (need > smem) smem = need;
     }
     zp.nblk = cdiv(zp.ncol, ZR_COLS);
     // windows of at most 128 bytes per column: ask for 64-byte fills
-    const bool sparse = maxnch * 16 <= 128 && zp.nz * 8 > 128 && !packed;     // packed windows are one dense stream
+    sparse = maxnch * 16 <= 128 && zp.nz * 8 > 128 && !packed;     // packed windows are one dense stream
+    return EPSGRAD_OK;
+}
+
+// packed: EF / EA hold only the union window of every column, [B,3,ncol][count] chunks (the host entry point's gather)
+int launch_zreduce(epsgrad_plan *P, int n_pairs, const void *const *EF, const void *const *EA, float *gbar, cudaStream_t st,
+                   bool host_src = false, bool packed = false)
+{
+    ZredParams zp;
+    size_t smem = 0;
+    bool sparse = false;
+    int maxnch = 1;
+    // x-slab: only the slab's rows have fields; the cotangent of every other column of the region is zero
+    if (P->slab_nx > 0 &&
+        cudaMemsetAsync(gbar, 0, (size_t)P->cfg.batch * 5 * P->nx * P->ny * sizeof(float), st) != cudaSuccess) { cudaGetLastError(); return EPSGRAD_ECUDA; }
+    int rcf = fill_zreduce(P, gbar, packed, zp, smem, sparse, maxnch);
+    if (rcf) return rcf;
     host_src = host_src || P->cur_host_src;
-    if (sparse && !host_src && P->use_tma && P->emb.nx_full == 0 && P->slab_nx == 0) {
+    if (!host_src && !packed && P->use_tma == 2 && P->tma_encode && P->emb.nx_full == 0 && maxnch <= 24) {
+        // thin persistent read stream (zreduce_pipe.cuh): TMA boxes {window, ZP_COLS columns} through a ring of stages
+        typedef CUresult (*EncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                     const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                     CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+        EncodeFn enc = (EncodeFn)P->tma_encode;
+        ZredPipeParams pp;
+        pp.gbar = zp.gbar; pp.zw = P->d_zw; pp.ncol = zp.ncol; pp.nz = zp.nz; pp.pstride = zp.pstride;
+        for (int g = 0; g < 2; ++g) { pp.ch0[g] = zp.ch0[g]; pp.nch[g] = zp.nch[g]; }
+        pp.wb = maxnch | 1;
+        pp.nblk = cdiv(zp.ncol, ZP_COLS);
+        const cuuint64_t dims[2] = {(cuuint64_t)zp.nz * 2, (cuuint64_t)P->cfg.batch * 3 * zp.ncol};
+        const cuuint64_t strides[1] = {(cuuint64_t)zp.nz * 8};
+        const cuuint32_t box[2] = {(cuuint32_t)pp.wb * 4, (cuuint32_t)ZP_COLS}, es[2] = {1, 1};
+        const int stage_b = 2 * ZP_COLS * pp.wb * 16;
+        pp.nstage = P->tune[2] > 0 ? P->tune[2] : std::max(2, std::min(8, 100 * 1024 / stage_b));
+        if (pp.nstage > ZP_MAX_STAGE) pp.nstage = ZP_MAX_STAGE;
+        const size_t smem_p = zpipe_smem_bytes(pp.wb, pp.nstage);
+        if (smem_p > 220 * 1024) return EPSGRAD_EUNSUPPORTED;
+        int rcp = set_smem(k_zreduce_pipe, smem_p);
+        if (rcp) return rcp;
+        const CUtensorMapL2promotion promo = sparse ? CU_TENSOR_MAP_L2_PROMOTION_L2_64B : CU_TENSOR_MAP_L2_PROMOTION_L2_128B;
+        const int n_items = 3 * pp.nblk, n_want = std::max(1, (P->tune[3] > 0 ? P->tune[3] : 1) * P->n_sm / P->cfg.batch);
+        const dim3 grid_p(std::min(n_items, n_want), 1, P->cfg.batch);
+        if (P->cfg.batch > 65535) return EPSGRAD_EUNSUPPORTED;
+        for (int p0 = 0; p0 < n_pairs; p0 += ZR_MAX_PAIRS) {
+            const int np = n_pairs - p0 < ZR_MAX_PAIRS ? n_pairs - p0 : ZR_MAX_PAIRS;
+            for (int p = 0; p < np; ++p) {
+                if (enc(&pp.mf[p], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void *>(EF[p0 + p]), dims, strides, box, es,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS ||
+                    enc(&pp.ma[p], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void *>(EA[p0 + p]), dims, strides, box, es,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+                    return EPSGRAD_ECUDA;
+            }
+            for (int p = np; p < ZR_MAX_PAIRS; ++p) { pp.mf[p] = pp.mf[0]; pp.ma[p] = pp.ma[0]; }
+            pp.n_pairs = np; pp.accumulate = p0 > 0;
+            k_zreduce_pipe<<<grid_p, ZP_THREADS, smem_p, st>>>(pp);
+            rcp = check_launch(P, "zreduce", st);
+            if (rcp) return rcp;
+        }
+        return EPSGRAD_OK;
+    }
+    if (sparse && !host_src && P->use_tma == 1 && P->emb.nx_full == 0 && P->slab_nx == 0) {
         // TMA variant (zreduce.cuh): one 2-D tensor map per field, rows = z columns, box = {window, 256 columns}
         typedef CUresult (*EncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
                                      const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -1021,7 +1186,7 @@ int launch_front(epsgrad_plan *P, const float *C, float beta, cudaStream_t st)
 }
 
 // ---- R2..R5
-int launch_maskgrad(epsgrad_plan *P, const float *phi, float beta, const float *gbar, const float *coef, float *v, cudaStream_t st)
+MaskGradParams fill_maskgrad(const epsgrad_plan *P, const float *phi, float beta, const float *gbar, const float *coef, float *v)
 {
     MaskGradParams mp;
     mp.phi = phi; mp.gbar = gbar; mp.coef = coef; mp.v = v; mp.nrm = make_nrm(P);
@@ -1030,6 +1195,12 @@ int launch_maskgrad(epsgrad_plan *P, const float *phi, float beta, const float *
     mp.use_den = 1;
     mp.dbeta_part = P->cur_dbeta ? ws_part(P) : nullptr;               // [B][n_part_mg]
     if (P->morph_R > 0) { mp.phi = ws_mc(P); mp.eta_r = 0.0f; mp.use_den = 0; }   // v holds the cotangent of rho~: the filters^T follow
+    return mp;
+}
+
+int launch_maskgrad(epsgrad_plan *P, const float *phi, float beta, const float *gbar, const float *coef, float *v, cudaStream_t st)
+{
+    const MaskGradParams mp = fill_maskgrad(P, phi, beta, gbar, coef, v);
     const size_t smem = maskgrad_smem_floats(mp.s) * 4;
     auto kern = mp.s == 2 ? k_maskgrad<2> : (mp.s == 4 ? k_maskgrad<4> : k_maskgrad<0>);
     int rc = set_smem(kern, smem);
@@ -1061,6 +1232,94 @@ struct DeviceGuard {
     ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
 };
 
+// ---- the whole step as one persistent dataflow kernel (mega.cuh)
+bool mega_applies(const epsgrad_plan *P, int n_pairs)
+{
+    return P->use_mega == 1 && P->d_sched && !P->cur_dbeta && P->slab_nx == 0 && !P->cur_host_src && !P->prof && n_pairs <= ZR_MAX_PAIRS;
+}
+
+template <int NTC>
+int launch_mega_nt(epsgrad_plan *P, MegaParams &mp, bool sparse, size_t smem, cudaStream_t st)
+{
+    auto kern = sparse ? k_mega<NTC, true> : k_mega<NTC, false>;
+    int rc = set_smem(kern, smem);
+    if (rc) return rc;
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, MK_THREADS, smem) != cudaSuccess || per_sm < 1) { cudaGetLastError(); return EPSGRAD_ECUDA; }
+    if (P->tune[4] > 0 && P->tune[4] < per_sm) per_sm = P->tune[4];
+    const int grid = per_sm * P->n_sm;
+    if (cudaMemsetAsync(P->d_sched, 0, P->sched_bytes, st) != cudaSuccess) { cudaGetLastError(); return EPSGRAD_ECUDA; }
+    kern<<<grid, MK_THREADS, smem, st>>>(mp);
+    return check_launch(P, "chain", st);
+}
+
+// phases: which steps this launch runs (bit PH_*); the others' outputs are taken as complete (an earlier launch made them)
+int launch_mega(epsgrad_plan *P, const float *C, float beta, int n_pairs, const void *const *EF, const void *const *EA,
+                float *eps, float *dFdC, cudaStream_t st, unsigned phases = 0x3f)
+{
+    MegaParams mp;
+    std::memset(&mp, 0, sizeof(mp));
+    const int T = P->T, NT = P->NT, nx = P->nx, ny = P->ny, mx = P->cfg.mx, my = P->cfg.my;
+    mp.f1 = fill_filter(P, C, ws_phi(P));
+    mp.f2 = fill_fwd2d(P, ws_phi(P), beta, eps ? ws_e2d(P) : nullptr, dFdC ? ws_coef(P) : nullptr, nullptr);
+    mp.sched = P->d_sched;
+    mp.prof = P->d_mprof;
+    mp.B = P->cfg.batch;
+    mp.nb = cdiv(nx, MK_BAND);
+    mp.nbx1 = cdiv(my, F4_TB);
+    mp.nbx2 = cdiv(ny, F2_TJ);
+    mp.w_floats = NT * NT * 16;
+    const int ntr = cdiv(mx, F4_TA), rows_last = nx - (mp.nb - 1) * MK_BAND;
+    size_t scratch = std::max((size_t)((F4_TA + 2 * T) * (F4_TB + 2 * T + 1) + 4 + MK_G * F4_THREADS * 16) * 4,
+                              fwd2d_smem_floats(2) * 4);
+    size_t zsmem = 0;
+    mp.full[PH_F1] = 2 * mp.nbx1;            mp.last[PH_F1] = (ntr - 2 * (mp.nb - 1)) * mp.nbx1;
+    mp.full[PH_F2] = mp.last[PH_F2] = mp.nbx2;
+    bool sparse = false;
+    if (eps) {
+        mp.ex = fill_extrude(P, ws_e2d(P), eps);
+        mp.xblk[0] = cdiv(MK_BAND * ny, mp.ex.cpb); mp.xblk[1] = cdiv(rows_last * ny, mp.ex.cpb);
+        mp.full[PH_X] = 3 * mp.xblk[0];      mp.last[PH_X] = 3 * mp.xblk[1];
+        scratch = std::max(scratch, (size_t)3 * mp.ex.cpb * 4);
+    }
+    if (dFdC) {
+        int maxnch = 1;
+        int rc = fill_zreduce(P, ws_gbar(P), false, mp.zr, zsmem, sparse, maxnch, MK_ZCOLS, MK_ZCOLS * 5);
+        if (rc) return rc;
+        for (int p = 0; p < ZR_MAX_PAIRS; ++p) {
+            mp.zr.ef[p] = (const float4 *)(p < n_pairs ? EF[p] : nullptr);
+            mp.zr.ea[p] = (const float4 *)(p < n_pairs ? EA[p] : nullptr);
+        }
+        mp.zr.n_pairs = n_pairs; mp.zr.accumulate = 0;
+        mp.zblk[0] = cdiv(MK_BAND * ny, MK_ZCOLS); mp.zblk[1] = cdiv(rows_last * ny, MK_ZCOLS);
+        mp.full[PH_Z] = 3 * mp.zblk[0];      mp.last[PH_Z] = 3 * mp.zblk[1];
+        mp.mg = fill_maskgrad(P, ws_phi(P), beta, ws_gbar(P), ws_coef(P), ws_v(P));
+        mp.full[PH_M] = mp.last[PH_M] = mp.nbx2;
+        mp.ft = fill_filterT(P, ws_v(P), dFdC);
+        mp.full[PH_T] = mp.full[PH_F1];      mp.last[PH_T] = mp.last[PH_F1];
+        scratch = std::max(scratch, maskgrad_smem_floats(2) * 4);
+        scratch = std::max(scratch, ((size_t)filterT4_tile_rows(NT, MK_TPASS) * filterT4_pitch(T) + (size_t)MK_G * F4_TA * F4_TB) * 4);
+    }
+    scratch = align_up(scratch, 16);
+    mp.scratch_floats = (int)(scratch / 4);
+    // pipeline step of band b: tau = b + lag; every dependence points to a smaller tau (mega.cuh)
+    // An item runs for several steps' worth of tickets (a step of 16 rows is ~190 tickets for ~600 CTAs), so the lag between a
+    // phase and its consumer is a few steps: the consumer's bands are then complete when its ticket comes up.
+    const int L = P->tune[6] > 0 ? P->tune[6] : 7;
+    mp.lag[PH_Z] = 0; mp.lag[PH_F1] = 0; mp.lag[PH_F2] = L; mp.lag[PH_X] = 2 * L; mp.lag[PH_M] = 2 * L; mp.lag[PH_T] = 3 * L;
+    for (int ph = 0; ph < PH_N; ++ph)
+        if (!(phases >> ph & 1)) mp.full[ph] = mp.last[ph] = 0;
+    if (!(phases >> PH_Z & 1)) zsmem = 0;
+    const size_t smem = (size_t)mp.w_floats * 4 + scratch + zsmem;
+    if (smem > 200 * 1024) return EPSGRAD_EUNSUPPORTED;
+    switch (NT) {
+    case 5: return launch_mega_nt<5>(P, mp, sparse, smem, st);
+    case 9: return launch_mega_nt<9>(P, mp, sparse, smem, st);
+    case 13: return launch_mega_nt<13>(P, mp, sparse, smem, st);
+    }
+    return EPSGRAD_EUNSUPPORTED;
+}
+
 // The whole path.  eps == nullptr skips F6, dFdC == nullptr skips R1-R6.
 // Dependencies: fwd2d <- filter;  extrude <- fwd2d;  maskgrad <- zreduce, fwd2d;  filterT <- maskgrad;  zreduce <- nothing.
 // Two HBM-bound kernels (zreduce: field reads; extrude: eps stores) and four small L2-resident ones.  Running the two
@@ -1074,6 +1333,7 @@ int run_chain(epsgrad_plan *P, const float *C, float beta, int n_pairs, const vo
               const void *const *EA, float *eps, float *dFdC, cudaStream_t st)
 {
     int rc = EPSGRAD_OK;
+    if (mega_applies(P, n_pairs)) return launch_mega(P, C, beta, n_pairs, EF, EA, eps, dFdC, st);
     if (!dFdC || !P->overlap || P->prof) {
         rc = launch_front(P, C, beta, st);
         if (!rc) rc = launch_fwd2d(P, ws_phi(P), beta, eps ? ws_e2d(P) : nullptr, dFdC ? ws_coef(P) : nullptr, nullptr, st);
@@ -1091,19 +1351,22 @@ int run_chain(epsgrad_plan *P, const float *C, float beta, int n_pairs, const vo
         cudaGetLastError();
         return EPSGRAD_ECUDA;
     }
-    rc = launch_front(P, C, beta, ax);
+    const bool chains = P->use_mega == 2 && P->d_sched && !P->cur_dbeta && P->slab_nx == 0;   // the 2-D chains as two persistent kernels
+    if (chains) rc = launch_mega(P, C, beta, n_pairs, EF, EA, eps, dFdC, ax, 1u << PH_F1 | 1u << PH_F2);
+    else rc = launch_front(P, C, beta, ax);
     if (!rc) rc = launch_zreduce(P, n_pairs, EF, EA, ws_gbar(P), st);
     if (!rc && cudaEventRecord(P->ev_r, st) != cudaSuccess) rc = EPSGRAD_ECUDA;
-    if (!rc) rc = launch_fwd2d(P, ws_phi(P), beta, eps ? ws_e2d(P) : nullptr, ws_coef(P), nullptr, ax);
+    if (!rc && !chains) rc = launch_fwd2d(P, ws_phi(P), beta, eps ? ws_e2d(P) : nullptr, ws_coef(P), nullptr, ax);
     if (!rc && cudaEventRecord(P->ev_2d, ax) != cudaSuccess) rc = EPSGRAD_ECUDA;
     if (!rc && cudaStreamWaitEvent(ax, P->ev_r, 0) != cudaSuccess) rc = EPSGRAD_ECUDA;
-    if (!rc) rc = launch_maskgrad(P, ws_phi(P), beta, ws_gbar(P), ws_coef(P), ws_v(P), ax);
+    if (!rc && chains) rc = launch_mega(P, C, beta, n_pairs, EF, EA, eps, dFdC, ax, 1u << PH_M | 1u << PH_T);
+    if (!rc && !chains) rc = launch_maskgrad(P, ws_phi(P), beta, ws_gbar(P), ws_coef(P), ws_v(P), ax);
     if (!rc && eps) {
         if (cudaStreamWaitEvent(st, P->ev_2d, 0) != cudaSuccess) rc = EPSGRAD_ECUDA;
         if (!rc) rc = launch_extrude(P, ws_e2d(P), eps, st);
     }
     if (!rc && P->morph_R > 0) rc = launch_morph_reverse(P, ws_phi(P), beta, ws_v(P), ax);
-    if (!rc) rc = launch_filterT(P, ws_v(P), dFdC, ax);
+    if (!rc && !chains) rc = launch_filterT(P, ws_v(P), dFdC, ax);
     if (!rc) rc = launch_dbeta_sum(P, ax);
     // always join, even on error, so that the auxiliary stream never outlives the call
     if (cudaEventRecord(P->ev_join, ax) != cudaSuccess || cudaStreamWaitEvent(st, P->ev_join, 0) != cudaSuccess) {

@@ -35,20 +35,62 @@ __host__ __device__ inline int extrude_cols_per_block(int nz)
     return EX_THREADS % nz4 == 0 ? (EX_THREADS / nz4) * EX_PASSES : 64;
 }
 
-// grid (nblk, 3, B): x fastest, so CTAs are dispatched component by component; dynamic shared memory 3 cpb floats
-__global__ void __launch_bounds__(EX_THREADS, EX_CTAS_PER_SM) k_extrude(const __grid_constant__ ExtrudeParams P)
+// Columns [col0, col0 + ncb) (ncb <= cpb) of component c of design b by a CTA of EX_THREADS threads; vsm: 3 cpb floats of shared
+// memory (plane values of the block).  No barrier at entry or exit.  The plane values are read through L2 (ld.global.cg): in
+// the persistent kernel (mega.cuh) other CTAs of the same launch produce them.
+__device__ __forceinline__ void block_extrude(const ExtrudeParams &P, int c, int col0, int ncb, int b, float *vsm)
 {
-    extern __shared__ float vsm[];                            // plane values of the block: [3][cpb]
-    const int tid = threadIdx.x, b = blockIdx.z, nz = P.nz, nz4 = nz >> 2, ncol = P.ncol;
-    const int c = blockIdx.y, blk = blockIdx.x;
-    const int cpb = P.cpb, col0 = blk * cpb, ncb = min(cpb, ncol - col0);
+    const int tid = threadIdx.x, nz = P.nz, nz4 = nz >> 2;
+    const int cpb = P.cpb;
     const float *ed = P.e2d + (size_t)b * 5 * P.pstride;
     float4 *out = reinterpret_cast<float4 *>(P.eps) + P.cm.plane(b, c);
     // stage: c = x, y need their own plane; c = z needs planes 2 (full cells), 3 and 4 (face cells)
     const int npl = c == 2 ? 3 : 1;
     for (int o = 0; o < npl; ++o)
-        for (int lc = tid; lc < ncb; lc += EX_THREADS) vsm[o * cpb + lc] = ed[(size_t)(c + o) * P.pstride + col0 + lc];
-    if (P.sh4 >= 0) {
+        for (int lc = tid; lc < ncb; lc += EX_THREADS) vsm[o * cpb + lc] = __ldcg(ed + (size_t)(c + o) * P.pstride + col0 + lc);
+    if (P.sh4 >= 0 && !P.cm.embedded) {
+        // region-sized eps: the block is one contiguous run; a thread walks it with a constant stride (few instructions per
+        // store: the kernel's issue slots are what the 2-D work beside it needs)
+        const int kq = tid & (nz4 - 1), k = kq << 2, cq = tid >> P.sh4, cpp = EX_THREADS >> P.sh4;
+        float4 *dst = out + (size_t)(col0 + cq) * nz4 + kq;
+        const size_t stride = (size_t)cpp * nz4;
+        const float *vp = vsm + cq;
+        if (c < 2) {
+            float wx[4], bx[4];
+#pragma unroll
+            for (int x = 0; x < 4; ++x) { wx[x] = __ldg(P.zw + k + x); bx[x] = __ldg(P.zw + 5 * nz + k + x); }
+            __syncthreads();
+            if (ncb == cpb) {
+#pragma unroll
+                for (int pass = 0; pass < EX_PASSES; ++pass) {
+                    const float v = vp[pass * cpp];
+                    __stcs(dst + pass * stride, make_float4(fmaf(wx[0], v, bx[0]), fmaf(wx[1], v, bx[1]), fmaf(wx[2], v, bx[2]), fmaf(wx[3], v, bx[3])));
+                }
+            } else {
+                for (int lc = cq; lc < ncb; lc += cpp, dst += stride) {
+                    const float v = vsm[lc];
+                    __stcs(dst, make_float4(fmaf(wx[0], v, bx[0]), fmaf(wx[1], v, bx[1]), fmaf(wx[2], v, bx[2]), fmaf(wx[3], v, bx[3])));
+                }
+            }
+        } else {
+            float bz[4], zf[4], zl[4], zh[4];
+#pragma unroll
+            for (int x = 0; x < 4; ++x) {
+                bz[x] = __ldg(P.zw + 6 * nz + k + x); zf[x] = __ldg(P.zw + 2 * nz + k + x);
+                zl[x] = __ldg(P.zw + 3 * nz + k + x); zh[x] = __ldg(P.zw + 4 * nz + k + x);
+            }
+            __syncthreads();
+            for (int lc = cq; lc < ncb; lc += cpp, dst += stride) {
+                const float v = vsm[lc], vl = vsm[cpb + lc], vh = vsm[2 * cpb + lc];
+                float4 o;
+                o.x = fmaf(zf[0], v, fmaf(zl[0], vl, fmaf(zh[0], vh, bz[0])));
+                o.y = fmaf(zf[1], v, fmaf(zl[1], vl, fmaf(zh[1], vh, bz[1])));
+                o.z = fmaf(zf[2], v, fmaf(zl[2], vl, fmaf(zh[2], vh, bz[2])));
+                o.w = fmaf(zf[3], v, fmaf(zl[3], vl, fmaf(zh[3], vh, bz[3])));
+                __stcs(dst, o);
+            }
+        }
+    } else if (P.sh4 >= 0) {
         const int kq = tid & (nz4 - 1), k = kq << 2, cq = tid >> P.sh4, cpp = EX_THREADS >> P.sh4;
         float4 *dst = out + kq;
         if (c < 2) {
@@ -104,6 +146,14 @@ __global__ void __launch_bounds__(EX_THREADS, EX_CTAS_PER_SM) k_extrude(const __
             __stcs(out + P.cm.col(col0 + lc) + (k >> 2), make_float4(o[0], o[1], o[2], o[3]));
         }
     }
+}
+
+// grid (nblk, 3, B): x fastest, so CTAs are dispatched component by component; dynamic shared memory 3 cpb floats
+__global__ void __launch_bounds__(EX_THREADS, EX_CTAS_PER_SM) k_extrude(const __grid_constant__ ExtrudeParams P)
+{
+    extern __shared__ float vsm[];                            // plane values of the block: [3][cpb]
+    const int col0 = blockIdx.x * P.cpb;
+    block_extrude(P, blockIdx.y, col0, min(P.cpb, P.ncol - col0), blockIdx.z, vsm);
 }
 
 }  // namespace epsgrad

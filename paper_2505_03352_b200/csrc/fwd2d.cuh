@@ -65,11 +65,12 @@ __device__ __forceinline__ void sobel_at(const float *A, int ci, int cj, int i, 
     gy = ((a02 - a00) + 2.0f * (a12 - a10) + (a22 - a20)) * 0.125f;
 }
 
-// grid (ceil(ny/TJ), ceil(nx/TI), B).  S > 0: compile-time subpixel count (index divisions fold to shifts); S = 0: runtime P.s.
+// One tile of TI x TJ cells by a CTA of F2_THREADS threads; sm: fwd2d_smem_floats(s) floats.  No barrier at entry or exit:
+// the caller separates calls that reuse sm.  Phi' is read through L2 (ld.global.cg): in the persistent kernel (mega.cuh)
+// other CTAs of the same launch produce it.  S > 0: compile-time subpixel count (index divisions fold to shifts); S = 0: runtime P.s.
 template <int S>
-__global__ void __launch_bounds__(F2_THREADS) k_fwd2d(const __grid_constant__ Fwd2dParams P)
+__device__ __forceinline__ void tile_fwd2d(const Fwd2dParams &P, int bx, int by, int b, float *sm)
 {
-    extern __shared__ __align__(16) float sm[];
     constexpr int TI = F2_TI, TJ = F2_TJ, NTH = F2_THREADS;
     constexpr int CI = TI + 2, CJ = TJ + 2;
     const int s = S > 0 ? S : P.s, hs = s >> 1;
@@ -82,7 +83,7 @@ __global__ void __launch_bounds__(F2_THREADS) k_fwd2d(const __grid_constant__ Fw
     float *Hy = Ay + CI * CJ;
 
     const int tid = threadIdx.x;
-    const int i0 = blockIdx.y * TI, j0 = blockIdx.x * TJ, b = blockIdx.z;
+    const int i0 = by * TI, j0 = bx * TJ;
     const int nx = P.nx, ny = P.ny, ncol = nx * ny;
     const float inv_s2 = 1.0f / (float)(s * s);
 
@@ -101,7 +102,7 @@ __global__ void __launch_bounds__(F2_THREADS) k_fwd2d(const __grid_constant__ Fw
                 if (base + u * NTH < MP * MQ) {
                     const int p = inside ? p_base + lp : clampi(p_base + lp, 0, P.px - 1);
                     const int q = inside ? q_base + lq : clampi(q_base + lq, 0, P.py - 1);
-                    ph[u] = phib[p * P.py + q];
+                    ph[u] = __ldcg(phib + p * P.py + q);
                 }
                 lp += dlp; lq += dlq;
                 if (lq >= MQ) { lq -= MQ; ++lp; }
@@ -188,6 +189,14 @@ __global__ void __launch_bounds__(F2_THREADS) k_fwd2d(const __grid_constant__ Fw
         cf[(size_t)8 * ncol] = P.w_lo > 0.f ? face_factor(P.w_lo, az, inv_ec) : 0.f;
         cf[(size_t)9 * ncol] = P.w_hi > 0.f ? face_factor(P.w_hi, az, inv_ec) : 0.f;
     }
+}
+
+// grid (ceil(ny/TJ), ceil(nx/TI), B)
+template <int S>
+__global__ void __launch_bounds__(F2_THREADS) k_fwd2d(const __grid_constant__ Fwd2dParams P)
+{
+    extern __shared__ __align__(16) float sm[];
+    tile_fwd2d<S>(P, blockIdx.x, blockIdx.y, blockIdx.z, sm);
 }
 
 }  // namespace epsgrad

@@ -37,11 +37,12 @@ __host__ __device__ inline size_t maskgrad_smem_floats(int s)
     return (size_t)10 * MG_CI * MG_CJ + MG_TI * MG_TJ + (size_t)s * (MG_TI + MG_TJ);
 }
 
-// grid (ceil(ny/TJ), ceil(nx/TI), B).  S > 0: compile-time subpixel count; S = 0: runtime P.s.
+// One tile of TI x TJ cells by a CTA of MG_THREADS threads; sm: maskgrad_smem_floats(s) floats; npart: tiles per design (the
+// pitch of dbeta_part).  No barrier at entry or exit.  G, the coefficients and Phi' are read through L2 (ld.global.cg): in the
+// persistent kernel (mega.cuh) other CTAs of the same launch produce them.  S > 0: compile-time subpixel count; S = 0: runtime P.s.
 template <int S>
-__global__ void __launch_bounds__(MG_THREADS) k_maskgrad(const __grid_constant__ MaskGradParams P)
+__device__ __forceinline__ void tile_maskgrad(const MaskGradParams &P, int bx, int by, int b, int tiles_x, int tiles_y, float *sm)
 {
-    extern __shared__ __align__(16) float sm[];
     constexpr int TI = MG_TI, TJ = MG_TJ, NTH = MG_THREADS, CI = MG_CI, CJ = MG_CJ, NC = CI * CJ;
     const int s = S > 0 ? S : P.s, hs = s >> 1;
     float *R = sm;                     // [8][NC] staged residual planes: Hb, Ab, Gx, Gy for c = x then c = y
@@ -50,7 +51,7 @@ __global__ void __launch_bounds__(MG_THREADS) k_maskgrad(const __grid_constant__
     int *nidx = reinterpret_cast<int *>(AbZ + TI * TJ);   // normaliser table row of each tile mask row, then column of each mask column
 
     const int tid = threadIdx.x;
-    const int i0 = blockIdx.y * TI, j0 = blockIdx.x * TJ, b = blockIdx.z;
+    const int i0 = by * TI, j0 = bx * TJ;
     const int oi = i0 - 2, oj = j0 - 2;            // cell origin of the staged arrays
     const int nx = P.nx, ny = P.ny, ncol = nx * ny;
     const float inv_s2 = 1.0f / (float)(s * s), inv_deps = 1.0f / P.deps;
@@ -71,11 +72,11 @@ __global__ void __launch_bounds__(MG_THREADS) k_maskgrad(const __grid_constant__
             float r8[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
             if (i >= 0 && i < nx && j >= 0 && j < ny) {
                 const int cell = i * ny + j;
-                const float gx = gb[cell], gy = gb[ncol + cell];
+                const float gx = __ldcg(gb + cell), gy = __ldcg(gb + ncol + cell);
 #pragma unroll
                 for (int o = 0; o < 4; ++o) {
-                    r8[o] = cb[(size_t)o * ncol + cell] * gx;
-                    r8[4 + o] = cb[(size_t)(4 + o) * ncol + cell] * gy;
+                    r8[o] = __ldcg(cb + (size_t)o * ncol + cell) * gx;
+                    r8[4 + o] = __ldcg(cb + (size_t)(4 + o) * ncol + cell) * gy;
                 }
             }
 #pragma unroll
@@ -87,8 +88,8 @@ __global__ void __launch_bounds__(MG_THREADS) k_maskgrad(const __grid_constant__
         float az = 0.f;
         if (i < nx && j < ny) {
             const int cell = i * ny + j;
-            az = fmaf(cb[(size_t)8 * ncol + cell], gb[(size_t)3 * ncol + cell],
-                      fmaf(cb[(size_t)9 * ncol + cell], gb[(size_t)4 * ncol + cell], gb[(size_t)2 * ncol + cell]));
+            az = fmaf(__ldcg(cb + (size_t)8 * ncol + cell), __ldcg(gb + (size_t)3 * ncol + cell),
+                      fmaf(__ldcg(cb + (size_t)9 * ncol + cell), __ldcg(gb + (size_t)4 * ncol + cell), __ldcg(gb + (size_t)2 * ncol + cell)));
         }
         AbZ[it] = az;
     }
@@ -163,8 +164,8 @@ __global__ void __launch_bounds__(MG_THREADS) k_maskgrad(const __grid_constant__
         ex[1] = mx * AbF[c0];  hx[1] = mx * R[c0];
         ey[1] = my * AbF[NC + c0];  hy[1] = my * R[4 * NC + c0];
         const int p = 2 * i, q = 2 * j;
-        const float2 ph0 = *reinterpret_cast<const float2 *>(phib + p * P.py + q);
-        const float2 ph1 = *reinterpret_cast<const float2 *>(phib + (p + 1) * P.py + q);
+        const float2 ph0 = __ldcg(reinterpret_cast<const float2 *>(phib + p * P.py + q));
+        const float2 ph1 = __ldcg(reinterpret_cast<const float2 *>(phib + (p + 1) * P.py + q));
         const float phv[2][2] = {{ph0.x, ph0.y}, {ph1.x, ph1.y}};
         const int nq0 = nidx[TP + 2 * tj], nq1 = nidx[TP + 2 * tj + 1];
         const float k0 = P.deps * inv_s2 * 2.0f * P.beta;
@@ -189,7 +190,7 @@ __global__ void __launch_bounds__(MG_THREADS) k_maskgrad(const __grid_constant__
         }
         if (P.dbeta_part) {                                         // block-uniform
             const float sdb = block_sum(db, reinterpret_cast<float *>(nidx));      // nidx is dead for every thread past block_sum's first barrier
-            if (tid == 0) P.dbeta_part[(size_t)b * gridDim.y * gridDim.x + blockIdx.y * gridDim.x + blockIdx.x] = sdb / P.beta;
+            if (tid == 0) P.dbeta_part[(size_t)b * tiles_y * tiles_x + by * tiles_x + bx] = sdb / P.beta;
         }
     } else {
     float db = 0.f;
@@ -199,7 +200,7 @@ __global__ void __launch_bounds__(MG_THREADS) k_maskgrad(const __grid_constant__
         for (int u = 0; u < 4; ++u) {
             const int it = base + u * NTH, tp = it / TQ, tq = it - tp * TQ;
             const int p = s * i0 + tp, q = s * j0 + tq;
-            if (it < TP * TQ && p < P.px && q < P.py) ph[u] = phib[p * P.py + q];
+            if (it < TP * TQ && p < P.px && q < P.py) ph[u] = __ldcg(phib + p * P.py + q);
         }
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
@@ -236,9 +237,17 @@ __global__ void __launch_bounds__(MG_THREADS) k_maskgrad(const __grid_constant__
     }
     if (P.dbeta_part) {
         const float sdb = block_sum(db, reinterpret_cast<float *>(nidx));
-        if (tid == 0) P.dbeta_part[(size_t)b * gridDim.y * gridDim.x + blockIdx.y * gridDim.x + blockIdx.x] = sdb / P.beta;
+        if (tid == 0) P.dbeta_part[(size_t)b * tiles_y * tiles_x + by * tiles_x + bx] = sdb / P.beta;
     }
     }
+}
+
+// grid (ceil(ny/TJ), ceil(nx/TI), B)
+template <int S>
+__global__ void __launch_bounds__(MG_THREADS) k_maskgrad(const __grid_constant__ MaskGradParams P)
+{
+    extern __shared__ __align__(16) float sm[];
+    tile_maskgrad<S>(P, blockIdx.x, blockIdx.y, blockIdx.z, gridDim.x, gridDim.y, sm);
 }
 
 }  // namespace epsgrad

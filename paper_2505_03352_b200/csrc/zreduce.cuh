@@ -38,11 +38,11 @@ struct ZredParams {
     int choff;             // chunk the stored columns start at: 0, or the first chunk of the union window for packed fields
 };
 
-__host__ __device__ inline int zred_cols_per_pass(int nch)
+__host__ __device__ inline int zred_cols_per_pass(int nch, int max_cols = ZR_COLS, int stage_chunks = ZR_STAGE_CHUNKS)
 {
-    int n = ZR_STAGE_CHUNKS / (nch | 1);
+    int n = stage_chunks / (nch | 1);
     if (n >= 32) n &= ~31;                 // whole warps of columns
-    return n > ZR_COLS ? ZR_COLS : n;
+    return n > max_cols ? max_cols : n;
 }
 
 // 16-byte asynchronous copy global -> shared (LDGSTS): completion by cp.async groups.
@@ -89,27 +89,43 @@ __device__ __forceinline__ void zwindow_issue(const ZredParams &P, float4 *buf, 
                 }
             }
         } else {
-            for (int lc = threadIdx.x >> sh; lc < nc; lc += lstep) {
-                const size_t o = P.cm.col(col0 + lc);
-                cp_async16<SPARSE>(df + lc * pitch, pf + o);
-                cp_async16<SPARSE>(da + lc * pitch, pa + o);
+            if (!P.cm.embedded) {
+                // region-sized fields: constant strides, few instructions per copy
+                const int lc0 = threadIdx.x >> sh;
+                const size_t o0 = (size_t)(col0 + lc0) * P.cm.col_pitch, ostep = (size_t)lstep * P.cm.col_pitch;
+                pf += o0; pa += o0; df += lc0 * pitch; da += lc0 * pitch;
+                const int sstep = lstep * pitch;
+                for (int lc = lc0; lc < nc; lc += lstep, pf += ostep, pa += ostep, df += sstep, da += sstep) {
+                    cp_async16<SPARSE>(df, pf);
+                    cp_async16<SPARSE>(da, pa);
+                }
+            } else {
+                for (int lc = threadIdx.x >> sh; lc < nc; lc += lstep) {
+                    const size_t o = P.cm.col(col0 + lc);
+                    cp_async16<SPARSE>(df + lc * pitch, pf + o);
+                    cp_async16<SPARSE>(da + lc * pitch, pa + o);
+                }
             }
         }
     }
     cp_async_commit();
 }
 
-// grid (nblk, 3, B): x fastest, so CTAs are dispatched component by component; dynamic shared memory: 2 fields x ncp x (nch | 1) chunks
+// Columns [colb, colb + ncb) (ncb <= ZR_COLS) of component c of design b by a CTA of ZR_THREADS threads; stage: 2 fields x ncp x
+// (nch | 1) chunks of shared memory.  In two halves, so that a caller can do other work while the first copies are in flight
+// (mega.cuh): _begin starts the copies of the first pass of the first pair; _finish waits, reduces and runs the remaining
+// passes and pairs.  No barrier at entry or exit: the caller separates calls that reuse `stage`.
 template <bool SPARSE, bool HOSTSRC>
-__global__ void __launch_bounds__(ZR_THREADS, 5) k_zreduce(const __grid_constant__ ZredParams P)
+__device__ __forceinline__ void block_zreduce_begin(const ZredParams &P, int c, int colb, int ncb, int b, float4 *stage)
 {
-    extern __shared__ __align__(16) float4 stage[];
-    const int tid = threadIdx.x;
-    const int c = blockIdx.y, blk = blockIdx.x, b = blockIdx.z;
-    const int grp = c == 2, nch = P.nch[grp], ch0 = P.ch0[grp], ncp = P.ncp[grp], nz = P.nz;
-    const int colb = blk * ZR_COLS, ncb = min(ZR_COLS, P.ncol - colb);
+    zwindow_issue<SPARSE, HOSTSRC>(P, stage, 0, b, c, colb, min(P.ncp[c == 2], ncb));
+}
 
-    zwindow_issue<SPARSE, HOSTSRC>(P, stage, 0, b, c, colb, min(ncp, ncb));
+template <bool SPARSE, bool HOSTSRC>
+__device__ __forceinline__ void block_zreduce_finish(const ZredParams &P, int c, int colb, int ncb, int b, float4 *stage)
+{
+    const int tid = threadIdx.x;
+    const int grp = c == 2, nch = P.nch[grp], ch0 = P.ch0[grp], ncp = P.ncp[grp], nz = P.nz;
     // a thread reduces one column; the extrusion weights (2 cells per chunk; three rows for component z) are warp-uniform
     // cached loads
     for (int c0 = 0; c0 < ncb; c0 += ncp) {
@@ -149,6 +165,22 @@ __global__ void __launch_bounds__(ZR_THREADS, 5) k_zreduce(const __grid_constant
             }
         }
     }
+}
+
+template <bool SPARSE, bool HOSTSRC>
+__device__ __forceinline__ void block_zreduce(const ZredParams &P, int c, int colb, int ncb, int b, float4 *stage)
+{
+    block_zreduce_begin<SPARSE, HOSTSRC>(P, c, colb, ncb, b, stage);
+    block_zreduce_finish<SPARSE, HOSTSRC>(P, c, colb, ncb, b, stage);
+}
+
+// grid (nblk, 3, B): x fastest, so CTAs are dispatched component by component; dynamic shared memory: 2 fields x ncp x (nch | 1) chunks
+template <bool SPARSE, bool HOSTSRC>
+__global__ void __launch_bounds__(ZR_THREADS, 5) k_zreduce(const __grid_constant__ ZredParams P)
+{
+    extern __shared__ __align__(16) float4 stage[];
+    const int colb = blockIdx.x * ZR_COLS;
+    block_zreduce<SPARSE, HOSTSRC>(P, blockIdx.y, colb, min(ZR_COLS, P.ncol - colb), blockIdx.z, stage);
 }
 
 // ---------------------------------------------------------------- TMA variant
