@@ -89,7 +89,10 @@ typedef struct {
     double  filter_sigma;     /* Gaussian sigma in Yee cells                                 */
     double  eta;              /* projection threshold: 0.5 -> Eq. (6), 0 -> Eq. (3) (S9)     */
     double  eps_core, eps_clad;
-    double  normal_delta;     /* guard in n_c^2 = g_c^2/(|g|^2 + delta) (S6; default 1e-12)  */
+    double  normal_delta;     /* guard in n_c^2 = g_c^2/(|g|^2 + delta) (S6).  Recommended (the binding's default) 1e-8: in
+                                 float32 the Sobel differences of a flat mask carry noise^2 ~ 1e-14, so a guard near it turns
+                                 rounding noise into normals.  Must be >= 1e-30: EPSGRAD_EINVAL below (0 and
+                                 denormals would give n^2 = 0/0 on every flat cell) */
     double  morph_diameter;   /* d of Eqs. (4)-(5) in Yee cells (minimum feature size); 0 = morphological
                                  filters off.  On: rho0 = projection(Phi), "dilate, erode, erode, dilate" (
                                  S17) with the disk K_m normalised over the in-region pixels (S18), then Eq. (6) */
@@ -196,16 +199,25 @@ int epsgrad_adam_step(float *C, float *M, float *V, const float *G, size_t n, in
  *   epsgrad_soap_eigh         Q, w <- eigenvectors / ascending eigenvalues [n] of the symmetric A [n,n] (A is not
  *                             written).  The library's one LIBRARY step (cuSOLVER syevd), loaded with dlopen on first use:
  *                             EPSGRAD_EUNSUPPORTED (and workspace_bytes = 0) when cuSOLVER is not on the machine.  Uses the
- *                             current device; one host thread at a time.  Eigenvector signs are the solver's: they do not
- *                             change the update (S23).
+ *                             current device; the per-device solver handle is bound to `stream` and the solver enqueued
+ *                             under one lock, so host threads may call it concurrently.  Eigenvector signs are the solver's:
+ *                             they do not change the update (S23).  The solver's status word stays in `work`:
+ *   epsgrad_soap_eigh_info    copies it to *info and synchronises `stream` (host-blocking): 0 = converged, i > 0 = i
+ *                             off-diagonal elements of the tridiagonal form did not converge (Q is then not to be used).
  *   epsgrad_soap_step         M <- b1 M + (1-b1) G;  G' = QL^T G QR;  M' = QL^T M QR;  V' <- b2 V' + (1-b2) G'^2;
  *                             N' = (M'/(1-b1^step)) / sqrt(V'/(1-b2^step) + eps)  (eps inside the root, as printed);
  *                             C <- C - lr QL N' QR^T                                                           (Eq. (13))
+ *                             Range of eps in float32: on the first steps L ~ G G^T and R ~ G^T G, so G' is diagonal up to
+ *                             rounding and every other entry of N' is noise/sqrt(noise^2 + eps) with noise ~ 1e-7 |G|: the
+ *                             update agrees with float64 (1e-4) for eps >= ~1e-2 mean(G^2) (what tests/test_gpu_soap.py and
+ *                             test_gpu_loop.py use); at App. B's "small number" 1e-8 with |G| ~ 1 the
+ *                             off-diagonal entries of the first update are wrong by ~1e-3 each.
  * `work` is caller-owned device scratch of at least the matching *_workspace_bytes.  Errors: EPSGRAD_EINVAL (null pointer,
  * size < 1, step < 1, b outside [0,1), lr <= 0, eps < 0), EPSGRAD_ENOWORKSPACE, EPSGRAD_ECUDA.  No host synchronisation.   */
 int    epsgrad_soap_accumulate(float *L, float *R, const float *G, int mx, int my, double b2, void *stream);
 size_t epsgrad_soap_eigh_workspace_bytes(int n);
 int    epsgrad_soap_eigh(const float *A, float *Q, float *w, int n, void *work, size_t work_bytes, void *stream);
+int    epsgrad_soap_eigh_info(const void *work, size_t work_bytes, int n, void *stream, int *info);
 size_t epsgrad_soap_step_workspace_bytes(int mx, int my);
 int    epsgrad_soap_step(float *C, float *M, float *Vp, const float *G, const float *QL, const float *QR, int mx, int my,
                          int step, double b1, double b2, double lr, double eps, void *work, size_t work_bytes, void *stream);

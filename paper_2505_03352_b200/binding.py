@@ -22,7 +22,7 @@ EXPORTS = (
     "epsgrad_plan_set_profiling", "epsgrad_plan_last_kernel_times", "epsgrad_plan_set_overlap", "epsgrad_plan_set_host_direct", "epsgrad_plan_set_embedding", "epsgrad_plan_set_slab", "epsgrad_plan_set_tma", "epsgrad_plan_set_bulk_stores", "epsgrad_plan_set_tuning", "epsgrad_plan_set_fused", "epsgrad_plan_fused_profile", "epsgrad_plan_set_timeline", "epsgrad_plan_read_timeline", 
     "eps_forward", "eps_vjp", "eps_forward_vjp", "eps_forward_vjp_host", "eps_vjp_beta", "eps_unbinarity",
     "epsgrad_beta_schedule", "epsgrad_beta_update", "epsgrad_adam_step",
-    "epsgrad_soap_accumulate", "epsgrad_soap_eigh_workspace_bytes", "epsgrad_soap_eigh",
+    "epsgrad_soap_accumulate", "epsgrad_soap_eigh_workspace_bytes", "epsgrad_soap_eigh", "epsgrad_soap_eigh_info",
     "epsgrad_soap_step_workspace_bytes", "epsgrad_soap_step",
     "epsgrad_stage_filter", "epsgrad_stage_eps2d", "epsgrad_stage_zreduce",
     "epsgrad_status_string", "epsgrad_version",
@@ -63,7 +63,7 @@ class Config(ctypes.Structure):
 
 def make_config(*, batch=1, mx, my, nz, z_lo, z_hi, upsample=2, subpixel=2, filter_kind=FILTER_CONIC,
                 filter_radius=4.0, filter_sigma=1.0, filter_normalize=1, eta=0.5, eps_core=12.11,
-                eps_clad=2.085, normal_delta=1e-12, morph_diameter=0.0, morph_alpha=20.0) -> Config:
+                eps_clad=2.085, normal_delta=1e-8, morph_diameter=0.0, morph_alpha=20.0) -> Config:
     return Config(batch, mx, my, upsample, subpixel, nz, filter_kind, filter_normalize, z_lo, z_hi,
                   filter_radius, filter_sigma, eta, eps_core, eps_clad, normal_delta, morph_diameter, morph_alpha)
 
@@ -122,8 +122,9 @@ class Soap:
             _check(lib().epsgrad_soap_accumulate(self.L.data_ptr(), self.R.data_ptr(), G.data_ptr(), self.mx, self.my, b2,
                                                  self._stream()), "epsgrad_soap_accumulate")
 
-    def eigh(self, A, Q, w) -> None:
-        """Q, w <- eigenvectors (columns) and ascending eigenvalues of the symmetric A"""
+    def eigh(self, A, Q, w, check: bool = False) -> None:
+        """Q, w <- eigenvectors (columns) and ascending eigenvalues of the symmetric A; check: read the solver's status back
+        (synchronises the stream) and raise if it did not converge"""
         t = self._torch
         self._chk(A, Q, w)
         n = A.shape[0]
@@ -136,6 +137,12 @@ class Soap:
                 self._ework = t.empty(need, dtype=t.uint8, device=self.device)
             _check(lib().epsgrad_soap_eigh(A.data_ptr(), Q.data_ptr(), w.data_ptr(), n, self._ework.data_ptr(), self._ework.numel(),
                                            self._stream()), "epsgrad_soap_eigh")
+            if check:
+                info = ctypes.c_int(-1)
+                _check(lib().epsgrad_soap_eigh_info(self._ework.data_ptr(), self._ework.numel(), n, self._stream(), ctypes.byref(info)),
+                       "epsgrad_soap_eigh_info")
+                if info.value != 0:
+                    raise RuntimeError(f"epsgrad_soap_eigh: the eigensolver did not converge (info = {info.value})")
 
     def refresh(self) -> None:
         """Q_L, Q_R <- eigenvectors of L, R"""
@@ -204,6 +211,7 @@ def lib() -> ctypes.CDLL:
     L.epsgrad_soap_eigh_workspace_bytes.restype = sz
     L.epsgrad_soap_eigh_workspace_bytes.argtypes = [i32]
     L.epsgrad_soap_eigh.argtypes = [vp, vp, vp, i32, vp, sz, vp]
+    L.epsgrad_soap_eigh_info.argtypes = [vp, sz, i32, vp, ctypes.POINTER(ctypes.c_int)]
     L.epsgrad_soap_step_workspace_bytes.restype = sz
     L.epsgrad_soap_step_workspace_bytes.argtypes = [i32, i32]
     L.epsgrad_soap_step.argtypes = [vp, vp, vp, vp, vp, vp, i32, i32, i32, ctypes.c_double, ctypes.c_double, ctypes.c_double,

@@ -137,7 +137,8 @@ static int validate(const epsgrad_config_t *c)
     if (c->filter_kind != EPSGRAD_FILTER_CONIC && c->filter_kind != EPSGRAD_FILTER_GAUSSIAN) return EPSGRAD_EINVAL;
     if (c->filter_kind == EPSGRAD_FILTER_GAUSSIAN && !(c->filter_sigma > 0.0)) return EPSGRAD_EINVAL;
     if (!(c->eps_core > 0.0) || !(c->eps_clad > 0.0) || c->eps_core == c->eps_clad) return EPSGRAD_EINVAL;
-    if (!(c->normal_delta >= 0.0)) return EPSGRAD_EINVAL;
+    if (!(c->normal_delta >= 1e-30) || !std::isfinite(c->normal_delta)) return EPSGRAD_EINVAL;   // 0 / denormal: n^2 = 0/0 on flat cells
+    if (!std::isfinite(c->eta) || !std::isfinite(c->z_lo) || !std::isfinite(c->z_hi)) return EPSGRAD_EINVAL;
     if (!(c->morph_diameter >= 0.0)) return EPSGRAD_EINVAL;
     if (c->morph_diameter > 0.0) {
         if (!(c->morph_alpha > 0.0)) return EPSGRAD_EINVAL;
@@ -1570,11 +1571,32 @@ extern "C" int epsgrad_soap_eigh(const float *A, float *Q, float *w, int n, void
     float *a = (float *)work, *lw = (float *)((char *)work + b_a);
     int *info = (int *)((char *)work + b_a + b_w);
     if (cudaMemcpyAsync(a, A, (size_t)n * n * 4, cudaMemcpyDeviceToDevice, st) != cudaSuccess) { cudaGetLastError(); return EPSGRAD_ECUDA; }
-    if (g_solver.set_stream(h, st) != CUSOLVER_STATUS_SUCCESS) return EPSGRAD_ECUDA;
-    // A is symmetric, so its row-major image is its column-major image; the eigenvectors come back as columns, column-major
-    if (g_solver.syevd(h, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER, n, a, n, w, lw, lwork, info) != CUSOLVER_STATUS_SUCCESS) return EPSGRAD_ECUDA;
+    {
+        // the per-device handle carries the stream: binding it and enqueueing the solver is one critical section
+        std::lock_guard<std::mutex> lock(g_solver_mutex);
+        if (g_solver.set_stream(h, st) != CUSOLVER_STATUS_SUCCESS) return EPSGRAD_ECUDA;
+        // A is symmetric, so its row-major image is its column-major image; the eigenvectors come back as columns, column-major
+        if (g_solver.syevd(h, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER, n, a, n, w, lw, lwork, info) != CUSOLVER_STATUS_SUCCESS) return EPSGRAD_ECUDA;
+    }
     k_transpose<<<dim3(cdiv(n, 32), cdiv(n, 32)), 256, 0, st>>>(a, Q, n);
     return cudaGetLastError() == cudaSuccess ? EPSGRAD_OK : EPSGRAD_ECUDA;
+}
+
+extern "C" int epsgrad_soap_eigh_info(const void *work, size_t work_bytes, int n, void *stream, int *info)
+{
+    if (!work || !info || n < 1) return EPSGRAD_EINVAL;
+    int device = 0;
+    if (cudaGetDevice(&device) != cudaSuccess) { cudaGetLastError(); return EPSGRAD_ECUDA; }
+    cusolverDnHandle_t h = solver_handle(device);
+    if (!h) return EPSGRAD_EUNSUPPORTED;
+    const int lwork = solver_lwork(h, n);
+    if (lwork < 0) return EPSGRAD_ECUDA;
+    const size_t b_a = align_up((size_t)n * n * 4, 256), b_w = align_up((size_t)lwork * 4, 256);
+    if (work_bytes < b_a + b_w + 256) return EPSGRAD_ENOWORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (cudaMemcpyAsync(info, (const char *)work + b_a + b_w, sizeof(int), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess) { cudaGetLastError(); return EPSGRAD_ECUDA; }
+    return EPSGRAD_OK;
 }
 
 extern "C" double epsgrad_beta_schedule(double beta_min, double beta_max, int i, int n_iter)

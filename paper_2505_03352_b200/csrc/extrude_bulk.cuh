@@ -47,7 +47,7 @@ __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.a
 __global__ void __launch_bounds__(EXB_THREADS) k_extrude_bulk(const __grid_constant__ ExtrudeBulkParams P)
 {
     extern __shared__ __align__(128) float exb_sm[];
-    const int tid = threadIdx.x, b = blockIdx.y, nz = P.nz, nz4 = nz >> 2, cols = P.cols;
+    const int tid = threadIdx.x, b = blockIdx.z, nz = P.nz, nz4 = nz >> 2, cols = P.cols;
     const int blk_floats = cols * nz;
     // constant part: eps_clad everywhere (the window pieces are rewritten for every item)
     {

@@ -51,7 +51,7 @@ __global__ void __launch_bounds__(ZP_THREADS) k_zreduce_pipe(const __grid_consta
     const unsigned stage_bytes = 2u * ZP_COLS * wb * 16u;
     unsigned long long *full = reinterpret_cast<unsigned long long *>(base + (size_t)NS * stage_bytes);
     unsigned long long *empty = full + ZP_MAX_STAGE;
-    const int tid = threadIdx.x, b = blockIdx.y, nz = P.nz, nblk = P.nblk, n_items = 3 * nblk;
+    const int tid = threadIdx.x, b = blockIdx.z, nz = P.nz, nblk = P.nblk, n_items = 3 * nblk;
 
     if (tid == 0) {
         for (int s = 0; s < NS; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, ZP_CONSUMERS); }

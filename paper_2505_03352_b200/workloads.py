@@ -34,7 +34,7 @@ class Workload:
     eta: float = 0.5
     eps_core: float = 12.11     # Si
     eps_clad: float = 2.085     # SiO2
-    normal_delta: float = 1e-12
+    normal_delta: float = 1e-8  # guard of the normals (S6): above float32 Sobel-difference noise^2
     morph_diameter: float = 0.0 # d of Eqs. (4)-(5) in Yee cells; 0 = morphological filters off (as in Fig. 4)
     morph_alpha: float = 20.0   # App. B
 

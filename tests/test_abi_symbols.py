@@ -55,6 +55,9 @@ def test_host_side_validation_and_no_cpu_fallback():
         B.make_config(mx=8, my=8, nz=8, z_lo=2.0, z_hi=5.0, filter_radius=-1.0),
         B.make_config(mx=8, my=8, nz=8, z_lo=2.0, z_hi=5.0, eps_clad=0.0),
         B.make_config(mx=8, my=8, nz=8, z_lo=2.0, z_hi=5.0, filter_kind=7),
+        B.make_config(mx=8, my=8, nz=8, z_lo=2.0, z_hi=5.0, normal_delta=0.0),    # n^2 = 0/0 on flat cells
+        B.make_config(mx=8, my=8, nz=8, z_lo=2.0, z_hi=5.0, normal_delta=1e-40),  # denormal: flushed to 0 on the device
+        B.make_config(mx=8, my=8, nz=8, z_lo=2.0, z_hi=5.0, eta=float("nan")),
     ]
     for cfg in bad:
         assert L.epsgrad_plan_create(ctypes.byref(cfg), 0, ctypes.byref(h)) == B.EINVAL

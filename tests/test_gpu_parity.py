@@ -347,6 +347,17 @@ def test_error_codes():
     with pytest.raises(B.EpsgradError) as e:
         plan.eps_forward(torch.rand(plan.ctrl_shape, device="cuda"), -1.0)
     assert e.value.status == B.EINVAL
+    # guard of the normals: 0, a denormal (rcp.approx.ftz would flush it) or NaN would make n^2 = 0/0 on every flat cell and break
+    # the uniform-C invariant; non-finite eta or slab faces
+    for bad in (dict(normal_delta=0.0), dict(normal_delta=1e-40), dict(normal_delta=float("nan")), dict(normal_delta=-1e-8),
+                dict(eta=float("nan")), dict(eta=float("inf")), dict(z_lo=float("-inf"))):
+        with pytest.raises(B.EpsgradError) as e:
+            B.Plan(B.make_config(**dict(dict(mx=8, my=8, nz=8, z_lo=2.0, z_hi=5.0), **bad)))
+        assert e.value.status == B.EINVAL, bad
+    # the smallest guard the library takes keeps a uniform design uniform
+    plan = B.Plan(B.make_config(mx=8, my=8, nz=8, z_lo=2.0, z_hi=5.0, normal_delta=1e-30))
+    e1 = plan.eps_forward(torch.full(plan.ctrl_shape, 0.5, device="cuda"), 8.0)
+    assert bool(torch.isfinite(e1).all()) and float((e1[:, :, :, :, 3] - 7.0975).abs().max()) < 1e-5
 
 
 def test_two_plans_on_two_streams_do_not_interfere():

@@ -43,7 +43,7 @@ def test_eigensolver_by_its_defining_properties(n):
     s = B.Soap(n, n)
     Q, w = torch.empty(n, n, device="cuda"), torch.empty(n, device="cuda")
     dA = dev(A)
-    s.eigh(dA, Q, w)
+    s.eigh(dA, Q, w, check=True)             # the solver status word (epsgrad_soap_eigh_info) must say "converged"
     torch.cuda.synchronize()
     assert torch.equal(dA, dev(A))                                          # the input is not written
     Qh, wh = host(Q), host(w)

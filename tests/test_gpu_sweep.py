@@ -67,7 +67,7 @@ def draw(i: int):
     if i % 9 == 0:
         kw["eps_core"], kw["eps_clad"] = 2.1, 12.0                    # inverted contrast
     if i % 3 == 2:
-        kw["normal_delta"] = float(rng.choice([1e-8, 1e-5]))          # guard of the normals (S6); default 1e-12 otherwise
+        kw["normal_delta"] = float(rng.choice([1e-8, 1e-5]))          # guard of the normals (S6); the default is 1e-8 too
     beta = float(np.exp(rng.uniform(0.0, np.log(64.0))))
     return kw, beta, int(rng.integers(1, 4))
 
@@ -106,26 +106,28 @@ def errors(kw, beta, n_pairs, i):
     return worst
 
 
-# the cases of the 1300-case hunt that needed the rules below always run
+# The cases of a 1300-case hunt at the guard SURVEY.md first proposed, delta = 1e-12: there the rounding noise of
+# the float32 Sobel differences (noise^2 ~ 1e-14) became normals on flat parts of the mask.  They always run, at the library's
+# default guard (1e-8) like every other case, and must pass at the same tolerances.
 HARD = [183, 214, 239, 547, 1092, 1239]
+AMPLIFIED = []                     # cases whose tolerances were widened by beta / 17 > 1 (printed by the last test)
 
 
 @pytest.mark.parametrize("i", list(range(N_CASES)) + [i for i in HARD if i >= N_CASES])
 def test_random_configuration(i):
     kw, beta, n_pairs = draw(i)
+    if beta > 17.0:
+        AMPLIFIED.append((i, round(beta, 1)))
     e = errors(kw, beta, n_pairs, i)
-    assert e[3] < 1, (kw, beta, e)
-    if np.any(e[:3] >= 1):
-        # The one known way past the tolerances is the conditioning of the normals: where the mask is flat
-        # to float32 rounding, n_c^2 = g_c^2/(|g|^2 + delta) turns the rounding noise of the Sobel differences (noise^2 ~
-        # 1e-14 against the default delta = 1e-12) into an error of n^2, and its derivative, ~ 1/|g|, into large terms of the
-        # reverse pass that only cancel further down.  Seen in 6 of 1300 cases: gray plateaus left by the morphological
-        # filters (eps off by 1.4e-4), beta ~ 1 under a wide filter, a control grid smaller than the filter, and fully
-        # binarised masks whose whole gradient is 1e-5 ... 1e-10 of the usual size.  Such a case must pass once the guard is
-        # well above the noise.
-        assert kw.get("normal_delta", 1e-12) < 1e-8, (kw, beta, e)
-        e2 = errors(dict(kw, normal_delta=1e-6), beta, n_pairs, i)
-        assert np.all(e2 < 1), (kw, beta, e, e2)
+    assert np.all(e < 1), (kw, beta, e)
+
+
+def test_report_amplified_tolerances():
+    """How many of the sweep's cases ran with tolerances above BASELINE.json's (beta > 17: the float32 rounding of the filter
+    output times beta).  Informational: run with -s to see the list."""
+    n = N_CASES + len([i for i in HARD if i >= N_CASES])
+    print(f"\nsweep: {len(AMPLIFIED)} of {n} cases ran with tolerances x beta/17 (beta > 17): {AMPLIFIED}")
+    assert len(AMPLIFIED) <= n
 
 
 @pytest.mark.parametrize("i", range(N_CASES))
@@ -154,9 +156,31 @@ def test_random_configuration_every_entry_point(i):
     assert torch.equal(eps1, eps0) and torch.equal(g1, g0) and torch.equal(gb1, g0) and torch.equal(db1, db0)
     plan.set_overlap(True)
     # TMA field stream: same windows, same per-column order
-    plan.set_tma(True)
-    assert torch.equal(plan.stage_zreduce(EF, EA), G0) and torch.equal(plan.eps_vjp(C, beta, EF, EA), g0)
-    plan.set_tma(False)
+    for mode in (1, 2):            # single-stage TMA; persistent TMA ring
+        plan.set_tma(mode)
+        plan._ws.fill_(255)                # NaN everywhere: a block this mode skipped cannot borrow the previous mode's result
+        assert torch.equal(plan.stage_zreduce(EF, EA), G0) and torch.equal(plan.eps_vjp(C, beta, EF, EA), g0), (kw, mode)
+    plan.set_tma(0)
+    # eps written by bulk copies out of shared memory: the same affine forms
+    plan.set_bulk_stores(True)
+    assert torch.equal(plan.eps_forward(C, beta), eps0), kw
+    plan.set_bulk_stores(False)
+    # the persistent dataflow kernel (whole step; 2-D chains only), where it applies: same tiles, the filter's tap rows summed
+    # in two groups instead of three
+    try:
+        plan.set_fused(1)
+        fused = True
+    except B.EpsgradError as err:
+        assert err.status == B.EUNSUPPORTED
+        fused = False
+    if fused:
+        for mode in (1, 2):
+            plan.set_fused(mode)
+            eps_f, g_f = plan.eps_forward_vjp(C, beta, EF, EA)
+            torch.cuda.synchronize()
+            assert float(((eps_f - eps0).abs() / eps0.abs()).max()) < 1e-5 * max(1.0, beta / 17.0), (kw, mode)
+            assert float((g_f - g0).abs().max()) <= 1e-4 * max(1.0, beta / 17.0) * float(g0.abs().max()) + 1e-30, (kw, mode)
+        plan.set_fused(0)
     # dense field stream: the cells outside the slab have zero weight, the order inside a column is the same
     plan.set_dense_reads(True)
     assert torch.equal(plan.eps_vjp(C, beta, EF, EA), g0)
