@@ -228,7 +228,7 @@ int eps_forward_vjp(epsgrad_plan_t *plan, const float *C, float beta, int n_pair
                     float *eps, float *dFdC, void *stream);
 
 /* ---- the same calls on HOST buffers (end-to-end path; copies included) --------------- */
-/* eps_host / dFdC_host may be NULL to skip that output (and its work).                  */
+/* eps_host / dFdC_host may be NULL to skip that output (and its work).  At most 64 pairs per call (EPSGRAD_EUNSUPPORTED beyond). */
 int eps_forward_vjp_host(epsgrad_plan_t *plan, const float *C_host, float beta, int n_pairs,
                          const void *const *EF_host, const void *const *EA_host,
                          float *eps_host, float *dFdC_host, void *stream);

@@ -50,11 +50,12 @@ def nvcc_path() -> str:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    """Compile csrc/epsgrad.cu (which includes every .cuh) into libepsgrad.so; returns its path."""
+    """Compile the translation units of csrc/ (plan.cu, launch.cu, hostpath.cu, optimizer.cu) into libepsgrad.so; returns its path."""
     if not force and not stale():
         return LIB
     tmp = LIB + f".tmp{os.getpid()}"
-    cmd = [nvcc_path(), *NVCC_FLAGS, "-I", INCLUDE, "-o", tmp, os.path.join(CSRC, "epsgrad.cu"), "-ldl"]
+    units = sorted(glob.glob(os.path.join(CSRC, "*.cu")))
+    cmd = [nvcc_path(), *NVCC_FLAGS, "--threads", str(len(units)), "-I", INCLUDE, "-o", tmp, *units, "-ldl"]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
     subprocess.check_call(cmd, cwd=CSRC)

@@ -12,12 +12,10 @@
 // Everything here is L2-resident (4 B read per mask pixel, 60 B written per cell); the kernel is ALU/latency bound.
 #pragma once
 #include "common.cuh"
+#include "sizes.cuh"
 
 namespace epsgrad {
 
-constexpr int F2_TI = 16, F2_TJ = 16, F2_THREADS = 256;
-constexpr int F2_NE2D = 5;        // planes: eps2d_x, eps2d_y, eps2d_z, eps_zz on the lower face cell, on the upper face cell
-constexpr int F2_NCOEF = 10;      // planes: [hbk, abk, gxk, gyk] for c = x, the same for c = y, flo, fhi
 
 struct Fwd2dParams {
     const float *phi;      // [B,px,py] centred filter output
@@ -29,12 +27,6 @@ struct Fwd2dParams {
     float w_lo, w_hi;      // fractional z-face weights of eps_zz (0 if that face cell is absent)
 };
 
-__host__ __device__ inline size_t fwd2d_smem_floats(int s)
-{
-    const int CI = F2_TI + 2, CJ = F2_TJ + 2;
-    const int MP = s * CI + s / 2, MQ = s * CJ + s / 2;
-    return (size_t)2 * MP * MQ + 4 * CI * CJ;
-}
 
 // d eps_zz / d eps2d_z on a face cell of weight w:  w (eps_zz/v)^2, eps_zz/v = 1/(w + (1-w) v/eps_clad)
 __device__ __forceinline__ float face_factor(float w, float v, float inv_ec)

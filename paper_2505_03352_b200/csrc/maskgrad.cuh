@@ -13,6 +13,7 @@
 // Sobel^T sources on [i0-2, i0+TI].
 #pragma once
 #include "common.cuh"
+#include "sizes.cuh"
 #include "reduce.cuh"
 
 namespace epsgrad {
@@ -29,13 +30,7 @@ struct MaskGradParams {
     float beta, eta_r, eps_clad, deps;
 };
 
-constexpr int MG_TI = 16, MG_TJ = 16, MG_THREADS = 256;
-constexpr int MG_CI = MG_TI + 3, MG_CJ = MG_TJ + 3;        // staged cells: [i0-2, i0+TI] x [j0-2, j0+TJ]
 
-__host__ __device__ inline size_t maskgrad_smem_floats(int s)
-{
-    return (size_t)10 * MG_CI * MG_CJ + MG_TI * MG_TJ + (size_t)s * (MG_TI + MG_TJ);
-}
 
 // One tile of TI x TJ cells by a CTA of MG_THREADS threads; sm: maskgrad_smem_floats(s) floats; npart: tiles per design (the
 // pitch of dbeta_part).  No barrier at entry or exit.  G, the coefficients and Phi' are read through L2 (ld.global.cg): in the

@@ -29,12 +29,10 @@
 
 namespace epsgrad {
 
-constexpr int MK_THREADS = 256, MK_G = 2, MK_BAND = 16;     // CTA size; tap-row groups of the filter tiles; Yee rows per band
+constexpr int MK_THREADS = 256, MK_G = 2;                   // CTA size; tap-row groups of the filter tiles (MK_BAND: sizes.cuh)
 constexpr int MK_TPASS = 2;                                  // passes of a transposed-filter tile over its tap rows (shared memory)
 constexpr int MK_ZCOLS = 128;                                // z columns per field block (20 KB of staging at 5 chunks per column)
-enum { PH_F1 = 0, PH_F2, PH_X, PH_M, PH_T, PH_Z, PH_N };    // the compute list's phases in within-step order, then the field blocks
 constexpr int MK_NCOMPUTE = 5;
-constexpr int MK_SCHED_HEAD = 8;                             // ints before the done counters in MegaParams::sched
 
 static_assert(F4_THREADS * MK_G == MK_THREADS && F2_THREADS == MK_THREADS && MG_THREADS == MK_THREADS &&
               ZR_THREADS == MK_THREADS && EX_THREADS == MK_THREADS, "one CTA size for every role");

@@ -19,11 +19,11 @@
 // (plain adds: no sliding-window subtraction, the staged values span e^-20..e^20).  Bound: shared-memory reads and FADD issue; L2-resident.
 #pragma once
 #include "common.cuh"
+#include "sizes.cuh"
 #include "reduce.cuh"
 
 namespace epsgrad {
 
-constexpr int MO_T = 32, MO_THREADS = 256, MO_MAX_R = 16;
 
 struct MorphParams {
     const float *x;        // [B,px,py] input of the forward op: first op: centred filter output Phi'; later ops: z of the previous op

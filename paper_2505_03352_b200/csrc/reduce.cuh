@@ -6,6 +6,7 @@
 // No atomics: the results are bitwise reproducible.
 #pragma once
 #include "common.cuh"
+#include "sizes.cuh"
 
 namespace epsgrad {
 
@@ -36,7 +37,6 @@ __global__ void __launch_bounds__(256) k_sum_partials(const float *pa, int na, c
     if (threadIdx.x == 0) out[blockIdx.x] = scale * s;
 }
 
-constexpr int UB_THREADS = 256, UB_PER_THREAD = 16;
 
 // partial sums of sech^2(beta (x - eta_r)) over the mask of design blockIdx.y; x: centred input of the last projection
 __global__ void __launch_bounds__(UB_THREADS) k_unbinarity(const float *x, size_t n_mask, float beta, float eta_r, float *part)
@@ -56,22 +56,6 @@ __global__ void __launch_bounds__(UB_THREADS) k_unbinarity(const float *x, size_
     }
     const float s = block_sum(v, scratch);
     if (threadIdx.x == 0) part[(size_t)blockIdx.y * gridDim.x + blockIdx.x] = s;
-}
-
-// Adam, Eqs. (10)-(11), one step in place on n control variables: M = b1 M + (1-b1) G, V = b2 V + (1-b2) G^2,
-// C -= lr (M/c1) / (sqrt(V/c2) + eps) with the bias corrections c1 = 1 - b1^i, c2 = 1 - b2^i formed on the host in float64.
-// IEEE division and square root (no approximations): the update is compared with the float64 oracle at 1e-6.
-__global__ void __launch_bounds__(256) k_adam(float *C, float *M, float *V, const float *G, size_t n,
-                                              float b1, float b2, float omb1, float omb2, float inv_c1, float inv_c2, float lr, float eps)
-{
-    const size_t k = (size_t)blockIdx.x * 256 + threadIdx.x;
-    if (k >= n) return;
-    const float g = G[k];
-    const float m = fmaf(b1, M[k], omb1 * g);          // omb = 1 - b, rounded once from float64 (1.0f - 0.999f is off by 5e-5)
-    const float v = fmaf(b2, V[k], omb2 * g * g);
-    M[k] = m;
-    V[k] = v;
-    C[k] -= lr * (m * inv_c1) / (sqrtf(v * inv_c2) + eps);
 }
 
 }  // namespace epsgrad

@@ -92,4 +92,20 @@ __global__ void __launch_bounds__(256) k_transpose(const float *in, float *out, 
         if (bx + r < n && by + tx < n) out[(size_t)(bx + r) * n + by + tx] = t[tx][r];
 }
 
+// Adam, Eqs. (10)-(11), one step in place on n control variables: M = b1 M + (1-b1) G, V = b2 V + (1-b2) G^2,
+// C -= lr (M/c1) / (sqrt(V/c2) + eps) with the bias corrections c1 = 1 - b1^i, c2 = 1 - b2^i formed on the host in float64.
+// IEEE division and square root (no approximations): the update is compared with the float64 oracle at 1e-6.
+__global__ void __launch_bounds__(256) k_adam(float *C, float *M, float *V, const float *G, size_t n,
+                                              float b1, float b2, float omb1, float omb2, float inv_c1, float inv_c2, float lr, float eps)
+{
+    const size_t k = (size_t)blockIdx.x * 256 + threadIdx.x;
+    if (k >= n) return;
+    const float g = G[k];
+    const float m = fmaf(b1, M[k], omb1 * g);          // omb = 1 - b, rounded once from float64 (1.0f - 0.999f is off by 5e-5)
+    const float v = fmaf(b2, V[k], omb2 * g * g);
+    M[k] = m;
+    V[k] = v;
+    C[k] -= lr * (m * inv_c1) / (sqrtf(v * inv_c2) + eps);
+}
+
 }  // namespace epsgrad
