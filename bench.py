@@ -232,25 +232,43 @@ def run_ours(args, w):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     dev = torch.device("cuda", local)
 
-    plan = B.Plan(B.config_of(w), local)
     from dataclasses import replace
-    C = torch.from_numpy(W.make_C(replace(w, index=w.index + 1000 * rank))).to(dev)
+    mode = args.shard
+    shard = sharding.make_shard(mode, w, rank, world)
+    plan = B.Plan(B.config_of(shard["sub"]), local)
+    if shard["slab"] is not None:
+        plan.set_slab(shard["slab"]["x_first"], shard["slab"]["x_count"])
+    # designs: every rank draws its own designs; pairs / xslab: ONE design, the same C on every rank
+    C = torch.from_numpy(W.make_C(replace(w, index=w.index + 1000 * rank) if mode == "designs" else w)).to(dev)
+    C_part = C if shard["slab"] is None else C[:, shard["slab"]["e0"]:shard["slab"]["e1"]].contiguous()
     gen = torch.Generator(device=dev)
     gen.manual_seed(1234 + rank)
-    shape = plan.eps_shape
+    shape = plan.field_shape                                   # this rank's rows of eps / E_F / E_A
+    n_my = len(shard["pairs"])                                 # this rank's field pairs
 
     def field():
         return torch.view_as_complex(torch.randn(*shape, 2, device=dev, dtype=torch.float32, generator=gen))
     NS = n_sets(w)
-    EF = [[field() for _ in range(w.n_pairs)] for _ in range(NS)]
-    EA = [[field() for _ in range(w.n_pairs)] for _ in range(NS)]
+    EF = [[field() for _ in range(n_my)] for _ in range(NS)]
+    EA = [[field() for _ in range(n_my)] for _ in range(NS)]
     eps = torch.empty(shape, dtype=torch.float32, device=dev)
-    grad = torch.empty(plan.ctrl_shape, dtype=torch.float32, device=dev)
+    grad = torch.empty((w.batch, w.mx, w.my), dtype=torch.float32, device=dev)         # the whole design's dF/dC
+    grad_part = grad if shard["slab"] is None else torch.empty(plan.ctrl_shape, dtype=torch.float32, device=dev)
+
+    def compute(Cp, EFs, EAs, beta):
+        if n_my == 0:                                          # more ranks than pairs: forward only, nothing to add
+            plan.eps_forward(Cp, beta, eps)
+            return eps, None
+        plan.eps_forward_vjp(Cp, beta, EFs, EAs, eps, grad_part)
+        return eps, grad_part
 
     def eager_step(i):
         s = i % NS
         for beta in w.betas:
-            plan.eps_forward_vjp(C, beta, EF[s], EA[s], eps, grad)
+            sharding.shard_step(shard, compute, C, (EF[s], EA[s]), beta, grad, C_part=C_part)
+
+    if mode != "designs" and world > 1:
+        args.graph = False                                     # the gradient all-reduce (NCCL) runs between the library calls
 
     # One CUDA graph per buffer set, captured through the C ABI (the calls enqueue only kernels and
     # fork/join events, so they are capturable); replaying removes the host's launch cost from the step.
@@ -294,7 +312,39 @@ def run_ours(args, w):
     clocks = sampler.stop()
     ms_total = sharding.max_over_ranks(ms_total, device=dev)
     cells_step = w.cells * len(w.betas)
-    value = sharding.job_throughput(cells_step, args.steps, ms_total, world)
+    # designs: every rank processed its own cells (weak scaling); pairs / xslab: the ranks shared ONE design (strong scaling)
+    value = sharding.job_throughput(cells_step, args.steps, ms_total, world if mode == "designs" else 1)
+
+    if mode != "designs":
+        # ONE design shared by the ranks: whole-job throughput with the gradient exchange inside the timed region.  The
+        # per-call breakdown, the per-kernel roofline and the host-buffer leg are those of the default (--shard designs) line.
+        if rank == 0:
+            peak, peak_src = measured_peak_gbs()
+            step_ms = ms_total / args.steps
+            step_bytes = (w.cells * 12 * world if mode == "pairs" else w.cells * 12) * len(w.betas) \
+                + zreduce_sector_bytes(w, w.n_pairs) * len(w.betas)
+            line = base_line(w, args, world)
+            line["config"]["per_gpu"] = {
+                "pairs": f"field pairs of ONE design over the ranks ({w.n_pairs} pairs / {world} ranks); every rank runs the forward "
+                         f"chain and writes its own eps; one all-reduce (sum) of dF/dC, {w.batch * w.mx * w.my * 4} bytes, per step",
+                "xslab": f"x-slabs of ONE design over the ranks (halo {sharding.slab_halo_cells(w.radius, w.morph_diameter)} cells); "
+                         f"eps and fields hold the own rows only; one all-reduce (sum) of dF/dC, {w.batch * w.mx * w.my * 4} bytes, per step",
+            }[mode]
+            if not args.graph:
+                line["config"]["launch"] = "eager eps_forward_vjp calls (the NCCL all-reduce runs between them)"
+            line.update({"value": value, "ms_per_step": step_ms, "dtype": "f32", "scaling": "strong", "shard": mode,
+                         "clocks": clocks, "gpu_launches": launches_per_step * args.steps,
+                         "e2e": {"skipped": "measured by the default line (--shard designs)"},
+                         "roofline": {"bound": "hbm", "kernel": "step", "unit": "GB/s", "peak": peak, "peak_source": peak_src,
+                                      "algorithmic_bytes": step_bytes, "achieved": step_bytes / (step_ms * 1e-3) / 1e9,
+                                      "frac": step_bytes / (step_ms * 1e-3) / 1e9 / (peak * world), "traffic": None,
+                                      "note": "eps stores (every rank's) + touched field sectors of the whole job over the step, "
+                                              "against the peak of all ranks' HBM"}})
+            print(json.dumps(line), flush=True)
+        if dist is not None:
+            dist.barrier()
+            dist.destroy_process_group()
+        return
 
     # ---- the three calls of the ABI, each timed repetition by repetition (median of >= 20 repetitions):
     # forward (eps_forward), vjp (eps_vjp), forward_vjp (the step above).  One CUDA graph per call and buffer set, one event
@@ -363,20 +413,31 @@ def run_ours(args, w):
     alg = {"extrude": w.cells * 12, "zreduce": zreduce_sector_bytes(w, w.n_pairs)}
     dom = max(alg, key=lambda k: kernels[k])
 
-    # the field stream alone (the stage tap of the ABI), cold L2: a 256 MB fill between repetitions, rotating field sets
+    # the field stream alone (the stage tap of the ABI), cold L2, rotating field sets, two ways of emptying L2 before each
+    # repetition: a 256 MB FILL (leaves L2 full of dirty lines, as the eps stores of the previous step do: the stream then
+    # also pays for their write-back) and a 256 MB READ (clean lines: nothing to write back)
     flush = torch.empty(64 << 20, dtype=torch.float32, device=dev)
-    ts = []
-    for i in range(min(reps, 30)):
-        flush.fill_(float(i))
-        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a0.record()
-        plan.stage_zreduce(EF[i % NS], EA[i % NS])
-        a1.record()
-        torch.cuda.synchronize()
-        ts.append(a0.elapsed_time(a1))
+    flush.zero_()
+
+    def z_alone(dirty):
+        ts = []
+        for i in range(min(reps, 30)):
+            if dirty:
+                flush.fill_(float(i))
+            else:
+                flush.sum()
+            a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a0.record()
+            plan.stage_zreduce(EF[i % NS], EA[i % NS])
+            a1.record()
+            torch.cuda.synchronize()
+            ts.append(a0.elapsed_time(a1))
+        ts.sort()
+        return ts[len(ts) // 2]
+    flush.sum(); flush.sum()
+    z_clean_ms = z_alone(False)
+    z_alone_ms = z_alone(True)
     del flush
-    ts.sort()
-    z_alone_ms = ts[len(ts) // 2]
 
     # DRAM bytes per launch from the committed ncu --set full capture, if it was taken on THIS build (source hash)
     traffic, traffic_note = None, "no ncu capture of this build under profiles/ (traffic.json names another source hash)"
@@ -400,8 +461,11 @@ def run_ours(args, w):
                 "kernels_ms": kernels,
                 "others": {k: {"algorithmic_bytes": alg[k], "kernel_ms": kernels[k], "GB/s": alg[k] / (kernels[k] * 1e-3) / 1e9,
                                "frac": alg[k] / (kernels[k] * 1e-3) / 1e9 / peak} for k in alg if k != dom},
-                "zreduce_alone": {"kernel_ms": z_alone_ms, "frac": alg["zreduce"] / (z_alone_ms * 1e-3) / 1e9 / peak,
-                                  "how": "epsgrad_stage_zreduce alone, cold L2 (256 MB fill before each repetition), median"},
+                "zreduce_alone": {"kernel_ms": z_clean_ms, "frac": alg["zreduce"] / (z_clean_ms * 1e-3) / 1e9 / peak,
+                                  "how": "epsgrad_stage_zreduce alone, cold and CLEAN L2 (256 MB read before each repetition), median",
+                                  "after_fill_ms": z_alone_ms, "after_fill_frac": alg["zreduce"] / (z_alone_ms * 1e-3) / 1e9 / peak,
+                                  "after_fill": "the same after a 256 MB FILL: L2 full of dirty lines, as after the eps stores of the "
+                                                "previous step; the difference is their write-back under the read stream"},
                 "frac_dense_equiv": {"value": dense_bytes / (kernels["zreduce"] * 1e-3) / 1e9 / peak,
                                      "bytes": dense_bytes,
                                      "note": "48 B per Yee cell and pair as if every z cell were read: not the method's work "
@@ -464,12 +528,17 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=300)
     ap.add_argument("--warmup", type=int, default=10)
-    ap.add_argument("--config", default="paper")
+    ap.add_argument("--config", default=None, help="workload name (default: paper; multiwavelength / large with --shard pairs / xslab)")
+    ap.add_argument("--shard", default="designs", choices=["designs", "pairs", "xslab"],
+                    help="how N ranks share the work: independent designs (default, weak scaling, no collective); the field pairs "
+                         "of one design; x-slabs of one design (both strong scaling, one all-reduce of dF/dC per step)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-graph", dest="graph", action="store_false",
                     help="launch every step eagerly from Python instead of replaying a captured CUDA graph")
     args = ap.parse_args()
     from paper_2505_03352_b200 import workloads as W
+    if args.config is None:
+        args.config = {"designs": "paper", "pairs": "multiwavelength", "xslab": "large"}[args.shard]
     w = W.BY_NAME[args.config]
     if args.impl == "reference":
         run_reference(args, w)

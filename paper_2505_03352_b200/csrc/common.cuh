@@ -57,6 +57,13 @@ __device__ __forceinline__ float4 ld_stream(const float4 *p)
     return r;
 }
 
+// Load of a plane that an earlier kernel of the stream produced (CG = false: default caching) or that other CTAs of the SAME
+// launch produce (CG = true, the persistent kernel of mega.cuh: L1 is not coherent, so the load goes to L2).
+template <bool CG>
+__device__ __forceinline__ float ld_plane(const float *p) { return CG ? __ldcg(p) : *p; }
+template <bool CG>
+__device__ __forceinline__ float2 ld_plane2(const float2 *p) { return CG ? __ldcg(p) : *p; }
+
 // 1/x on the special-function unit (MUFU.RCP, <= 1 ulp; 1/inf = 0).  The 2-D chain needs ~1e-7
 // relative accuracy (tolerances 1e-5 / 1e-4), not IEEE rounding.
 __device__ __forceinline__ float fast_rcp(float x)

@@ -36,8 +36,9 @@ __host__ __device__ inline int extrude_cols_per_block(int nz)
 }
 
 // Columns [col0, col0 + ncb) (ncb <= cpb) of component c of design b by a CTA of EX_THREADS threads; vsm: 3 cpb floats of shared
-// memory (plane values of the block).  No barrier at entry or exit.  The plane values are read through L2 (ld.global.cg): in
-// the persistent kernel (mega.cuh) other CTAs of the same launch produce them.
+// memory (plane values of the block).  No barrier at entry or exit.  CG: the plane values are read through L2 (ld.global.cg) -- for
+// the persistent kernel (mega.cuh), where other CTAs of the same launch produce them.
+template <bool CG>
 __device__ __forceinline__ void block_extrude(const ExtrudeParams &P, int c, int col0, int ncb, int b, float *vsm)
 {
     const int tid = threadIdx.x, nz = P.nz, nz4 = nz >> 2;
@@ -47,7 +48,7 @@ __device__ __forceinline__ void block_extrude(const ExtrudeParams &P, int c, int
     // stage: c = x, y need their own plane; c = z needs planes 2 (full cells), 3 and 4 (face cells)
     const int npl = c == 2 ? 3 : 1;
     for (int o = 0; o < npl; ++o)
-        for (int lc = tid; lc < ncb; lc += EX_THREADS) vsm[o * cpb + lc] = __ldcg(ed + (size_t)(c + o) * P.pstride + col0 + lc);
+        for (int lc = tid; lc < ncb; lc += EX_THREADS) vsm[o * cpb + lc] = ld_plane<CG>(ed + (size_t)(c + o) * P.pstride + col0 + lc);
     if (P.sh4 >= 0 && !P.cm.embedded) {
         // region-sized eps: the block is one contiguous run; a thread walks it with a constant stride (few instructions per
         // store: the kernel's issue slots are what the 2-D work beside it needs)
@@ -153,7 +154,7 @@ __global__ void __launch_bounds__(EX_THREADS, EX_CTAS_PER_SM) k_extrude(const __
 {
     extern __shared__ float vsm[];                            // plane values of the block: [3][cpb]
     const int col0 = blockIdx.x * P.cpb;
-    block_extrude(P, blockIdx.y, col0, min(P.cpb, P.ncol - col0), blockIdx.z, vsm);
+    block_extrude<false>(P, blockIdx.y, col0, min(P.cpb, P.ncol - col0), blockIdx.z, vsm);
 }
 
 }  // namespace epsgrad

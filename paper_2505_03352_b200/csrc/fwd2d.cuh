@@ -58,9 +58,9 @@ __device__ __forceinline__ void sobel_at(const float *A, int ci, int cj, int i, 
 }
 
 // One tile of TI x TJ cells by a CTA of F2_THREADS threads; sm: fwd2d_smem_floats(s) floats.  No barrier at entry or exit:
-// the caller separates calls that reuse sm.  Phi' is read through L2 (ld.global.cg): in the persistent kernel (mega.cuh)
-// other CTAs of the same launch produce it.  S > 0: compile-time subpixel count (index divisions fold to shifts); S = 0: runtime P.s.
-template <int S>
+// the caller separates calls that reuse sm.  CG: Phi' is read through L2 (ld.global.cg) -- for the persistent kernel (mega.cuh),
+// where other CTAs of the same launch produce it.  S > 0: compile-time subpixel count (index divisions fold to shifts); S = 0: runtime P.s.
+template <int S, bool CG>
 __device__ __forceinline__ void tile_fwd2d(const Fwd2dParams &P, int bx, int by, int b, float *sm)
 {
     constexpr int TI = F2_TI, TJ = F2_TJ, NTH = F2_THREADS;
@@ -94,7 +94,7 @@ __device__ __forceinline__ void tile_fwd2d(const Fwd2dParams &P, int bx, int by,
                 if (base + u * NTH < MP * MQ) {
                     const int p = inside ? p_base + lp : clampi(p_base + lp, 0, P.px - 1);
                     const int q = inside ? q_base + lq : clampi(q_base + lq, 0, P.py - 1);
-                    ph[u] = __ldcg(phib + p * P.py + q);
+                    ph[u] = ld_plane<CG>(phib + p * P.py + q);
                 }
                 lp += dlp; lq += dlq;
                 if (lq >= MQ) { lq -= MQ; ++lp; }
@@ -185,10 +185,10 @@ __device__ __forceinline__ void tile_fwd2d(const Fwd2dParams &P, int bx, int by,
 
 // grid (ceil(ny/TJ), ceil(nx/TI), B)
 template <int S>
-__global__ void __launch_bounds__(F2_THREADS) k_fwd2d(const __grid_constant__ Fwd2dParams P)
+__global__ void __launch_bounds__(F2_THREADS, 8) k_fwd2d(const __grid_constant__ Fwd2dParams P)
 {
     extern __shared__ __align__(16) float sm[];
-    tile_fwd2d<S>(P, blockIdx.x, blockIdx.y, blockIdx.z, sm);
+    tile_fwd2d<S, false>(P, blockIdx.x, blockIdx.y, blockIdx.z, sm);
 }
 
 }  // namespace epsgrad

@@ -32,11 +32,11 @@ struct MaskGradParams {
 
 
 
-// One tile of TI x TJ cells by a CTA of MG_THREADS threads; sm: maskgrad_smem_floats(s) floats; npart: tiles per design (the
-// pitch of dbeta_part).  No barrier at entry or exit.  G, the coefficients and Phi' are read through L2 (ld.global.cg): in the
-// persistent kernel (mega.cuh) other CTAs of the same launch produce them.  S > 0: compile-time subpixel count; S = 0: runtime P.s.
-template <int S>
-__device__ __forceinline__ void tile_maskgrad(const MaskGradParams &P, int bx, int by, int b, int tiles_x, int tiles_y, float *sm)
+// One tile of TI x TJ cells by a CTA of MG_THREADS threads; sm: maskgrad_smem_floats(s) floats; part_idx: the tile's slot in
+// dbeta_part ([B][tile rows][tiles per row]).  No barrier at entry or exit.  CG: G, the coefficients and Phi' are read through L2 (ld.global.cg) -- for the
+// persistent kernel (mega.cuh), where other CTAs of the same launch produce them.  S > 0: compile-time subpixel count; S = 0: runtime P.s.
+template <int S, bool CG>
+__device__ __forceinline__ void tile_maskgrad(const MaskGradParams &P, int bx, int by, int b, int part_idx, float *sm)
 {
     constexpr int TI = MG_TI, TJ = MG_TJ, NTH = MG_THREADS, CI = MG_CI, CJ = MG_CJ, NC = CI * CJ;
     const int s = S > 0 ? S : P.s, hs = s >> 1;
@@ -67,11 +67,11 @@ __device__ __forceinline__ void tile_maskgrad(const MaskGradParams &P, int bx, i
             float r8[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
             if (i >= 0 && i < nx && j >= 0 && j < ny) {
                 const int cell = i * ny + j;
-                const float gx = __ldcg(gb + cell), gy = __ldcg(gb + ncol + cell);
+                const float gx = ld_plane<CG>(gb + cell), gy = ld_plane<CG>(gb + ncol + cell);
 #pragma unroll
                 for (int o = 0; o < 4; ++o) {
-                    r8[o] = __ldcg(cb + (size_t)o * ncol + cell) * gx;
-                    r8[4 + o] = __ldcg(cb + (size_t)(4 + o) * ncol + cell) * gy;
+                    r8[o] = ld_plane<CG>(cb + (size_t)o * ncol + cell) * gx;
+                    r8[4 + o] = ld_plane<CG>(cb + (size_t)(4 + o) * ncol + cell) * gy;
                 }
             }
 #pragma unroll
@@ -83,8 +83,8 @@ __device__ __forceinline__ void tile_maskgrad(const MaskGradParams &P, int bx, i
         float az = 0.f;
         if (i < nx && j < ny) {
             const int cell = i * ny + j;
-            az = fmaf(__ldcg(cb + (size_t)8 * ncol + cell), __ldcg(gb + (size_t)3 * ncol + cell),
-                      fmaf(__ldcg(cb + (size_t)9 * ncol + cell), __ldcg(gb + (size_t)4 * ncol + cell), __ldcg(gb + (size_t)2 * ncol + cell)));
+            az = fmaf(ld_plane<CG>(cb + (size_t)8 * ncol + cell), ld_plane<CG>(gb + (size_t)3 * ncol + cell),
+                      fmaf(ld_plane<CG>(cb + (size_t)9 * ncol + cell), ld_plane<CG>(gb + (size_t)4 * ncol + cell), ld_plane<CG>(gb + (size_t)2 * ncol + cell)));
         }
         AbZ[it] = az;
     }
@@ -159,8 +159,8 @@ __device__ __forceinline__ void tile_maskgrad(const MaskGradParams &P, int bx, i
         ex[1] = mx * AbF[c0];  hx[1] = mx * R[c0];
         ey[1] = my * AbF[NC + c0];  hy[1] = my * R[4 * NC + c0];
         const int p = 2 * i, q = 2 * j;
-        const float2 ph0 = __ldcg(reinterpret_cast<const float2 *>(phib + p * P.py + q));
-        const float2 ph1 = __ldcg(reinterpret_cast<const float2 *>(phib + (p + 1) * P.py + q));
+        const float2 ph0 = ld_plane2<CG>(reinterpret_cast<const float2 *>(phib + p * P.py + q));
+        const float2 ph1 = ld_plane2<CG>(reinterpret_cast<const float2 *>(phib + (p + 1) * P.py + q));
         const float phv[2][2] = {{ph0.x, ph0.y}, {ph1.x, ph1.y}};
         const int nq0 = nidx[TP + 2 * tj], nq1 = nidx[TP + 2 * tj + 1];
         const float k0 = P.deps * inv_s2 * 2.0f * P.beta;
@@ -185,7 +185,7 @@ __device__ __forceinline__ void tile_maskgrad(const MaskGradParams &P, int bx, i
         }
         if (P.dbeta_part) {                                         // block-uniform
             const float sdb = block_sum(db, reinterpret_cast<float *>(nidx));      // nidx is dead for every thread past block_sum's first barrier
-            if (tid == 0) P.dbeta_part[(size_t)b * tiles_y * tiles_x + by * tiles_x + bx] = sdb / P.beta;
+            if (tid == 0) P.dbeta_part[part_idx] = sdb / P.beta;
         }
     } else {
     float db = 0.f;
@@ -195,7 +195,7 @@ __device__ __forceinline__ void tile_maskgrad(const MaskGradParams &P, int bx, i
         for (int u = 0; u < 4; ++u) {
             const int it = base + u * NTH, tp = it / TQ, tq = it - tp * TQ;
             const int p = s * i0 + tp, q = s * j0 + tq;
-            if (it < TP * TQ && p < P.px && q < P.py) ph[u] = __ldcg(phib + p * P.py + q);
+            if (it < TP * TQ && p < P.px && q < P.py) ph[u] = ld_plane<CG>(phib + p * P.py + q);
         }
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
@@ -232,17 +232,17 @@ __device__ __forceinline__ void tile_maskgrad(const MaskGradParams &P, int bx, i
     }
     if (P.dbeta_part) {
         const float sdb = block_sum(db, reinterpret_cast<float *>(nidx));
-        if (tid == 0) P.dbeta_part[(size_t)b * tiles_y * tiles_x + by * tiles_x + bx] = sdb / P.beta;
+        if (tid == 0) P.dbeta_part[part_idx] = sdb / P.beta;
     }
     }
 }
 
 // grid (ceil(ny/TJ), ceil(nx/TI), B)
 template <int S>
-__global__ void __launch_bounds__(MG_THREADS) k_maskgrad(const __grid_constant__ MaskGradParams P)
+__global__ void __launch_bounds__(MG_THREADS, 8) k_maskgrad(const __grid_constant__ MaskGradParams P)
 {
     extern __shared__ __align__(16) float sm[];
-    tile_maskgrad<S>(P, blockIdx.x, blockIdx.y, blockIdx.z, gridDim.x, gridDim.y, sm);
+    tile_maskgrad<S, false>(P, blockIdx.x, blockIdx.y, blockIdx.z, (blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x, sm);
 }
 
 }  // namespace epsgrad

@@ -214,8 +214,8 @@ __global__ void __launch_bounds__(MK_THREADS, 4) k_mega(const __grid_constant__ 
                 const int tr = idx / P.nbx1;
                 tile_filter_conic4<NTC, MK_G>(P.f1, idx - tr * P.nbx1, 2 * b + tr, d, w_s, scratch);
             } break;
-            case PH_F2: tile_fwd2d<2>(P.f2, idx, b, d, scratch); break;
-            case PH_M: tile_maskgrad<2>(P.mg, idx, b, d, P.nbx2, P.nb, scratch); break;
+            case PH_F2: tile_fwd2d<2, true>(P.f2, idx, b, d, scratch); break;
+            case PH_M: tile_maskgrad<2, true>(P.mg, idx, b, d, (d * P.nb + b) * P.nbx2 + idx, scratch); break;
             case PH_T: {
                 const int tr = idx / P.nbx1;
                 tile_filterT_conic4<NTC, MK_G, MK_TPASS>(P.ft, idx - tr * P.nbx1, 2 * b + tr, d, w_s, scratch);
@@ -225,7 +225,7 @@ __global__ void __launch_bounds__(MK_THREADS, 4) k_mega(const __grid_constant__ 
                 const int c = idx / nblk, blk = idx - c * nblk;
                 const int col0 = b * MK_BAND * P.f2.ny, cend = min(P.f2.nx, (b + 1) * MK_BAND) * P.f2.ny;
                 const int colb = col0 + blk * P.ex.cpb;
-                block_extrude(P.ex, c, colb, min(P.ex.cpb, cend - colb), d, scratch);
+                block_extrude<true>(P.ex, c, colb, min(P.ex.cpb, cend - colb), d, scratch);
             } break;
             }
             __syncthreads();                                   // the item's global writes are ordered before the release

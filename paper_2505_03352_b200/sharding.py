@@ -57,3 +57,54 @@ def slab_partition(mx: int, upsample: int, rank: int, world: int, halo_cells: in
     h = -(-halo_cells // upsample)                     # control rows
     e0, e1 = max(0, a0 - h), min(mx, a1 + h)
     return dict(a0=a0, a1=a1, e0=e0, e1=e1, x_first=upsample * (a0 - e0), x_count=upsample * (a1 - a0))
+
+
+# ---- one sharded step (bench.py --shard, tests/test_sharding_gloo.py).  Control flow only: `compute` does the arithmetic
+# (the CUDA library in bench.py; any implementation of the chain in a test).
+def make_shard(mode: str, w, rank: int, world: int) -> dict:
+    """This rank's share of workload w (a workloads.Workload) under sharding `mode`:
+    "designs": its own batch of designs, nothing shared (weak scaling, no collective);
+    "pairs":   field pairs shard_range(n_pairs) of ONE design -- every rank runs the forward chain (its solver needs eps), reads
+               only its pairs' fields, and the partial gradients are summed (one all-reduce of B*Mx*My floats; P:L167, L173);
+    "xslab":   control rows [a0, a1) of ONE design plus a halo (slab_partition); eps and the fields hold only the rows it owns;
+               the partial gradient covers the slab's control rows and the halo parts add into the neighbours' (all-reduce).
+    Returns dict(mode, sub = the Workload of this rank's plan, pairs = range, slab = slab_partition(...) or None)."""
+    from dataclasses import replace
+    if mode == "designs":
+        return dict(mode=mode, sub=w, pairs=range(w.n_pairs), slab=None)
+    if mode == "pairs":
+        mine = shard_range(w.n_pairs, rank, world)
+        return dict(mode=mode, sub=replace(w, n_pairs=len(mine)), pairs=mine, slab=None)
+    if mode == "xslab":
+        p = slab_partition(w.mx, w.upsample, rank, world, slab_halo_cells(w.radius, w.morph_diameter))
+        return dict(mode=mode, sub=replace(w, mx=p["e1"] - p["e0"]), pairs=range(w.n_pairs), slab=p)
+    raise ValueError(mode)
+
+
+def shard_step(shard: dict, compute, C_full, fields, beta: float, grad_full, group=None, C_part=None):
+    """One forward + VJP of this rank's share, then the gradient exchange.
+    C_full [B,Mx,My]: the whole design's control variables (every rank has them: 250 KB at paper scale);
+    fields: (EF, EA) lists of this rank's OWN pairs on its OWN rows (what its solver produced);
+    compute(C_part, EF, EA, beta) -> (eps_part, grad_part [B, rows of C_part, My]);
+    grad_full: output [B,Mx,My], overwritten with the sum over the ranks;
+    C_part: this rank's rows of C_full if the caller has cut them out already (C does not change within a step).
+    Returns eps_part (this rank's eps: the whole region, or its rows of it)."""
+    EF, EA = fields
+    p = shard["slab"]
+    if C_part is None:
+        C_part = C_full if p is None else C_full[:, p["e0"]:p["e1"]].contiguous()
+    eps_part, grad_part = compute(C_part, EF, EA, beta)
+    if shard["mode"] == "designs":
+        if grad_part is not grad_full:
+            grad_full.copy_(grad_part)
+        return eps_part
+    if p is None:
+        if grad_part is None:                       # a rank without pairs adds nothing
+            grad_full.zero_()
+        elif grad_part is not grad_full:
+            grad_full.copy_(grad_part)
+    else:
+        grad_full.zero_()
+        grad_full[:, p["e0"]:p["e1"]].copy_(grad_part)
+    sum_gradients(grad_full, group)
+    return eps_part

@@ -38,6 +38,26 @@ def test_bench_line_has_the_contract_keys():
     c = d["cpu_baseline"]
     assert c["kind"] == "oracle" and c["cores"] >= 1 and 0 < c["value"] < d["value"] and c["sample"]
     assert set(d["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
+    # the three calls separately, medians of >= 20 repetitions; the slab-only fraction as the headline and the
+    # dense-equivalent one beside it; the field stream also timed alone; traffic only from a capture of this very build
+    m = d["modes"]
+    assert set(m) == {"forward", "vjp", "forward_vjp"}
+    for k in m:
+        assert m[k]["reps"] >= 20 and m[k]["ms_min"] <= m[k]["ms_median"] and m[k]["cells_per_s"] > 1e10
+    assert m["forward"]["ms_median"] < m["forward_vjp"]["ms_median"] and m["vjp"]["ms_median"] < m["forward_vjp"]["ms_median"]
+    assert abs(d["ms_per_step_median"] - m["forward_vjp"]["ms_median"]) < 1e-12
+    assert r["frac_dense_equiv"]["value"] > r["others"].get("zreduce", r)["frac"] and "not the method's work" in r["frac_dense_equiv"]["note"]
+    assert 0.05 < r["zreduce_alone"]["frac"] < 1.0 and 0.05 < r["step"]["frac"] < 1.0
+    assert set(r["modes_frac"]) == {"forward", "vjp", "vjp_dense_equiv"} and "traffic_source" in r
+    assert c["forward_cells_per_s"] > 0 and c["vjp_cells_per_s"] > 0
+
+
+@pytest.mark.parametrize("shard,config", [("pairs", "multiwavelength"), ("xslab", "paper")])
+def test_sharded_bench_lines_at_one_rank(shard, config):
+    # the N > 1 modes at N = 1: the same control flow (sharding.shard_step) with a world of one
+    d = run_bench("--shard", shard, "--config", config, "--steps", "3", "--warmup", "3")
+    assert d["shard"] == shard and d["scaling"] == "strong" and d["n_gpus"] == 1 and d["value"] > 1e9
+    assert d["gpu_launches"] > 0 and 0.01 < d["roofline"]["frac"] < 1.0 and "all-reduce" in d["config"]["per_gpu"]
 
 
 def test_reference_arm_times_the_oracle():

@@ -128,3 +128,69 @@ def test_slab_partition_covers_the_region_once():
             assert p["e0"] == max(0, p["a0"] - h) and p["e1"] == min(mx, p["a1"] + h)
             assert p["x_first"] == u * (p["a0"] - p["e0"]) and p["x_count"] == u * (p["a1"] - p["a0"])
             assert 0 <= p["x_first"] and p["x_first"] + p["x_count"] <= u * (p["e1"] - p["e0"])
+
+
+# ---- the control flow bench.py --shard runs (sharding.make_shard / shard_step), with the float64 oracle as the compute
+def _oracle_compute(w_sub, slab):
+    import oracle as O
+    from helpers import cfg_of
+
+    def compute(C_part, EF, EA, beta):
+        cfg = cfg_of(w_sub)
+        C = C_part.numpy()[0]
+        eps = O.forward(cfg, C, beta)
+        if slab is None:
+            g = O.vjp(cfg, C, beta, [f.numpy()[0] for f in EF], [f.numpy()[0] for f in EA]) if len(EF) else None
+            return torch.from_numpy(eps)[None], None if g is None else torch.from_numpy(g)[None]
+        rows = slice(slab["x_first"], slab["x_first"] + slab["x_count"])
+        full = (3, cfg.nx, cfg.ny, cfg.nz)
+        fs, as_ = [], []
+        for f, a in zip(EF, EA):                    # the rank's arrays hold its own rows only: zero elsewhere in the slab's region
+            ff, aa = np.zeros(full, np.complex64), np.zeros(full, np.complex64)
+            ff[:, rows], aa[:, rows] = f.numpy()[0], a.numpy()[0]
+            fs.append(ff); as_.append(aa)
+        g = O.vjp(cfg, C, beta, fs, as_)
+        return torch.from_numpy(np.ascontiguousarray(eps[:, rows]))[None], torch.from_numpy(g)[None]
+    return compute
+
+
+def _bench_flow_worker(rank, world, port, out_dir, mode):
+    import sys
+    from dataclasses import replace
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    sys.path[:0] = [root, os.path.join(root, "tests")]
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    from paper_2505_03352_b200 import workloads as W
+    w = replace(W.BY_NAME["multiwavelength"], mx=22, my=9, nz=8, z_lo=2.25, z_hi=5.75, radius=3.0)   # 3 pairs
+    beta = 8.0
+    C = torch.from_numpy(W.make_C(w))
+    EF = [torch.from_numpy(W.make_field(w, p, 0))[None] for p in range(w.n_pairs)]
+    EA = [torch.from_numpy(W.make_field(w, p, 1))[None] for p in range(w.n_pairs)]
+    sh = sharding.make_shard(mode, w, rank, world)
+    u = w.upsample
+    own = slice(None) if sh["slab"] is None else slice(u * sh["slab"]["a0"], u * sh["slab"]["a1"])
+    mine = ([EF[p][:, :, own].contiguous() for p in sh["pairs"]], [EA[p][:, :, own].contiguous() for p in sh["pairs"]])
+    grad = torch.full((1, w.mx, w.my), float("nan"), dtype=torch.float64)
+    eps = sharding.shard_step(sh, _oracle_compute(sh["sub"], sh["slab"]), C, mine, beta, grad)
+    # the 1-rank result of the same flow
+    one = sharding.make_shard(mode, w, 0, 1)
+    grad1 = torch.empty_like(grad)
+    dist_group = dist.new_group([rank])            # a world of one: the all-reduce is the identity
+    eps1 = sharding.shard_step(one, _oracle_compute(one["sub"], one["slab"]), C, (EF, EA), beta, grad1, group=dist_group)
+    err = torch.tensor([float((grad - grad1).abs().max() / grad1.abs().max()),
+                        float(((eps - eps1[:, :, own]).abs() / eps1[:, :, own]).max())])
+    dist.all_reduce(err, op=dist.ReduceOp.MAX)
+    if rank == 0:
+        np.save(os.path.join(out_dir, "res.npy"), err.numpy())
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("mode,world", [("pairs", 2), ("xslab", 2), ("pairs", 4), ("xslab", 3), ("designs", 2)])
+def test_bench_shard_flow_matches_the_one_rank_result(tmp_path, mode, world):
+    """bench.py --shard pairs | xslab: partition, per-rank compute, gradient all-reduce -- against the same flow on one rank.
+    pairs with 4 ranks leaves one rank without a pair."""
+    mp.spawn(_bench_flow_worker, args=(world, _free_port(), str(tmp_path), mode), nprocs=world, join=True)
+    err_g, err_e = np.load(tmp_path / "res.npy")
+    assert err_g < 1e-12 and err_e < 1e-12, (mode, world, err_g, err_e)
