@@ -55,7 +55,7 @@ extern "C" {
 #define EPSGRAD_OK             0
 #define EPSGRAD_EINVAL        -1   /* null / misaligned pointer, bad size, beta <= 0, eps <= 0, a normalised filter whose
                                       support leaves a mask pixel without any control pixel (R <= (u - 1/s)/sqrt(2)), ... */
-#define EPSGRAD_EUNSUPPORTED  -2   /* upsample*subpixel not in {2,4,6,8}, Nz % 4 != 0, tables too large (conic filter: taps x
+#define EPSGRAD_EUNSUPPORTED  -2   /* upsample*subpixel not in {2,4,6,8} (unless nx_cells, ny_cells are given), tables too large (conic filter: taps x
                                       phases beyond 200 KB of shared memory, e.g. R = 12 cells at 8 mask pixels per control pixel),
                                       morphological disk radius > 16 mask pixels or wider than the mask */
 #define EPSGRAD_ENOWORKSPACE  -3   /* workspace / staging buffer missing or too small */
@@ -81,9 +81,14 @@ typedef struct {
     int32_t mx, my;           /* control grid (Eq. (2) nodes, pixel-centred; S3)             */
     int32_t upsample;         /* u: Yee cells per control pixel, Nx = u*Mx, Ny = u*My        */
     int32_t subpixel;         /* s: mask pixels per Yee cell per axis, even (S4; default 2)  */
-    int32_t nz;               /* Yee cells in z (multiple of 4)                              */
+    int32_t nz;               /* Yee cells in z (multiples of 4 take the 16-byte paths; any other nz a scalar one) */
     int32_t filter_kind;      /* EPSGRAD_FILTER_*                                            */
     int32_t filter_normalize; /* 1: density filter, renormalised at borders (S2); 0: raw Eq. (2) */
+    int32_t nx_cells, ny_cells; /* 0, 0: Nx = upsample*Mx, Ny = upsample*My.  Otherwise the Yee cells of the design region, any
+                                 numbers >= Mx, My: control node a sits at x_a = (Nx/Mx)(a + 1/2), a non-integer number of cells per
+                                 control pixel (Fig. 4: 36 x 36 control variables on 210 x 210 cells).  Such plans run
+                                 Eq. (2) and its transpose with weights evaluated on the fly (filter_general.cuh) and `upsample`
+                                 is ignored; no x-slab, no persistent kernel for them                              */
     double  z_lo, z_hi;       /* slab extent in cell units, may be fractional (S8)           */
     double  filter_radius;    /* R in Yee cells                                              */
     double  filter_sigma;     /* Gaussian sigma in Yee cells                                 */

@@ -46,6 +46,7 @@ class Config(ctypes.Structure):
         ("batch", ctypes.c_int32), ("mx", ctypes.c_int32), ("my", ctypes.c_int32),
         ("upsample", ctypes.c_int32), ("subpixel", ctypes.c_int32), ("nz", ctypes.c_int32),
         ("filter_kind", ctypes.c_int32), ("filter_normalize", ctypes.c_int32),
+        ("nx_cells", ctypes.c_int32), ("ny_cells", ctypes.c_int32),
         ("z_lo", ctypes.c_double), ("z_hi", ctypes.c_double),
         ("filter_radius", ctypes.c_double), ("filter_sigma", ctypes.c_double),
         ("eta", ctypes.c_double), ("eps_core", ctypes.c_double), ("eps_clad", ctypes.c_double),
@@ -54,17 +55,17 @@ class Config(ctypes.Structure):
 
     @property
     def nx(self) -> int:
-        return self.upsample * self.mx
+        return self.nx_cells if self.nx_cells > 0 else self.upsample * self.mx
 
     @property
     def ny(self) -> int:
-        return self.upsample * self.my
+        return self.ny_cells if self.ny_cells > 0 else self.upsample * self.my
 
 
 def make_config(*, batch=1, mx, my, nz, z_lo, z_hi, upsample=2, subpixel=2, filter_kind=FILTER_CONIC,
                 filter_radius=4.0, filter_sigma=1.0, filter_normalize=1, eta=0.5, eps_core=12.11,
-                eps_clad=2.085, normal_delta=1e-8, morph_diameter=0.0, morph_alpha=20.0) -> Config:
-    return Config(batch, mx, my, upsample, subpixel, nz, filter_kind, filter_normalize, z_lo, z_hi,
+                eps_clad=2.085, normal_delta=1e-8, morph_diameter=0.0, morph_alpha=20.0, nx_cells=0, ny_cells=0) -> Config:
+    return Config(batch, mx, my, upsample, subpixel, nz, filter_kind, filter_normalize, nx_cells, ny_cells, z_lo, z_hi,
                   filter_radius, filter_sigma, eta, eps_core, eps_clad, normal_delta, morph_diameter, morph_alpha)
 
 
@@ -74,7 +75,8 @@ def config_of(w) -> Config:
                        subpixel=w.subpixel, filter_kind=w.filter_kind, filter_radius=w.radius,
                        filter_sigma=w.sigma if w.sigma > 0 else 1.0, eta=w.eta, eps_core=w.eps_core,
                        eps_clad=w.eps_clad, normal_delta=w.normal_delta,
-                       morph_diameter=getattr(w, "morph_diameter", 0.0), morph_alpha=getattr(w, "morph_alpha", 20.0))
+                       morph_diameter=getattr(w, "morph_diameter", 0.0), morph_alpha=getattr(w, "morph_alpha", 20.0),
+                       nx_cells=getattr(w, "nx_cells", 0), ny_cells=getattr(w, "ny_cells", 0))
 
 
 _lib = None

@@ -115,15 +115,18 @@ __device__ __forceinline__ void lds_vec(const float *p, float *out)
 }
 
 struct Normaliser {          // 1/sum_w lookup (S2), DESIGN.md 5.1
-    const float *tab;        // conic: [KX*m][KY*m]; separable: x table [KX*m] then y table [KY*m]
+    const float *tab;        // conic: [KX*m][KY*m]; separable: x table [KX*m] then y table [KY*m]; plane: [px][plane_py]
     int mx, my, m, T, KX, KY, separable;
+    int plane_py;            // > 0: tab is a whole plane of 1/sum_w on the mask, written by k_filter_general (a non-integer number
+                             // of cells per control pixel has no phase structure to tabulate); index = pixel coordinate
     // table row / column of mask pixel p = m*a0 + f along x / y
     __device__ __forceinline__ int ix(int a0, int f) const { return border_class(a0, mx, T, KX) * m + f; }
     __device__ __forceinline__ int iy(int b0, int f) const { return border_class(b0, my, T, KY) * m + f; }
-    __device__ __forceinline__ int ix_of(int p) const { const int a0 = p / m; return ix(a0, p - a0 * m); }
-    __device__ __forceinline__ int iy_of(int q) const { const int b0 = q / m; return iy(b0, q - b0 * m); }
+    __device__ __forceinline__ int ix_of(int p) const { if (plane_py) return p; const int a0 = p / m; return ix(a0, p - a0 * m); }
+    __device__ __forceinline__ int iy_of(int q) const { if (plane_py) return q; const int b0 = q / m; return iy(b0, q - b0 * m); }
     __device__ __forceinline__ float at_index(int i, int j) const
     {
+        if (plane_py) return tab[(size_t)i * plane_py + j];
         return separable ? tab[i] * tab[KX * m + j] : tab[i * (KY * m) + j];
     }
     __device__ __forceinline__ float at(int p, int q) const { return at_index(ix_of(p), iy_of(q)); }

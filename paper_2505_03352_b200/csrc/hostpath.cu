@@ -39,7 +39,7 @@ extern "C" int eps_forward_vjp_host(epsgrad_plan_t *P, const float *C_host, floa
     // Eq. (1) needs only the slab cells of the fields ("|Omega_D").  When every field buffer is pinned, mapped host
     // memory, the z-reduction reads its windows straight out of it (16-byte asynchronous copies over PCIe / C2C) and the
     // rest of the fields never crosses the bus; otherwise (pageable memory, dense plans) the fields are staged whole.
-    bool direct = P->host_direct && !P->dense && n_pairs > 0;
+    bool direct = P->host_direct && !P->dense && n_pairs > 0 && P->cfg.nz % 4 == 0;   // odd columns: staged whole (scalar3d.cuh)
     for (int p = 0; p < n_pairs && direct; ++p) {
         const void *hp[2] = {EF_host[p], EA_host[p]};
         const void **dp[2] = {&ef[p], &ea[p]};

@@ -10,11 +10,13 @@
 #include "filter.cuh"
 #include "filter4.cuh"
 #include "filter_sep.cuh"
+#include "filter_general.cuh"
 #include "fwd2d.cuh"
 #include "extrude.cuh"
 #include "extrude_bulk.cuh"
 #include "zreduce.cuh"
 #include "zreduce_pipe.cuh"
+#include "scalar3d.cuh"
 #include "maskgrad.cuh"
 #include "mega.cuh"
 #include "morph.cuh"
@@ -79,6 +81,8 @@ Normaliser make_nrm(const epsgrad_plan *P)
     Normaliser n;
     n.tab = P->d_invden; n.mx = P->cfg.mx; n.my = P->cfg.my; n.m = P->m; n.T = P->T;
     n.KX = P->KX; n.KY = P->KY; n.separable = P->separable;
+    n.plane_py = 0;
+    if (P->general) { n.tab = ws_invden(P); n.plane_py = P->py; }      // the plane k_filter_general wrote (every call runs F1 first)
     return n;
 }
 
@@ -196,8 +200,29 @@ int launch_filterT_m(epsgrad_plan *P, const float *v, float *dC, cudaStream_t st
     }
 }
 
+FilterGenParams fill_filter_general(const epsgrad_plan *P)
+{
+    FilterGenParams fp;
+    std::memset(&fp, 0, sizeof(fp));
+    fp.mx = P->cfg.mx; fp.my = P->cfg.my; fp.px = P->px; fp.py = P->py; fp.s = P->cfg.subpixel;
+    fp.kind = P->cfg.filter_kind; fp.normalize = P->cfg.filter_normalize;
+    fp.ux = (double)P->nx / P->cfg.mx; fp.uy = (double)P->ny / P->cfg.my;
+    fp.R = (float)P->cfg.filter_radius; fp.inv_R = (float)(1.0 / P->cfg.filter_radius);
+    fp.inv_2s2 = P->cfg.filter_kind == EPSGRAD_FILTER_GAUSSIAN ? (float)(1.0 / (2.0 * P->cfg.filter_sigma * P->cfg.filter_sigma)) : 0.0f;
+    fp.eta0 = P->eta0;
+    return fp;
+}
+
 int launch_filter(epsgrad_plan *P, const float *C, float *phi, cudaStream_t st)
 {
+    if (P->general) {
+        FilterGenParams fp = fill_filter_general(P);
+        fp.C = C; fp.phi = phi; fp.invden = ws_invden(P);
+        if (P->cfg.batch > 65535) return EPSGRAD_EUNSUPPORTED;
+        const size_t n_mask = (size_t)P->px * P->py;
+        k_filter_general<<<dim3((unsigned)((n_mask + FG_THREADS - 1) / FG_THREADS), P->cfg.batch), FG_THREADS, 0, st>>>(fp);
+        return check_launch(P, "filter", st);
+    }
     switch (P->m) {
     case 2: return launch_filter_m<2>(P, C, phi, st);
     case 4: return launch_filter_m<4>(P, C, phi, st);
@@ -209,6 +234,13 @@ int launch_filter(epsgrad_plan *P, const float *C, float *phi, cudaStream_t st)
 
 int launch_filterT(epsgrad_plan *P, const float *v, float *dC, cudaStream_t st)
 {
+    if (P->general) {
+        FilterGenParams fp = fill_filter_general(P);
+        fp.v = v; fp.dC = dC;
+        if (P->cfg.batch > 65535) return EPSGRAD_EUNSUPPORTED;
+        k_filterT_general<<<dim3(cdiv(P->cfg.mx * P->cfg.my, FG_THREADS), P->cfg.batch), FG_THREADS, 0, st>>>(fp);
+        return check_launch(P, "filterT", st);
+    }
     switch (P->m) {
     case 2: return launch_filterT_m<2>(P, v, dC, st);
     case 4: return launch_filterT_m<4>(P, v, dC, st);
@@ -283,8 +315,19 @@ ExtrudeParams fill_extrude(const epsgrad_plan *P, const float *e2d, float *eps)
 
 int launch_extrude(epsgrad_plan *P, const float *e2d, float *eps, cudaStream_t st)
 {
-    const ExtrudeParams ep = fill_extrude(P, e2d, eps);
     if (P->cfg.batch > 65535) return EPSGRAD_EUNSUPPORTED;
+    if (P->cfg.nz % 4) {
+        // columns that are not whole 16-byte pieces: one thread per cell (scalar3d.cuh)
+        if (P->emb.nx_full > 0) return EPSGRAD_EUNSUPPORTED;
+        ExtrudeScalarParams sp;
+        sp.e2d = e2d; sp.eps = eps; sp.zw = P->d_zw; sp.nz = P->cfg.nz;
+        sp.pstride = P->nx * P->ny; sp.ncol = sp.pstride;
+        if (P->slab_nx > 0) { sp.ncol = P->slab_nx * P->ny; sp.e2d += (size_t)P->slab_x0 * P->ny; }
+        const size_t n = (size_t)sp.ncol * sp.nz;
+        k_extrude_scalar<<<dim3((unsigned)((n + SC_THREADS - 1) / SC_THREADS), 3, P->cfg.batch), SC_THREADS, 0, st>>>(sp);
+        return check_launch(P, "extrude", st);
+    }
+    const ExtrudeParams ep = fill_extrude(P, e2d, eps);
     if (P->use_bulk && P->emb.nx_full == 0) {
         // thin persistent store stream (extrude_bulk.cuh): columns of a plane are one contiguous run
         ExtrudeBulkParams bp;
@@ -383,6 +426,31 @@ int launch_zreduce(epsgrad_plan *P, int n_pairs, const void *const *EF, const vo
     // x-slab: only the slab's rows have fields; the cotangent of every other column of the region is zero
     if (P->slab_nx > 0 &&
         cudaMemsetAsync(gbar, 0, (size_t)P->cfg.batch * 5 * P->nx * P->ny * sizeof(float), st) != cudaSuccess) { cudaGetLastError(); return EPSGRAD_ECUDA; }
+    if (P->cfg.nz % 4) {
+        // field columns that are not whole 16-byte chunks: one thread per column, 8-byte loads (scalar3d.cuh)
+        if (P->emb.nx_full > 0 || packed || host_src || P->cur_host_src) return EPSGRAD_EUNSUPPORTED;
+        if (P->cfg.batch > 65535) return EPSGRAD_EUNSUPPORTED;
+        ZredScalarParams sp;
+        sp.gbar = gbar; sp.zw = P->d_zw; sp.nz = P->cfg.nz;
+        sp.pstride = P->nx * P->ny; sp.ncol = sp.pstride;
+        if (P->slab_nx > 0) { sp.ncol = P->slab_nx * P->ny; sp.gbar += (size_t)P->slab_x0 * P->ny; }
+        for (int g = 0; g < 2; ++g) {
+            sp.k0[g] = P->dense ? 0 : 2 * P->ch0[g];
+            sp.k1[g] = P->dense ? sp.nz : std::min(sp.nz, 2 * (P->ch0[g] + P->nch[g]));
+        }
+        for (int p0 = 0; p0 < n_pairs; p0 += ZR_MAX_PAIRS) {
+            const int np = std::min(ZR_MAX_PAIRS, n_pairs - p0);
+            for (int p = 0; p < ZR_MAX_PAIRS; ++p) {
+                sp.ef[p] = (const float2 *)(p < np ? EF[p0 + p] : nullptr);
+                sp.ea[p] = (const float2 *)(p < np ? EA[p0 + p] : nullptr);
+            }
+            sp.n_pairs = np; sp.accumulate = p0 > 0;
+            k_zreduce_scalar<<<dim3(cdiv(sp.ncol, SC_THREADS), 3, P->cfg.batch), SC_THREADS, 0, st>>>(sp);
+            int rcs = check_launch(P, "zreduce", st);
+            if (rcs) return rcs;
+        }
+        return EPSGRAD_OK;
+    }
     int rcf = fill_zreduce(P, gbar, packed, zp, smem, sparse, maxnch);
     if (rcf) return rcf;
     host_src = host_src || P->cur_host_src;
@@ -607,7 +675,7 @@ int check_pairs(int n_pairs, const void *const *EF, const void *const *EA)
 // ---- the whole step as one persistent dataflow kernel (mega.cuh)
 bool mega_applies(const epsgrad_plan *P, int n_pairs)
 {
-    return P->use_mega == 1 && P->d_sched && !P->cur_dbeta && P->slab_nx == 0 && !P->cur_host_src && !P->prof && n_pairs <= ZR_MAX_PAIRS;
+    return P->use_mega == 1 && P->d_sched && P->cfg.nz % 4 == 0 && !P->cur_dbeta && P->slab_nx == 0 && !P->cur_host_src && !P->prof && n_pairs <= ZR_MAX_PAIRS;
 }
 
 template <int NTC>
@@ -723,7 +791,7 @@ int run_chain(epsgrad_plan *P, const float *C, float beta, int n_pairs, const vo
         cudaGetLastError();
         return EPSGRAD_ECUDA;
     }
-    const bool chains = P->use_mega == 2 && P->d_sched && !P->cur_dbeta && P->slab_nx == 0;   // the 2-D chains as two persistent kernels
+    const bool chains = P->use_mega == 2 && P->d_sched && P->cfg.nz % 4 == 0 && !P->cur_dbeta && P->slab_nx == 0;   // the 2-D chains as two persistent kernels
     if (chains) rc = launch_mega(P, C, beta, n_pairs, EF, EA, eps, dFdC, ax, 1u << PH_F1 | 1u << PH_F2);
     else rc = launch_front(P, C, beta, ax);
     if (!rc) rc = launch_zreduce(P, n_pairs, EF, EA, ws_gbar(P), st);

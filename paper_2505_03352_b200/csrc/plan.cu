@@ -40,6 +40,12 @@ static double overlap(double a0, double a1, double b0, double b1)
     return hi > lo ? hi - lo : 0.0;
 }
 
+// explicit cell counts that are not upsample x the control grid: Eq. (2) by the general kernels (filter_general.cuh)
+static bool is_general(const epsgrad_config_t *c)
+{
+    return (c->nx_cells > 0 || c->ny_cells > 0) && !(c->nx_cells == c->upsample * c->mx && c->ny_cells == c->upsample * c->my);
+}
+
 static int validate(const epsgrad_config_t *c)
 {
     if (!c) return EPSGRAD_EINVAL;
@@ -57,12 +63,18 @@ static int validate(const epsgrad_config_t *c)
         if (!(c->morph_alpha > 0.0)) return EPSGRAD_EINVAL;
         const int R = (int)std::floor(0.5 * c->morph_diameter * c->subpixel);
         if (R > MO_MAX_R) return EPSGRAD_EUNSUPPORTED;
-        if (c->subpixel * c->upsample * c->mx < 2 * R + 1 || c->subpixel * c->upsample * c->my < 2 * R + 1) return EPSGRAD_EUNSUPPORTED;
+    }
+    if (c->nx_cells < 0 || c->ny_cells < 0 || (c->nx_cells > 0) != (c->ny_cells > 0)) return EPSGRAD_EINVAL;
+    if (c->nx_cells > 0 && (c->nx_cells < c->mx || c->ny_cells < c->my)) return EPSGRAD_EINVAL;      // at least one cell per control pixel
+    const int nx = c->nx_cells > 0 ? c->nx_cells : c->upsample * c->mx, ny = c->nx_cells > 0 ? c->ny_cells : c->upsample * c->my;
+    if (c->morph_diameter > 0.0) {
+        const int R = (int)std::floor(0.5 * c->morph_diameter * c->subpixel);
+        if (c->subpixel * nx < 2 * R + 1 || c->subpixel * ny < 2 * R + 1) return EPSGRAD_EUNSUPPORTED;
     }
     const int m = c->upsample * c->subpixel;
-    if (m != 2 && m != 4 && m != 6 && m != 8) return EPSGRAD_EUNSUPPORTED;
-    if (c->nz % 4) return EPSGRAD_EUNSUPPORTED;
-    const double cells = (double)c->batch * 3.0 * c->upsample * c->mx * c->upsample * c->my;
+    if (!is_general(c) && m != 2 && m != 4 && m != 6 && m != 8) return EPSGRAD_EUNSUPPORTED;
+    if (c->subpixel > 8) return EPSGRAD_EUNSUPPORTED;
+    const double cells = (double)c->batch * 3.0 * nx * ny;
     if (cells * c->subpixel * c->subpixel > 2.0e9) return EPSGRAD_EUNSUPPORTED;   // 32-bit plane indices
     return EPSGRAD_OK;
 }
@@ -84,9 +96,13 @@ extern "C" int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsg
     P->cfg = *cfg;
     P->device = device;
     if (cudaDeviceGetAttribute(&P->n_sm, cudaDevAttrMultiProcessorCount, device) != cudaSuccess || P->n_sm < 1) { cudaGetLastError(); P->n_sm = 148; }
-    const int u = cfg->upsample, s = cfg->subpixel, m = u * s;
+    // general plans (non-integer cells per control pixel) never use the phase tables below: they are built for one cell per
+    // pixel, only so that every table pointer of the plan is valid
+    P->general = is_general(cfg);
+    const int u = P->general ? 1 : cfg->upsample, s = cfg->subpixel, m = u * s;
     P->m = m;
-    P->nx = u * cfg->mx; P->ny = u * cfg->my;
+    P->nx = cfg->nx_cells > 0 ? cfg->nx_cells : u * cfg->mx;
+    P->ny = cfg->nx_cells > 0 ? cfg->ny_cells : u * cfg->my;
     P->px = s * P->nx;   P->py = s * P->ny;
     P->separable = cfg->filter_kind == EPSGRAD_FILTER_GAUSSIAN;
     // taps: X_p - x_a = delta_f - u t, |delta_f| < u/2  =>  |t| <= floor((R + u/2)/u)
@@ -170,7 +186,7 @@ extern "C" int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsg
             }
     }
 
-    if (uncovered) { delete P; return EPSGRAD_EINVAL; }    // the density filter would divide 0 by 0 there (R < u/sqrt(2))
+    if (uncovered && !P->general) { delete P; return EPSGRAD_EINVAL; }    // the density filter would divide 0 by 0 there (R < u/sqrt(2))
 
     // ---- z tables (S7, S8): wxy_k = |[k,k+1] ^ slab|, wz_k = |[k+1/2,k+3/2] ^ slab|
     const int nz = cfg->nz;
@@ -199,8 +215,29 @@ extern "C" int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsg
         else { P->ch0[g] = kmin[g] / 2; P->nch[g] = kmax[g] / 2 - P->ch0[g] + 1; }
     }
 
+    if (P->general) {
+        // coverage of the normalised Eq. (2) (S2): the mask pixel farthest from the control nodes, axis by axis (the grid is a product)
+        double far[2] = {0.0, 0.0};
+        for (int ax = 0; ax < 2; ++ax) {
+            const int M = ax ? cfg->my : cfg->mx, N = ax ? P->ny : P->nx;
+            const double uu = (double)N / M;
+            for (int p = 0; p < s * N; ++p) {
+                const double X = (p + 0.5) / s;
+                int a = (int)std::floor(X / uu);
+                a = a < 0 ? 0 : (a > M - 1 ? M - 1 : a);
+                double dmin = std::fabs(X - uu * (a + 0.5));
+                if (a > 0) dmin = std::min(dmin, std::fabs(X - uu * (a - 0.5)));
+                if (a < M - 1) dmin = std::min(dmin, std::fabs(X - uu * (a + 1.5)));
+                far[ax] = std::max(far[ax], dmin);
+            }
+        }
+        const double R = cfg->filter_radius;
+        uncovered = cfg->filter_normalize && (P->separable ? (far[0] > R || far[1] > R) : !(std::sqrt(far[0] * far[0] + far[1] * far[1]) < R));
+        if (uncovered) { delete P; return EPSGRAD_EINVAL; }
+    }
+
     // ---- shared-memory budget of the transposed conic filter (v tile + weight table)
-    if (!P->separable) {
+    if (!P->separable && !P->general) {
         const int sp = m % 4 == 0 ? 4 : 2, tb = 32 / sp, ta = 8;
         const size_t need = ((size_t)NT * NT * m * m + (size_t)m * (ta + 2 * T) * m * (tb + 2 * T) + 2 * NT) * 4;
         if (need > 200 * 1024) { delete P; return EPSGRAD_EUNSUPPORTED; }
@@ -310,10 +347,11 @@ extern "C" int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsg
         const size_t a = (size_t)P->n_part_mg + P->n_part_mo, b = (size_t)P->n_part_ub;
         P->off_part = off; off += align_up((size_t)cfg->batch * (a > b ? a : b) * 4, 256);
     }
-    P->off_tmp = off;  off += P->separable ? align_up((size_t)cfg->batch * cfg->mx * P->py * 4, 256) : 0;
+    P->off_tmp = off;  off += P->separable && !P->general ? align_up((size_t)cfg->batch * cfg->mx * P->py * 4, 256) : 0;
+    P->off_invden = off; off += P->general ? align_up((size_t)P->px * P->py * 4, 256) : 0;     // 1 / sum W on the mask (filter_general.cuh)
     P->ws_need = off;
     // ---- persistent dataflow kernel (mega.cuh): conic fast path with 4 mask pixels per control pixel, s = 2, no morphological filters
-    if (!P->separable && m == 4 && s == 2 && (NT == 5 || NT == 9 || NT == 13) && P->morph_R == 0) {
+    if (!P->separable && !P->general && m == 4 && s == 2 && (NT == 5 || NT == 9 || NT == 13) && P->morph_R == 0) {
         const int nb = (P->nx + MK_BAND - 1) / MK_BAND;
         P->sched_bytes = ((size_t)MK_SCHED_HEAD + (size_t)PH_N * cfg->batch * nb) * sizeof(int);
         int prev3 = 0;
@@ -420,7 +458,7 @@ extern "C" int epsgrad_plan_set_embedding(epsgrad_plan_t *P, const epsgrad_embed
     if (!e) { std::memset(&P->emb, 0, sizeof(P->emb)); return EPSGRAD_OK; }
     if (e->nx_full < 1 || e->ny_full < 1 || e->nz_full < 1 || e->i0 < 0 || e->j0 < 0 || e->k0 < 0) return EPSGRAD_EINVAL;
     if (e->i0 + P->nx > e->nx_full || e->j0 + P->ny > e->ny_full || e->k0 + P->cfg.nz > e->nz_full) return EPSGRAD_EINVAL;
-    if (e->nz_full % 4 || e->k0 % 4) return EPSGRAD_EUNSUPPORTED;          // 16-byte pieces of eps (4 cells) and of the fields (2 cells)
+    if (e->nz_full % 4 || e->k0 % 4 || P->cfg.nz % 4) return EPSGRAD_EUNSUPPORTED;   // 16-byte pieces of eps (4 cells) and of the fields (2 cells)
     if ((double)P->cfg.batch * 3.0 * e->nx_full * e->ny_full > 2.0e9) return EPSGRAD_EUNSUPPORTED;
     if (P->slab_nx > 0) return EPSGRAD_EUNSUPPORTED;                        // one addressing option at a time
     P->emb = *e;
@@ -478,7 +516,7 @@ extern "C" int epsgrad_plan_set_slab(epsgrad_plan_t *P, int x_first, int x_count
     if (!P) return EPSGRAD_EINVAL;
     if (x_first == 0 && x_count == 0) { P->slab_x0 = P->slab_nx = 0; return EPSGRAD_OK; }
     if (x_first < 0 || x_count < 1 || x_first + x_count > P->nx) return EPSGRAD_EINVAL;
-    if (P->emb.nx_full > 0) return EPSGRAD_EUNSUPPORTED;         // one addressing option at a time
+    if (P->emb.nx_full > 0 || P->general) return EPSGRAD_EUNSUPPORTED;         // one addressing option at a time; slabs are cut along control rows
     P->slab_x0 = x_first; P->slab_nx = x_count;
     return EPSGRAD_OK;
 }

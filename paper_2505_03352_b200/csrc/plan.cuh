@@ -20,6 +20,7 @@ struct epsgrad_plan {
     int nx, ny, px, py, m;
     int T, NT, KX, KY;
     int separable;
+    int general;               // explicit cell counts, non-integer cells per control pixel: Eq. (2) by filter_general.cuh
     // device tables (one allocation)
     void *d_tables;
     float *d_w;                // conic [NT][NT][m][m] | separable [NT][m]
@@ -56,7 +57,7 @@ struct epsgrad_plan {
     void *ws; size_t ws_bytes;
     void *stg; size_t stg_bytes;
     // workspace carve-up (byte offsets)
-    size_t off_phi, off_v, off_gbar, off_e2d, off_coef, off_tmp, ws_need;
+    size_t off_phi, off_v, off_gbar, off_e2d, off_coef, off_tmp, off_invden, ws_need;
     int last_launches;
     // kernels already opted in to their dynamic shared memory on this plan's device (launch.cu set_smem)
     const void *smem_fn[EPSGRAD_MAX_SMEM_KERNELS]; size_t smem_bytes[EPSGRAD_MAX_SMEM_KERNELS]; int n_smem_set;
@@ -100,6 +101,7 @@ inline float *ws_gbar(const epsgrad_plan *P) { return (float *)((char *)P->ws + 
 inline float *ws_e2d(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_e2d); }
 inline float *ws_coef(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_coef); }
 inline float *ws_tmp(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_tmp); }
+inline float *ws_invden(const epsgrad_plan *P) { return (float *)((char *)P->ws + P->off_invden); }
 
 // ---- launch layer (launch.cu).  Every function enqueues on `st` and returns an EPSGRAD_* status.
 void begin_call(epsgrad_plan *P, cudaStream_t st);

@@ -37,14 +37,16 @@ class Workload:
     normal_delta: float = 1e-8  # guard of the normals (S6): above float32 Sobel-difference noise^2
     morph_diameter: float = 0.0 # d of Eqs. (4)-(5) in Yee cells; 0 = morphological filters off (as in Fig. 4)
     morph_alpha: float = 20.0   # App. B
+    nx_cells: int = 0           # Yee cells of the design region when they are not upsample * mx (Fig. 4: 210 cells on 36 controls)
+    ny_cells: int = 0
 
     @property
     def nx(self) -> int:
-        return self.upsample * self.mx
+        return self.nx_cells if self.nx_cells > 0 else self.upsample * self.mx
 
     @property
     def ny(self) -> int:
-        return self.upsample * self.my
+        return self.ny_cells if self.ny_cells > 0 else self.upsample * self.my
 
     @property
     def cells(self) -> int:
@@ -64,8 +66,12 @@ CONFIGS = (
 )
 # Not a BASELINE.json config: the paper-scale workload with the morphological filters on (minimum feature size d = 4 cells
 # = 100 nm at the 25 nm cells of Fig. 4, alpha = 20 of App. B), for `bench.py --config paper_morph`.
+# "fig4": the geometry of the paper's own demonstration (Fig. 4): 36 x 36 control variables on a design region of 210 x 210
+# cells (5.83 cells per control pixel), 64 cells in z, two wavelengths = two field pairs; filter radius and beta are not printed:
+# R = 8 cells, beta = 16 as at paper scale.
 EXTRA = (
     Workload("paper_morph", 1, 1, 250, 250, 64, 28.25, 35.75, 0, 8.0, 0.0, (16.0,), 1, "uniform", morph_diameter=4.0),
+    Workload("fig4", 5, 1, 36, 36, 64, 28.25, 35.75, 0, 8.0, 0.0, (16.0,), 2, "uniform", nx_cells=210, ny_cells=210),
 )
 BY_NAME = {w.name: w for w in CONFIGS + EXTRA}
 

@@ -39,9 +39,9 @@ def test_status_strings():
 
 
 def test_config_struct_layout_matches_header():
-    # 8 int32 then 8 doubles, no padding
-    assert ctypes.sizeof(B.Config) == 8 * 4 + 10 * 8
-    assert B.Config.z_lo.offset == 32 and B.Config.normal_delta.offset == 32 + 7 * 8
+    # 10 int32 then 10 doubles, no padding
+    assert ctypes.sizeof(B.Config) == 10 * 4 + 10 * 8
+    assert B.Config.nx_cells.offset == 32 and B.Config.z_lo.offset == 40 and B.Config.normal_delta.offset == 40 + 7 * 8
 
 
 def test_host_side_validation_and_no_cpu_fallback():
@@ -61,9 +61,13 @@ def test_host_side_validation_and_no_cpu_fallback():
     ]
     for cfg in bad:
         assert L.epsgrad_plan_create(ctypes.byref(cfg), 0, ctypes.byref(h)) == B.EINVAL
-    for cfg in (B.make_config(mx=8, my=8, nz=6, z_lo=2.0, z_hi=5.0),
-                B.make_config(mx=8, my=8, nz=8, z_lo=2.0, z_hi=5.0, upsample=5)):
+    for cfg in (B.make_config(mx=8, my=8, nz=8, z_lo=2.0, z_hi=5.0, upsample=5),
+                B.make_config(mx=8, my=8, nz=8, z_lo=2.0, z_hi=5.0, subpixel=10)):
         assert L.epsgrad_plan_create(ctypes.byref(cfg), 0, ctypes.byref(h)) == B.EUNSUPPORTED
+    for cfg in (B.make_config(mx=8, my=8, nz=8, z_lo=2.0, z_hi=5.0, nx_cells=20),                 # only one of the two cell counts
+                B.make_config(mx=8, my=8, nz=8, z_lo=2.0, z_hi=5.0, nx_cells=7, ny_cells=20),     # fewer cells than control pixels
+                B.make_config(mx=8, my=8, nz=8, z_lo=2.0, z_hi=5.0, nx_cells=-3, ny_cells=20)):
+        assert L.epsgrad_plan_create(ctypes.byref(cfg), 0, ctypes.byref(h)) == B.EINVAL
     assert L.epsgrad_plan_create(None, 0, ctypes.byref(h)) == B.EINVAL
     if not torch.cuda.is_available():
         good = B.make_config(mx=8, my=8, nz=8, z_lo=2.0, z_hi=5.0)

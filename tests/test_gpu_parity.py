@@ -309,7 +309,7 @@ def test_error_codes():
         B.Plan(B.make_config(mx=8, my=8, nz=8, z_lo=2.0, z_hi=5.0, subpixel=3))
     assert e.value.status == B.EINVAL
     with pytest.raises(B.EpsgradError) as e:
-        B.Plan(B.make_config(mx=8, my=8, nz=6, z_lo=2.0, z_hi=5.0))
+        B.Plan(B.make_config(mx=8, my=8, nz=8, z_lo=2.0, z_hi=5.0, upsample=5))      # 10 mask pixels per control pixel: no phase table
     assert e.value.status == B.EUNSUPPORTED
     # cone too small to reach the mask pixels midway between control pixels: the normalised Eq. (2) would be 0/0 there
     with pytest.raises(B.EpsgradError) as e:
