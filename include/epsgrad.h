@@ -163,8 +163,9 @@ int eps_forward(epsgrad_plan_t *plan, const float *C, float beta, float *eps, vo
 /* Eq. (1): dFdC = -2 Re((d eps/dC)^T (E_F (.) E_A)) summed over n_pairs >= 1
  * pairs.  EF, EA: HOST arrays of n_pairs DEVICE pointers to complex64 [B,3,Nx,Ny,Nz].
  * A real cotangent w can be fed as E_F = -w/2 + 0i, E_A = 1 + 0i.
- * Limit: the z window of the field reads (the slab's cells; the whole column for dense
- * plans) must not exceed 512 cells, else EPSGRAD_EUNSUPPORTED.                         */
+ * A z window of the field reads (the slab's cells; the whole column for dense plans) wider
+ * than 512 cells takes the scalar kernel (region-sized or x-slab device arrays; embedded
+ * or host-resident fields: EPSGRAD_EUNSUPPORTED).                                      */
 int eps_vjp(epsgrad_plan_t *plan, const float *C, float beta, int n_pairs,
             const void *const *EF, const void *const *EA, float *dFdC, void *stream);
 
@@ -263,6 +264,12 @@ int epsgrad_plan_set_slab(epsgrad_plan_t *plan, int x_first, int x_count);
  * host-resident fields fall back to 0).  Same bytes, bitwise the same results; a measurement switch.
  * EPSGRAD_EUNSUPPORTED when TMA descriptors cannot be built on this driver.                                               */
 int epsgrad_plan_set_tma(epsgrad_plan_t *plan, int mode);
+
+/* Programmatic dependent launch (default on).  Consecutive kernels of a stream -- filter -> 2-D stage (-> eps stores in
+ * eps_forward), mask cotangent -> transposed filter -- are launched with the programmatic-stream-serialization attribute: the
+ * next kernel's CTAs are scheduled, and stage their tables, while the previous kernel drains, and wait (griddepcontrol.wait)
+ * before they read what it wrote.  Bitwise the same results; 0 = plain stream order.  CUDA-graph capturable either way.   */
+int epsgrad_plan_set_pdl(epsgrad_plan_t *plan, int enable);
 
 /* How eps is written.  0: per-thread 16-byte streaming stores (k_extrude).  1: thin persistent store stream -- the columns
  * are assembled in shared memory (only the slab pieces change from column to column) and written by bulk asynchronous copies

@@ -64,6 +64,14 @@ __device__ __forceinline__ float ld_plane(const float *p) { return CG ? __ldcg(p
 template <bool CG>
 __device__ __forceinline__ float2 ld_plane2(const float2 *p) { return CG ? __ldcg(p) : *p; }
 
+// Programmatic dependent launch (sm_90+): a kernel launched with the programmatic-stream-serialization attribute may start
+// while the kernel before it on the stream is still running; pdl_wait() blocks until that kernel has completed and its writes
+// are visible (a no-op for a normal launch), pdl_launch() lets the NEXT kernel's CTAs be scheduled early (a no-op without a
+// dependent).  The kernels of the path call pdl_launch() first and pdl_wait() before they touch anything another kernel
+// wrote: launch latency, CTA ramp-up and table staging of a kernel then overlap the tail of its predecessor.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // 1/x on the special-function unit (MUFU.RCP, <= 1 ulp; 1/inf = 0).  The 2-D chain needs ~1e-7
 // relative accuracy (tolerances 1e-5 / 1e-4), not IEEE rounding.
 __device__ __forceinline__ float fast_rcp(float x)

@@ -153,6 +153,8 @@ __device__ __forceinline__ void block_extrude(const ExtrudeParams &P, int c, int
 __global__ void __launch_bounds__(EX_THREADS, EX_CTAS_PER_SM) k_extrude(const __grid_constant__ ExtrudeParams P)
 {
     extern __shared__ float vsm[];                            // plane values of the block: [3][cpb]
+    pdl_launch();
+    pdl_wait();
     const int col0 = blockIdx.x * P.cpb;
     block_extrude<false>(P, blockIdx.y, col0, min(P.cpb, P.ncol - col0), blockIdx.z, vsm);
 }

@@ -131,6 +131,8 @@ __global__ void __launch_bounds__(F4F_THREADS) k_filter_conic4(const FilterParam
 {
     extern __shared__ __align__(16) float sm[];
     f4_stage_weights<NTC>(sm, P.w, F4F_THREADS);
+    pdl_launch();
+    pdl_wait();                                    // Phi' may still be read by the kernel before (the previous call's reverse pass)
     tile_filter_conic4<NTC, F4_G>(P, blockIdx.x, blockIdx.y, blockIdx.z, sm, sm + NTC * NTC * 16);
 }
 
@@ -243,7 +245,9 @@ template <int NTC>
 __global__ void __launch_bounds__(F4T_THREADS) k_filterT_conic4(const FilterTParams P)
 {
     extern __shared__ __align__(16) float sm[];
-    f4_stage_weights<NTC>(sm, P.w, F4T_THREADS);
+    f4_stage_weights<NTC>(sm, P.w, F4T_THREADS);      // the table is the plan's: staged while the mask cotangent is still being written
+    pdl_launch();
+    pdl_wait();
     tile_filterT_conic4<NTC, F4T_G, 1>(P, blockIdx.x, blockIdx.y, blockIdx.z, sm, sm + NTC * NTC * 16);
 }
 

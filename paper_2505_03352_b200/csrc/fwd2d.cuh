@@ -188,6 +188,8 @@ template <int S>
 __global__ void __launch_bounds__(F2_THREADS, 8) k_fwd2d(const __grid_constant__ Fwd2dParams P)
 {
     extern __shared__ __align__(16) float sm[];
+    pdl_launch();
+    pdl_wait();
     tile_fwd2d<S, false>(P, blockIdx.x, blockIdx.y, blockIdx.z, sm);
 }
 

@@ -5,6 +5,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstring>
+#include <utility>
 
 #include "common.cuh"
 #include "filter.cuh"
@@ -43,6 +44,25 @@ int set_smem(epsgrad_plan *P, K kernel, size_t bytes)
     return EPSGRAD_OK;
 }
 
+// Launch with the programmatic-dependent-launch attribute when the operation before it on `st` was a kernel of this call that
+// releases its dependents early (common.cuh pdl_launch / pdl_wait): the plan remembers that stream in pdl_stream.
+template <typename... KArgs, typename... Args>
+cudaError_t launch_k(epsgrad_plan *P, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args &&...args)
+{
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = P->use_pdl && P->pdl_valid && P->pdl_stream == st ? 1 : 0;
+    const cudaError_t e = cudaLaunchKernelEx(&cfg, kern, std::forward<Args>(args)...);
+    P->pdl_stream = st; P->pdl_valid = 1; P->pdl_mark = 1;
+    return e;
+}
+// any other operation on a stream (event record / wait, copy, a kernel without pdl_launch) ends the chain
+inline void pdl_break(epsgrad_plan *P) { P->pdl_valid = 0; }
+
 __global__ void k_stamp(unsigned long long *slot)
 {
     unsigned long long t;
@@ -62,11 +82,15 @@ void begin_call(epsgrad_plan *P, cudaStream_t st)
 {
     P->last_launches = 0;
     P->n_tl = 0;
+    P->pdl_valid = P->pdl_mark = 0;
     if (P->prof) cudaEventRecord(P->ev[0], st);
 }
 
 int check_launch(epsgrad_plan *P, const char *name, cudaStream_t st)
 {
+    // a kernel launched without launch_k, the profiling events and the timeline stamps all end a dependent-launch chain
+    if (!P->pdl_mark || P->prof || P->d_tl) P->pdl_valid = 0;
+    P->pdl_mark = 0;
     const int idx = P->last_launches++;
     if (idx < EPSGRAD_MAX_KERNELS) {
         P->kname[idx] = name;
@@ -116,7 +140,7 @@ int launch_filter_m(epsgrad_plan *P, const float *C, float *phi, cudaStream_t st
             const size_t smem4 = (filter4_smem_floats(NT) + 4) * 4;
             int rc4 = set_smem(P, kern, smem4);
             if (rc4) return rc4;
-            kern<<<dim3(cdiv(my, F4_TB), cdiv(mx, F4_TA), B), F4F_THREADS, smem4, st>>>(fp);
+            launch_k(P, kern, dim3(cdiv(my, F4_TB), cdiv(mx, F4_TA), B), dim3(F4F_THREADS), smem4, st, fp);
             return check_launch(P, "filter", st);
         }
         const size_t smem = ((size_t)NT * NT * M * M + (size_t)(TA + 2 * T) * (TB + 2 * T + 1) + 2 * NT) * 4;
@@ -160,7 +184,7 @@ int launch_filterT_conic(epsgrad_plan *P, const float *v, float *dC, cudaStream_
         const size_t smem4 = filterT4_smem_floats(NT) * 4;
         int rc4 = set_smem(P, kern, smem4);
         if (rc4) return rc4;
-        kern<<<dim3(cdiv(fp.my, F4_TB), cdiv(fp.mx, F4_TA), P->cfg.batch), F4T_THREADS, smem4, st>>>(fp);
+        launch_k(P, kern, dim3(cdiv(fp.my, F4_TB), cdiv(fp.mx, F4_TA), P->cfg.batch), dim3(F4T_THREADS), smem4, st, fp);
         return check_launch(P, "filterT", st);
     }
     const size_t smem = ((size_t)NT * NT * M * M + (size_t)M * (S::TA + 2 * T) * M * (S::TB + 2 * T) + 2 * NT) * 4;
@@ -269,7 +293,7 @@ int launch_fwd2d(epsgrad_plan *P, const float *phi, float beta, float *e2d, floa
     auto kern = fp.s == 2 ? k_fwd2d<2> : (fp.s == 4 ? k_fwd2d<4> : k_fwd2d<0>);
     int rc = set_smem(P, kern, smem);
     if (rc) return rc;
-    kern<<<dim3(cdiv(P->ny, F2_TJ), cdiv(P->nx, F2_TI), P->cfg.batch), F2_THREADS, smem, st>>>(fp);
+    launch_k(P, kern, dim3(cdiv(P->ny, F2_TJ), cdiv(P->nx, F2_TI), P->cfg.batch), dim3(F2_THREADS), smem, st, fp);
     return check_launch(P, "fwd2d", st);
 }
 
@@ -356,7 +380,7 @@ int launch_extrude(epsgrad_plan *P, const float *e2d, float *eps, cudaStream_t s
     const size_t smem = (size_t)3 * ep.cpb * 4;
     int rc = set_smem(P, k_extrude, smem);
     if (rc) return rc;
-    k_extrude<<<dim3(ep.nblk, 3, P->cfg.batch), EX_THREADS, smem, st>>>(ep);
+    launch_k(P, k_extrude, dim3(ep.nblk, 3, P->cfg.batch), dim3(EX_THREADS), smem, st, ep);
     return check_launch(P, "extrude", st);
 }
 
@@ -426,8 +450,11 @@ int launch_zreduce(epsgrad_plan *P, int n_pairs, const void *const *EF, const vo
     // x-slab: only the slab's rows have fields; the cotangent of every other column of the region is zero
     if (P->slab_nx > 0 &&
         cudaMemsetAsync(gbar, 0, (size_t)P->cfg.batch * 5 * P->nx * P->ny * sizeof(float), st) != cudaSuccess) { cudaGetLastError(); return EPSGRAD_ECUDA; }
-    if (P->cfg.nz % 4) {
-        // field columns that are not whole 16-byte chunks: one thread per column, 8-byte loads (scalar3d.cuh)
+    int widest = 0;                                               // slab window in 16-byte chunks
+    for (int g = 0; g < 2; ++g) widest = std::max(widest, P->dense ? P->cfg.nz / 2 : P->nch[g]);
+    if (P->cfg.nz % 4 || (widest > 256 && P->emb.nx_full == 0 && !packed && !host_src && !P->cur_host_src)) {
+        // field columns that are not whole 16-byte chunks, or a window wider than one CTA pass of the vector kernel (512
+        // cells): one thread per column, 8-byte loads (scalar3d.cuh)
         if (P->emb.nx_full > 0 || packed || host_src || P->cur_host_src) return EPSGRAD_EUNSUPPORTED;
         if (P->cfg.batch > 65535) return EPSGRAD_EUNSUPPORTED;
         ZredScalarParams sp;
@@ -652,7 +679,7 @@ int launch_maskgrad(epsgrad_plan *P, const float *phi, float beta, const float *
     auto kern = mp.s == 2 ? k_maskgrad<2> : (mp.s == 4 ? k_maskgrad<4> : k_maskgrad<0>);
     int rc = set_smem(P, kern, smem);
     if (rc) return rc;
-    kern<<<dim3(cdiv(P->ny, MG_TJ), cdiv(P->nx, MG_TI), P->cfg.batch), MG_THREADS, smem, st>>>(mp);
+    launch_k(P, kern, dim3(cdiv(P->ny, MG_TJ), cdiv(P->nx, MG_TI), P->cfg.batch), dim3(MG_THREADS), smem, st, mp);
     return check_launch(P, "maskgrad", st);
 }
 
@@ -787,6 +814,8 @@ int run_chain(epsgrad_plan *P, const float *C, float beta, int n_pairs, const vo
     }
     cudaStream_t ax = P->aux;
     stamp(P, "begin", st);
+    // (event records and waits sit between most kernels of the two streams: only filter -> 2-D stage and mask cotangent ->
+    // transposed filter are adjacent launches, and those two pairs chain by programmatic dependent launch)
     if (cudaEventRecord(P->ev_fork, st) != cudaSuccess || cudaStreamWaitEvent(ax, P->ev_fork, 0) != cudaSuccess) {
         cudaGetLastError();
         return EPSGRAD_ECUDA;
@@ -795,8 +824,10 @@ int run_chain(epsgrad_plan *P, const float *C, float beta, int n_pairs, const vo
     if (chains) rc = launch_mega(P, C, beta, n_pairs, EF, EA, eps, dFdC, ax, 1u << PH_F1 | 1u << PH_F2);
     else rc = launch_front(P, C, beta, ax);
     if (!rc) rc = launch_zreduce(P, n_pairs, EF, EA, ws_gbar(P), st);
+    pdl_break(P);
     if (!rc && cudaEventRecord(P->ev_r, st) != cudaSuccess) rc = EPSGRAD_ECUDA;
     if (!rc && !chains) rc = launch_fwd2d(P, ws_phi(P), beta, eps ? ws_e2d(P) : nullptr, ws_coef(P), nullptr, ax);
+    pdl_break(P);
     if (!rc && cudaEventRecord(P->ev_2d, ax) != cudaSuccess) rc = EPSGRAD_ECUDA;
     if (!rc && cudaStreamWaitEvent(ax, P->ev_r, 0) != cudaSuccess) rc = EPSGRAD_ECUDA;
     if (!rc && chains) rc = launch_mega(P, C, beta, n_pairs, EF, EA, eps, dFdC, ax, 1u << PH_M | 1u << PH_T);

@@ -242,6 +242,8 @@ template <int S>
 __global__ void __launch_bounds__(MG_THREADS, 8) k_maskgrad(const __grid_constant__ MaskGradParams P)
 {
     extern __shared__ __align__(16) float sm[];
+    pdl_launch();
+    pdl_wait();
     tile_maskgrad<S, false>(P, blockIdx.x, blockIdx.y, blockIdx.z, (blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x, sm);
 }
 

@@ -317,6 +317,7 @@ extern "C" int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsg
         cudaSetDevice(prev2);
         if (!ok) { cudaGetLastError(); epsgrad_plan_destroy(P); return EPSGRAD_ECUDA; }
         P->overlap = 1;
+        P->use_pdl = 1;
         P->host_direct = 2;
         {
             cudaDriverEntryPointQueryResult qres;
@@ -470,6 +471,13 @@ extern "C" int epsgrad_plan_set_tma(epsgrad_plan_t *P, int enable)
     if (!P) return EPSGRAD_EINVAL;
     if (enable && !P->tma_encode) return EPSGRAD_EUNSUPPORTED;
     P->use_tma = enable < 0 ? 0 : (enable > 2 ? 2 : enable);
+    return EPSGRAD_OK;
+}
+
+extern "C" int epsgrad_plan_set_pdl(epsgrad_plan_t *P, int enable)
+{
+    if (!P) return EPSGRAD_EINVAL;
+    P->use_pdl = enable != 0;
     return EPSGRAD_OK;
 }
 

@@ -42,6 +42,8 @@ struct epsgrad_plan {
     // embedding of the design region in the caller's simulation-domain arrays (epsgrad_plan_set_embedding); emb.nx_full = 0: none
     epsgrad_embedding_t emb;
     int use_tma;               // field windows by TMA bulk tensor copies where possible (epsgrad_plan_set_tma): 1 single-stage, 2 pipelined
+    int use_pdl;               // programmatic dependent launch between consecutive kernels of a stream (epsgrad_plan_set_pdl)
+    int pdl_valid, pdl_mark; cudaStream_t pdl_stream;     // the last operation of the call in flight was a kernel on pdl_stream that releases its dependents early
     int use_bulk;              // eps columns written by bulk copies from shared memory (epsgrad_plan_set_bulk_stores)
     int tune[8];               // measurement knobs (epsgrad_plan_set_tuning)
     int use_mega;              // the whole step as one persistent dataflow kernel where the configuration allows (epsgrad_plan_set_fused)

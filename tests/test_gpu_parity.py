@@ -321,12 +321,18 @@ def test_error_codes():
     with pytest.raises(B.EpsgradError) as e:
         B.Plan(B.make_config(mx=40, my=40, nz=8, z_lo=2.0, z_hi=5.0, upsample=1, subpixel=8, filter_radius=12.0))
     assert e.value.status == B.EUNSUPPORTED
-    # field window wider than 512 cells: the forward call works, the reverse pass says so
-    plan = B.Plan(B.make_config(mx=4, my=4, nz=1024, z_lo=3.5, z_hi=1000.0))
-    plan.eps_forward(torch.rand(plan.ctrl_shape, device="cuda"), 8.0)
-    f = torch.zeros(plan.eps_shape, dtype=torch.complex64, device="cuda")
+    # field window wider than 512 cells: the scalar field kernel; refused only where that one does not apply (embedded fields)
+    cfg = B.make_config(mx=4, my=4, nz=1024, z_lo=3.5, z_hi=1000.0)
+    plan = B.Plan(cfg)
+    Cw = rand_C(cfg, 1)
+    EFw, EAw = rand_fields(cfg, 1, 2)
+    gw = plan.eps_vjp(dev(Cw), 8.0, [dev(EFw[0])], [dev(EAw[0])]).cpu().numpy().astype(np.float64)[0]
+    gw_ref = O.vjp(oracle_cfg(cfg), Cw[0], 8.0, [EFw[0][0]], [EAw[0][0]])
+    assert np.max(np.abs(gw - gw_ref)) < TOL_GRAD * np.max(np.abs(gw_ref))
+    plan.set_embedding(8, 8, 1024, 0, 0, 0)
+    f = torch.zeros(plan.field_shape, dtype=torch.complex64, device="cuda")
     with pytest.raises(B.EpsgradError) as e:
-        plan.eps_vjp(torch.rand(plan.ctrl_shape, device="cuda"), 8.0, [f], [f])
+        plan.eps_vjp(dev(Cw), 8.0, [f], [f])
     assert e.value.status == B.EUNSUPPORTED
     # beyond the 32-bit plane indices: refused at plan creation, before anything is allocated
     with pytest.raises(B.EpsgradError) as e:
