@@ -19,7 +19,7 @@ EXPORTS = (
     "epsgrad_plan_create", "epsgrad_plan_destroy", "epsgrad_workspace_bytes",
     "epsgrad_plan_set_workspace", "epsgrad_staging_bytes", "epsgrad_plan_set_staging",
     "epsgrad_plan_set_dense_reads", "epsgrad_plan_last_launches", "epsgrad_plan_last_copy_bytes",
-    "epsgrad_plan_set_profiling", "epsgrad_plan_last_kernel_times", "epsgrad_plan_set_overlap", "epsgrad_plan_set_host_direct", "epsgrad_plan_set_embedding", "epsgrad_plan_set_slab", "epsgrad_plan_set_tma", "epsgrad_plan_set_bulk_stores", "epsgrad_plan_set_pdl", "epsgrad_plan_set_tuning", "epsgrad_plan_set_fused", "epsgrad_plan_fused_profile", "epsgrad_plan_set_timeline", "epsgrad_plan_read_timeline", 
+    "epsgrad_plan_set_profiling", "epsgrad_plan_last_kernel_times", "epsgrad_plan_set_overlap", "epsgrad_plan_set_host_direct", "epsgrad_plan_set_embedding", "epsgrad_plan_set_slab", "epsgrad_plan_set_tma", "epsgrad_plan_set_bulk_stores", "epsgrad_plan_set_pdl", "epsgrad_plan_set_tensor_cores", "epsgrad_plan_set_tuning", "epsgrad_plan_set_fused", "epsgrad_plan_fused_profile", "epsgrad_plan_set_timeline", "epsgrad_plan_read_timeline", 
     "eps_forward", "eps_vjp", "eps_forward_vjp", "eps_forward_vjp_host", "eps_vjp_beta", "eps_unbinarity",
     "epsgrad_beta_schedule", "epsgrad_beta_update", "epsgrad_adam_step",
     "epsgrad_soap_accumulate", "epsgrad_soap_eigh_workspace_bytes", "epsgrad_soap_eigh", "epsgrad_soap_eigh_info",
@@ -229,6 +229,7 @@ def lib() -> ctypes.CDLL:
     L.epsgrad_plan_set_tma.argtypes = [vp, i32]
     L.epsgrad_plan_set_bulk_stores.argtypes = [vp, i32]
     L.epsgrad_plan_set_pdl.argtypes = [vp, i32]
+    L.epsgrad_plan_set_tensor_cores.argtypes = [vp, i32]
     L.epsgrad_plan_set_tuning.argtypes = [vp, i32, i32]
     L.epsgrad_plan_set_fused.argtypes = [vp, i32]
     L.epsgrad_plan_fused_profile.argtypes = [vp, i32, vp]
@@ -360,6 +361,10 @@ class Plan:
     def set_tma(self, mode) -> None:
         """0: LDGSTS field reads; 1: single-stage TMA; 2: thin persistent TMA read stream"""
         _check(lib().epsgrad_plan_set_tma(self._h, int(mode)), "epsgrad_plan_set_tma")
+
+    def set_tensor_cores(self, mode) -> None:
+        """Eq. (2) on the tensor cores: 0 / False never, 1 / True wherever it applies, 2 where it measured faster (default)"""
+        _check(lib().epsgrad_plan_set_tensor_cores(self._h, int(mode)), "epsgrad_plan_set_tensor_cores")
 
     def set_pdl(self, enable: bool) -> None:
         _check(lib().epsgrad_plan_set_pdl(self._h, int(bool(enable))), "epsgrad_plan_set_pdl")

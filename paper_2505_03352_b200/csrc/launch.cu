@@ -12,6 +12,7 @@
 #include "filter4.cuh"
 #include "filter_sep.cuh"
 #include "filter_general.cuh"
+#include "filter_tc.cuh"
 #include "fwd2d.cuh"
 #include "extrude.cuh"
 #include "extrude_bulk.cuh"
@@ -135,6 +136,40 @@ int launch_filter_m(epsgrad_plan *P, const float *C, float *phi, cudaStream_t st
     if (!P->separable) {
         constexpr int TA = 8, TB = 16;
         const FilterParams fp = fill_filter(P, C, phi);
+        // tensor cores (filter_tc.cuh): always when asked for (use_tc = 1); by default (2) where they measured faster than the
+        // FFMA stencil -- enough tiles to amortise the per-CTA set-up (weights, TMEM): R = 12 from ~500 x 500 control pixels
+        // (31 against 47 us; 75 against 159 us at 1000 x 1000), R <= 8 from ~375 x 375 (16.5 against 20.4 us; a tie at 250 x 250)
+        bool tc = M == 4 && P->use_tc && P->d_atc && (NT == 5 || NT == 9 || NT == 13);
+        if (tc && P->use_tc == 2) {
+            const bool big = NT == 13;
+            const int nt = cdiv(my, FTC_TB) * cdiv(mx, big ? FTC_N_STREAM : FTC_N_RESIDENT) * B;
+            tc = big ? 2 * nt >= P->n_sm : 2 * nt >= 3 * P->n_sm;
+        }
+        if (tc) {
+            FilterTcParams tp;
+            tp.C = C; tp.phi = phi; tp.a_tab = P->d_atc; tp.nrm = fp.nrm;
+            tp.mx = mx; tp.my = my; tp.px = P->px; tp.py = P->py; tp.eta0 = P->eta0;
+            tp.dbg = P->d_mprof;          // cycle accounting, when epsgrad_plan_fused_profile is on
+            const bool stream = NT == 13 || P->tune[7] == 1;          // R = 12: the weight matrices do not fit in shared memory
+            const int Nt = stream ? FTC_N_STREAM : FTC_N_RESIDENT;
+            tp.tiles_x = cdiv(my, FTC_TB); tp.tiles_y = cdiv(mx, Nt); tp.n_tiles = tp.tiles_x * tp.tiles_y * B;
+            const size_t smem_tc = ftc_smem_bytes(NT, Nt, stream);
+            const int grid_tc = std::min(tp.n_tiles, P->n_sm);
+            int rct = EPSGRAD_OK;
+#define EPSGRAD_TC_LAUNCH(NTC_, N_, S_)                                                         \
+            do {                                                                                \
+                rct = set_smem(P, k_filter_tc<NTC_, N_, S_>, smem_tc);                          \
+                if (!rct) k_filter_tc<NTC_, N_, S_><<<grid_tc, FTC_THREADS, smem_tc, st>>>(tp);  \
+            } while (0)
+            if (NT == 13) EPSGRAD_TC_LAUNCH(13, FTC_N_STREAM, true);
+            else if (NT == 9 && stream) EPSGRAD_TC_LAUNCH(9, FTC_N_STREAM, true);
+            else if (NT == 9) EPSGRAD_TC_LAUNCH(9, FTC_N_RESIDENT, false);
+            else if (stream) EPSGRAD_TC_LAUNCH(5, FTC_N_STREAM, true);
+            else EPSGRAD_TC_LAUNCH(5, FTC_N_RESIDENT, false);
+#undef EPSGRAD_TC_LAUNCH
+            if (rct) return rct;
+            return check_launch(P, "filter", st);
+        }
         if (M == 4 && (NT == 5 || NT == 9 || NT == 13)) {      // fast path (filter4.cuh)
             auto kern = NT == 5 ? k_filter_conic4<5> : (NT == 9 ? k_filter_conic4<9> : k_filter_conic4<13>);
             const size_t smem4 = (filter4_smem_floats(NT) + 4) * 4;

@@ -270,6 +270,34 @@ extern "C" int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsg
         return EPSGRAD_ECUDA;
     }
 
+    // ---- tensor-core filter (filter_tc.cuh): per tap row tx the banded matrix A_tx[(fx, beta, fy), j] = W[tx][j - beta][fx][fy],
+    // split into two tf32 terms (hi + lo = the float32 weight up to 2^-21), in the K-major chunk layout the MMA descriptors name
+    if (!P->separable && !P->general && m == 4 && (NT == 5 || NT == 9 || NT == 13)) {
+        const int K = ftc_k(NT), KC = K / 4;
+        std::vector<float> atc(ftc_a_floats(NT), 0.0f);
+        const size_t half = atc.size() / 2;
+        for (int tx = 0; tx < NT; ++tx)
+            for (int fx = 0; fx < 4; ++fx)
+                for (int beta = 0; beta < FTC_TB; ++beta)
+                    for (int fy = 0; fy < 4; ++fy)
+                        for (int j = 0; j < K; ++j) {
+                            const int ty = j - beta, row = fx * 32 + beta * 4 + fy;
+                            if (ty < 0 || ty >= NT) continue;
+                            const float wv = w[(((size_t)tx * NT + ty) * m + fx) * m + fy];
+                            const float hi = tf32_trunc(wv), lo = tf32_trunc(wv - hi);
+                            const size_t o = (((size_t)tx * KC + (j >> 2)) * FTC_M + row) * 4 + (j & 3);
+                            atc[o] = hi; atc[half + o] = lo;
+                        }
+        int prevt = 0;
+        cudaGetDevice(&prevt);
+        cudaSetDevice(device);
+        const bool okt = cudaMalloc(&P->d_atc, atc.size() * 4) == cudaSuccess &&
+                         cudaMemcpy(P->d_atc, atc.data(), atc.size() * 4, cudaMemcpyHostToDevice) == cudaSuccess;
+        cudaSetDevice(prevt);
+        if (!okt) { cudaGetLastError(); epsgrad_plan_destroy(P); return EPSGRAD_ECUDA; }
+        P->use_tc = 2;           // where it measured faster (launch.cu)
+    }
+
     // ---- morphological disk: K_m = 1 for dp^2 + dq^2 <= (d s / 2)^2, unit sum over the in-region pixels (S18)
     if (cfg->morph_diameter > 0.0) {
         const double rp = 0.5 * cfg->morph_diameter * s;
@@ -375,6 +403,7 @@ extern "C" int epsgrad_plan_destroy(epsgrad_plan_t *P)
     if (P->d_hl) cudaFree(P->d_hl);
     if (P->d_invn) cudaFree(P->d_invn);
     if (P->d_sched) cudaFree(P->d_sched);
+    if (P->d_atc) cudaFree(P->d_atc);
     if (P->d_mprof) cudaFree(P->d_mprof);
     if (P->aux) cudaStreamDestroy(P->aux);
     if (P->ev_fork) cudaEventDestroy(P->ev_fork);
@@ -471,6 +500,14 @@ extern "C" int epsgrad_plan_set_tma(epsgrad_plan_t *P, int enable)
     if (!P) return EPSGRAD_EINVAL;
     if (enable && !P->tma_encode) return EPSGRAD_EUNSUPPORTED;
     P->use_tma = enable < 0 ? 0 : (enable > 2 ? 2 : enable);
+    return EPSGRAD_OK;
+}
+
+extern "C" int epsgrad_plan_set_tensor_cores(epsgrad_plan_t *P, int enable)
+{
+    if (!P) return EPSGRAD_EINVAL;
+    if (enable && !P->d_atc) return EPSGRAD_EUNSUPPORTED;
+    P->use_tc = enable < 0 ? 0 : (enable > 2 ? 2 : enable);
     return EPSGRAD_OK;
 }
 

@@ -32,6 +32,25 @@ constexpr int MO_T = 32, MO_THREADS = 256, MO_MAX_R = 16;
 // u(beta) partial sums (reduce.cuh)
 constexpr int UB_THREADS = 256, UB_PER_THREAD = 16;
 
+// tensor-core filter (filter_tc.cuh): 128 = 4 phases x 32 mask columns (8 control columns) by FTC_N control rows per tile
+constexpr int FTC_WORKERS = 256, FTC_THREADS = FTC_WORKERS + 64, FTC_TB = 8, FTC_M = 128;   // + the weight-producer warp and the MMA warp
+constexpr int FTC_N_RESIDENT = 64, FTC_N_STREAM = 256, FTC_STAGES = 3;   // control rows per tile; stages of the streamed weights' ring
+__host__ __device__ constexpr int ftc_k(int NT) { return ((FTC_TB + NT - 1) + 7) / 8 * 8; }          // FTC_TB + 2T rounded up to 8
+__host__ __device__ constexpr size_t ftc_a_floats(int NT) { return (size_t)2 * NT * ftc_k(NT) * FTC_M; }   // hi and lo tables
+__host__ __device__ constexpr size_t ftc_smem_bytes(int NT, int N, bool stream)
+{
+    return ((stream ? (size_t)FTC_STAGES * 2 * ftc_k(NT) * FTC_M : ftc_a_floats(NT)) + (size_t)4 * ftc_k(NT) * (N + NT - 1)) * 4 + 128;
+}
+// low 13 mantissa bits cleared: exactly representable as tf32 whatever the unit does with the bits it does not read
+__host__ __device__ inline float tf32_trunc(float x)
+{
+#ifdef __CUDA_ARCH__
+    return __uint_as_float(__float_as_uint(x) & 0xffffe000u);
+#else
+    union { float f; unsigned u; } v; v.f = x; v.u &= 0xffffe000u; return v.f;
+#endif
+}
+
 // persistent dataflow kernel (mega.cuh): Yee rows per band, phases, ints before the per-band counters of the schedule buffer
 constexpr int MK_BAND = 16;
 enum { PH_F1 = 0, PH_F2, PH_X, PH_M, PH_T, PH_Z, PH_N };    // the compute list's phases in within-step order, then the field blocks

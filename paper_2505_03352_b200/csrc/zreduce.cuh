@@ -212,6 +212,11 @@ __device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"((unsigned)__cvta_generic_to_shared(bar)), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive(unsigned long long *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+}
+
 __device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned phase)
 {
     asm volatile(

@@ -37,11 +37,6 @@ __host__ __device__ inline size_t zpipe_smem_bytes(int wb, int nstage)
     return (size_t)nstage * 2 * ZP_COLS * wb * 16 + 128 /* alignment slack */ + 2 * ZP_MAX_STAGE * 8;
 }
 
-__device__ __forceinline__ void mbar_arrive(unsigned long long *bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
-}
-
 // grid (n_cta, 1, B): persistent CTAs, each walking the (component, column block) items n_cta apart, component by component
 __global__ void __launch_bounds__(ZP_THREADS) k_zreduce_pipe(const __grid_constant__ ZredPipeParams P)
 {

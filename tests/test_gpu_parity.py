@@ -407,3 +407,32 @@ def test_plans_are_released():
             free0 = torch.cuda.mem_get_info()[0]
     torch.cuda.empty_cache()
     assert torch.cuda.mem_get_info()[0] >= free0 - (8 << 20)          # device tables, streams and events go with the plan
+
+
+@pytest.mark.parametrize("kw,beta", [
+    (dict(mx=32, my=32, nz=16, z_lo=6.25, z_hi=9.75, filter_radius=4.0), 8.0),                 # Tiny's geometry: one ragged tile per block
+    (dict(mx=67, my=13, nz=8, z_lo=2.25, z_hi=5.75, filter_radius=4.0), 16.0),                 # 2 row blocks (64 + 3), 2 column blocks (8 + 5)
+    (dict(batch=3, mx=5, my=70, nz=8, z_lo=2.25, z_hi=5.75, filter_radius=8.0), 64.0),         # fewer control rows than taps; saturated tanh
+    (dict(mx=130, my=41, nz=8, z_lo=2.25, z_hi=5.75, filter_radius=8.0, filter_normalize=0, eta=0.0), 1.5),
+    (dict(mx=270, my=23, nz=4, z_lo=0.5, z_hi=3.5, filter_radius=12.0), 32.0),                 # streamed weights: 256 + 14 rows
+    (dict(batch=2, mx=9, my=9, nz=4, z_lo=0.5, z_hi=3.5, filter_radius=12.0), 8.0),            # a grid smaller than the filter
+])
+def test_tensor_core_filter_matches_the_oracle(kw, beta):
+    """Eq. (2) by tcgen05 MMAs (filter_tc.cuh, forced on: by default it runs only on large control grids): the filter output
+    against the FFMA stencil, and eps / dF/dC against the oracle at BASELINE.json's tolerances."""
+    cfg = B.make_config(**kw)
+    C = rand_C(cfg, 21)
+    plan = B.Plan(cfg)
+    plan.set_tensor_cores(0)
+    phi0 = plan.stage_filter(dev(C))
+    plan.set_tensor_cores(1)
+    phi1 = plan.stage_filter(dev(C))
+    torch.cuda.synchronize()
+    # the tensor core accumulates in float32 with a coarser rounding than FFMA: a few 1e-6 of the largest |Phi|
+    assert float((phi1 - phi0).abs().max()) < 8e-6 * max(0.5, float(phi0.abs().max())), float((phi1 - phi0).abs().max())
+    check_forward(cfg, C, beta, plan)
+    EF, EA = rand_fields(cfg, 2, 22)
+    check_vjp(cfg, C, beta, EF, EA, plan)
+    with pytest.raises(B.EpsgradError) as e:                      # the Gaussian filter is separable: no banded matrices for it
+        B.Plan(B.make_config(mx=16, my=16, nz=8, z_lo=2.0, z_hi=5.0, filter_kind=1, filter_radius=6.0, filter_sigma=2.0)).set_tensor_cores(1)
+    assert e.value.status == B.EUNSUPPORTED
