@@ -116,19 +116,27 @@ def zreduce_sector_bytes(w, n_pairs: int) -> int:
     return w.batch * w.nx * w.ny * per_column * 2 * n_pairs
 
 
+def crop(w, mx, my):
+    """workload w on an mx x my control grid (same cells per control pixel, also when that is not an integer)"""
+    from dataclasses import replace
+    if w.nx_cells > 0:
+        return replace(w, mx=mx, my=my, batch=1, nx_cells=max(mx, round(mx * w.nx_cells / w.mx)), ny_cells=max(my, round(my * w.ny_cells / w.my)))
+    return replace(w, mx=mx, my=my, batch=1)
+
+
 def oracle_cfg(w, mx=None, my=None):
     import oracle as O
     mx, my = mx or w.mx, my or w.my
-    return O.OracleConfig(mx=mx, my=my, nx=w.upsample * mx, ny=w.upsample * my, nz=w.nz, z_lo=w.z_lo, z_hi=w.z_hi,
+    wc = crop(w, mx, my)
+    return O.OracleConfig(mx=mx, my=my, nx=wc.nx, ny=wc.ny, nz=w.nz, z_lo=w.z_lo, z_hi=w.z_hi,
                           s=w.subpixel, filter_kind=w.filter_kind, radius=w.radius, sigma=w.sigma or 1.0, eta=w.eta,
                           eps_core=w.eps_core, eps_clad=w.eps_clad, delta=w.normal_delta,
                           morph_diam=w.morph_diameter, morph_alpha=w.morph_alpha)
 
 
 def oracle_step_inputs(w, mx, my):
-    from dataclasses import replace
     from paper_2505_03352_b200 import workloads as W
-    ws = replace(w, mx=mx, my=my, batch=1)
+    ws = crop(w, mx, my)
     C = W.make_C(ws)[0]
     EF = [W.make_field(ws, p, 0) for p in range(w.n_pairs)]
     EA = [W.make_field(ws, p, 1) for p in range(w.n_pairs)]

@@ -183,7 +183,10 @@ __global__ void __launch_bounds__(FTC_THREADS, 1) k_filter_tc(const FilterTcPara
         }
     } else {
         // ---- workers: stage tile it, then read out and store tile it - 1 (while the tensor core works on tile it)
-        const int fx = warp & 3, half = warp >> 2, beta = lane >> 2, fy = lane & 3;   // warps w and w + 4 share TMEM lanes 32 fx ..
+        // warps w, w + 4, w + 8, .. share TMEM lanes 32 fx .. 32 fx + 31 and split the control rows: a warp has one store in flight at
+        // a time (~120 cycles per 128-byte row segment, measured), so the read-out scales with the number of warps doing it
+        constexpr int NPART = FTC_WORKERS / 128;
+        const int fx = warp & 3, part = warp >> 2, beta = lane >> 2, fy = lane & 3;
         for (int it = 0; it <= my_tiles; ++it) {
             const long long t0 = clock64();
             if (it < my_tiles) {
@@ -195,7 +198,7 @@ __global__ void __launch_bounds__(FTC_THREADS, 1) k_filter_tc(const FilterTcPara
                 // buffer was last read by the MMAs of tile it - 2, which completed before that tile's read-out began.
                 float *Bh = Bs + (size_t)(it & 1) * 2 * K * RB, *Bl = Bh + K * RB;
                 const float *Cb = P.C + (size_t)b * P.mx * P.my;
-                constexpr int U = 4;                   // loads in flight per thread
+                constexpr int U = 8;                   // loads in flight per thread
                 for (int base = tid; base < RB * K; base += U * FTC_WORKERS) {
                     float v[U];
 #pragma unroll
@@ -237,7 +240,7 @@ __global__ void __launch_bounds__(FTC_THREADS, 1) k_filter_tc(const FilterTcPara
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                 const long long t2 = clock64();
 #pragma unroll 1
-                for (int n0 = half * (N / 2); n0 < (half + 1) * (N / 2); n0 += 16) {
+                for (int n0 = part * (N / NPART); n0 < (part + 1) * (N / NPART); n0 += 16) {
                     unsigned v[16];
                     const unsigned taddr = tmem + ((unsigned)(fx * 32) << 16) + (unsigned)(buf * N + n0);
                     asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
@@ -251,7 +254,7 @@ __global__ void __launch_bounds__(FTC_THREADS, 1) k_filter_tc(const FilterTcPara
                         const int a0 = a_base + n0 + i;
                         if (col_ok && a0 < P.mx) {
                             const float inv = (a0 >= T && a0 < P.mx - T) ? inv_in : P.nrm.at_index(P.nrm.ix(a0, fx), niy);
-                            *orow = __uint_as_float(v[i]) * inv;
+                            __stcg(orow, __uint_as_float(v[i]) * inv);      // L2: the 2-D stage reads Phi' from there
                         }
                     }
                 }

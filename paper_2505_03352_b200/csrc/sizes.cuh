@@ -33,7 +33,7 @@ constexpr int MO_T = 32, MO_THREADS = 256, MO_MAX_R = 16;
 constexpr int UB_THREADS = 256, UB_PER_THREAD = 16;
 
 // tensor-core filter (filter_tc.cuh): 128 = 4 phases x 32 mask columns (8 control columns) by FTC_N control rows per tile
-constexpr int FTC_WORKERS = 256, FTC_THREADS = FTC_WORKERS + 64, FTC_TB = 8, FTC_M = 128;   // + the weight-producer warp and the MMA warp
+constexpr int FTC_WORKERS = 512, FTC_THREADS = FTC_WORKERS + 64, FTC_TB = 8, FTC_M = 128;   // + the weight-producer warp and the MMA warp
 constexpr int FTC_N_RESIDENT = 64, FTC_N_STREAM = 256, FTC_STAGES = 3;   // control rows per tile; stages of the streamed weights' ring
 __host__ __device__ constexpr int ftc_k(int NT) { return ((FTC_TB + NT - 1) + 7) / 8 * 8; }          // FTC_TB + 2T rounded up to 8
 __host__ __device__ constexpr size_t ftc_a_floats(int NT) { return (size_t)2 * NT * ftc_k(NT) * FTC_M; }   // hi and lo tables
