@@ -384,7 +384,8 @@ class Plan:
             return None
         names = ("F1", "F2", "X", "M", "T", "Z")
         return {"busy": {n: int(out[i]) for i, n in enumerate(names)}, "items": {n: int(out[6 + i]) for i, n in enumerate(names)},
-                "tickets": int(out[12]), "total": int(out[13]), "wait": int(out[14]), "release": int(out[15]), "zbegin": int(out[16]), "endsync": int(out[17])}
+                "tickets": int(out[12]), "total": int(out[13]), "wait": int(out[14]), "release": int(out[15]), "zbegin": int(out[16]), "endsync": int(out[17]),
+                "raw": [int(x) for x in out]}
 
     def set_tuning(self, knob: int, value: int) -> None:
         _check(lib().epsgrad_plan_set_tuning(self._h, int(knob), int(value)), "epsgrad_plan_set_tuning")

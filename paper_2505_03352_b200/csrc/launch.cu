@@ -13,6 +13,7 @@
 #include "filter_sep.cuh"
 #include "filter_general.cuh"
 #include "filter_tc.cuh"
+#include "filterT_tc.cuh"
 #include "fwd2d.cuh"
 #include "extrude.cuh"
 #include "extrude_bulk.cuh"
@@ -214,6 +215,28 @@ int launch_filterT_conic(epsgrad_plan *P, const float *v, float *dC, cudaStream_
     using S = FilterTShape<M>;
     const int T = P->T, NT = P->NT;
     const FilterTParams fp = fill_filterT(P, v, dC);
+    // tensor cores (filterT_tc.cuh): when asked for (use_tc = 1); by default (2) where they measured faster than the FFMA kernel:
+    // R = 12 from ~500 x 500 control pixels (44 against 58 us; 112 against 203 us at 1000 x 1000), R <= 8 at 1000 x 1000
+    // (87 against 125 us; within 2 us of each other at 375 and 500, slower at 250)
+    bool tc = M == 4 && P->use_tc && P->d_att && (NT == 5 || NT == 9 || NT == 13);
+    if (tc) {
+        FilterTTcParams tp;
+        tp.v = v; tp.dC = dC; tp.a_tab = P->d_att;
+        tp.mx = fp.mx; tp.my = fp.my; tp.px = fp.px; tp.py = fp.py; tp.dbg = P->d_mprof;
+        const int nb = cdiv(fp.mx, FTT_MAXN - 2 * T);                      // row blocks; rows per block rounded so that n_in % 16 == 0
+        tp.n_in = std::min(FTT_MAXN, (cdiv(fp.mx, nb) + 2 * T + 15) / 16 * 16);
+        tp.n_out = tp.n_in - 2 * T;
+        tp.tiles_x = cdiv(fp.my, FTC_TB); tp.tiles_y = cdiv(fp.mx, tp.n_out); tp.n_tiles = tp.tiles_x * tp.tiles_y * P->cfg.batch;
+        if (P->use_tc == 2) tc = NT == 13 ? tp.n_tiles >= P->n_sm : 2 * tp.n_tiles >= 3 * P->n_sm;
+        if (tc) {
+            auto kern = NT == 5 ? k_filterT_tc<5> : (NT == 9 ? k_filterT_tc<9> : k_filterT_tc<13>);
+            const size_t smem_t = ftt_smem_bytes(NT);
+            int rct = set_smem(P, kern, smem_t);
+            if (rct) return rct;
+            kern<<<std::min(tp.n_tiles, P->n_sm), FTC_THREADS, smem_t, st>>>(tp);
+            return check_launch(P, "filterT", st);
+        }
+    }
     if (M == 4 && (NT == 5 || NT == 9 || NT == 13)) {          // fast path (filter4.cuh)
         auto kern = NT == 5 ? k_filterT_conic4<5> : (NT == 9 ? k_filterT_conic4<9> : k_filterT_conic4<13>);
         const size_t smem4 = filterT4_smem_floats(NT) * 4;

@@ -294,7 +294,28 @@ extern "C" int epsgrad_plan_create(const epsgrad_config_t *cfg, int device, epsg
         const bool okt = cudaMalloc(&P->d_atc, atc.size() * 4) == cudaSuccess &&
                          cudaMemcpy(P->d_atc, atc.data(), atc.size() * 4, cudaMemcpyHostToDevice) == cudaSuccess;
         cudaSetDevice(prevt);
-        if (!okt) { cudaGetLastError(); epsgrad_plan_destroy(P); return EPSGRAD_ECUDA; }
+        // the transpose (filterT_tc.cuh): A[(tx, beta), (fx, qq)] = W[tx][beta + 2T - qq/4][fx][qq % 4], in k-step slabs of 8 (fx, qq) values
+        const int KQ = ftt_kq(NT), KS = ftt_ksteps(NT);
+        std::vector<float> att(ftt_a_floats(NT), 0.0f);
+        for (int ks = 0; ks < KS; ++ks) {
+            const int fx = ks / (KQ / 8), q8 = 8 * (ks - fx * (KQ / 8));
+            for (int c = 0; c < 2; ++c)
+                for (int tx = 0; tx < NT; ++tx)
+                    for (int beta = 0; beta < FTC_TB; ++beta)
+                        for (int e = 0; e < 4; ++e) {
+                            const int qq = q8 + 4 * c + e, ty = beta + 2 * T - (qq >> 2), fy = qq & 3, row = tx * FTC_TB + beta;
+                            if (ty < 0 || ty >= NT) continue;
+                            const float wv = w[(((size_t)tx * NT + ty) * m + fx) * m + fy];
+                            const float hi = tf32_trunc(wv), lo = tf32_trunc(wv - hi);
+                            const size_t o = ((size_t)ks * 2 * 2 + c) * FTC_M * 4 + (size_t)row * 4 + e;      // [ks][hi][c][row][e]; lo one [2][128][4] further
+                            att[o] = hi; att[o + 2 * FTC_M * 4] = lo;
+                        }
+        }
+        cudaSetDevice(device);
+        const bool oka = cudaMalloc(&P->d_att, att.size() * 4) == cudaSuccess &&
+                         cudaMemcpy(P->d_att, att.data(), att.size() * 4, cudaMemcpyHostToDevice) == cudaSuccess;
+        cudaSetDevice(prevt);
+        if (!okt || !oka) { cudaGetLastError(); epsgrad_plan_destroy(P); return EPSGRAD_ECUDA; }
         P->use_tc = 2;           // where it measured faster (launch.cu)
     }
 
@@ -404,6 +425,7 @@ extern "C" int epsgrad_plan_destroy(epsgrad_plan_t *P)
     if (P->d_invn) cudaFree(P->d_invn);
     if (P->d_sched) cudaFree(P->d_sched);
     if (P->d_atc) cudaFree(P->d_atc);
+    if (P->d_att) cudaFree(P->d_att);
     if (P->d_mprof) cudaFree(P->d_mprof);
     if (P->aux) cudaStreamDestroy(P->aux);
     if (P->ev_fork) cudaEventDestroy(P->ev_fork);

@@ -26,6 +26,7 @@ struct epsgrad_plan {
     float *d_w;                // conic [NT][NT][m][m] | separable [NT][m]
     int *d_tyrange;            // conic [NT][2]
     float *d_atc;              // tensor-core filter (filter_tc.cuh): banded weight matrices [2 (hi, lo)][NT][K/4][128][4], or nullptr
+    float *d_att;              // transposed tensor-core filter (filterT_tc.cuh): weight slabs of the k-steps, two tf32 terms
     int use_tc;                // Eq. (2) forward on the tensor cores where d_atc exists (epsgrad_plan_set_tensor_cores)
     float *d_invden;           // conic [KX*m][KY*m] | separable [KX*m] + [KY*m]
     float *d_zw;               // [7][nz]: wxy, wz, z-full / lower-face / upper-face indicators, eps_clad(1-wxy), eps_clad[wz=0]

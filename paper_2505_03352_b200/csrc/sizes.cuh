@@ -41,6 +41,18 @@ __host__ __device__ constexpr size_t ftc_smem_bytes(int NT, int N, bool stream)
 {
     return ((stream ? (size_t)FTC_STAGES * 2 * ftc_k(NT) * FTC_M : ftc_a_floats(NT)) + (size_t)4 * ftc_k(NT) * (N + NT - 1)) * 4 + 128;
 }
+// tensor-core transposed filter (filterT_tc.cuh): k-steps of 8 of the K = 16 (8 + 2T) values; weight slabs [KS][hi, lo][2][128][4]
+__host__ __device__ constexpr int ftt_kq(int NT) { return 4 * (FTC_TB + NT - 1); }            // mask columns a block of 8 control columns reads
+__host__ __device__ constexpr int ftt_ksteps(int NT) { return 4 * ftt_kq(NT) / 8; }
+__host__ __device__ constexpr size_t ftt_a_floats(int NT) { return (size_t)ftt_ksteps(NT) * 2 * 2 * FTC_M * 4; }
+constexpr int FTT_GROUP = 4, FTT_RING = 2, FTT_MAXN = 256;   // k-steps per group (the unit of the rings: 32 KB of weights, 65 KB of data); groups per ring
+__host__ __device__ constexpr unsigned ftt_b_step_floats() { return 2 * 2 * (FTT_MAXN * 4 + 16); }   // a data slab: [hi, lo][2 chunks][256 rows + 64 bytes][4 floats]
+__host__ __device__ constexpr size_t ftt_smem_bytes(int NT)
+{
+    // the read-out buffer E [8 NT][FTT_MAXN + 1] reuses the data ring (idle between the last MMA of a tile and the first slab of the next)
+    return (size_t)FTT_RING * FTT_GROUP * ((size_t)2 * 2 * FTC_M * 16 + (size_t)ftt_b_step_floats() * 4) + 128;
+}
+
 // low 13 mantissa bits cleared: exactly representable as tf32 whatever the unit does with the bits it does not read
 __host__ __device__ inline float tf32_trunc(float x)
 {

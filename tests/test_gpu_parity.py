@@ -416,6 +416,8 @@ def test_plans_are_released():
     (dict(mx=130, my=41, nz=8, z_lo=2.25, z_hi=5.75, filter_radius=8.0, filter_normalize=0, eta=0.0), 1.5),
     (dict(mx=270, my=23, nz=4, z_lo=0.5, z_hi=3.5, filter_radius=12.0), 32.0),                 # streamed weights: 256 + 14 rows
     (dict(batch=2, mx=9, my=9, nz=4, z_lo=0.5, z_hi=3.5, filter_radius=12.0), 8.0),            # a grid smaller than the filter
+    (dict(batch=2, mx=500, my=19, nz=4, z_lo=0.5, z_hi=3.5, filter_radius=12.0), 16.0),        # transposed filter: 3 row blocks of 192 staged rows
+    (dict(mx=21, my=300, nz=4, z_lo=0.5, z_hi=3.5, filter_radius=8.0), 16.0),                  # 38 column blocks, the last one ragged
 ])
 def test_tensor_core_filter_matches_the_oracle(kw, beta):
     """Eq. (2) by tcgen05 MMAs (filter_tc.cuh, forced on: by default it runs only on large control grids): the filter output
@@ -433,6 +435,12 @@ def test_tensor_core_filter_matches_the_oracle(kw, beta):
     check_forward(cfg, C, beta, plan)
     EF, EA = rand_fields(cfg, 2, 22)
     check_vjp(cfg, C, beta, EF, EA, plan)
+    # the transposed filter (filterT_tc.cuh) against the FFMA kernel on the same cotangent: two-term tf32 operands, float32 sums
+    g1 = plan.eps_vjp(dev(C), beta, [dev(f) for f in EF], [dev(f) for f in EA]).clone()
+    plan.set_tensor_cores(0)
+    g0 = plan.eps_vjp(dev(C), beta, [dev(f) for f in EF], [dev(f) for f in EA])
+    torch.cuda.synchronize()
+    assert float((g1 - g0).abs().max()) <= 1e-5 * float(g0.abs().max()), float((g1 - g0).abs().max() / g0.abs().max())
     with pytest.raises(B.EpsgradError) as e:                      # the Gaussian filter is separable: no banded matrices for it
         B.Plan(B.make_config(mx=16, my=16, nz=8, z_lo=2.0, z_hi=5.0, filter_kind=1, filter_radius=6.0, filter_sigma=2.0)).set_tensor_cores(1)
     assert e.value.status == B.EUNSUPPORTED
