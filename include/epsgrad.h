@@ -265,13 +265,15 @@ int epsgrad_plan_set_slab(epsgrad_plan_t *plan, int x_first, int x_count);
  * EPSGRAD_EUNSUPPORTED when TMA descriptors cannot be built on this driver.                                               */
 int epsgrad_plan_set_tma(epsgrad_plan_t *plan, int mode);
 
-/* Eq. (2) on the tensor cores (tcgen05.mma kind::tf32, accumulators in tensor memory; both operands split into two tf32 terms
- * and three products accumulated in float32; filter_tc.cuh).  Applies to the conic filter with upsample * subpixel = 4 and
- * R <= 12 cells (EPSGRAD_EUNSUPPORTED when set on another plan).  Mode 2 (default on such plans): where it measured faster
- * than the FFMA stencil, i.e. on control grids large enough to amortise the per-CTA set-up (from ~500 x 500 at R = 12: 75 us
- * against 159 us at 1000 x 1000; from ~375 x 375 at R <= 8); 1: wherever it applies; 0: never (filter4.cuh).  The tensor
- * core's float32 accumulation is coarser than FFMA's: measured against the oracle, eps errors grow from 7e-7 to 3.3e-6 at
- * beta = 64 (tolerance 1e-5).                                                                                            */
+/* Eq. (2) and its transpose on the tensor cores (tcgen05.mma kind::tf32, accumulators in tensor memory; both operands split
+ * into two tf32 terms and three products accumulated in float32; filter_tc.cuh, filterT_tc.cuh).  Applies to the conic filter
+ * with upsample * subpixel = 4 and R <= 12 cells (EPSGRAD_EUNSUPPORTED when set on another plan).  Mode 2 (default on such
+ * plans): where each kernel measured faster than its FFMA stencil, i.e. on control grids with enough tiles for every SM --
+ * the filter from ~500 x 500 control pixels at R = 12 (55 us against 158 us at 1000 x 1000) and from ~375 x 375 at R <= 8
+ * (52 against 97 us at 1000 x 1000); its transpose from ~500 x 500 at R = 12 (112 against 203 us at 1000 x 1000) and at
+ * 1000 x 1000 for R <= 8 (87 against 125 us).  1: wherever they apply; 0: never (filter4.cuh).  The tensor core's float32
+ * accumulation is coarser than FFMA's: measured against the oracle, eps errors grow from 7e-7 to 3.3e-6 at beta = 64
+ * (tolerance 1e-5); dF/dC differs from the FFMA kernel's by <= 2.5e-6 of its largest entry (tolerance 1e-4).              */
 int epsgrad_plan_set_tensor_cores(epsgrad_plan_t *plan, int enable);
 
 /* Programmatic dependent launch (default on).  Consecutive kernels of a stream -- filter -> 2-D stage (-> eps stores in

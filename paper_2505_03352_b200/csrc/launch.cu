@@ -139,7 +139,7 @@ int launch_filter_m(epsgrad_plan *P, const float *C, float *phi, cudaStream_t st
         const FilterParams fp = fill_filter(P, C, phi);
         // tensor cores (filter_tc.cuh): always when asked for (use_tc = 1); by default (2) where they measured faster than the
         // FFMA stencil -- enough tiles to amortise the per-CTA set-up (weights, TMEM): R = 12 from ~500 x 500 control pixels
-        // (31 against 47 us; 75 against 159 us at 1000 x 1000), R <= 8 from ~375 x 375 (16.5 against 20.4 us; a tie at 250 x 250)
+        // (27 against 47 us; 55 against 158 us at 1000 x 1000), R <= 8 from ~375 x 375 (14.5 against 20.5 us; a tie at 250 x 250)
         bool tc = M == 4 && P->use_tc && P->d_atc && (NT == 5 || NT == 9 || NT == 13);
         if (tc && P->use_tc == 2) {
             const bool big = NT == 13;
