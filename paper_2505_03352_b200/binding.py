@@ -363,7 +363,7 @@ class Plan:
         _check(lib().epsgrad_plan_set_tma(self._h, int(mode)), "epsgrad_plan_set_tma")
 
     def set_tensor_cores(self, mode) -> None:
-        """Eq. (2) on the tensor cores: 0 / False never, 1 / True wherever it applies, 2 where it measured faster (default)"""
+        """Eq. (2) and its transpose on the tensor cores: 0 / False never, 1 / True wherever it applies, 2 where it measured faster (default)"""
         _check(lib().epsgrad_plan_set_tensor_cores(self._h, int(mode)), "epsgrad_plan_set_tensor_cores")
 
     def set_pdl(self, enable: bool) -> None:
@@ -372,8 +372,9 @@ class Plan:
     def set_bulk_stores(self, enable: bool) -> None:
         _check(lib().epsgrad_plan_set_bulk_stores(self._h, int(bool(enable))), "epsgrad_plan_set_bulk_stores")
 
-    def set_fused(self, enable: bool) -> None:
-        """one persistent dataflow kernel per call (default where it applies) / the step as separate kernels"""
+    def set_fused(self, enable) -> None:
+        """0 / False: the step as separate kernels (default); 1: one persistent dataflow kernel per call; 2: persistent 2-D chains
+        beside the separate stream kernels (measurement switches: both are slower)"""
         _check(lib().epsgrad_plan_set_fused(self._h, int(enable)), "epsgrad_plan_set_fused")
 
     def fused_profile(self, enable: bool, read: bool = False):

@@ -5,8 +5,8 @@
 // (exact), the basis itself in float32:
 //   forward  Phi'[p,q] = sum_ab W(X_p - x_a, Y_q - y_b) (C[a,b] - eta0) / sum_ab W(...)       one thread per mask pixel; it also
 //            leaves 1/sum_ab W on a mask-sized plane, which the reverse pass reads through Normaliser::plane_py (S2);
-//   reverse  dC[a,b] = sum_pq W(X_p - x_a, Y_q - y_b) v[p,q]                                  one thread per control node
-//            (gather, deterministic; v already carries 1/sum W).
+//   reverse  dC[a,b] = sum_pq W(X_p - x_a, Y_q - y_b) v[p,q]                                  one warp per control node
+//            (gather, fixed summation order: deterministic; v already carries 1/sum W).
 // A coverage path, not a tuned one: the BASELINE configs have 2 cells per control pixel and take filter4.cuh / filter_sep.cuh.
 #pragma once
 #include "common.cuh"
@@ -67,24 +67,29 @@ __global__ void __launch_bounds__(FG_THREADS) k_filter_general(const FilterGenPa
     if (b == 0) P.invden[i] = inv;
 }
 
-// grid (ceil(mx*my / FG_THREADS), B)
+// grid (ceil(mx*my / (FG_THREADS / 32)), B): one WARP per control node -- its window of mask pixels ((2 R s + 3)^2, 35 x 35 for
+// Fig. 4) is split over the lanes and the 32 partial sums are added in a fixed butterfly order (deterministic).  One thread per
+// node left 1296 threads with 1225 dependent evaluations each: 246 us for Fig. 4's 36 x 36 nodes.
 __global__ void __launch_bounds__(FG_THREADS) k_filterT_general(const FilterGenParams P)
 {
-    const int n_ctrl = P.mx * P.my, i = blockIdx.x * FG_THREADS + threadIdx.x;
-    if (i >= n_ctrl) return;
+    const int n_ctrl = P.mx * P.my, lane = threadIdx.x & 31, i = blockIdx.x * (FG_THREADS / 32) + (threadIdx.x >> 5);
+    if (i >= n_ctrl) return;                       // whole warps leave
     const int b = blockIdx.y, a = i / P.my, bb = i - a * P.my;
     const double xa = P.ux * (a + 0.5), yb = P.uy * (bb + 0.5), R = (double)P.R;
     // mask pixels within reach: |(p + 1/2)/s - x_a| <= R, one pixel of slack, clamped (the basis is zero beyond its support)
     const int plo = max(0, (int)floor((xa - R) * P.s - 0.5) - 1), phi_ = min(P.px - 1, (int)ceil((xa + R) * P.s - 0.5) + 1);
     const int qlo = max(0, (int)floor((yb - R) * P.s - 0.5) - 1), qhi = min(P.py - 1, (int)ceil((yb + R) * P.s - 0.5) + 1);
+    const int nq = qhi - qlo + 1, n_win = (phi_ - plo + 1) * nq;
     const float *vb = P.v + (size_t)b * P.px * P.py;
+    const double inv_s = 1.0 / P.s;                // a multiplication per pixel instead of a float64 division (1 ulp of float64 apart at most)
     float acc = 0.0f;
-    for (int p = plo; p <= phi_; ++p) {
-        const float dx = (float)((p + 0.5) / P.s - xa);
-        for (int q = qlo; q <= qhi; ++q)
-            acc = fmaf(fg_basis(P, dx, (float)((q + 0.5) / P.s - yb)), vb[(size_t)p * P.py + q], acc);
+    for (int k = lane; k < n_win; k += 32) {
+        const int kp = k / nq, p = plo + kp, q = qlo + (k - kp * nq);
+        acc = fmaf(fg_basis(P, (float)((p + 0.5) * inv_s - xa), (float)((q + 0.5) * inv_s - yb)), vb[(size_t)p * P.py + q], acc);
     }
-    P.dC[(size_t)b * n_ctrl + i] = acc;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (lane == 0) P.dC[(size_t)b * n_ctrl + i] = acc;
 }
 
 }  // namespace epsgrad

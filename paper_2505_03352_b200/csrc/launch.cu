@@ -320,7 +320,7 @@ int launch_filterT(epsgrad_plan *P, const float *v, float *dC, cudaStream_t st)
         FilterGenParams fp = fill_filter_general(P);
         fp.v = v; fp.dC = dC;
         if (P->cfg.batch > 65535) return EPSGRAD_EUNSUPPORTED;
-        k_filterT_general<<<dim3(cdiv(P->cfg.mx * P->cfg.my, FG_THREADS), P->cfg.batch), FG_THREADS, 0, st>>>(fp);
+        k_filterT_general<<<dim3(cdiv(P->cfg.mx * P->cfg.my, FG_THREADS / 32), P->cfg.batch), FG_THREADS, 0, st>>>(fp);
         return check_launch(P, "filterT", st);
     }
     switch (P->m) {
