@@ -84,3 +84,16 @@ def test_product_does_not_import_the_oracle():
                 text = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(import|from)\s+oracle\b", text, flags=re.M), f
                 assert "epsgrad_oracle" not in text, f
+
+
+def test_abtest_module_needs_a_gpu_and_names_its_modes(capsys):
+    """`python -m paper_2505_03352_b200.abtest`: usage without arguments; no CPU path behind any of its modes."""
+    import torch
+    from paper_2505_03352_b200 import abtest
+    assert abtest.main([]) == 2
+    text = capsys.readouterr().out
+    for mode in ("streams", "pdl", "fused", "tc"):
+        assert mode in text
+    if not torch.cuda.is_available():
+        with pytest.raises(RuntimeError):
+            abtest.main(["pdl", "tiny"])
