@@ -257,6 +257,17 @@ int epsgrad_plan_set_embedding(epsgrad_plan_t *plan, const epsgrad_embedding_t *
  * in the *_host entry points.                                                                                              */
 int epsgrad_plan_set_slab(epsgrad_plan_t *plan, int x_first, int x_count);
 
+/* Fields on the design region only (Eq. (1) is restricted to Omega_D, and in z the design region is the slab).  After
+ * epsgrad_plan_set_packed_fields(plan, 1) the DEVICE entry points take every E_F / E_A as [B, 3, Nx, Ny, n_cells] complex64:
+ * the z cells [first_cell, first_cell + n_cells) of each column, contiguous -- the union of the slab windows of the x|y and z
+ * components, rounded to 16-byte pieces (two cells), as epsgrad_plan_packed_window returns them (paper scale: cells 26..35 of
+ * 64).  This is what a solver holds when it accumulates its frequency-domain fields on Omega_D only; the field stream then
+ * reads one dense array (80 instead of 512 bytes per column, no half-used fills).  Same arithmetic in the same order as with
+ * full columns: bitwise the same dFdC.  eps is unaffected (full columns).  EPSGRAD_EUNSUPPORTED together with an embedding, an
+ * x-slab, dense reads or nz % 4 != 0, and in the *_host entry point (which gathers the windows itself).                      */
+int epsgrad_plan_set_packed_fields(epsgrad_plan_t *plan, int enable);
+int epsgrad_plan_packed_window(const epsgrad_plan_t *plan, int *first_cell, int *n_cells);
+
 /* How the device-resident field windows are fetched.  0: by 16-byte asynchronous copies (LDGSTS), 5 CTAs per SM.
  * 1: by the tensor memory accelerator, one bulk tensor copy per field and 256 columns, one stage per CTA (region-sized
  * fields with sparse windows only; other cases fall back).  2: thin persistent read stream -- one CTA per SM, TMA copies

@@ -19,7 +19,7 @@ EXPORTS = (
     "epsgrad_plan_create", "epsgrad_plan_destroy", "epsgrad_workspace_bytes",
     "epsgrad_plan_set_workspace", "epsgrad_staging_bytes", "epsgrad_plan_set_staging",
     "epsgrad_plan_set_dense_reads", "epsgrad_plan_last_launches", "epsgrad_plan_last_copy_bytes",
-    "epsgrad_plan_set_profiling", "epsgrad_plan_last_kernel_times", "epsgrad_plan_set_overlap", "epsgrad_plan_set_host_direct", "epsgrad_plan_set_embedding", "epsgrad_plan_set_slab", "epsgrad_plan_set_tma", "epsgrad_plan_set_bulk_stores", "epsgrad_plan_set_pdl", "epsgrad_plan_set_tensor_cores", "epsgrad_plan_set_tuning", "epsgrad_plan_set_fused", "epsgrad_plan_fused_profile", "epsgrad_plan_set_timeline", "epsgrad_plan_read_timeline", 
+    "epsgrad_plan_set_profiling", "epsgrad_plan_last_kernel_times", "epsgrad_plan_set_overlap", "epsgrad_plan_set_host_direct", "epsgrad_plan_set_embedding", "epsgrad_plan_set_slab", "epsgrad_plan_set_packed_fields", "epsgrad_plan_packed_window", "epsgrad_plan_set_tma", "epsgrad_plan_set_bulk_stores", "epsgrad_plan_set_pdl", "epsgrad_plan_set_tensor_cores", "epsgrad_plan_set_tuning", "epsgrad_plan_set_fused", "epsgrad_plan_fused_profile", "epsgrad_plan_set_timeline", "epsgrad_plan_read_timeline", 
     "eps_forward", "eps_vjp", "eps_forward_vjp", "eps_forward_vjp_host", "eps_vjp_beta", "eps_unbinarity",
     "epsgrad_beta_schedule", "epsgrad_beta_update", "epsgrad_adam_step",
     "epsgrad_soap_accumulate", "epsgrad_soap_eigh_workspace_bytes", "epsgrad_soap_eigh", "epsgrad_soap_eigh_info",
@@ -227,6 +227,8 @@ def lib() -> ctypes.CDLL:
     L.epsgrad_plan_set_slab.argtypes = [vp, i32, i32]
     L.epsgrad_plan_set_embedding.argtypes = [vp, vp]
     L.epsgrad_plan_set_tma.argtypes = [vp, i32]
+    L.epsgrad_plan_set_packed_fields.argtypes = [vp, i32]
+    L.epsgrad_plan_packed_window.argtypes = [vp, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_int)]
     L.epsgrad_plan_set_bulk_stores.argtypes = [vp, i32]
     L.epsgrad_plan_set_pdl.argtypes = [vp, i32]
     L.epsgrad_plan_set_tensor_cores.argtypes = [vp, i32]
@@ -275,6 +277,7 @@ class Plan:
         self._stg = None
         self._stg_pairs = -1
         self._field_shape = None          # set_embedding: shape of the solver's arrays
+        self._packed_shape = None         # set_packed_fields: shape of E_F / E_A
 
     def close(self) -> None:
         if getattr(self, "_h", None):
@@ -320,8 +323,8 @@ class Plan:
         t = self._torch
         assert len(EF) == len(EA) and len(EF) >= 1
         for f in list(EF) + list(EA):
-            assert f.is_cuda and f.dtype == t.complex64 and f.is_contiguous() and tuple(f.shape) == self.field_shape, \
-                (f.shape, f.dtype, self.field_shape)
+            want = self._packed_shape or self.field_shape
+            assert f.is_cuda and f.dtype == t.complex64 and f.is_contiguous() and tuple(f.shape) == tuple(want), (f.shape, f.dtype, want)
         return _ptr_array(EF), _ptr_array(EA)
 
     def _out(self, out, shape):
@@ -357,6 +360,21 @@ class Plan:
         """eps / E_F / E_A hold only Yee rows [x_first, x_first + x_count) of the region: [B,3,x_count,Ny,Nz]; (0, 0): off"""
         _check(lib().epsgrad_plan_set_slab(self._h, x_first, x_count), "epsgrad_plan_set_slab")
         self._field_shape = (self.eps_shape[0], 3, x_count, self.eps_shape[3], self.eps_shape[4]) if x_count > 0 else None
+
+    def set_packed_fields(self, enable: bool) -> None:
+        """E_F / E_A as [B,3,Nx,Ny,n] complex64 holding only z cells packed_window() of every column (fields on Omega_D only)"""
+        _check(lib().epsgrad_plan_set_packed_fields(self._h, int(bool(enable))), "epsgrad_plan_set_packed_fields")
+        if enable:
+            k0, n = self.packed_window()
+            self._packed_shape = tuple(self.eps_shape[:4]) + (n,)
+        else:
+            self._packed_shape = None
+
+    def packed_window(self):
+        """(first z cell, number of z cells) of the packed field layout"""
+        a, b = ctypes.c_int(0), ctypes.c_int(0)
+        _check(lib().epsgrad_plan_packed_window(self._h, ctypes.byref(a), ctypes.byref(b)), "epsgrad_plan_packed_window")
+        return int(a.value), int(b.value)
 
     def set_tma(self, mode) -> None:
         """0: LDGSTS field reads; 1: single-stage TMA; 2: thin persistent TMA read stream"""

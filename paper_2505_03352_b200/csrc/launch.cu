@@ -453,6 +453,24 @@ void window_union(const epsgrad_plan *P, int *first, int *count)
     *count = hi > lo ? hi - lo : 0;
 }
 
+extern "C" int epsgrad_plan_set_packed_fields(epsgrad_plan_t *P, int enable)
+{
+    if (!P) return EPSGRAD_EINVAL;
+    if (enable && (P->emb.nx_full > 0 || P->slab_nx > 0 || P->dense || P->cfg.nz % 4)) return EPSGRAD_EUNSUPPORTED;
+    P->packed_fields = enable != 0;
+    return EPSGRAD_OK;
+}
+
+extern "C" int epsgrad_plan_packed_window(const epsgrad_plan_t *P, int *first_cell, int *n_cells)
+{
+    if (!P || !first_cell || !n_cells) return EPSGRAD_EINVAL;
+    int u0 = 0, un = 0;
+    window_union(P, &u0, &un);
+    *first_cell = 2 * u0;                  // 16-byte chunks of two complex64 cells
+    *n_cells = 2 * un;
+    return EPSGRAD_OK;
+}
+
 // everything of ZredParams but the field pointers; smem: bytes of staging a CTA needs; sparse: windows worth 64-byte fills
 int fill_zreduce(const epsgrad_plan *P, float *gbar, bool packed, ZredParams &zp, size_t &smem, bool &sparse, int &maxnch,
                  int max_cols = ZR_COLS, int stage_chunks = ZR_STAGE_CHUNKS)
@@ -505,6 +523,10 @@ int launch_zreduce(epsgrad_plan *P, int n_pairs, const void *const *EF, const vo
     size_t smem = 0;
     bool sparse = false;
     int maxnch = 1;
+    if (P->packed_fields && !host_src && !P->cur_host_src) {      // device fields on the slab window only (epsgrad_plan_set_packed_fields)
+        if (P->emb.nx_full > 0 || P->slab_nx > 0 || P->dense || P->cfg.nz % 4) return EPSGRAD_EUNSUPPORTED;
+        packed = true;
+    }
     // x-slab: only the slab's rows have fields; the cotangent of every other column of the region is zero
     if (P->slab_nx > 0 &&
         cudaMemsetAsync(gbar, 0, (size_t)P->cfg.batch * 5 * P->nx * P->ny * sizeof(float), st) != cudaSuccess) { cudaGetLastError(); return EPSGRAD_ECUDA; }
@@ -760,7 +782,7 @@ int check_pairs(int n_pairs, const void *const *EF, const void *const *EA)
 // ---- the whole step as one persistent dataflow kernel (mega.cuh)
 bool mega_applies(const epsgrad_plan *P, int n_pairs)
 {
-    return P->use_mega == 1 && P->d_sched && P->cfg.nz % 4 == 0 && !P->cur_dbeta && P->slab_nx == 0 && !P->cur_host_src && !P->prof && n_pairs <= ZR_MAX_PAIRS;
+    return P->use_mega == 1 && P->d_sched && P->cfg.nz % 4 == 0 && !P->cur_dbeta && P->slab_nx == 0 && !P->packed_fields && !P->cur_host_src && !P->prof && n_pairs <= ZR_MAX_PAIRS;
 }
 
 template <int NTC>

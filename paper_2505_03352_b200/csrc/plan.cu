@@ -500,6 +500,7 @@ extern "C" int epsgrad_plan_set_staging(epsgrad_plan_t *P, void *p, size_t bytes
 extern "C" int epsgrad_plan_set_dense_reads(epsgrad_plan_t *P, int dense)
 {
     if (!P) return EPSGRAD_EINVAL;
+    if (dense && P->packed_fields) return EPSGRAD_EUNSUPPORTED;            // packed fields have no cells outside the window to read
     P->dense = dense != 0;
     return EPSGRAD_OK;
 }
@@ -512,7 +513,7 @@ extern "C" int epsgrad_plan_set_embedding(epsgrad_plan_t *P, const epsgrad_embed
     if (e->i0 + P->nx > e->nx_full || e->j0 + P->ny > e->ny_full || e->k0 + P->cfg.nz > e->nz_full) return EPSGRAD_EINVAL;
     if (e->nz_full % 4 || e->k0 % 4 || P->cfg.nz % 4) return EPSGRAD_EUNSUPPORTED;   // 16-byte pieces of eps (4 cells) and of the fields (2 cells)
     if ((double)P->cfg.batch * 3.0 * e->nx_full * e->ny_full > 2.0e9) return EPSGRAD_EUNSUPPORTED;
-    if (P->slab_nx > 0) return EPSGRAD_EUNSUPPORTED;                        // one addressing option at a time
+    if (P->slab_nx > 0 || P->packed_fields) return EPSGRAD_EUNSUPPORTED;   // one addressing option at a time
     P->emb = *e;
     return EPSGRAD_OK;
 }
@@ -583,7 +584,7 @@ extern "C" int epsgrad_plan_set_slab(epsgrad_plan_t *P, int x_first, int x_count
     if (!P) return EPSGRAD_EINVAL;
     if (x_first == 0 && x_count == 0) { P->slab_x0 = P->slab_nx = 0; return EPSGRAD_OK; }
     if (x_first < 0 || x_count < 1 || x_first + x_count > P->nx) return EPSGRAD_EINVAL;
-    if (P->emb.nx_full > 0 || P->general) return EPSGRAD_EUNSUPPORTED;         // one addressing option at a time; slabs are cut along control rows
+    if (P->emb.nx_full > 0 || P->general || P->packed_fields) return EPSGRAD_EUNSUPPORTED;   // one addressing option at a time; slabs are cut along control rows
     P->slab_x0 = x_first; P->slab_nx = x_count;
     return EPSGRAD_OK;
 }

@@ -444,3 +444,58 @@ def test_tensor_core_filter_matches_the_oracle(kw, beta):
     with pytest.raises(B.EpsgradError) as e:                      # the Gaussian filter is separable: no banded matrices for it
         B.Plan(B.make_config(mx=16, my=16, nz=8, z_lo=2.0, z_hi=5.0, filter_kind=1, filter_radius=6.0, filter_sigma=2.0)).set_tensor_cores(1)
     assert e.value.status == B.EUNSUPPORTED
+
+
+@pytest.mark.parametrize("kw,beta,n_pairs", [
+    (dict(mx=33, my=21, nz=64, z_lo=28.25, z_hi=35.75, filter_radius=8.0), 16.0, 2),          # the paper's slab: cells 26..35 of 64
+    (dict(batch=2, mx=17, my=40, nz=32, z_lo=14.25, z_hi=17.75, filter_kind=1, filter_radius=6.0, filter_sigma=2.0), 8.0, 1),   # Wide batch's slab
+    (dict(mx=12, my=12, nz=16, z_lo=0.0, z_hi=16.0, filter_radius=4.0), 8.0, 3),                 # the slab is the whole column
+    (dict(mx=20, my=9, nz=24, z_lo=3.5, z_hi=4.25, filter_radius=4.0), 32.0, 9),                # a slab inside one cell; more than 8 pairs
+])
+def test_packed_fields_give_the_same_gradient(kw, beta, n_pairs):
+    """epsgrad_plan_set_packed_fields: E_F / E_A restricted to the z cells of the slab window (fields on Omega_D only)
+    give bit for bit the dF/dC of full columns, through every entry point that reads fields; what lies outside the window
+    never mattered (NaNs there change nothing); options that address the fields differently are refused."""
+    cfg = B.make_config(**kw)
+    C = rand_C(cfg, 31)
+    EF, EA = rand_fields(cfg, n_pairs, 32)
+    plan = B.Plan(cfg)
+    full = lambda fs: [dev(f) for f in fs]
+    g0 = plan.eps_vjp(dev(C), beta, full(EF), full(EA)).clone()
+    gb0, db0 = plan.eps_vjp_beta(dev(C), beta, full(EF), full(EA))
+    gb0, db0 = gb0.clone(), db0.clone()
+    z0 = plan.stage_zreduce(full(EF), full(EA)).clone()
+    check_vjp(cfg, C, beta, EF, EA, plan)
+    k0, n = plan.packed_window()
+    assert 0 <= k0 and k0 + n <= cfg.nz and k0 % 2 == 0 and n % 2 == 0
+    assert k0 <= int(np.floor(kw["z_lo"])) and k0 + n >= min(cfg.nz, int(np.ceil(kw["z_hi"]))), (k0, n)     # the window holds the slab
+    # full columns with NaNs outside the window: same bits
+    def poisoned(fs):
+        out = []
+        for f in fs:
+            t = dev(f).clone()
+            v = torch.view_as_real(t)
+            v[..., :k0, :] = float("nan")
+            v[..., k0 + n:, :] = float("nan")
+            out.append(t)
+        return out
+    assert torch.equal(plan.eps_vjp(dev(C), beta, poisoned(EF), poisoned(EA)), g0)
+    plan.set_packed_fields(True)
+    pack = lambda fs: [dev(f)[..., k0:k0 + n].contiguous() for f in fs]
+    assert torch.equal(plan.eps_vjp(dev(C), beta, pack(EF), pack(EA)), g0)
+    eps1, g1 = plan.eps_forward_vjp(dev(C), beta, pack(EF), pack(EA))
+    assert torch.equal(g1, g0) and tuple(eps1.shape) == plan.eps_shape
+    gb1, db1 = plan.eps_vjp_beta(dev(C), beta, pack(EF), pack(EA))
+    assert torch.equal(gb1, gb0) and torch.equal(db1, db0)
+    assert torch.equal(plan.stage_zreduce(pack(EF), pack(EA)), z0)
+    for call in (lambda: plan.set_embedding(cfg.nx + 8, cfg.ny + 8, cfg.nz, 4, 4, 0), lambda: plan.set_slab(0, cfg.nx // 2),
+                 lambda: plan.set_dense_reads(True)):
+        with pytest.raises(B.EpsgradError) as e:
+            call()
+        assert e.value.status == B.EUNSUPPORTED
+    plan.set_packed_fields(False)
+    assert torch.equal(plan.eps_vjp(dev(C), beta, full(EF), full(EA)), g0)
+    plan.set_dense_reads(True)
+    with pytest.raises(B.EpsgradError) as e:
+        plan.set_packed_fields(True)
+    assert e.value.status == B.EUNSUPPORTED
