@@ -179,6 +179,19 @@ int eps_vjp_beta(epsgrad_plan_t *plan, const float *C, float beta, int n_pairs,
  * (S20): the mean over the design mask of 4 rho (1 - rho), rho the final projected mask; u: DEVICE array of B floats.   */
 int eps_unbinarity(epsgrad_plan_t *plan, const float *C, float beta, float *u, void *stream);
 
+/* The same u(beta) for callers that may not allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): of a mask the caller already holds -- phi: DEVICE array [B, s Nx, s Ny], the centred filter output
+ * (what epsgrad_stage_filter writes) -- with the partial sums of the two-stage reduction in a file-scope device array of the
+ * library instead of the plan's workspace.  The call needs no workspace and calls no cudaMalloc / cudaFree / allocating
+ * library routine: two kernel launches on `stream`.  Bitwise the same u as eps_unbinarity (same sums in the same order).
+ * LIMIT: the array holds epsgrad_static_scratch_partials() = 4096 floats (16 KB, resident on every GPU that loads the library
+ * until exit): B * ceil(s Nx * s Ny / 4096) must not exceed it (16.7 M mask pixels in all; paper scale uses 245), else
+ * EPSGRAD_EUNSUPPORTED -- as with the morphological filters on (the last projection's input is then not the filter output).
+ * Every call, whatever its plan or stream, SHARES the array: a call writes every slot before it reads it, so what an earlier
+ * call left does not matter, but calls that overlap on the GPU (different streams) race -- serialise them.              */
+int eps_unbinarity_static(const epsgrad_plan_t *plan, const float *phi, float beta, float *u, void *stream);
+int epsgrad_static_scratch_partials(void);
+
 /* The paper's update rule for the projection strength (host scalars).  Eq. (14), P:L150:
  *   beta_i = beta_min + (beta_max - beta_min) (exp((i/N)^2) - 1)/(e - 1);
  * Eq. (15), moving averages with decay gamma that steer beta_max so that u reaches u0 at the last iteration:

@@ -21,6 +21,7 @@ EXPORTS = (
     "epsgrad_plan_set_dense_reads", "epsgrad_plan_last_launches", "epsgrad_plan_last_copy_bytes",
     "epsgrad_plan_set_profiling", "epsgrad_plan_last_kernel_times", "epsgrad_plan_set_overlap", "epsgrad_plan_set_host_direct", "epsgrad_plan_set_embedding", "epsgrad_plan_set_slab", "epsgrad_plan_set_packed_fields", "epsgrad_plan_packed_window", "epsgrad_plan_set_tma", "epsgrad_plan_set_bulk_stores", "epsgrad_plan_set_pdl", "epsgrad_plan_set_tensor_cores", "epsgrad_plan_set_tuning", "epsgrad_plan_set_fused", "epsgrad_plan_fused_profile", "epsgrad_plan_set_timeline", "epsgrad_plan_read_timeline", 
     "eps_forward", "eps_vjp", "eps_forward_vjp", "eps_forward_vjp_host", "eps_vjp_beta", "eps_unbinarity",
+    "eps_unbinarity_static", "epsgrad_static_scratch_partials",
     "epsgrad_beta_schedule", "epsgrad_beta_update", "epsgrad_adam_step",
     "epsgrad_soap_accumulate", "epsgrad_soap_eigh_workspace_bytes", "epsgrad_soap_eigh", "epsgrad_soap_eigh_info",
     "epsgrad_soap_step_workspace_bytes", "epsgrad_soap_step",
@@ -238,6 +239,8 @@ def lib() -> ctypes.CDLL:
     L.epsgrad_plan_set_timeline.argtypes = [vp, i32]
     L.epsgrad_plan_read_timeline.argtypes = [vp, i32, vp, vp]
     L.epsgrad_stage_zreduce.argtypes = [vp, i32, vp, vp, vp, vp]
+    L.eps_unbinarity_static.argtypes = [vp, vp, ctypes.c_float, vp, vp]
+    L.epsgrad_static_scratch_partials.restype = i32
     L.epsgrad_status_string.argtypes = [i32]
     L.epsgrad_status_string.restype = ctypes.c_char_p
     L.epsgrad_version.restype = i32
@@ -453,6 +456,20 @@ class Plan:
         _check(lib().eps_vjp_beta(self._h, self._c(C).data_ptr(), beta, len(EF), pf, pa, g.data_ptr(), db.data_ptr(),
                                   self._stream()), "eps_vjp_beta")
         return g, db
+
+    def unbinarity_static(self, phi, beta: float, out=None):
+        """u(beta) [B] of a centred filter output the caller holds (stage_filter), partial sums in the library's static device
+        array: no workspace, no allocation inside the call (`out` given).  Limit: B * ceil(mask pixels / 4096) <= 4096."""
+        t = self._torch
+        assert phi.is_cuda and phi.dtype == t.float32 and phi.is_contiguous() and tuple(phi.shape) == self.mask_shape, (phi.shape, self.mask_shape)
+        u = out if out is not None else t.empty(self.ctrl_shape[0], dtype=t.float32, device=self.device)
+        assert u.is_cuda and u.dtype == t.float32 and u.is_contiguous() and u.numel() == self.ctrl_shape[0]
+        rc = lib().eps_unbinarity_static(self._h, phi.data_ptr(), beta, u.data_ptr(), self._stream())
+        if rc == EUNSUPPORTED:
+            raise EpsgradError(rc, "eps_unbinarity_static (morphological filters on, or B * ceil(mask pixels / 4096) exceeds the static "
+                                   f"scratch of {lib().epsgrad_static_scratch_partials()} partial sums)")
+        _check(rc, "eps_unbinarity_static")
+        return u
 
     def unbinarity(self, C, beta: float):
         """u(beta) [B]: mean over the design mask of 4 rho (1 - rho) (S20)"""

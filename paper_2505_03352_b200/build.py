@@ -50,7 +50,7 @@ def nvcc_path() -> str:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    """Compile the translation units of csrc/ (plan.cu, launch.cu, hostpath.cu, optimizer.cu) into libepsgrad.so; returns its path."""
+    """Compile the translation units of csrc/ (plan.cu, launch.cu, hostpath.cu, optimizer.cu, noalloc.cu) into libepsgrad.so; returns its path."""
     if not force and not stale():
         return LIB
     tmp = LIB + f".tmp{os.getpid()}"
