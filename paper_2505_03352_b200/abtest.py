@@ -101,8 +101,8 @@ def streams(args):
     steps = 100 if c.w.cells < 1e8 else 10
     c.reset()
     e0, g0 = c.result()
-    # (name, bulk stores, TMA mode, tuning knobs): knob 0 bulk bytes, 1 store CTAs / SM, 2 ring stages, 3 read CTAs / SM
-    variants = [("base", 0, 0, ()), ("bulk stores", 1, 0, ()), ("bulk 32 KB", 1, 0, ((0, 32768),)), ("bulk 3 CTAs/SM", 1, 0, ((1, 3),)),
+    # (name, bulk stores, TMA mode, tuning knobs): knob 0 bulk bytes, 1 store CTAs / SM, 2 ring stages, 3 read CTAs / SM, 5 fill policy
+    variants = [("base", 0, 0, ()), ("field fills without the evict-first policy", 0, 0, ((5, 2),)), ("bulk stores", 1, 0, ()), ("bulk 32 KB", 1, 0, ((0, 32768),)), ("bulk 3 CTAs/SM", 1, 0, ((1, 3),)),
                 ("TMA ring", 0, 2, ()), ("TMA ring 4 stages", 0, 2, ((2, 4),)), ("TMA ring 4 stages 2 CTAs/SM", 0, 2, ((2, 4), (3, 2))),
                 ("TMA per block", 0, 1, ()), ("bulk + TMA ring", 1, 2, ())]
     for name, bulk, tma, tune in variants:

@@ -15,6 +15,30 @@
 
 namespace epsgrad {
 
+// the eps store: 16 bytes, streaming (st.global.cs).  EPSGRAD_EPS_STORE selects the alternatives that were timed against it
+// (DESIGN.md 5.6): 1 = .cg, 2 = .wt (write-through), 3 = L2 evict-first policy, 4 = L2 evict-last policy.
+#ifndef EPSGRAD_EPS_STORE
+#define EPSGRAD_EPS_STORE 0
+#endif
+__device__ __forceinline__ void st_eps(float4 *p, const float4 v)
+{
+#if EPSGRAD_EPS_STORE == 0
+    __stcs(p, v);
+#elif EPSGRAD_EPS_STORE == 1
+    __stcg(p, v);
+#elif EPSGRAD_EPS_STORE == 2
+    __stwt(p, v);
+#else
+    unsigned long long pol;
+#if EPSGRAD_EPS_STORE == 3
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+#else
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+#endif
+    asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1, %2, %3, %4}, %5;" :: "l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w), "l"(pol) : "memory");
+#endif
+}
+
 constexpr int EX_THREADS = 256, EX_PASSES = 16, EX_CTAS_PER_SM = 8;
 
 struct ExtrudeParams {
@@ -65,12 +89,12 @@ __device__ __forceinline__ void block_extrude(const ExtrudeParams &P, int c, int
 #pragma unroll
                 for (int pass = 0; pass < EX_PASSES; ++pass) {
                     const float v = vp[pass * cpp];
-                    __stcs(dst + pass * stride, make_float4(fmaf(wx[0], v, bx[0]), fmaf(wx[1], v, bx[1]), fmaf(wx[2], v, bx[2]), fmaf(wx[3], v, bx[3])));
+                    st_eps(dst + pass * stride, make_float4(fmaf(wx[0], v, bx[0]), fmaf(wx[1], v, bx[1]), fmaf(wx[2], v, bx[2]), fmaf(wx[3], v, bx[3])));
                 }
             } else {
                 for (int lc = cq; lc < ncb; lc += cpp, dst += stride) {
                     const float v = vsm[lc];
-                    __stcs(dst, make_float4(fmaf(wx[0], v, bx[0]), fmaf(wx[1], v, bx[1]), fmaf(wx[2], v, bx[2]), fmaf(wx[3], v, bx[3])));
+                    st_eps(dst, make_float4(fmaf(wx[0], v, bx[0]), fmaf(wx[1], v, bx[1]), fmaf(wx[2], v, bx[2]), fmaf(wx[3], v, bx[3])));
                 }
             }
         } else {
@@ -88,7 +112,7 @@ __device__ __forceinline__ void block_extrude(const ExtrudeParams &P, int c, int
                 o.y = fmaf(zf[1], v, fmaf(zl[1], vl, fmaf(zh[1], vh, bz[1])));
                 o.z = fmaf(zf[2], v, fmaf(zl[2], vl, fmaf(zh[2], vh, bz[2])));
                 o.w = fmaf(zf[3], v, fmaf(zl[3], vl, fmaf(zh[3], vh, bz[3])));
-                __stcs(dst, o);
+                st_eps(dst, o);
             }
         }
     } else if (P.sh4 >= 0) {
@@ -107,7 +131,7 @@ __device__ __forceinline__ void block_extrude(const ExtrudeParams &P, int c, int
                     float4 o;
                     o.x = fmaf(wx[0], v, bx[0]); o.y = fmaf(wx[1], v, bx[1]);
                     o.z = fmaf(wx[2], v, bx[2]); o.w = fmaf(wx[3], v, bx[3]);
-                    __stcs(dst + P.cm.col(col0 + lc), o);
+                    st_eps(dst + P.cm.col(col0 + lc), o);
                 }
             }
         } else {
@@ -128,7 +152,7 @@ __device__ __forceinline__ void block_extrude(const ExtrudeParams &P, int c, int
                     o.y = fmaf(zf[1], v, fmaf(zl[1], vl, fmaf(zh[1], vh, bz[1])));
                     o.z = fmaf(zf[2], v, fmaf(zl[2], vl, fmaf(zh[2], vh, bz[2])));
                     o.w = fmaf(zf[3], v, fmaf(zl[3], vl, fmaf(zh[3], vh, bz[3])));
-                    __stcs(dst + P.cm.col(col0 + lc), o);
+                    st_eps(dst + P.cm.col(col0 + lc), o);
                 }
             }
         }
@@ -144,7 +168,7 @@ __device__ __forceinline__ void block_extrude(const ExtrudeParams &P, int c, int
             for (int x = 0; x < 4; ++x)
                 o[x] = c < 2 ? fmaf(w_xy[k + x], v, b_xy[k + x])
                              : fmaf(i_f[k + x], v, fmaf(i_l[k + x], vsm[cpb + lc], fmaf(i_h[k + x], vsm[2 * cpb + lc], b_z[k + x])));
-            __stcs(out + P.cm.col(col0 + lc) + (k >> 2), make_float4(o[0], o[1], o[2], o[3]));
+            st_eps(out + P.cm.col(col0 + lc) + (k >> 2), make_float4(o[0], o[1], o[2], o[3]));
         }
     }
 }

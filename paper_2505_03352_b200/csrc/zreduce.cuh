@@ -36,6 +36,8 @@ struct ZredParams {
     ColumnMap cm;          // where the columns sit in E_F / E_A (16-byte pieces = 2 cells)
     int ncp[2];            // columns staged per pass (<= ZR_COLS): ncp (nch | 1) <= ZR_STAGE_CHUNKS
     int choff;             // chunk the stored columns start at: 0, or the first chunk of the union window for packed fields
+    int evict_first;       // field fills carry an L2 evict-first policy: they recycle each other's lines instead of pushing out the
+                           // dirty eps lines of the step before
 };
 
 __host__ __device__ inline int zred_cols_per_pass(int nch, int max_cols = ZR_COLS, int stage_chunks = ZR_STAGE_CHUNKS)
@@ -46,10 +48,22 @@ __host__ __device__ inline int zred_cols_per_pass(int nch, int max_cols = ZR_COL
 }
 
 // 16-byte asynchronous copy global -> shared (LDGSTS): completion by cp.async groups.
+__device__ __forceinline__ unsigned long long policy_evict_first()
+{
+    unsigned long long pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+// pol: 0, or an L2 cache policy (createpolicy) for the fill
 template <bool SPARSE>
-__device__ __forceinline__ void cp_async16(float4 *smem, const float4 *g)
+__device__ __forceinline__ void cp_async16(float4 *smem, const float4 *g, unsigned long long pol = 0)
 {
     const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+    if (pol) {
+        if (SPARSE) asm volatile("cp.async.cg.shared.global.L2::cache_hint.L2::64B [%0], [%1], 16, %2;" :: "r"(sa), "l"(g), "l"(pol) : "memory");
+        else asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;" :: "r"(sa), "l"(g), "l"(pol) : "memory");
+        return;
+    }
     if (SPARSE) asm volatile("cp.async.cg.shared.global.L2::64B [%0], [%1], 16;" :: "r"(sa), "l"(g) : "memory");
     else asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(sa), "l"(g) : "memory");
 }
@@ -69,6 +83,7 @@ __device__ __forceinline__ void zwindow_issue(const ZredParams &P, float4 *buf, 
 {
     const int grp = c == 2, nch = P.nch[grp], sh = P.chs[grp], ncp = P.ncp[grp];
     const int ch = threadIdx.x & ((1 << sh) - 1), lstep = ZR_THREADS >> sh;
+    const unsigned long long pol = P.evict_first ? policy_evict_first() : 0ull;
     if (ch < nch) {
         const size_t first = P.cm.plane(b, c) + (P.ch0[grp] - P.choff) + ch;
         const float4 *pf = P.ef[p] + first, *pa = P.ea[p] + first;
@@ -96,14 +111,14 @@ __device__ __forceinline__ void zwindow_issue(const ZredParams &P, float4 *buf, 
                 pf += o0; pa += o0; df += lc0 * pitch; da += lc0 * pitch;
                 const int sstep = lstep * pitch;
                 for (int lc = lc0; lc < nc; lc += lstep, pf += ostep, pa += ostep, df += sstep, da += sstep) {
-                    cp_async16<SPARSE>(df, pf);
-                    cp_async16<SPARSE>(da, pa);
+                    cp_async16<SPARSE>(df, pf, pol);
+                    cp_async16<SPARSE>(da, pa, pol);
                 }
             } else {
                 for (int lc = threadIdx.x >> sh; lc < nc; lc += lstep) {
                     const size_t o = P.cm.col(col0 + lc);
-                    cp_async16<SPARSE>(df + lc * pitch, pf + o);
-                    cp_async16<SPARSE>(da + lc * pitch, pa + o);
+                    cp_async16<SPARSE>(df + lc * pitch, pf + o, pol);
+                    cp_async16<SPARSE>(da + lc * pitch, pa + o, pol);
                 }
             }
         }

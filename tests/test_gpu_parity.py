@@ -110,8 +110,11 @@ def test_tma_field_reads_give_the_same_bits():
         g0, G0 = plan.eps_vjp(C, 16.0, EF, EA), plan.stage_zreduce(EF, EA)
         plan.set_tma(True)
         g1, G1 = plan.eps_vjp(C, 16.0, EF, EA), plan.stage_zreduce(EF, EA)
+        plan.set_tma(False)
+        plan.set_tuning(5, 2)                                     # field fills without the evict-first L2 policy (the default has it)
+        g2, G2 = plan.eps_vjp(C, 16.0, EF, EA), plan.stage_zreduce(EF, EA)
         torch.cuda.synchronize()
-        assert torch.equal(G0, G1) and torch.equal(g0, g1)
+        assert torch.equal(G0, G1) and torch.equal(g0, g1) and torch.equal(G0, G2) and torch.equal(g0, g2)
 
 
 def test_dense_reads_give_the_same_gradient():
