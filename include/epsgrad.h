@@ -330,7 +330,7 @@ int epsgrad_plan_set_fused(epsgrad_plan_t *plan, int enable);
 int epsgrad_plan_fused_profile(epsgrad_plan_t *plan, int enable, uint64_t *out20);
 
 /* Measurement knobs of the two stream kernels (0 = the default of each): knob 0 = bytes per bulk store, 1 = store-stream
- * CTAs per SM, 2 = stages of the read stream's ring, 3 = read-stream CTAs per SM; 4 = CTAs per SM of the persistent kernel, 6 = pipeline lag (steps) between a phase of the persistent kernel and its consumer; 5 = L2 policy of the field fills (0, 1: evict-first, the default; 2: none); 7 = force streamed tensor-core weights.  EPSGRAD_EINVAL for a
+ * CTAs per SM, 2 = stages of the read stream's ring, 3 = read-stream CTAs per SM; 4 = CTAs per SM of the persistent kernel, 6 = pipeline lag (steps) between a phase of the persistent kernel and its consumer; 5 = L2 evict-first policy of the field fills (0: on for field arrays up to 4 GB per launch, the default; 1: always; 2: never); 7 = force streamed tensor-core weights.  EPSGRAD_EINVAL for a
  * knob outside 0..7.  Values are clamped to what the kernels support; results never depend on them.                      */
 int epsgrad_plan_set_tuning(epsgrad_plan_t *plan, int knob, int value);
 

@@ -476,7 +476,7 @@ int fill_zreduce(const epsgrad_plan *P, float *gbar, bool packed, ZredParams &zp
                  int max_cols = ZR_COLS, int stage_chunks = ZR_STAGE_CHUNKS)
 {
     zp.gbar = gbar; zp.zw = P->d_zw; zp.ncol = P->nx * P->ny; zp.nz = P->cfg.nz;
-    zp.evict_first = P->tune[5] != 2;      // default on: 104 -> 98 us per step at paper scale, neutral at Large
+    zp.evict_first = P->tune[5] == 1;      // the launch decides for knob value 0 (launch_zreduce)
     zp.pstride = zp.ncol;
     if (P->slab_nx > 0) {
         zp.ncol = P->slab_nx * P->ny;
@@ -561,6 +561,11 @@ int launch_zreduce(epsgrad_plan *P, int n_pairs, const void *const *EF, const vo
     }
     int rcf = fill_zreduce(P, gbar, packed, zp, smem, sparse, maxnch);
     if (rcf) return rcf;
+    // L2 evict-first fills: they keep the field stream from pushing the previous step's dirty eps lines (at most
+    // one L2 of them) out under itself -- 104 -> 96 us per step at paper scale.  That cost is fixed, so it only matters for
+    // streams of a few L2 sizes; on the multi-GB streams of Large / Wide batch the policy costs ~1 % instead, so by default it
+    // is on up to 4 GB of field columns per launch (knob 5: 1 always, 2 never).
+    if (P->tune[5] == 0) zp.evict_first = (double)P->cfg.batch * 3.0 * zp.ncol * zp.nz * 16.0 * std::min(n_pairs, ZR_MAX_PAIRS) <= 4.0e9;
     host_src = host_src || P->cur_host_src;
     if (!host_src && !packed && P->use_tma == 2 && P->tma_encode && P->emb.nx_full == 0 && maxnch <= 24) {
         // thin persistent read stream (zreduce_pipe.cuh): TMA boxes {window, ZP_COLS columns} through a ring of stages
