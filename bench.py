@@ -448,6 +448,21 @@ def run_ours(args, w):
     z_clean_ms = z_alone(False)
     z_alone_ms = z_alone(True)
 
+    # ---- where the kernels END inside the OVERLAPPED schedule (the per-kernel times above come from the serial one): timeline
+    # stamps of the library's hook (a one-thread kernel writing %globaltimer after each kernel, on the stream it ran on), median
+    # over a few eager steps, us since the step's first stamp
+    plan.set_timeline(True)
+    tls = []
+    for i in range(8):
+        plan.eps_forward_vjp(C, w.betas[-1], EF[i % NS], EA[i % NS], eps, grad)
+        tl = plan.read_timeline()
+        if i >= 3:
+            tls.append(tl)
+    plan.set_timeline(False)
+    timeline = None
+    if tls and all(len(t) == len(tls[0]) for t in tls):
+        timeline = [[tls[0][k][0], sorted(t[k][1] for t in tls)[len(tls) // 2] / 1e3] for k in range(len(tls[0]))]
+
     # ---- the same step with the fields given on the design region only (epsgrad_plan_set_packed_fields: E_F / E_A hold the z
     # cells of the slab window, "restricted to Omega_D"): NOT the BASELINE layout, reported beside the headline only
     packed = None
@@ -512,6 +527,8 @@ def run_ours(args, w):
                 "step": {"algorithmic_bytes": step_bytes, "ms": step_ms, "GB/s": step_bytes / (step_ms * 1e-3) / 1e9,
                          "frac": step_bytes / (step_ms * 1e-3) / 1e9 / peak,
                          "note": "eps stores + touched field sectors over the whole overlapped step (2-D chain included)"},
+                "timeline_us": timeline,
+                "timeline": "end of each kernel inside the overlapped two-stream schedule (eager calls, stamps on the kernels' own streams)",
                 "packed_fields": packed,
                 "modes_frac": {"forward": alg["extrude"] * len(w.betas) / (modes["forward"]["ms_median"] * 1e-3) / 1e9 / peak,
                                "vjp": alg["zreduce"] * len(w.betas) / (modes["vjp"]["ms_median"] * 1e-3) / 1e9 / peak,

@@ -49,6 +49,9 @@ def test_bench_line_has_the_contract_keys():
     assert r["frac_dense_equiv"]["value"] > r["others"].get("zreduce", r)["frac"] and "not the method's work" in r["frac_dense_equiv"]["note"]
     assert 0.05 < r["zreduce_alone"]["frac"] < 1.0 and 0.05 < r["step"]["frac"] < 1.0
     assert set(r["modes_frac"]) == {"forward", "vjp", "vjp_dense_equiv"} and "traffic_source" in r
+    tl = r["timeline_us"]                         # kernel ends inside the overlapped schedule
+    assert [n for n, _ in tl][0] == "begin" and {n for n, _ in tl} >= {"filter", "fwd2d", "zreduce", "extrude", "maskgrad", "filterT"}
+    assert all(0.0 <= t < 1e4 for _, t in tl)
     pk = r["packed_fields"]                       # the same step with the fields on the design region only: beside the headline, not it
     assert pk["window_cells"][1] > 0 and pk["bytes_read"] > 0 and "not the headline" in pk["note"]
     assert 0 < pk["zreduce_alone_ms"] <= r["zreduce_alone"]["kernel_ms"] * 1.5 and 0 < pk["forward_vjp_ms_median"] and 0 < pk["zreduce_in_step_frac"] < 1.2
