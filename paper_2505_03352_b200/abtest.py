@@ -5,6 +5,7 @@ is faster on THIS size.  Every variant computes the same path; the switches are 
     python -m paper_2505_03352_b200.abtest pdl [workload ...]     # programmatic dependent launch on / off
     python -m paper_2505_03352_b200.abtest fused [workload]       # separate kernels / one persistent dataflow kernel / 2-D chains only
     python -m paper_2505_03352_b200.abtest tc [mx:R ...]          # FFMA stencils against the tensor-core filters (+ cycle accounting)
+    python -m paper_2505_03352_b200.abtest replay [workload] [knob=value ...]   # graph replays of the step: a target for ncu
 
 One JSON line per variant: step time of a replayed CUDA graph (us, mean of `steps` replays over rotating field sets), the
 event-timed kernels of the serial schedule, and whether the results equal the baseline's bit for bit (or how far they are).
@@ -189,9 +190,21 @@ def tc(args):
         torch.cuda.empty_cache()
 
 
+def replay(args):
+    """replays CUDA graphs of eps_forward_vjp (3 rotating field sets, 9 replays) with the given tuning knobs: a target for
+    `ncu --graph-profiling node --cache-control none`, which then sees every kernel with the L2 state its predecessors left"""
+    c = _Case(W.BY_NAME[args[0] if args else "paper"])
+    c.reset()
+    for kv in args[1:]:
+        k, v = kv.split("=")
+        c.plan.set_tuning(int(k), int(v))
+    print(json.dumps({"workload": c.w.name, "tuning": args[1:], "step_us": c._replay_us(
+        lambda s: c.plan.eps_forward_vjp(c.C, c.beta, c.EF[s], c.EA[s], c.eps, c.g), 9)}), flush=True)
+
+
 def main(argv=None):
     argv = list(sys.argv[1:] if argv is None else argv)
-    table = {"streams": streams, "pdl": pdl, "fused": fused, "tc": tc}
+    table = {"streams": streams, "pdl": pdl, "fused": fused, "tc": tc, "replay": replay}
     if not argv or argv[0] not in table:
         print(__doc__)
         return 2
