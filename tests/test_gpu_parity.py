@@ -454,6 +454,8 @@ def test_tensor_core_filter_matches_the_oracle(kw, beta):
     (dict(batch=2, mx=17, my=40, nz=32, z_lo=14.25, z_hi=17.75, filter_kind=1, filter_radius=6.0, filter_sigma=2.0), 8.0, 1),   # Wide batch's slab
     (dict(mx=12, my=12, nz=16, z_lo=0.0, z_hi=16.0, filter_radius=4.0), 8.0, 3),                 # the slab is the whole column
     (dict(mx=20, my=9, nz=24, z_lo=3.5, z_hi=4.25, filter_radius=4.0), 32.0, 9),                # a slab inside one cell; more than 8 pairs
+    (dict(mx=12, my=14, nx_cells=70, ny_cells=81, nz=64, z_lo=28.25, z_hi=35.75, filter_radius=8.0), 16.0, 2),   # Fig. 4's 5.8 cells per control pixel
+    (dict(batch=2, mx=24, my=20, nz=32, z_lo=14.25, z_hi=17.75, filter_radius=6.0, morph_diameter=3.0), 12.0, 1),  # morphological filters on
 ])
 def test_packed_fields_give_the_same_gradient(kw, beta, n_pairs):
     """epsgrad_plan_set_packed_fields: E_F / E_A restricted to the z cells of the slab window (fields on Omega_D only)
