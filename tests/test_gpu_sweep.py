@@ -185,6 +185,25 @@ def test_random_configuration_every_entry_point(i):
     plan.set_dense_reads(True)
     assert torch.equal(plan.eps_vjp(C, beta, EF, EA), g0)
     plan.set_dense_reads(False)
+    # field fills with the L2 evict-first policy forced on / off (by default the size of the launch decides): a cache hint only
+    for knob in (1, 2):
+        plan.set_tuning(5, knob)
+        assert torch.equal(plan.stage_zreduce(EF, EA), G0) and torch.equal(plan.eps_vjp(C, beta, EF, EA), g0), (kw, knob)
+    plan.set_tuning(5, 0)
+    # fields on the design region only: the slab window of every z column, packed (where the layout applies)
+    try:
+        plan.set_packed_fields(True)
+        packed = True
+    except B.EpsgradError as err:
+        assert err.status == B.EUNSUPPORTED
+        packed = False
+    if packed:
+        k0, nk = plan.packed_window()
+        pEF = [f[..., k0:k0 + nk].contiguous() for f in EF]
+        pEA = [f[..., k0:k0 + nk].contiguous() for f in EA]
+        plan._ws.fill_(255)
+        assert torch.equal(plan.stage_zreduce(pEF, pEA), G0) and torch.equal(plan.eps_vjp(C, beta, pEF, pEA), g0), kw
+        plan.set_packed_fields(False)
     # CUDA graph replay of the fused call
     eps_g, g_g = torch.empty_like(eps0), torch.empty_like(g0)
     s = torch.cuda.Stream()
