@@ -279,6 +279,16 @@ int epsgrad_plan_set_slab(epsgrad_plan_t *plan, int x_first, int x_count);
  * full columns: bitwise the same dFdC.  eps is unaffected (full columns).  EPSGRAD_EUNSUPPORTED together with an embedding, an
  * x-slab, dense reads or nz % 4 != 0, and in the *_host entry point (which gathers the windows itself).                      */
 int epsgrad_plan_set_packed_fields(epsgrad_plan_t *plan, int enable);
+
+/* eps on the design region only (the layout is extruded to the device layer; every cell of a z column outside the slab
+ * is eps_clad whatever C and beta are).  After epsgrad_plan_set_eps_window_only(plan, 1) the DEVICE entry points rewrite only
+ * the z cells of every column that depend on the design -- the union of the slab windows of the three components, rounded
+ * outwards to whole 32-byte sectors (paper scale: cells 24..39 of 64) -- and touch nothing else of `eps`.  The caller's eps
+ * array must therefore already hold the result of ONE earlier full call (enable = 0) of the same plan geometry: a design loop
+ * makes its first eps_forward a full one and every later one a window one (48 instead of 192 MB stored per call at paper
+ * scale).  Inside the window the bits are those of the full call.  EPSGRAD_EUNSUPPORTED when nz % 4 != 0 and in the *_host
+ * entry point (its eps buffer is written whole).  Works with an embedding and with x-slabs.                              */
+int epsgrad_plan_set_eps_window_only(epsgrad_plan_t *plan, int enable);
 int epsgrad_plan_packed_window(const epsgrad_plan_t *plan, int *first_cell, int *n_cells);
 
 /* How the device-resident field windows are fetched.  0: by 16-byte asynchronous copies (LDGSTS), 5 CTAs per SM.

@@ -19,7 +19,7 @@ EXPORTS = (
     "epsgrad_plan_create", "epsgrad_plan_destroy", "epsgrad_workspace_bytes",
     "epsgrad_plan_set_workspace", "epsgrad_staging_bytes", "epsgrad_plan_set_staging",
     "epsgrad_plan_set_dense_reads", "epsgrad_plan_last_launches", "epsgrad_plan_last_copy_bytes",
-    "epsgrad_plan_set_profiling", "epsgrad_plan_last_kernel_times", "epsgrad_plan_set_overlap", "epsgrad_plan_set_host_direct", "epsgrad_plan_set_embedding", "epsgrad_plan_set_slab", "epsgrad_plan_set_packed_fields", "epsgrad_plan_packed_window", "epsgrad_plan_set_tma", "epsgrad_plan_set_bulk_stores", "epsgrad_plan_set_pdl", "epsgrad_plan_set_tensor_cores", "epsgrad_plan_set_tuning", "epsgrad_plan_set_fused", "epsgrad_plan_fused_profile", "epsgrad_plan_set_timeline", "epsgrad_plan_read_timeline", 
+    "epsgrad_plan_set_profiling", "epsgrad_plan_last_kernel_times", "epsgrad_plan_set_overlap", "epsgrad_plan_set_host_direct", "epsgrad_plan_set_embedding", "epsgrad_plan_set_slab", "epsgrad_plan_set_packed_fields", "epsgrad_plan_packed_window", "epsgrad_plan_set_eps_window_only", "epsgrad_plan_set_tma", "epsgrad_plan_set_bulk_stores", "epsgrad_plan_set_pdl", "epsgrad_plan_set_tensor_cores", "epsgrad_plan_set_tuning", "epsgrad_plan_set_fused", "epsgrad_plan_fused_profile", "epsgrad_plan_set_timeline", "epsgrad_plan_read_timeline", 
     "eps_forward", "eps_vjp", "eps_forward_vjp", "eps_forward_vjp_host", "eps_vjp_beta", "eps_unbinarity",
     "eps_unbinarity_static", "epsgrad_static_scratch_partials",
     "epsgrad_beta_schedule", "epsgrad_beta_update", "epsgrad_adam_step",
@@ -229,6 +229,7 @@ def lib() -> ctypes.CDLL:
     L.epsgrad_plan_set_embedding.argtypes = [vp, vp]
     L.epsgrad_plan_set_tma.argtypes = [vp, i32]
     L.epsgrad_plan_set_packed_fields.argtypes = [vp, i32]
+    L.epsgrad_plan_set_eps_window_only.argtypes = [vp, i32]
     L.epsgrad_plan_packed_window.argtypes = [vp, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_int)]
     L.epsgrad_plan_set_bulk_stores.argtypes = [vp, i32]
     L.epsgrad_plan_set_pdl.argtypes = [vp, i32]
@@ -363,6 +364,11 @@ class Plan:
         """eps / E_F / E_A hold only Yee rows [x_first, x_first + x_count) of the region: [B,3,x_count,Ny,Nz]; (0, 0): off"""
         _check(lib().epsgrad_plan_set_slab(self._h, x_first, x_count), "epsgrad_plan_set_slab")
         self._field_shape = (self.eps_shape[0], 3, x_count, self.eps_shape[3], self.eps_shape[4]) if x_count > 0 else None
+
+    def set_eps_window_only(self, enable: bool) -> None:
+        """eps_forward / eps_forward_vjp rewrite only the z cells of `eps` that depend on the design (the slab window of every
+        column); the array must already hold the result of one full call"""
+        _check(lib().epsgrad_plan_set_eps_window_only(self._h, int(bool(enable))), "epsgrad_plan_set_eps_window_only")
 
     def set_packed_fields(self, enable: bool) -> None:
         """E_F / E_A as [B,3,Nx,Ny,n] complex64 holding only z cells packed_window() of every column (fields on Omega_D only)"""

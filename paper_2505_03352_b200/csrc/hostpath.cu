@@ -20,7 +20,7 @@ extern "C" int eps_forward_vjp_host(epsgrad_plan_t *P, const float *C_host, floa
         n_pairs = 0;
     }
     if (n_pairs > EPSGRAD_MAX_HOST_PAIRS) return EPSGRAD_EUNSUPPORTED;
-    if (P->emb.nx_full > 0 || P->slab_nx > 0 || P->packed_fields) return EPSGRAD_EUNSUPPORTED;     // host buffers are region-sized, full z columns: no embedding, slab or packed windows here
+    if (P->emb.nx_full > 0 || P->slab_nx > 0 || P->packed_fields || P->eps_window_only) return EPSGRAD_EUNSUPPORTED;     // host buffers are region-sized, full z columns: no embedding, slab or packed windows here
     if (!P->ws) return EPSGRAD_ENOWORKSPACE;
     if (!P->stg || P->stg_bytes < epsgrad_staging_bytes(P, n_pairs)) return EPSGRAD_ENOWORKSPACE;
     DeviceGuard g(P->device);

@@ -17,6 +17,7 @@
 #include "fwd2d.cuh"
 #include "extrude.cuh"
 #include "extrude_bulk.cuh"
+#include "extrude_window.cuh"
 #include "zreduce.cuh"
 #include "zreduce_pipe.cuh"
 #include "scalar3d.cuh"
@@ -410,6 +411,22 @@ int launch_extrude(epsgrad_plan *P, const float *e2d, float *eps, cudaStream_t s
         return check_launch(P, "extrude", st);
     }
     const ExtrudeParams ep = fill_extrude(P, e2d, eps);
+    if (P->eps_window_only) {
+        // only the z cells that depend on the design (extrude_window.cuh): the union of the slab windows, in whole 32-byte sectors
+        ExtrudeWindowParams wp;
+        wp.e = ep;
+        int lo = ep.nz, hi = -1;
+        for (int g = 0; g < 2; ++g)
+            if (P->nch[g] > 0) { lo = std::min(lo, 2 * P->ch0[g]); hi = std::max(hi, 2 * (P->ch0[g] + P->nch[g]) - 1); }
+        if (hi < lo) return EPSGRAD_OK;                          // no cell of any column depends on the design
+        const int nz4 = ep.nz / 4;
+        wp.q0 = (lo / 4) & ~1;
+        wp.nq = std::min(nz4, (std::min(hi, ep.nz - 1) / 4 + 2) & ~1) - wp.q0;
+        if ((double)ep.ncol * wp.nq > 2.0e9) return EPSGRAD_EUNSUPPORTED;
+        const unsigned nblk = (unsigned)(((size_t)ep.ncol * wp.nq + EW_THREADS - 1) / EW_THREADS);
+        launch_k(P, k_extrude_window, dim3(nblk, 3, P->cfg.batch), dim3(EW_THREADS), 0, st, wp);
+        return check_launch(P, "extrude", st);
+    }
     if (P->use_bulk && P->emb.nx_full == 0) {
         // thin persistent store stream (extrude_bulk.cuh): columns of a plane are one contiguous run
         ExtrudeBulkParams bp;
@@ -451,6 +468,14 @@ void window_union(const epsgrad_plan *P, int *first, int *count)
         if (P->nch[g] > 0) { lo = std::min(lo, P->ch0[g]); hi = std::max(hi, P->ch0[g] + P->nch[g]); }
     *first = hi > lo ? lo : 0;
     *count = hi > lo ? hi - lo : 0;
+}
+
+extern "C" int epsgrad_plan_set_eps_window_only(epsgrad_plan_t *P, int enable)
+{
+    if (!P) return EPSGRAD_EINVAL;
+    if (enable && P->cfg.nz % 4) return EPSGRAD_EUNSUPPORTED;
+    P->eps_window_only = enable != 0;
+    return EPSGRAD_OK;
 }
 
 extern "C" int epsgrad_plan_set_packed_fields(epsgrad_plan_t *P, int enable)
@@ -788,7 +813,7 @@ int check_pairs(int n_pairs, const void *const *EF, const void *const *EA)
 // ---- the whole step as one persistent dataflow kernel (mega.cuh)
 bool mega_applies(const epsgrad_plan *P, int n_pairs)
 {
-    return P->use_mega == 1 && P->d_sched && P->cfg.nz % 4 == 0 && !P->cur_dbeta && P->slab_nx == 0 && !P->packed_fields && !P->cur_host_src && !P->prof && n_pairs <= ZR_MAX_PAIRS;
+    return P->use_mega == 1 && P->d_sched && P->cfg.nz % 4 == 0 && !P->cur_dbeta && P->slab_nx == 0 && !P->packed_fields && !P->eps_window_only && !P->cur_host_src && !P->prof && n_pairs <= ZR_MAX_PAIRS;
 }
 
 template <int NTC>

@@ -44,6 +44,7 @@ struct epsgrad_plan {
     float *cur_dbeta;
     // embedding of the design region in the caller's simulation-domain arrays (epsgrad_plan_set_embedding); emb.nx_full = 0: none
     epsgrad_embedding_t emb;
+    int eps_window_only;       // eps_forward rewrites only the slab window of every z column (epsgrad_plan_set_eps_window_only)
     int packed_fields;         // device E_F / E_A hold only the union slab window of every z column (epsgrad_plan_set_packed_fields)
     int use_tma;               // field windows by TMA bulk tensor copies where possible (epsgrad_plan_set_tma): 1 single-stage, 2 pipelined
     int use_pdl;               // programmatic dependent launch between consecutive kernels of a stream (epsgrad_plan_set_pdl)

@@ -52,6 +52,9 @@ def test_bench_line_has_the_contract_keys():
     tl = r["timeline_us"]                         # kernel ends inside the overlapped schedule
     assert [n for n, _ in tl][0] == "begin" and {n for n, _ in tl} >= {"filter", "fwd2d", "zreduce", "extrude", "maskgrad", "filterT"}
     assert all(0.0 <= t < 1e4 for _, t in tl)
+    wn = r["eps_window_only"]                     # eps rewritten on the slab window only: also beside the headline
+    assert 0 < wn["forward_ms_median"] <= m["forward"]["ms_median"] * 1.05 and "not the headline" in wn["note"]
+    assert 0 < wn["with_packed_fields_forward_vjp_ms_median"] <= m["forward_vjp"]["ms_median"] * 1.05
     pk = r["packed_fields"]                       # the same step with the fields on the design region only: beside the headline, not it
     assert pk["window_cells"][1] > 0 and pk["bytes_read"] > 0 and "not the headline" in pk["note"]
     assert 0 < pk["zreduce_alone_ms"] <= r["zreduce_alone"]["kernel_ms"] * 1.5 and 0 < pk["forward_vjp_ms_median"] and 0 < pk["zreduce_in_step_frac"] < 1.2

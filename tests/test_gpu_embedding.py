@@ -62,6 +62,16 @@ def test_embedded_calls_equal_region_calls_on_the_cropped_block(kw, full, org):
         assert max_rel(eps_f[blk][b].cpu().numpy().astype(np.float64), ref) < TOL_EPS
         gref = O.vjp(oc, C[b], 9.0, [f[blk][b] for f in EF], [f[blk][b] for f in EA])
         assert rel_inf(g_e[b].cpu().numpy().astype(np.float64), gref) < TOL_GRAD
+    # window-only eps (epsgrad_plan_set_eps_window_only) inside the embedded block: after the full call above, a window call on
+    # another design leaves the solver's array as a full call would, and still touches nothing outside the block
+    C2 = rand_C(cfg, 63)
+    eps_w = eps_f.clone()
+    eps_full2 = torch.full(shape, sentinel, device="cuda")
+    plan.eps_forward(dev(C2), 9.0, out=eps_full2)
+    plan.set_eps_window_only(True)
+    plan.eps_forward(dev(C2), 9.0, out=eps_w)
+    plan.set_eps_window_only(False)
+    assert torch.equal(eps_w, eps_full2)
     plan.set_embedding()                                               # back to region-sized arrays
     eps_b, g_b = plan.eps_forward_vjp(dev(C), 9.0, cEF, cEA)
     assert torch.equal(eps_b, eps_r) and torch.equal(g_b, g_r)

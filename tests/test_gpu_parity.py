@@ -504,3 +504,65 @@ def test_packed_fields_give_the_same_gradient(kw, beta, n_pairs):
     with pytest.raises(B.EpsgradError) as e:
         plan.set_packed_fields(True)
     assert e.value.status == B.EUNSUPPORTED
+
+
+@pytest.mark.parametrize("kw,beta", [
+    (dict(mx=33, my=21, nz=64, z_lo=28.25, z_hi=35.75, filter_radius=8.0), 16.0),               # the paper's slab: sectors of cells 24..39
+    (dict(batch=2, mx=17, my=40, nz=32, z_lo=14.25, z_hi=17.75, filter_kind=1, filter_radius=6.0, filter_sigma=2.0), 8.0),
+    (dict(mx=12, my=12, nz=16, z_lo=0.0, z_hi=16.0, filter_radius=4.0), 8.0),                    # the slab is the whole column
+    (dict(mx=20, my=9, nz=12, z_lo=3.5, z_hi=4.25, filter_radius=4.0), 32.0),                   # a slab inside one cell; nz/4 odd
+    (dict(mx=14, my=10, nz=24, z_lo=20.5, z_hi=24.0, filter_radius=4.0), 8.0),                  # the slab ends at the top of the column
+    (dict(mx=12, my=14, nx_cells=70, ny_cells=81, nz=64, z_lo=28.25, z_hi=35.75, filter_radius=8.0), 16.0),
+])
+def test_eps_window_only_rewrites_the_slab_window_and_nothing_else(kw, beta):
+    """epsgrad_plan_set_eps_window_only: after ONE full call, a window call on a NEW design leaves the array bit for bit
+    equal to a full call on the new design; on an array of sentinels it writes whole 32-byte sectors around the slab and nothing
+    else; the oracle agrees on every cell; eps_forward_vjp does the same and its gradient does not change."""
+    cfg = B.make_config(**kw)
+    C1, C2 = rand_C(cfg, 61), rand_C(cfg, 62)
+    EF, EA = rand_fields(cfg, 1, 63)
+    plan = B.Plan(cfg)
+    full2 = plan.eps_forward(dev(C2), beta).clone()
+    g2 = plan.eps_vjp(dev(C2), beta, [dev(f) for f in EF], [dev(f) for f in EA]).clone()
+    buf = plan.eps_forward(dev(C1), beta).clone()                 # the one full call
+    assert not torch.equal(buf, full2)
+    plan.set_eps_window_only(True)
+    plan.eps_forward(dev(C2), beta, buf)
+    assert torch.equal(buf, full2)
+    ref = np.stack([O.forward(oracle_cfg(cfg), C2[b], beta) for b in range(cfg.batch)])
+    assert max_rel(buf.cpu().numpy().astype(np.float64), ref) < TOL_EPS
+    # what is written: whole sectors (8 cells) around the slab, nothing else
+    SENT = -7.0
+    s = torch.full(plan.eps_shape, SENT, dtype=torch.float32, device="cuda")
+    plan.eps_forward(dev(C2), beta, s)
+    written = (s != SENT)
+    per_k = written.reshape(-1, cfg.nz).any(dim=0).cpu().numpy()
+    assert (written.reshape(-1, cfg.nz).all(dim=0).cpu().numpy() == per_k).all()      # a z cell is written in every column or in none
+    ks = np.nonzero(per_k)[0]
+    k_lo, k_hi = int(np.floor(kw["z_lo"])), int(np.ceil(kw["z_hi"]))               # the slab's cells: [k_lo, k_hi)
+    assert ks.min() <= k_lo and ks.max() >= min(cfg.nz, k_hi) - 1, (ks.min(), ks.max())
+    assert ks.min() % 8 == 0 and ((ks.max() + 1) % 8 == 0 or ks.max() + 1 == cfg.nz), (ks.min(), ks.max())
+    assert len(ks) == ks.max() - ks.min() + 1 and len(ks) <= min(cfg.nz, (k_hi - k_lo) + 1 + 16)
+    assert torch.equal(s[written], full2[written])
+    assert bool((full2[~written] == float(np.float32(cfg.eps_clad))).all())           # everything it skips is cladding
+    # the one-call path, and the gradient
+    plan.set_eps_window_only(False)
+    buf2 = plan.eps_forward(dev(C1), beta).clone()
+    plan.set_eps_window_only(True)
+    e3, g3 = plan.eps_forward_vjp(dev(C2), beta, [dev(f) for f in EF], [dev(f) for f in EA], buf2)
+    assert torch.equal(e3, full2) and torch.equal(g3, g2)
+    plan.set_eps_window_only(False)
+    assert torch.equal(plan.eps_forward(dev(C2), beta), full2)
+    if cfg.nx_cells == 0 and cfg.batch == 1:
+        # the host entry point writes its eps buffer whole: refused while the option is on, as with packed fields
+        plan.set_eps_window_only(True)
+        with pytest.raises(B.EpsgradError) as e:
+            plan.eps_forward_vjp_host(torch.from_numpy(C2).pin_memory(), beta, [torch.from_numpy(f).pin_memory() for f in EF],
+                                      [torch.from_numpy(f).pin_memory() for f in EA],
+                                      torch.empty(plan.eps_shape, dtype=torch.float32).pin_memory(),
+                                      torch.empty(plan.ctrl_shape, dtype=torch.float32).pin_memory())
+        assert e.value.status == B.EUNSUPPORTED
+        plan.set_eps_window_only(False)
+    with pytest.raises(B.EpsgradError) as e:                              # columns that are not whole 16-byte pieces
+        B.Plan(B.make_config(mx=8, my=8, nz=10, z_lo=2.0, z_hi=5.0, filter_radius=3.0)).set_eps_window_only(True)
+    assert e.value.status == B.EUNSUPPORTED

@@ -46,6 +46,12 @@ def test_slabs_reproduce_the_undivided_plan(kw, world):
         assert torch.equal(plan.eps_forward(C_r, beta), eps_r) and torch.equal(plan.eps_vjp(C_r, beta, EF_r, EA_r), g_r)
         g_b, db_r = plan.eps_vjp_beta(C_r, beta, EF_r, EA_r)
         assert torch.equal(g_b, g_r)
+        # window-only eps on the slab's own rows: one full call on another design first, then the window call
+        buf = plan.eps_forward((1.0 - C_r).contiguous(), beta).clone()
+        plan.set_eps_window_only(True)
+        plan.eps_forward(C_r, beta, buf)
+        plan.set_eps_window_only(False)
+        assert torch.equal(buf, eps_r), (rank, p)
         g_sum[:, p["e0"]:p["e1"]] += g_r                 # what sharding.sum_gradients does across ranks
         db_sum += db_r
         # rows of the halo beyond the dependency cone get nothing at all

@@ -190,6 +190,20 @@ def test_random_configuration_every_entry_point(i):
         plan.set_tuning(5, knob)
         assert torch.equal(plan.stage_zreduce(EF, EA), G0) and torch.equal(plan.eps_vjp(C, beta, EF, EA), g0), (kw, knob)
     plan.set_tuning(5, 0)
+    # eps on the design region only: after a full call on another design, the window call gives the full call's array
+    try:
+        plan.set_eps_window_only(True)
+        windowed = True
+    except B.EpsgradError as err:
+        assert err.status == B.EUNSUPPORTED
+        windowed = False
+    if windowed:
+        plan.set_eps_window_only(False)
+        buf = plan.eps_forward((1.0 - C).contiguous(), beta).clone()
+        plan.set_eps_window_only(True)
+        ew, gw = plan.eps_forward_vjp(C, beta, EF, EA, eps_out=buf)
+        assert torch.equal(ew, eps0) and torch.equal(gw, g0), kw
+        plan.set_eps_window_only(False)
     # fields on the design region only: the slab window of every z column, packed (where the layout applies)
     try:
         plan.set_packed_fields(True)
