@@ -207,3 +207,41 @@ def test_repeated_calls_give_the_same_bits(name):
         gb, db = plan.eps_vjp_beta(C, w.betas[0], EF, EA)
         assert torch.equal(eps, eps0) and torch.equal(g, g0) and torch.equal(gb, gb0) and torch.equal(db, db0), rep
     torch.cuda.synchronize()
+
+
+@pytest.mark.skipif(not __import__("os").environ.get("EPSGRAD_FULL_WIDE"), reason="opt-in (EPSGRAD_FULL_WIDE=<designs>, e.g. 0,5 or all): 4 minutes of oracle time per design")
+def test_widebatch_full_size_elementwise():
+    """Wide batch (8 designs of 2048x2048x32, Gaussian filter of radius 32 cells) element by element against the oracle: the GPU
+    runs the whole batch in one call, the oracle takes the chosen designs one after the other (3.2 GB of fields and 3.2 GB of
+    float64 eps each; its reverse pass does 0.6 M cells/s on this filter).  Opt-in: the default suite compares a window on
+    every design (test_widebatch_full_size_sampled_windows).  Measured on a B200 box: DESIGN.md 6.2."""
+    w = W.BY_NAME["widebatch"]
+    if _mem_available_gb() < 60.0:
+        pytest.skip(f"needs 60 GB of free host memory, {_mem_available_gb():.0f} GB available")
+    C = W.make_C(w)
+    plan = B.Plan(B.config_of(w))
+    beta = w.betas[0]
+    dEF = torch.empty(plan.eps_shape, dtype=torch.complex64, device="cuda")
+    dEA = torch.empty(plan.eps_shape, dtype=torch.complex64, device="cuda")
+    for b in range(w.batch):
+        dEF[b] = torch.from_numpy(W.make_field(w, 0, 0, design=b)).cuda()
+        dEA[b] = torch.from_numpy(W.make_field(w, 0, 1, design=b)).cuda()
+    eps, g = plan.eps_forward_vjp(dev(C), beta, [dEF], [dEA])
+    torch.cuda.synchronize()
+    g = g.cpu().numpy().astype(np.float64)
+    del dEF, dEA
+    oc = cfg_of(replace(w, batch=1))
+    worst_e = worst_g = 0.0
+    sel = __import__("os").environ["EPSGRAD_FULL_WIDE"]
+    for b in (range(w.batch) if sel in ("1", "all") else [int(x) for x in sel.split(",")]):
+        EF, EA = W.make_field(w, 0, 0, design=b), W.make_field(w, 0, 1, design=b)
+        gref = O.vjp(oc, C[b], beta, [EF], [EA])
+        err_g = max(rel_inf(g[b], gref), rel_l2(g[b], gref))
+        del EF, EA
+        ref = O.forward(oc, C[b], beta)
+        eb = eps[b].cpu().numpy()
+        err_e = max(float(np.max(np.abs(eb[c] - ref[c]) / ref[c])) for c in range(3))
+        print(f"widebatch design {b}, every element: eps {err_e:.2e} on {ref.size} cells, dF/dC {err_g:.2e} on {gref.size} nodes", flush=True)
+        worst_e, worst_g = max(worst_e, err_e), max(worst_g, err_g)
+        del ref, eb
+    assert worst_e < TOL_EPS and worst_g < TOL_GRAD, (worst_e, worst_g)
